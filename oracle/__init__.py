@@ -1,0 +1,195 @@
+"""TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes binding of the plain CPU fp64 oracle in ``oracle/pdf_oracle.c`` (written
+from PAPER.md section 3.2; see the C header for the citations).
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
+/ ``--impl reference`` legs may import this package.  It imports nothing from
+``paper_2302_03343_b200`` and shares no code with the CUDA path.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pdf_oracle.c")
+_HDR = os.path.join(_HERE, "pdf_oracle.h")
+_LIB = os.path.join(_HERE, "libpdf_oracle.so")
+
+REGION_INTERIOR, REGION_LOWX, REGION_LOWQ, REGION_HIGHQ = 0, 1, 2, 3
+REGION_LOWX_LOWQ, REGION_LOWX_HIGHQ, REGION_INVALID = 4, 5, 6
+ALPHAS_FREEZE, ALPHAS_LOGGRAD = 0, 1
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, OpenMP, no FMA contraction)."""
+    stale = (not os.path.exists(_LIB)) or any(
+        os.path.getmtime(p) > os.path.getmtime(_LIB) for p in (_SRC, _HDR))
+    if force or stale:
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
+               "-ffp-contract=off", "-Wall", "-Wextra", "-o", _LIB + ".tmp", _SRC, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+        os.replace(_LIB + ".tmp", _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        dp, ip, vp = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p
+        ll = C.c_longlong
+        L.oracle_grid_create.argtypes = [C.POINTER(vp), C.c_int, dp, C.c_int, ip, dp, dp, C.c_int, ip, C.c_int]
+        L.oracle_grid_set_alphas.argtypes = [vp, C.c_int, dp, dp]
+        L.oracle_grid_set_alphas_mode.argtypes = [vp, C.c_int]
+        L.oracle_grid_set_coupling.argtypes = [vp, dp]
+        L.oracle_grid_limits.argtypes = [vp, dp, dp, dp, dp]
+        L.oracle_grid_destroy.argtypes = [vp]
+        L.oracle_locate.argtypes = [vp, ll, dp, dp, ip, ip, ip, ip]
+        L.oracle_xfxq2.argtypes = [vp, ip, C.c_int, ll, dp, dp, ip, dp, dp]
+        L.oracle_alphas_q2.argtypes = [vp, ll, dp, dp]
+        L.oracle_lumi.argtypes = [vp, ll, dp, dp, dp, dp, dp, dp]
+        L.oracle_interior_order.argtypes = [vp, C.c_int, C.c_int, C.c_int, ll, dp, dp, dp]
+        L.oracle_weights_1d.argtypes = [C.c_int, dp, C.c_double, C.c_int, dp]
+        L.oracle_num_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _i(a):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(C.POINTER(C.c_int))
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def weights_1d(knots_log, wlog: float, cell: int) -> np.ndarray:
+    k, kp = _d(knots_log)
+    w = np.zeros(4)
+    rc = lib().oracle_weights_1d(len(k), kp, float(wlog), int(cell), w.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc:
+        raise ValueError(f"oracle_weights_1d: {rc}")
+    return w
+
+
+class OracleGrid:
+    """Handle on an oracle grid.  ``values`` is [nmem] lists of per-sub-grid
+    arrays [nx][nq_k][nflav], or the flat concatenation the C call takes."""
+
+    def __init__(self, x_knots, q2_subgrids, values, pids, nmem: int = 1):
+        self._h = C.c_void_p()
+        x, xp = _d(x_knots)
+        nq = [len(q) for q in q2_subgrids]
+        q2, qp = _d(np.concatenate([np.asarray(q, dtype=np.float64) for q in q2_subgrids]))
+        nqa, nqp = _i(nq)
+        v, vp = _d(np.asarray(values, dtype=np.float64).ravel())
+        pid, pp = _i(pids)
+        expect = len(x) * sum(nq) * len(pid) * nmem
+        if v.size != expect:
+            raise ValueError(f"values has {v.size} entries, expected {expect}")
+        rc = lib().oracle_grid_create(C.byref(self._h), len(x), xp, len(nq), nqp, qp, vp, len(pid), pp, nmem)
+        if rc:
+            raise ValueError(f"oracle_grid_create failed: {rc}")
+        self.nflav, self.nmem = len(pid), nmem
+
+    def close(self):
+        if self._h:
+            lib().oracle_grid_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_alphas(self, q2_knots, values, mode: int = ALPHAS_FREEZE):
+        q, qp = _d(q2_knots)
+        v, vp = _d(values)
+        if lib().oracle_grid_set_alphas(self._h, len(q), qp, vp):
+            raise ValueError("oracle_grid_set_alphas failed")
+        if lib().oracle_grid_set_alphas_mode(self._h, mode):
+            raise ValueError("oracle_grid_set_alphas_mode failed")
+
+    def set_coupling(self, Cmat):
+        c, cp = _d(Cmat)
+        if c.size != self.nflav ** 2 or lib().oracle_grid_set_coupling(self._h, cp):
+            raise ValueError("oracle_grid_set_coupling failed")
+
+    def limits(self):
+        a = [C.c_double() for _ in range(4)]
+        lib().oracle_grid_limits(self._h, *[C.byref(t) for t in a])
+        return tuple(t.value for t in a)
+
+    def locate(self, x, q2):
+        x, xp = _d(x)
+        q, qp = _d(q2)
+        n = x.size
+        outs = [np.empty(n, dtype=np.int32) for _ in range(4)]
+        rc = lib().oracle_locate(self._h, n, xp, qp, *[o.ctypes.data_as(C.POINTER(C.c_int)) for o in outs])
+        if rc:
+            raise ValueError(f"oracle_locate: {rc}")
+        return tuple(outs)  # ix, iq, isub, region
+
+    def xfxq2(self, pids, x, q2, member=None, want_scale: bool = False):
+        x, xp = _d(x)
+        q, qp = _d(q2)
+        pid, pp = _i(pids)
+        n = x.size
+        out = np.empty((n, len(pid)))
+        sc = np.empty((n, len(pid))) if want_scale else None
+        mp = None
+        if member is not None:
+            member, mp = _i(member)
+        rc = lib().oracle_xfxq2(self._h, pp, len(pid), n, xp, qp, mp,
+                                out.ctypes.data_as(C.POINTER(C.c_double)),
+                                sc.ctypes.data_as(C.POINTER(C.c_double)) if want_scale else None)
+        if rc:
+            raise ValueError(f"oracle_xfxq2: {rc}")
+        return (out, sc) if want_scale else out
+
+    def alphas_q2(self, q2):
+        q, qp = _d(q2)
+        out = np.empty(q.size)
+        rc = lib().oracle_alphas_q2(self._h, q.size, qp, out.ctypes.data_as(C.POINTER(C.c_double)))
+        if rc:
+            raise ValueError(f"oracle_alphas_q2: {rc}")
+        return out
+
+    def lumi(self, x1, x2, q2, weights, want_scale: bool = False):
+        a, ap = _d(x1)
+        b, bp = _d(x2)
+        q, qp = _d(q2)
+        w, wp = _d(weights)
+        out = np.empty(a.size)
+        sc = np.empty(a.size) if want_scale else None
+        rc = lib().oracle_lumi(self._h, a.size, ap, bp, qp, wp,
+                               out.ctypes.data_as(C.POINTER(C.c_double)),
+                               sc.ctypes.data_as(C.POINTER(C.c_double)) if want_scale else None)
+        if rc:
+            raise ValueError(f"oracle_lumi: {rc}")
+        return (out, sc) if want_scale else out
+
+    def interior_order(self, order: int, flavour_col: int, x, q2, member: int = 0):
+        x, xp = _d(x)
+        q, qp = _d(q2)
+        out = np.empty(x.size)
+        rc = lib().oracle_interior_order(self._h, order, flavour_col, member, x.size, xp, qp,
+                                         out.ctypes.data_as(C.POINTER(C.c_double)))
+        if rc:
+            raise ValueError(f"oracle_interior_order: {rc}")
+        return out
