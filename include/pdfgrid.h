@@ -1,0 +1,161 @@
+/*
+ * pdfgrid.h -- C ABI of the B200-native (sm_100a) batched PDF interpolation library.
+ *
+ * What it computes (citations: /root/reference/PAPER.md = M. Rossi, arXiv:2302.03343):
+ *   - xf_i(x,Q2) by LHAPDF-style log-bicubic interpolation: cubic Hermite splines in
+ *     (log x, log Q2) on the 4 neighbour knots per axis (section 3.2, Fig. 3.1(a)),
+ *     on knot grids split in Q2 sub-grids at quark-mass thresholds (L1714, L1833);
+ *   - the default (MSTW / LHAPDF5) extrapolation outside the grid: low-x and high-Q linear
+ *     continuation from the two outermost knots, of log(xf) when both values exceed 1e-3
+ *     (L1720-1722); low-Q anomalous-dimension continuation eq. 3.4 with the limits of eq. 3.5
+ *     (L1724-1742); corners: x rule first, then Q rule (L1744);
+ *   - alpha_s(Q2): cubic Hermite spline on the log Q2 line, constant beyond the knots
+ *     (L1746, L1835);
+ *   - the two-parton luminosity  w * sum_ij C_ij f_i(x1,Q2) f_j(x2,Q2),  f = xf/x
+ *     (eq. 3.3, eq. 4.1).
+ * Readings of every point the paper leaves open are listed in DESIGN.md (C-1..C-L, S-1..S-22).
+ *
+ * Conventions
+ *   - Every function returns an int status: PDF_OK (0) or a negative code; nothing throws.
+ *   - HOST / DEVICE says where a pointer must live.  `stream` is a cudaStream_t passed as void*
+ *     (NULL = the legacy default stream).  Evaluation calls only ENQUEUE work on `stream` and
+ *     return; they never synchronise.  HOST arrays (pids, knots, values) are consumed before the
+ *     call returns.
+ *   - Ownership: pdf_grid_create copies its host arrays into device tables owned by the handle;
+ *     query / output / workspace buffers are caller-owned (e.g. torch tensors, data_ptr()).
+ *     The library allocates device memory only in pdf_grid_create / set_* and, for the *_host
+ *     convenience calls, a staging area kept in the handle.
+ *   - q2 is Q^2 in GeV^2; outputs are x*f (L1712 "always in the xf(x,Q2) format").
+ *   - Per-query domain errors (x <= 0, x > xmax, Q2 <= 0, non-finite, member out of range) write
+ *     quiet NaN to every requested column of that row and increment a device counter that
+ *     pdf_error_count reads.
+ *   - A requested pid that is not in the grid's flavour list yields a column of 0.0; pid 0 is
+ *     an alias of 21 (gluon).
+ */
+#ifndef PDFGRID_H
+#define PDFGRID_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    PDF_OK = 0,
+    PDF_EINVAL = -1,     /* bad argument (NULL, size, non-monotonic knots, non-finite value ...) */
+    PDF_ENOMEM = -2,     /* host or device allocation failed                                     */
+    PDF_ECUDA = -3,      /* a CUDA runtime call failed (see pdf_last_cuda_error)                 */
+    PDF_EWORKSPACE = -4, /* the binned path needs a workspace and none / too small was supplied  */
+    PDF_ESTATE = -5      /* call needs data that was not set (alpha_s knots, coupling matrix)    */
+};
+
+/* region codes written by pdf_locate (Fig. 3.1(b)) */
+enum {
+    PDF_REGION_INTERIOR = 0,
+    PDF_REGION_LOWX = 1,
+    PDF_REGION_LOWQ = 2,
+    PDF_REGION_HIGHQ = 3,
+    PDF_REGION_LOWX_LOWQ = 4,
+    PDF_REGION_LOWX_HIGHQ = 5,
+    PDF_REGION_INVALID = 6
+};
+
+/* alpha_s below its first knot: PDFFlow's constant (L1835, default) or LHAPDF's logarithmic
+ * gradient continuation (L1746) */
+enum { PDF_ALPHAS_FREEZE = 0, PDF_ALPHAS_LOGGRAD = 1 };
+
+/* evaluation strategy of pdf_xfxq2 / pdf_lumi (pdf_grid_set_option(PDF_OPT_PATH, ...)) */
+enum {
+    PDF_PATH_AUTO = 0,    /* binned when a workspace is attached and the call qualifies, else direct */
+    PDF_PATH_DIRECT = 1,  /* one thread per query, stencil gathered through L1/L2                   */
+    PDF_PATH_BINNED = 2   /* queries binned by cell so that warps share one stencil (needs workspace) */
+};
+enum { PDF_OPT_PATH = 1, PDF_OPT_ALPHAS_MODE = 2, PDF_OPT_CHUNK = 3 };
+
+typedef struct pdf_grid pdf_grid; /* opaque; owns its device tables */
+
+/* ---- grid handle (a-1: grid layout; L1714, L1833) -------------------------------------------
+ * x_knots   HOST [nx], strictly increasing, > 0, nx >= 2.
+ * nq        HOST [nsub], every nq[k] >= 2.
+ * q2_knots  HOST, the sub-grids' knots concatenated ([sum nq]); strictly increasing inside a
+ *           sub-grid; last knot of sub-grid k == first knot of sub-grid k+1 (bitwise).
+ * values    HOST [nmem][ block 0 | block 1 | ... ], block k = [nx][nq[k]][nflav] row-major,
+ *           all finite.  values are x*f at the knots.
+ * flavour_pids HOST [nflav] PDG ids of the value columns.
+ * The device currently selected (cudaGetDevice) becomes the grid's device.
+ * Errors: PDF_EINVAL on any violated condition, PDF_ENOMEM / PDF_ECUDA on allocation failure. */
+int pdf_grid_create(pdf_grid **g, int nx, const double *x_knots, int nsub, const int *nq,
+                    const double *q2_knots, const double *values, int nflav,
+                    const int *flavour_pids, int nmem);
+int pdf_grid_destroy(pdf_grid *g);
+
+/* alpha_s knots (HOST [n], Q2 strictly increasing > 0, n >= 2) and values (HOST [n]); L1746 */
+int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double *values);
+/* flavour-pair coupling C, HOST [nflav][nflav] row-major, in the grid's column order; eq. 4.1 */
+int pdf_grid_set_coupling(pdf_grid *g, const double *C);
+/* caller-owned DEVICE scratch for the binned path; must stay valid until replaced or the grid is
+ * destroyed; bytes >= pdf_workspace_bytes(g, n) for the largest n it will be used with.
+ * dev_ptr == NULL detaches. */
+int pdf_grid_set_workspace(pdf_grid *g, void *dev_ptr, size_t bytes);
+size_t pdf_workspace_bytes(const pdf_grid *g, long long n);
+int pdf_grid_set_option(pdf_grid *g, int option, long long value);
+/* xMin/xMax/Q2Min/Q2Max of L1714; any output pointer may be NULL */
+int pdf_grid_limits(const pdf_grid *g, double *xmin, double *xmax, double *q2min, double *q2max);
+
+/* ---- evaluation (a-2 ... a-5, a-8) ----------------------------------------------------------
+ * pids HOST [npid]; x, q2 DEVICE [n]; out DEVICE [n][npid] row-major (leading dimension npid).
+ * n == 0 is a no-op.  Enqueues on `stream`. */
+int pdf_xfxq2(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+              const double *q2, double *out, void *stream);
+/* as above with a per-query member index (DEVICE int32 [n] or NULL = member 0) and an explicit
+ * leading dimension ld_out >= npid (in doubles). */
+int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+                 const double *q2, const int *member, double *out, long long ld_out, void *stream);
+
+/* a-6: alpha_s(Q2); q2, out DEVICE [n].  PDF_ESTATE if no alpha_s knots were set. */
+int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out, void *stream);
+
+/* a-7: out[e] = weights[e] * sum_ij C_ij [xf_i(x1,q2)/x1] [xf_j(x2,q2)/x2] over the grid's own
+ * flavour columns (member 0); all arrays DEVICE [n].  PDF_ESTATE if no coupling was set. */
+int pdf_lumi(const pdf_grid *g, long long n, const double *x1, const double *x2, const double *q2,
+             const double *weights, double *out, void *stream);
+
+/* a-2 exposed for validation: region class, sub-grid, lower-left knot of the cell (ix, and iq
+ * local to the sub-grid); DEVICE int32 [n] each, any may be NULL.  For extrapolated queries the
+ * indices are those of the knots the continuation is anchored on (low-x: ix = 0; low-Q:
+ * isub = 0, iq = 0; high-Q: last sub-grid, iq = nq-2); invalid queries get -1. */
+int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2, int *ix,
+               int *iq, int *isub, int *region, void *stream);
+
+/* number of invalid queries seen by this grid since creation / the last call of this function
+ * (reads and resets the device counter; synchronises `stream`). */
+int pdf_error_count(const pdf_grid *g, long long *n_invalid, void *stream);
+
+/* ---- host-buffer convenience calls (the e2e path) -------------------------------------------
+ * Same results as the calls above, but x, q2, out (x1, x2, weights) are HOST pointers, pinned
+ * memory recommended.  The call copies inputs to the device in chunks, evaluates, copies the
+ * results back, overlapping the three on internal streams, and returns when `out` is complete. */
+int pdf_xfxq2_host(pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+                   const double *q2, double *out);
+int pdf_alphas_q2_host(pdf_grid *g, long long n, const double *q2, double *out);
+int pdf_lumi_host(pdf_grid *g, long long n, const double *x1, const double *x2, const double *q2,
+                  const double *weights, double *out);
+
+/* ---- diagnostics ---------------------------------------------------------------------------- */
+const char *pdf_status_string(int status);
+const char *pdf_last_cuda_error(void);
+/* kernels launched by this library in this process since load (the bench's gpu_launches) */
+long long pdf_launch_count(void);
+/* name and launch time (ms, CUDA events on `stream`) of the kernels of the last evaluation call
+ * when profiling was switched on with pdf_profile_enable(1); returns the number of entries. */
+int pdf_profile_enable(int on);
+int pdf_profile_read(int max_entries, const char **names, float *ms);
+/* sustained fp64 FMA throughput of the device (an independent-DFMA-chain kernel), in TFLOP/s;
+ * the measured denominator of the "alu" roofline of pdf_lumi. */
+int pdf_measure_fp64_tflops(double *tflops, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,284 @@
+"""Thin ctypes binding of ``libpdfgrid.so`` (C ABI: ``include/pdfgrid.h``).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels.  The
+function names mirror the C calls (``pdf_grid_create`` ... ``pdf_lumi``).  PyTorch is
+used for device memory and streams (``tensor.data_ptr()``, the current CUDA stream).
+
+There is NO CPU fallback: if the shared library is missing or cannot be loaded,
+importing a symbol raises ``PdfGridError``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import torch
+
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpdfgrid.so")
+
+PDF_OK, PDF_EINVAL, PDF_ENOMEM, PDF_ECUDA, PDF_EWORKSPACE, PDF_ESTATE = 0, -1, -2, -3, -4, -5
+PDF_PATH_AUTO, PDF_PATH_DIRECT, PDF_PATH_BINNED = 0, 1, 2
+PDF_OPT_PATH, PDF_OPT_ALPHAS_MODE, PDF_OPT_CHUNK = 1, 2, 3
+PDF_ALPHAS_FREEZE, PDF_ALPHAS_LOGGRAD = 0, 1
+
+# every symbol include/pdfgrid.h declares (tests check the library exports all of them)
+SYMBOLS = (
+    "pdf_grid_create", "pdf_grid_destroy", "pdf_grid_set_alphas", "pdf_grid_set_coupling",
+    "pdf_grid_set_workspace", "pdf_workspace_bytes", "pdf_grid_set_option", "pdf_grid_limits",
+    "pdf_xfxq2", "pdf_xfxq2_ex", "pdf_alphas_q2", "pdf_lumi", "pdf_locate", "pdf_error_count",
+    "pdf_xfxq2_host", "pdf_alphas_q2_host", "pdf_lumi_host", "pdf_status_string",
+    "pdf_last_cuda_error", "pdf_launch_count", "pdf_profile_enable", "pdf_profile_read",
+    "pdf_measure_fp64_tflops",
+)
+
+
+class PdfGridError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load libpdfgrid.so (never builds at import time on the GPU box; fails loudly if absent)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise PdfGridError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                           "(nvcc, sm_100a). There is no CPU fallback.")
+    L = C.CDLL(LIB_PATH)
+    vp, ip, dp, ll = C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_double), C.c_longlong
+    L.pdf_grid_create.argtypes = [C.POINTER(vp), C.c_int, dp, C.c_int, ip, dp, dp, C.c_int, ip, C.c_int]
+    L.pdf_grid_destroy.argtypes = [vp]
+    L.pdf_grid_set_alphas.argtypes = [vp, C.c_int, dp, dp]
+    L.pdf_grid_set_coupling.argtypes = [vp, dp]
+    L.pdf_grid_set_workspace.argtypes = [vp, vp, C.c_size_t]
+    L.pdf_workspace_bytes.argtypes = [vp, ll]
+    L.pdf_workspace_bytes.restype = C.c_size_t
+    L.pdf_grid_set_option.argtypes = [vp, C.c_int, ll]
+    L.pdf_grid_limits.argtypes = [vp, dp, dp, dp, dp]
+    L.pdf_xfxq2.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp]
+    L.pdf_xfxq2_ex.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp, ll, vp]
+    L.pdf_alphas_q2.argtypes = [vp, ll, vp, vp, vp]
+    L.pdf_lumi.argtypes = [vp, ll, vp, vp, vp, vp, vp, vp]
+    L.pdf_locate.argtypes = [vp, ll, vp, vp, vp, vp, vp, vp, vp]
+    L.pdf_error_count.argtypes = [vp, C.POINTER(ll), vp]
+    L.pdf_xfxq2_host.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp]
+    L.pdf_alphas_q2_host.argtypes = [vp, ll, vp, vp]
+    L.pdf_lumi_host.argtypes = [vp, ll, vp, vp, vp, vp, vp]
+    L.pdf_status_string.argtypes = [C.c_int]
+    L.pdf_status_string.restype = C.c_char_p
+    L.pdf_last_cuda_error.restype = C.c_char_p
+    L.pdf_launch_count.restype = ll
+    L.pdf_profile_enable.argtypes = [C.c_int]
+    L.pdf_profile_read.argtypes = [C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
+    L.pdf_measure_fp64_tflops.argtypes = [dp, vp]
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str):
+    if rc != PDF_OK:
+        L = lib()
+        msg = L.pdf_status_string(rc).decode()
+        if rc == PDF_ECUDA or rc == PDF_ENOMEM:
+            msg += " [" + L.pdf_last_cuda_error().decode() + "]"
+        raise PdfGridError(f"{what}: {msg} ({rc})")
+
+
+def _hd(t) -> torch.Tensor:
+    return torch.as_tensor(t, dtype=torch.float64, device="cpu").contiguous()
+
+
+def _hi(t) -> torch.Tensor:
+    return torch.as_tensor(t, dtype=torch.int32, device="cpu").contiguous()
+
+
+def _dptr(t: torch.Tensor):
+    return C.cast(t.data_ptr(), C.POINTER(C.c_double))
+
+
+def _iptr(t: torch.Tensor):
+    return C.cast(t.data_ptr(), C.POINTER(C.c_int))
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype, what: str):
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise PdfGridError(f"{what} must be a contiguous CUDA tensor of dtype {dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def pdf_launch_count() -> int:
+    return int(lib().pdf_launch_count())
+
+
+def pdf_profile_enable(on: bool):
+    lib().pdf_profile_enable(1 if on else 0)
+
+
+def pdf_profile_read(max_entries: int = 4096):
+    names = (C.c_char_p * max_entries)()
+    ms = (C.c_float * max_entries)()
+    n = lib().pdf_profile_read(max_entries, names, ms)
+    return [(names[i].decode(), float(ms[i])) for i in range(n)]
+
+
+def pdf_measure_fp64_tflops(stream=None) -> float:
+    v = C.c_double()
+    _check(lib().pdf_measure_fp64_tflops(C.byref(v), _stream_ptr(stream)), "pdf_measure_fp64_tflops")
+    return v.value
+
+
+class PdfGrid:
+    """Owner of a ``pdf_grid*`` handle.  Methods are 1:1 with the C calls."""
+
+    def __init__(self, x_knots, q2_subgrids: Sequence, values, pids: Sequence[int], nmem: int = 1):
+        L = lib()
+        x = _hd(x_knots)
+        nq = _hi([len(q) for q in q2_subgrids])
+        q2 = _hd(torch.cat([_hd(q) for q in q2_subgrids]))
+        v = _hd(values).reshape(-1)
+        pid = _hi(list(pids))
+        expect = x.numel() * int(nq.sum()) * pid.numel() * nmem
+        if v.numel() != expect:
+            raise PdfGridError(f"values has {v.numel()} entries, expected {expect}")
+        self._h = C.c_void_p()
+        _check(L.pdf_grid_create(C.byref(self._h), x.numel(), _dptr(x), nq.numel(), _iptr(nq), _dptr(q2),
+                                 _dptr(v), pid.numel(), _iptr(pid), nmem), "pdf_grid_create")
+        self.nflav, self.nmem, self.pids = pid.numel(), nmem, tuple(int(p) for p in pids)
+        self._ws = None
+
+    @classmethod
+    def from_spec(cls, spec, workspace_for: int = 0):
+        g = cls(spec.x_knots, spec.q2_subgrids, spec.values, spec.pids, nmem=spec.nmem)
+        if spec.alphas_q2 is not None:
+            g.pdf_grid_set_alphas(spec.alphas_q2, spec.alphas_val)
+        if spec.coupling is not None:
+            g.pdf_grid_set_coupling(spec.coupling)
+        if workspace_for:
+            g.attach_workspace(workspace_for)
+        return g
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().pdf_grid_destroy(self._h)
+            self._h = C.c_void_p()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- configuration -------------------------------------------------------------------
+    def pdf_grid_set_alphas(self, q2_knots, values):
+        q, v = _hd(q2_knots), _hd(values)
+        _check(lib().pdf_grid_set_alphas(self._h, q.numel(), _dptr(q), _dptr(v)), "pdf_grid_set_alphas")
+
+    def pdf_grid_set_coupling(self, Cmat):
+        c = _hd(Cmat).reshape(-1)
+        if c.numel() != self.nflav ** 2:
+            raise PdfGridError("coupling must be [nflav][nflav]")
+        _check(lib().pdf_grid_set_coupling(self._h, _dptr(c)), "pdf_grid_set_coupling")
+
+    def pdf_grid_set_option(self, option: int, value: int):
+        _check(lib().pdf_grid_set_option(self._h, option, value), "pdf_grid_set_option")
+
+    def pdf_workspace_bytes(self, n: int) -> int:
+        return int(lib().pdf_workspace_bytes(self._h, n))
+
+    def pdf_grid_set_workspace(self, ws: Optional[torch.Tensor]):
+        if ws is None:
+            _check(lib().pdf_grid_set_workspace(self._h, None, 0), "pdf_grid_set_workspace")
+        else:
+            _check(lib().pdf_grid_set_workspace(self._h, C.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size()),
+                   "pdf_grid_set_workspace")
+        self._ws = ws
+
+    def attach_workspace(self, n: int, device="cuda"):
+        """Allocate (torch) and attach the scratch the binned path needs for calls of up to n queries."""
+        nbytes = self.pdf_workspace_bytes(n)
+        if nbytes:
+            self.pdf_grid_set_workspace(torch.empty(nbytes, dtype=torch.uint8, device=device))
+        return nbytes
+
+    def pdf_grid_limits(self):
+        a = [C.c_double() for _ in range(4)]
+        _check(lib().pdf_grid_limits(self._h, *[C.byref(t) for t in a]), "pdf_grid_limits")
+        return tuple(t.value for t in a)
+
+    # ---- evaluation (device tensors) -----------------------------------------------------
+    def pdf_xfxq2(self, pids, x: torch.Tensor, q2: torch.Tensor, out: Optional[torch.Tensor] = None,
+                  member: Optional[torch.Tensor] = None, ld_out: Optional[int] = None, stream=None):
+        pid = _hi(list(pids))
+        n = x.numel()
+        ld = ld_out or pid.numel()
+        if out is None:
+            out = torch.empty((n, ld), dtype=torch.float64, device=x.device)
+        xp, qp, op = _dev(x, torch.float64, "x"), _dev(q2, torch.float64, "q2"), _dev(out, torch.float64, "out")
+        if q2.numel() != n or out.numel() < n * ld:
+            raise PdfGridError("size mismatch")
+        if member is None and ld == pid.numel():
+            rc = lib().pdf_xfxq2(self._h, _iptr(pid), pid.numel(), n, xp, qp, op, _stream_ptr(stream))
+        else:
+            mp = _dev(member, torch.int32, "member") if member is not None else None
+            rc = lib().pdf_xfxq2_ex(self._h, _iptr(pid), pid.numel(), n, xp, qp, mp, op, ld, _stream_ptr(stream))
+        _check(rc, "pdf_xfxq2")
+        return out
+
+    def pdf_alphas_q2(self, q2: torch.Tensor, out: Optional[torch.Tensor] = None, stream=None):
+        if out is None:
+            out = torch.empty_like(q2)
+        _check(lib().pdf_alphas_q2(self._h, q2.numel(), _dev(q2, torch.float64, "q2"),
+                                   _dev(out, torch.float64, "out"), _stream_ptr(stream)), "pdf_alphas_q2")
+        return out
+
+    def pdf_lumi(self, x1, x2, q2, weights, out: Optional[torch.Tensor] = None, stream=None):
+        if out is None:
+            out = torch.empty_like(x1)
+        f = torch.float64
+        _check(lib().pdf_lumi(self._h, x1.numel(), _dev(x1, f, "x1"), _dev(x2, f, "x2"), _dev(q2, f, "q2"),
+                              _dev(weights, f, "weights"), _dev(out, f, "out"), _stream_ptr(stream)), "pdf_lumi")
+        return out
+
+    def pdf_locate(self, x: torch.Tensor, q2: torch.Tensor, stream=None):
+        n = x.numel()
+        outs = [torch.empty(n, dtype=torch.int32, device=x.device) for _ in range(4)]
+        _check(lib().pdf_locate(self._h, n, _dev(x, torch.float64, "x"), _dev(q2, torch.float64, "q2"),
+                                *[C.c_void_p(o.data_ptr()) for o in outs], _stream_ptr(stream)), "pdf_locate")
+        return tuple(outs)  # ix, iq, isub, region
+
+    def pdf_error_count(self, stream=None) -> int:
+        v = C.c_longlong()
+        _check(lib().pdf_error_count(self._h, C.byref(v), _stream_ptr(stream)), "pdf_error_count")
+        return int(v.value)
+
+    # ---- evaluation (host tensors; the e2e path) -------------------------------------------
+    def pdf_xfxq2_host(self, pids, x: torch.Tensor, q2: torch.Tensor, out: torch.Tensor):
+        pid = _hi(list(pids))
+        for t in (x, q2, out):
+            if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+                raise PdfGridError("host call takes contiguous CPU float64 tensors")
+        _check(lib().pdf_xfxq2_host(self._h, _iptr(pid), pid.numel(), x.numel(), C.c_void_p(x.data_ptr()),
+                                    C.c_void_p(q2.data_ptr()), C.c_void_p(out.data_ptr())), "pdf_xfxq2_host")
+        return out
+
+    def pdf_alphas_q2_host(self, q2: torch.Tensor, out: torch.Tensor):
+        _check(lib().pdf_alphas_q2_host(self._h, q2.numel(), C.c_void_p(q2.data_ptr()),
+                                        C.c_void_p(out.data_ptr())), "pdf_alphas_q2_host")
+        return out
+
+    def pdf_lumi_host(self, x1, x2, q2, weights, out):
+        _check(lib().pdf_lumi_host(self._h, x1.numel(), *[C.c_void_p(t.data_ptr()) for t in (x1, x2, q2, weights, out)]),
+               "pdf_lumi_host")
+        return out

@@ -1,0 +1,249 @@
+// pdf_common.cuh -- device-side data layout and the per-query arithmetic shared by all kernels.
+//
+// Method: PAPER.md section 3.2 (L1714-1746) in the readings of DESIGN.md (C-1 ... C-L).
+// This file is part of the CUDA product path; it shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pdfg {
+
+constexpr int kMaxLumiFlav = 16;   // generic pdf_lumi keeps both flavour vectors in registers/local
+constexpr int kRegionInterior = 0, kRegionLowX = 1, kRegionLowQ = 2, kRegionHighQ = 3,
+              kRegionLowXLowQ = 4, kRegionLowXHighQ = 5, kRegionInvalid = 6;
+
+// Per-cell constants of the 1-D Hermite operator in its 4-node-weight form (C-5):
+//   W[-1] = -bL h10;  W[0] = h00 + (bL-aL) h10 - aR h11;  W[+1] = h01 + aL h10 + (aR-bR) h11;
+//   W[+2] = bR h11,   with (aL,bL) = (1/2, rho_-/2) if the left neighbour exists else (1,0),
+//   (aR,bR) likewise on the right (one-sided secant at a grid / sub-grid end, L1833).
+struct CellTab {
+    double lo_log;   // ln of the cell's lower knot
+    double inv_d;    // 1 / (ln upper - ln lower)
+    double aL, bL, aR, bR;
+};
+
+// Device view of one grid (a-1).  Values are re-laid as V[mem][jg][ix][nfp]: one node = one
+// padded flavour row, the 4 x-neighbours of a Q2 row contiguous, jg = global Q2 knot index over
+// the concatenated sub-grids (a threshold appears twice, once per sub-grid, L1714).
+struct GridDev {
+    int nx, nsub, nflav, nfp, nmem, nqtot;
+    const double *xk, *qk;        // raw knots [nx], [nqtot]
+    const double *uk, *sk;        // ln knots (device log: the same routine the queries go through)
+    const int *sub_of;            // [nqtot] sub-grid of global knot jg
+    const int *qoff;              // [nsub+1]
+    const CellTab *cx;            // [nx-1]
+    const CellTab *cq;            // [nqtot], entry jg valid when jg is not the last knot of its sub-grid
+    const double *V;
+    size_t memstride;             // nqtot*nx*nfp
+    double q2plus;                // 1.01 * Q2min (C-9)
+    // alpha_s (a-6)
+    int na, alphas_mode;
+    const double *ak, *alk, *av;  // raw knots, ln knots, values
+    const CellTab *ca;            // [na-1]
+    // luminosity coupling [nflav][nflav]
+    const double *C;
+    unsigned long long *err_count;
+};
+
+struct Point1D {      // a cell, its 4 clamped node indices and node weights
+    int idx[4];
+    double w[4];
+};
+
+__device__ __forceinline__ bool finite_pos(double v) { return v > 0.0 && v < __longlong_as_double(0x7ff0000000000000LL); }
+
+// largest c in [0, m-2] with k[c] <= v (0 if none): C-4, comparisons on RAW values
+__device__ __forceinline__ int find_cell(const double *__restrict__ k, int m, double v)
+{
+    int lo = 0, hi = m - 1;
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (k[mid] <= v) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// largest jg in [0, m-1] with k[jg] <= v (0 if none); duplicates (thresholds) resolve to the
+// later copy, i.e. the UPPER sub-grid (C-3, S-6)
+__device__ __forceinline__ int find_last_le(const double *__restrict__ k, int m, double v)
+{
+    int lo = 0, hi = m;
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (k[mid] <= v) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+__device__ __forceinline__ void hermite_weights(double t, const CellTab &c, double w[4])
+{
+    double t2 = t * t, t3 = t2 * t;
+    double h00 = 2.0 * t3 - 3.0 * t2 + 1.0;
+    double h10 = t3 - 2.0 * t2 + t;
+    double h01 = -2.0 * t3 + 3.0 * t2;
+    double h11 = t3 - t2;
+    w[0] = -c.bL * h10;
+    w[1] = h00 + (c.bL - c.aL) * h10 - c.aR * h11;
+    w[2] = h01 + c.aL * h10 + (c.aR - c.bR) * h11;
+    w[3] = c.bR * h11;
+}
+
+__device__ __forceinline__ int classify(const GridDev &G, double x, double q2)
+{
+    if (!(finite_pos(x) && finite_pos(q2)) || x > G.xk[G.nx - 1]) return kRegionInvalid;
+    bool lowx = x < G.xk[0], lowq = q2 < G.qk[0], highq = q2 > G.qk[G.nqtot - 1];
+    if (lowx) return lowq ? kRegionLowXLowQ : highq ? kRegionLowXHighQ : kRegionLowX;
+    return lowq ? kRegionLowQ : highq ? kRegionHighQ : kRegionInterior;
+}
+
+// x-axis point inside the knot range: cell i, t = (ln x - u_i)/(u_{i+1}-u_i)
+__device__ __forceinline__ void x_point_cell(const GridDev &G, int i, double t, Point1D &p)
+{
+    CellTab c = G.cx[i];
+    hermite_weights(t, c, p.w);
+    p.idx[0] = i > 0 ? i - 1 : i;
+    p.idx[1] = i;
+    p.idx[2] = i + 1;
+    p.idx[3] = i + 2 < G.nx ? i + 2 : i + 1;
+}
+
+__device__ __forceinline__ int x_point(const GridDev &G, double x, Point1D &p)
+{
+    int i = find_cell(G.xk, G.nx, x);
+    // t = 1 exactly on the last knot (the only knot that belongs to the cell on its left, C-4)
+    double t = (x == G.xk[i + 1]) ? 1.0 : (log(x) - G.cx[i].lo_log) * G.cx[i].inv_d;
+    x_point_cell(G, i, t, p);
+    return i;
+}
+
+// Q2-axis point: jg = global index of the cell's lower knot
+__device__ __forceinline__ void q_point_cell(const GridDev &G, int jg, double t, Point1D &p)
+{
+    CellTab c = G.cq[jg];
+    hermite_weights(t, c, p.w);
+    p.idx[0] = (c.aL == 1.0) ? jg : jg - 1;     // no left neighbour inside the sub-grid
+    p.idx[1] = jg;
+    p.idx[2] = jg + 1;
+    p.idx[3] = (c.aR == 1.0) ? jg + 1 : jg + 2;
+}
+
+// in-range Q2: returns sub-grid k; writes local cell j
+__device__ __forceinline__ int q_locate(const GridDev &G, double q2, int &j, int &jg)
+{
+    int g = find_last_le(G.qk, G.nqtot, q2);
+    int k = G.sub_of[g];
+    int nqk = G.qoff[k + 1] - G.qoff[k];
+    j = g - G.qoff[k];
+    if (j > nqk - 2) j = nqk - 2;               // only Q2 == Q2max lands on a last knot
+    jg = G.qoff[k] + j;
+    return k;
+}
+
+__device__ __forceinline__ void q_point(const GridDev &G, double q2, Point1D &p)
+{
+    int j, jg;
+    q_locate(G, q2, j, jg);
+    double t = (q2 == G.qk[jg + 1]) ? 1.0 : (log(q2) - G.cq[jg].lo_log) * G.cq[jg].inv_d;
+    q_point_cell(G, jg, t, p);
+}
+
+// x-axis descriptor: in range -> one point; below X_0 -> the two anchor points + theta (C-7)
+struct XDesc { bool low; Point1D p0, p1; double theta; };
+// Q2-axis descriptor for Q2 >= Q2min: in range -> one point; above -> two anchors + theta (C-8)
+struct QDesc { bool high; Point1D p0, p1; double theta; };
+
+__device__ __forceinline__ void make_xdesc(const GridDev &G, double x, XDesc &d)
+{
+    d.low = x < G.xk[0];
+    if (!d.low) { x_point(G, x, d.p0); return; }
+    x_point_cell(G, 0, 0.0, d.p0);
+    if (G.nx >= 3) x_point_cell(G, 1, 0.0, d.p1); else x_point_cell(G, 0, 1.0, d.p1);
+    d.theta = (log(x) - G.uk[0]) / (G.uk[1] - G.uk[0]);
+}
+
+__device__ __forceinline__ void make_qdesc(const GridDev &G, double q2, QDesc &d)
+{
+    int last = G.nqtot - 1;
+    d.high = q2 > G.qk[last];
+    if (!d.high) { q_point(G, q2, d.p0); return; }
+    q_point_cell(G, last - 1, 0.0, d.p0);
+    q_point_cell(G, last - 1, 1.0, d.p1);
+    d.theta = (log(q2) - G.sk[last - 1]) / (G.sk[last] - G.sk[last - 1]);
+}
+
+// C-7 / C-8 switch (L1722): log form iff both anchors exceed 1e-3, per flavour
+__device__ __forceinline__ double continue_two(double f0, double f1, double theta)
+{
+    if (f0 > 1e-3 && f1 > 1e-3) {
+        double l0 = log(f0), l1 = log(f1);
+        return exp(l0 + theta * (l1 - l0));
+    }
+    return f0 + theta * (f1 - f0);
+}
+
+// C-9, eq. 3.4 with the limits of eq. 3.5
+__device__ __forceinline__ double lowq_continue(double fmin, double fplus, double r)
+{
+    double gamma = 1.0;
+    if (fmin > 1e-5) gamma = fmax(-2.5, (fplus - fmin) / (0.01 * fmin));
+    return fmin * pow(r, (gamma - 1.0) * r + 1.0);
+}
+
+// C-6 as a 16-term tensor sum for one flavour column
+__device__ __forceinline__ double stencil_col(const GridDev &G, const double *__restrict__ Vm,
+                                              const Point1D &xp, const Point1D &qp, int col)
+{
+    double acc = 0.0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        const double *row = Vm + (size_t)qp.idx[b] * G.nx * G.nfp + col;
+        double rb = 0.0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) rb = fma(xp.w[a], __ldg(row + (size_t)xp.idx[a] * G.nfp), rb);
+        acc = fma(qp.w[b], rb, acc);
+    }
+    return acc;
+}
+
+__device__ __forceinline__ double value_inq(const GridDev &G, const double *Vm, const XDesc &X,
+                                            const Point1D &qp, int col)
+{
+    if (!X.low) return stencil_col(G, Vm, X.p0, qp, col);
+    return continue_two(stencil_col(G, Vm, X.p0, qp, col), stencil_col(G, Vm, X.p1, qp, col), X.theta);
+}
+
+__device__ __forceinline__ double value_geq(const GridDev &G, const double *Vm, const XDesc &X,
+                                            const QDesc &Q, int col)
+{
+    if (!Q.high) return value_inq(G, Vm, X, Q.p0, col);
+    return continue_two(value_inq(G, Vm, X, Q.p0, col), value_inq(G, Vm, X, Q.p1, col), Q.theta);
+}
+
+// everything a thread needs to evaluate any flavour column of one valid query
+struct QueryPlan {
+    XDesc X;
+    QDesc Q;        // for q2 (in range / high) or for Q2min when lowq
+    QDesc Qplus;    // for 1.01*Q2min, only when lowq
+    bool lowq;
+    double r;       // q2 / Q2min when lowq
+};
+
+__device__ __forceinline__ void make_plan(const GridDev &G, double x, double q2, QueryPlan &P)
+{
+    make_xdesc(G, x, P.X);
+    P.lowq = q2 < G.qk[0];
+    if (!P.lowq) { make_qdesc(G, q2, P.Q); return; }
+    make_qdesc(G, G.qk[0], P.Q);
+    make_qdesc(G, G.q2plus, P.Qplus);
+    P.r = q2 / G.qk[0];
+}
+
+__device__ __forceinline__ double plan_value(const GridDev &G, const double *Vm, const QueryPlan &P, int col)
+{
+    if (!P.lowq) return value_geq(G, Vm, P.X, P.Q, col);
+    return lowq_continue(value_geq(G, Vm, P.X, P.Q, col), value_geq(G, Vm, P.X, P.Qplus, col), P.r);
+}
+
+__device__ __forceinline__ double qnan() { return __longlong_as_double(0x7ff8000000000000LL); }
+
+}  // namespace pdfg

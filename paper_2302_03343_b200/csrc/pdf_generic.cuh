@@ -1,0 +1,179 @@
+// pdf_generic.cuh -- layout kernels (a-1) and the DIRECT evaluation kernels: one thread per
+// query, any nflav / pid list / member axis, stencil gathered through L1/L2.  These are the
+// general-purpose path (PDF_PATH_DIRECT); the binned, warp-coherent path lives in pdf_binned.cuh.
+#pragma once
+#include "pdf_common.cuh"
+
+namespace pdfg {
+
+// ---- a-1: grid layout ------------------------------------------------------------------------
+// ln of the knots with the device log (so that t == 0 exactly on a knot), one thread per knot
+__global__ void k_log_knots(const double *__restrict__ k, double *__restrict__ lk, int n)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) lk[i] = log(k[i]);
+}
+
+// per-cell Hermite constants of one knot line [first, first+m) (a sub-grid, the x line, alpha_s)
+__global__ void k_cell_tables(const double *__restrict__ lk, CellTab *__restrict__ tab, int first, int m)
+{
+    int c = blockIdx.x * blockDim.x + threadIdx.x;      // local cell
+    if (c >= m - 1) return;
+    const double *w = lk + first;
+    double d = w[c + 1] - w[c];
+    CellTab t;
+    t.lo_log = w[c];
+    t.inv_d = 1.0 / d;
+    bool left = c > 0, right = c + 2 < m;
+    t.aL = left ? 0.5 : 1.0;
+    t.bL = left ? 0.5 * (d / (w[c] - w[c - 1])) : 0.0;
+    t.aR = right ? 0.5 : 1.0;
+    t.bR = right ? 0.5 * (d / (w[c + 2] - w[c + 1])) : 0.0;
+    tab[first + c] = t;
+}
+
+// values [mem][block k: [ix][iq][f]]  ->  V[mem][jg][ix][nfp] (pad columns = 0)
+__global__ void k_relayout(const double *__restrict__ src, double *__restrict__ dst, int nx, int nqk,
+                           int nflav, int nfp, int nqtot, int qoff_k, size_t src_memstride,
+                           size_t src_suboff, int nmem)
+{
+    size_t per_mem = (size_t)nx * nqk * nfp;
+    size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= per_mem * nmem) return;
+    int mem = (int)(e / per_mem);
+    size_t r = e % per_mem;
+    int f = (int)(r % nfp);
+    size_t node = r / nfp;
+    int ix = (int)(node % nx);
+    int iq = (int)(node / nx);
+    double v = 0.0;
+    if (f < nflav) v = src[(size_t)mem * src_memstride + src_suboff + ((size_t)ix * nqk + iq) * nflav + f];
+    dst[(size_t)mem * ((size_t)nqtot * nx * nfp) + ((size_t)(qoff_k + iq) * nx + ix) * nfp + f] = v;
+}
+
+// ---- a-2: locate -----------------------------------------------------------------------------
+__global__ void k_locate(GridDev G, long long n, const double *__restrict__ x, const double *__restrict__ q2,
+                         int *ix, int *iq, int *isub, int *region)
+{
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double xv = x[e], qv = q2[e];
+    int r = classify(G, xv, qv);
+    int i = -1, j = -1, k = -1;
+    if (r != kRegionInvalid) {
+        bool lowx = (r == kRegionLowX || r == kRegionLowXLowQ || r == kRegionLowXHighQ);
+        i = lowx ? 0 : find_cell(G.xk, G.nx, xv);
+        if (r == kRegionLowQ || r == kRegionLowXLowQ) { k = 0; j = 0; }
+        else if (r == kRegionHighQ || r == kRegionLowXHighQ) { k = G.nsub - 1; j = G.qoff[k + 1] - G.qoff[k] - 2; }
+        else { int jg; k = q_locate(G, qv, j, jg); }
+    }
+    if (ix) ix[e] = i;
+    if (iq) iq[e] = j;
+    if (isub) isub[e] = k;
+    if (region) region[e] = r;
+}
+
+// ---- a-3 ... a-5, a-8: direct evaluation -----------------------------------------------------
+// cols[p] = value column of requested pid p, or -1 (unknown pid -> 0.0)
+struct ColMap { int n; int col[64]; };
+
+__global__ void __launch_bounds__(128)
+k_xfxq2_direct(GridDev G, ColMap cm, long long n, const double *__restrict__ x,
+               const double *__restrict__ q2, const int *__restrict__ member,
+               double *__restrict__ out, long long ld)
+{
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double xv = x[e], qv = q2[e];
+    int mem = member ? member[e] : 0;
+    int r = classify(G, xv, qv);
+    double *o = out + e * ld;
+    if (r == kRegionInvalid || mem < 0 || mem >= G.nmem) {
+        for (int p = 0; p < cm.n; ++p) o[p] = qnan();
+        atomicAdd(G.err_count, 1ULL);
+        return;
+    }
+    const double *Vm = G.V + (size_t)mem * G.memstride;
+    QueryPlan P;
+    make_plan(G, xv, qv, P);
+    for (int p = 0; p < cm.n; ++p) {
+        int c = cm.col[p];
+        o[p] = c < 0 ? 0.0 : plan_value(G, Vm, P, c);
+    }
+}
+
+// ---- a-6: alpha_s ----------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_alphas(GridDev G, long long n, const double *__restrict__ q2, double *__restrict__ out)
+{
+    extern __shared__ double sm[];
+    double *ak = sm;                 // [na] raw knots
+    double *av = sm + G.na;          // [na] values
+    for (int i = threadIdx.x; i < G.na; i += blockDim.x) { ak[i] = G.ak[i]; av[i] = G.av[i]; }
+    __syncthreads();
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
+        double q = q2[e];
+        double v;
+        int m = G.na;
+        if (!finite_pos(q)) v = qnan();
+        else if (q > ak[m - 1]) v = av[m - 1];
+        else if (q < ak[0])   // L1835 constant (default) or L1746 logarithmic-gradient continuation
+            v = G.alphas_mode ? av[0] * pow(q / ak[0], log(av[1] / av[0]) / log(ak[1] / ak[0])) : av[0];
+        else {
+            int c = find_cell(ak, m, q);
+            CellTab ct = G.ca[c];
+            double t = (q == ak[c + 1]) ? 1.0 : (log(q) - ct.lo_log) * ct.inv_d;
+            double w[4];
+            hermite_weights(t, ct, w);
+            int i0 = c > 0 ? c - 1 : c, i3 = c + 2 < m ? c + 2 : c + 1;
+            v = fma(w[0], av[i0], fma(w[1], av[c], fma(w[2], av[c + 1], w[3] * av[i3])));
+        }
+        out[e] = v;
+    }
+}
+
+// ---- a-7: direct luminosity ------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+k_lumi_direct(GridDev G, long long n, const double *__restrict__ x1, const double *__restrict__ x2,
+              const double *__restrict__ q2, const double *__restrict__ w, double *__restrict__ out)
+{
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double a = x1[e], b = x2[e], qv = q2[e];
+    if (classify(G, a, qv) == kRegionInvalid || classify(G, b, qv) == kRegionInvalid) {
+        out[e] = qnan();
+        atomicAdd(G.err_count, 1ULL);
+        return;
+    }
+    double f2[kMaxLumiFlav];
+    QueryPlan P;
+    make_plan(G, b, qv, P);
+    double inv_b = 1.0 / b;
+    for (int j = 0; j < G.nflav; ++j) f2[j] = plan_value(G, G.V, P, j) * inv_b;
+    make_plan(G, a, qv, P);
+    double inv_a = 1.0 / a;
+    double acc = 0.0;
+    for (int i = 0; i < G.nflav; ++i) {
+        double f1 = plan_value(G, G.V, P, i) * inv_a;
+        double row = 0.0;
+        for (int j = 0; j < G.nflav; ++j) row = fma(__ldg(G.C + i * G.nflav + j), f2[j], row);
+        acc = fma(f1, row, acc);
+    }
+    out[e] = w[e] * acc;
+}
+
+// ---- fp64 peak micro-benchmark (denominator of the "alu" roofline) ----------------------------
+__global__ void __launch_bounds__(256)
+k_dfma_chain(double *sink, int iters, double a, double b)
+{
+    double r0 = threadIdx.x, r1 = r0 + 1, r2 = r0 + 2, r3 = r0 + 3, r4 = r0 + 4, r5 = r0 + 5, r6 = r0 + 6, r7 = r0 + 7;
+    for (int i = 0; i < iters; ++i) {
+        r0 = fma(r0, a, b); r1 = fma(r1, a, b); r2 = fma(r2, a, b); r3 = fma(r3, a, b);
+        r4 = fma(r4, a, b); r5 = fma(r5, a, b); r6 = fma(r6, a, b); r7 = fma(r7, a, b);
+    }
+    double s = r0 + r1 + r2 + r3 + r4 + r5 + r6 + r7;
+    if (s == 12345.678) sink[0] = s;
+}
+
+}  // namespace pdfg

@@ -1,0 +1,174 @@
+// pdfgrid_eval.inl -- evaluation entry points of the C ABI (included at the end of pdfgrid.cu).
+
+namespace {
+
+int build_colmap(const pdf_grid *g, const int *pids, int npid, ColMap &cm)
+{
+    if (!pids || npid < 1 || npid > 64) return PDF_EINVAL;
+    cm.n = npid;
+    for (int p = 0; p < npid; ++p) cm.col[p] = col_of_pid(g, pids[p]);
+    return PDF_OK;
+}
+
+inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+// direct path in slices of < 2^31 blocks (n is long long)
+int launch_direct(const pdf_grid *g, const ColMap &cm, long long n, const double *x, const double *q2,
+                  const int *member, double *out, long long ld, cudaStream_t s)
+{
+    const long long slice = 1LL << 30;
+    for (long long off = 0; off < n; off += slice) {
+        long long m = n - off < slice ? n - off : slice;
+        LaunchScope a(s, "k_xfxq2_direct");
+        k_xfxq2_direct<<<blocks_for(m, 128), 128, 0, s>>>(g->d, cm, m, x + off, q2 + off,
+                                                         member ? member + off : nullptr, out + off * ld, ld);
+    }
+    CK(cudaGetLastError());
+    return PDF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+                 const double *q2, const int *member, double *out, long long ld_out, void *stream)
+{
+    if (!g || n < 0 || ld_out < npid) return PDF_EINVAL;
+    ColMap cm;
+    int rc = build_colmap(g, pids, npid, cm);
+    if (rc) return rc;
+    if (n == 0) return PDF_OK;
+    if (!x || !q2 || !out) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    bool want_binned = g->path == PDF_PATH_BINNED ||
+                       (g->path == PDF_PATH_AUTO && g->ws && binned_qualifies(g->bplan, cm, member, n));
+    if (want_binned) {
+        if (!binned_qualifies(g->bplan, cm, member, n)) return PDF_EINVAL;
+        size_t need = pdf_workspace_bytes(g, n);
+        if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
+        return binned_xfxq2(g->d, g->bplan, cm, n, x, q2, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
+    }
+    return launch_direct(g, cm, n, x, q2, member, out, ld_out, s);
+}
+
+int pdf_xfxq2(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+              const double *q2, double *out, void *stream)
+{
+    return pdf_xfxq2_ex(g, pids, npid, n, x, q2, nullptr, out, npid, stream);
+}
+
+size_t pdf_workspace_bytes(const pdf_grid *g, long long n)
+{
+    if (!g || n < 0) return 0;
+    return binned_workspace_bytes(g->bplan, n, g->chunk);
+}
+
+int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out, void *stream)
+{
+    if (!g || n < 0) return PDF_EINVAL;
+    if (g->d.na < 2) return PDF_ESTATE;
+    if (n == 0) return PDF_OK;
+    if (!q2 || !out) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device);
+    long long want = (n + 255) / 256;
+    unsigned grid = (unsigned)(want < (long long)sms * 16 ? want : (long long)sms * 16);
+    LaunchScope a(s, "k_alphas");
+    k_alphas<<<grid, 256, sizeof(double) * 2 * g->d.na, s>>>(g->d, n, q2, out);
+    CK(cudaGetLastError());
+    return PDF_OK;
+}
+
+int pdf_lumi(const pdf_grid *g, long long n, const double *x1, const double *x2, const double *q2,
+             const double *weights, double *out, void *stream)
+{
+    if (!g || n < 0) return PDF_EINVAL;
+    if (!g->d.C) return PDF_ESTATE;
+    if (g->d.nflav > kMaxLumiFlav) return PDF_EINVAL;
+    if (n == 0) return PDF_OK;
+    if (!x1 || !x2 || !q2 || !weights || !out) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    bool want_binned = g->path == PDF_PATH_BINNED ||
+                       (g->path == PDF_PATH_AUTO && g->ws && binned_lumi_qualifies(g->bplan, n));
+    if (want_binned) {
+        if (!binned_lumi_qualifies(g->bplan, n)) return PDF_EINVAL;
+        size_t need = pdf_workspace_bytes(g, n);
+        if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
+        return binned_lumi(g->d, g->bplan, n, x1, x2, q2, weights, out, g->ws, g->ws_bytes, g->chunk, s);
+    }
+    const long long slice = 1LL << 30;
+    for (long long off = 0; off < n; off += slice) {
+        long long m = n - off < slice ? n - off : slice;
+        LaunchScope a(s, "k_lumi_direct");
+        k_lumi_direct<<<blocks_for(m, 128), 128, 0, s>>>(g->d, m, x1 + off, x2 + off, q2 + off, weights + off, out + off);
+    }
+    CK(cudaGetLastError());
+    return PDF_OK;
+}
+
+int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2, int *ix,
+               int *iq, int *isub, int *region, void *stream)
+{
+    if (!g || n < 0) return PDF_EINVAL;
+    if (n == 0) return PDF_OK;
+    if (!x || !q2) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const long long slice = 1LL << 30;
+    for (long long off = 0; off < n; off += slice) {
+        long long m = n - off < slice ? n - off : slice;
+        LaunchScope a(s, "k_locate");
+        k_locate<<<blocks_for(m, 256), 256, 0, s>>>(g->d, m, x + off, q2 + off, ix ? ix + off : nullptr,
+                                                   iq ? iq + off : nullptr, isub ? isub + off : nullptr,
+                                                   region ? region + off : nullptr);
+    }
+    CK(cudaGetLastError());
+    return PDF_OK;
+}
+
+int pdf_error_count(const pdf_grid *g, long long *n_invalid, void *stream)
+{
+    if (!g || !n_invalid) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    unsigned long long v = 0;
+    CK(cudaMemcpyAsync(&v, g->d_err, sizeof v, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemsetAsync(g->d_err, 0, sizeof v, s));
+    CK(cudaStreamSynchronize(s));
+    *n_invalid = (long long)v;
+    return PDF_OK;
+}
+
+int pdf_measure_fp64_tflops(double *tflops, void *stream)
+{
+    if (!tflops) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    double *sink = nullptr;
+    int rc = dev_alloc(&sink, 1);
+    if (rc) return rc;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    const int iters = 1 << 15, blocks = sms * 8, threads = 256;
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(a, s);
+        { LaunchScope l(s, "k_dfma_chain"); k_dfma_chain<<<blocks, threads, 0, s>>>(sink, iters, 0.999999, 1e-9); }
+        cudaEventRecord(b, s);
+        cudaEventSynchronize(b);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        if (rep && ms < best) best = ms;
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
+    CK(cudaGetLastError());
+    double flops = 2.0 * 8.0 * (double)iters * (double)blocks * threads;
+    *tflops = flops / (best * 1e-3) / 1e12;
+    return PDF_OK;
+}
+
+}  // extern "C"
+
+#include "pdfgrid_host.inl"

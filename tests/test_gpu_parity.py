@@ -1,0 +1,267 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Integer results (region, sub-grid, cell) must be bit-exact; values obey the
+tolerance of tests/parity.py (C-12)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2302_03343_b200 import synth
+from conftest import make_oracle_grid
+from parity import assert_values, value_errors
+
+pytestmark = pytest.mark.gpu
+
+PATHS = ["direct", "auto"]
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2302_03343_b200 import binding
+    assert torch.cuda.is_available()
+    binding.lib()
+    return binding
+
+
+def gpu_grid(B, spec, path="direct", n=0):
+    g = B.PdfGrid.from_spec(spec, workspace_for=n if path != "direct" else 0)
+    g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_DIRECT if path == "direct" else B.PDF_PATH_AUTO)
+    return g
+
+
+def knot_neighbour_queries(spec):
+    """every knot and its nextafter neighbours on both axes, crossed with a few fixed partners"""
+    xk = spec.x_knots.numpy()
+    qk = np.unique(np.concatenate([q.numpy() for q in spec.q2_subgrids]))
+    xs = np.concatenate([xk, np.nextafter(xk[1:], 0), np.nextafter(xk[:-1], 2)])
+    qs = np.concatenate([qk, np.nextafter(qk[1:], 0), np.nextafter(qk[:-1], 1e300)])
+    X = np.concatenate([xs, np.full(len(qs), 0.0123), np.full(len(qs), xk[0]), np.full(len(qs), xk[-1])])
+    Q = np.concatenate([np.full(len(xs), float(qk[len(qk) // 2]) * 1.01), qs, qs, qs])
+    return X, Q
+
+
+def check_locate(B, og, g, x, q):
+    ix, iq, isub, reg = og.locate(x, q)
+    gx, gq, gs, gr = [t.cpu().numpy() for t in g.pdf_locate(torch.tensor(x).cuda(), torch.tensor(q).cuda())]
+    assert np.array_equal(reg, gr) and np.array_equal(isub, gs)
+    assert np.array_equal(ix, gx) and np.array_equal(iq, gq)
+
+
+@pytest.mark.parametrize("cfg", ["c0", "c1"])
+def test_locate_bitexact(B, oracle_mod, cfg):
+    spec = synth.grid_c0() if cfg == "c0" else synth.grid_c1()
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec)
+    x, q = synth.queries_c2(spec, 300_001, seed=17)
+    check_locate(B, og, g, x.numpy(), q.numpy())
+    X, Q = knot_neighbour_queries(spec)
+    check_locate(B, og, g, X, Q)
+    bad_x = np.array([0.0, -1.0, 1.5, np.nan, np.inf, 0.1, 0.1, 0.1])
+    bad_q = np.array([10.0, 10.0, 10.0, 10.0, 10.0, 0.0, -3.0, np.nan])
+    check_locate(B, og, g, bad_x, bad_q)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_c0_parity(B, oracle_mod, path):
+    """configs[0]: 1e5 queries strictly inside the 50x30 single-sub-grid grid"""
+    spec = synth.grid_c0()
+    n = 100_000
+    x, q = synth.queries_inside(spec, n, synth.BASE_SEED + 10, strict=True)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda()).cpu().numpy()
+    st = assert_values(out, ref, S, "c0")
+    assert st["frac_within_strict"] > 0.99
+    assert g.pdf_error_count() == 0
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_c1_parity(B, oracle_mod, path):
+    """configs[1] shape (1e6-query slice of the 1e7 recipe; several tiles and a ragged tail)"""
+    spec = synth.grid_c1()
+    n = 1_000_003
+    x, q = synth.queries_inside(spec, n, synth.BASE_SEED + 11)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda()).cpu().numpy()
+    assert_values(out, ref, S, "c1")
+    check_locate(B, og, g, x.numpy()[:200_000], q.numpy()[:200_000])
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_c2_extrapolation_parity(B, oracle_mod, path):
+    """configs[2]: 5 % of the queries outside the grid (all five extrapolation classes)"""
+    spec = synth.grid_c1()
+    n = 1_000_000
+    x, q = synth.queries_c2(spec, n)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda()).cpu().numpy()
+    _, _, _, reg = og.locate(x.numpy(), q.numpy())
+    for r in range(6):
+        sel = reg == r
+        assert sel.sum() > 1000
+        assert_values(out[sel], ref[sel], S[sel], f"c2 region {r}")
+    a = g.pdf_alphas_q2(q.cuda()).cpu().numpy()
+    aref = og.alphas_q2(q.numpy())
+    assert np.max(np.abs(a - aref) / np.abs(aref)) < 1e-12
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_scan_lines_and_knots(B, oracle_mod, path):
+    """the thesis' accuracy-scan pattern (Fig. 3.5) + every knot and its neighbours;
+    P-1 on the GPU: stored node values come back bitwise"""
+    spec = synth.grid_c1()
+    og = make_oracle_grid(oracle_mod, spec)
+    X, Q = synth.scan_lines(spec)
+    Xk, Qk = knot_neighbour_queries(spec)
+    x = np.concatenate([X.numpy(), Xk])
+    q = np.concatenate([Q.numpy(), Qk])
+    g = gpu_grid(B, spec, path, len(x))
+    ref, S = og.xfxq2(spec.pids, x, q, want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, torch.tensor(x).cuda(), torch.tensor(q).cuda()).cpu().numpy()
+    assert_values(out, ref, S, "scan")
+    for k, qk in enumerate(spec.q2_subgrids):
+        top = len(qk) - 1 if k < len(spec.q2_subgrids) - 1 else len(qk)
+        XX, QQ = torch.meshgrid(spec.x_knots, qk[:top], indexing="ij")
+        got = g.pdf_xfxq2(spec.pids, XX.reshape(-1).cuda(), QQ.reshape(-1).cuda()).cpu()
+        want = spec.block(0, k)[:, :top, :].reshape(-1, spec.nflav)
+        assert torch.equal(got, want)
+
+
+def test_c3_members_parity(B, oracle_mod):
+    """configs[3]: replica batch, per-query member index (20 members here; the 100-member grid runs in bench)"""
+    spec = synth.grid_c1(nmem=20)
+    n = 400_000
+    x, q = synth.queries_inside(spec, n, synth.BASE_SEED + 13)
+    mem = synth.members(spec, n)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec)
+    ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), member=mem.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda(), member=mem.cuda()).cpu().numpy()
+    assert_values(out, ref, S, "c3")
+    bad = mem.clone()
+    bad[:5] = 20
+    bad[5:9] = -1
+    out = g.pdf_xfxq2(spec.pids, x[:100].cuda(), q[:100].cuda(), member=bad[:100].cuda()).cpu().numpy()
+    assert np.all(np.isnan(out[:9])) and not np.any(np.isnan(out[9:]))
+    assert g.pdf_error_count() == 9
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_c4_lumi_parity(B, oracle_mod, path):
+    """configs[4]: luminosity; ~20 % of the events take the low-Q branch"""
+    spec = synth.grid_c1()
+    n = 300_000
+    x1, x2, q2, w = synth.events_c4(n)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    ref, S = og.lumi(x1.numpy(), x2.numpy(), q2.numpy(), w.numpy(), want_scale=True)
+    out = g.pdf_lumi(x1.cuda(), x2.cuda(), q2.cuda(), w.cuda()).cpu().numpy()
+    assert_values(out, ref, S, "lumi")
+    # invalid events
+    x1b = x1[:64].clone()
+    x1b[3] = 1.5
+    x1b[7] = float("nan")
+    out = g.pdf_lumi(x1b.cuda(), x2[:64].cuda(), q2[:64].cuda(), w[:64].cuda()).cpu().numpy()
+    assert np.isnan(out[3]) and np.isnan(out[7]) and np.isnan(out).sum() == 2
+    assert g.pdf_error_count() == 2
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_pids_ld_and_edge_sizes(B, oracle_mod, path):
+    spec = synth.grid_c1()
+    og = make_oracle_grid(oracle_mod, spec)
+    g = gpu_grid(B, spec, path, 5000)
+    x, q = synth.queries_c2(spec, 5000, seed=3)
+    pids = [21, -3, 99, 0, 5]
+    ref, S = og.xfxq2(pids, x.numpy(), q.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(pids, x.cuda(), q.cuda()).cpu().numpy()
+    assert_values(out, ref, S, "pids")
+    assert np.all(out[:, 2] == 0.0) and np.array_equal(out[:, 0], out[:, 3])
+    # explicit leading dimension: untouched padding
+    buf = torch.full((5000, 12), -7.0, dtype=torch.float64, device="cuda")
+    g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda(), out=buf, ld_out=12)
+    ref11, S11 = og.xfxq2(spec.pids, x.numpy(), q.numpy(), want_scale=True)
+    assert_values(buf[:, :11].cpu().numpy(), ref11, S11, "ld12")
+    assert torch.all(buf[:, 11] == -7.0)
+    # empty and ragged sizes
+    for n in (0, 1, 31, 33, 127, 129, 1025):
+        o = g.pdf_xfxq2(spec.pids, x[:n].cuda(), q[:n].cuda())
+        assert o.shape == (n, 11)
+        if n:
+            assert_values(o.cpu().numpy(), ref11[:n], S11[:n], f"n={n}")
+    # invalid rows -> NaN + counter
+    bx = x[:10].clone()
+    bq = q[:10].clone()
+    bx[0], bx[1], bq[2], bq[3], bx[4] = 0.0, 1.0000001, -1.0, float("inf"), float("nan")
+    g.pdf_error_count()
+    o = g.pdf_xfxq2(spec.pids, bx.cuda(), bq.cuda()).cpu().numpy()
+    assert np.all(np.isnan(o[:5])) and not np.any(np.isnan(o[5:]))
+    assert g.pdf_error_count() == 5 and g.pdf_error_count() == 0
+
+
+def test_tiny_nonuniform_grids(B, oracle_mod):
+    """degenerate shapes: 2-knot axes, 2- and 3-knot sub-grids, non-uniform knots, all regions"""
+    rng = np.random.default_rng(4)
+    for nx, nq in [(2, [2]), (3, [3]), (4, [2, 3]), (5, [4, 2, 5]), (3, [2, 2, 2])]:
+        spec = synth.tiny_grid(200 + nx + len(nq), nx, nq, nflav=3)
+        og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec)
+        xmin, xmax, qmin, qmax = og.limits()
+        n = 4000
+        x = np.exp(rng.uniform(math.log(xmin) - 3, math.log(xmax), n)).clip(max=xmax)
+        q = np.exp(rng.uniform(math.log(qmin) - 3, math.log(qmax) + 3, n))
+        Xk, Qk = knot_neighbour_queries(spec)
+        x, q = np.concatenate([x, Xk]), np.concatenate([q, Qk])
+        check_locate(B, og, g, x, q)
+        ref, S = og.xfxq2(spec.pids, x, q, want_scale=True)
+        out = g.pdf_xfxq2(spec.pids, torch.tensor(x).cuda(), torch.tensor(q).cuda()).cpu().numpy()
+        assert_values(out, ref, S, f"tiny {nx} {nq}")
+
+
+def test_alphas_modes_and_nodes(B, oracle_mod):
+    spec = synth.grid_c1()
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec)
+    aq = spec.alphas_q2
+    assert torch.equal(g.pdf_alphas_q2(aq.cuda()).cpu(), spec.alphas_val)
+    q = torch.exp(torch.linspace(math.log(1e-3), math.log(1e13), 200_001, dtype=torch.float64))
+    a = g.pdf_alphas_q2(q.cuda()).cpu().numpy()
+    ref = og.alphas_q2(q.numpy())
+    assert np.max(np.abs(a - ref) / ref) < 1e-12
+    g.pdf_grid_set_option(B.PDF_OPT_ALPHAS_MODE, B.PDF_ALPHAS_LOGGRAD)
+    og.set_alphas(spec.alphas_q2.numpy(), spec.alphas_val.numpy(), mode=oracle_mod.ALPHAS_LOGGRAD)
+    a = g.pdf_alphas_q2(q.cuda()).cpu().numpy()
+    ref = og.alphas_q2(q.numpy())
+    assert np.max(np.abs(a - ref) / ref) < 1e-12
+    bad = torch.tensor([0.0, -1.0, float("nan")], dtype=torch.float64)
+    assert torch.all(torch.isnan(g.pdf_alphas_q2(bad.cuda())))
+
+
+def test_host_calls_match_device_calls(B, oracle_mod):
+    spec = synth.grid_c1()
+    g = gpu_grid(B, spec, "auto", 1 << 22)
+    n = (1 << 22) + 12345          # more than one pipeline chunk
+    x, q = synth.queries_c2(spec, n, seed=21)
+    out_h = torch.empty((n, 11), dtype=torch.float64).pin_memory()
+    g.pdf_xfxq2_host(spec.pids, x.pin_memory(), q.pin_memory(), out_h)
+    out_d = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda()).cpu()
+    assert torch.equal(torch.nan_to_num(out_h, nan=-1.0), torch.nan_to_num(out_d, nan=-1.0))
+    a_h = torch.empty(n, dtype=torch.float64)
+    g.pdf_alphas_q2_host(q, a_h)
+    assert torch.equal(a_h, g.pdf_alphas_q2(q.cuda()).cpu())
+    x1, x2, q2, w = synth.events_c4(100_000)
+    l_h = torch.empty(100_000, dtype=torch.float64)
+    g.pdf_lumi_host(x1, x2, q2, w, l_h)
+    assert torch.equal(l_h, g.pdf_lumi(x1.cuda(), x2.cuda(), q2.cuda(), w.cuda()).cpu())
+
+
+def test_missing_state_and_workspace_errors(B):
+    spec = synth.grid_c0()
+    g = B.PdfGrid(spec.x_knots, spec.q2_subgrids, spec.values, spec.pids)
+    q = torch.ones(4, dtype=torch.float64, device="cuda")
+    with pytest.raises(B.PdfGridError):
+        g.pdf_alphas_q2(q)
+    with pytest.raises(B.PdfGridError):
+        g.pdf_lumi(q, q, q, q)
+    g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_BINNED)
+    if g.pdf_workspace_bytes(4) > 0:
+        with pytest.raises(B.PdfGridError):
+            g.pdf_xfxq2(spec.pids, q * 0.1, q * 10)
