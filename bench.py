@@ -139,13 +139,15 @@ def timed_steps(torch, dist, world, fn, steps, warmup, sampler_index=None):
     """W untimed + K timed steps, barrier + synchronize on both sides, CUDA events on the launching
     stream, MAX over ranks.  Returns (seconds for K steps, clocks dict, per-kernel profile list)."""
     from paper_2302_03343_b200 import binding
+    sampler = ClockSampler(sampler_index) if sampler_index is not None else None
+    if sampler is not None:
+        time.sleep(1.0)                  # nvidia-smi start-up; its samples then cover warm-up + timed region
     for _ in range(warmup):
         fn()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
-    sampler = ClockSampler(sampler_index) if sampler_index is not None else None
     binding.pdf_profile_enable(True)
     launches0 = binding.pdf_launch_count()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -220,6 +222,7 @@ def run_ours(args):
 
     secs, clocks, prof, launches = timed_steps(torch, dist, world, step, args.steps, args.warmup, sampler_index=local)
     n_invalid = g.pdf_error_count()
+    out_sample = out[:200_000].clone()
     table = kernel_table(prof, args.steps)
     value = world * n * 11 * args.steps / secs
     xf_kernels = [k for k in table if k != "k_alphas"]
@@ -235,14 +238,14 @@ def run_ours(args):
             "clocks": clocks, "gpu_launches": launches, "kernels": table, "roofline": roof}
 
     if not args.skip_extras:
-        extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2, out, aout, line, peak_gbs, peak_src)
+        extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2, out, aout, line, peak_gbs, peak_src, out_sample)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
 
-def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2, out, aout, line, peak_gbs, peak_src):
+def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2, out, aout, line, peak_gbs, peak_src, out_sample):
     n = args.n
     steps, warm = max(2, min(args.steps, 3)), 3
     # ---- fp64 peak of this device (denominator of the "alu" roofline of pdf_lumi) -------------
@@ -331,10 +334,10 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
                                 "sample": f"first {ns} queries of this run's C2 batch, xfxq2 (11 flavours) + alphas, {dt:.1f} s"}
         # sampled parity at full size, in the timed launch configuration (oracle one by one on the sample)
         import numpy as np
-        got = out[:ns].cpu().numpy()
+        got = out_sample.cpu().numpy()
         _, S = og.xfxq2(spec.pids, cx[:200_000], cq[:200_000], want_scale=True)
         err = np.abs(got[:200_000] - ref[:200_000])
-        tol = 1e-12 * np.abs(ref[:200_000]) + 1e-13 * S
+        tol = 1e-12 * np.abs(ref[:200_000]) + 1e-14 * S
         okn = ~np.isnan(ref[:200_000])
         line["parity_sample"] = {"n": 200_000, "worst_err_over_tol": float(np.max(err[okn] / np.maximum(tol[okn], 1e-300))),
                                  "nan_match": bool(np.array_equal(np.isnan(got[:200_000]), ~okn))}

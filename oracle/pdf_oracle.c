@@ -189,15 +189,40 @@ static double hermite_cell(int m, const double *w, const double *v, long stride,
 {
     double delta = w[c + 1] - w[c];
     double t = (wpt - w[c]) / delta;
-    double t2 = t * t, t3 = t2 * t;
-    double h00 = 2.0 * t3 - 3.0 * t2 + 1.0;
-    double h10 = t3 - 2.0 * t2 + t;
-    double h01 = -2.0 * t3 + 3.0 * t2;
-    double h11 = t3 - t2;
+    /* the four Hermite basis cubics 2t^3-3t^2+1, t^3-2t^2+t, -2t^3+3t^2, t^3-t^2, written in
+     * factored form so that each keeps its relative accuracy where it vanishes (t -> 0, 1) */
+    double omt = 1.0 - t;
+    double h00 = (1.0 + 2.0 * t) * (omt * omt);
+    double h10 = t * (omt * omt);
+    double h01 = (t * t) * (3.0 - 2.0 * t);
+    double h11 = -((t * t) * omt);
     double mc = knot_slope(m, w, v, stride, c);
     double mc1 = knot_slope(m, w, v, stride, c + 1);
     return h00 * v[(long)c * stride] + h10 * (delta * mc)
          + h01 * v[(long)(c + 1) * stride] + h11 * (delta * mc1);
+}
+
+/* dp/dt of the same cubic (used only for the condition scale of the parity metric) */
+static double hermite_cell_dt(int m, const double *w, const double *v, long stride,
+                              int c, double wpt)
+{
+    double delta = w[c + 1] - w[c];
+    double t = (wpt - w[c]) / delta;
+    double omt = 1.0 - t;
+    double d00 = -6.0 * t * omt, d10 = omt * (1.0 - 3.0 * t), d01 = 6.0 * t * omt, d11 = t * (3.0 * t - 2.0);
+    double mc = knot_slope(m, w, v, stride, c);
+    double mc1 = knot_slope(m, w, v, stride, c + 1);
+    return d00 * v[(long)c * stride] + d10 * (delta * mc)
+         + d01 * v[(long)(c + 1) * stride] + d11 * (delta * mc1);
+}
+
+/* KT converts a first-order t-rounding term into units of the scale S:
+ * tol = 1e-12 |ref| + 1e-14 * scale, and t = (ln v - ln knot)/delta carries a rounding error of
+ * up to 2^-52 (2 + 2 |ln v|/delta); a factor 2 covers the two sides  ->  KT = 4 * 2^-52 / 1e-14 */
+#define KT 0.0888178419700125
+static double t_cond(const double *w, int c, double wpt)
+{
+    return 1.0 + fabs(wpt) / (w[c + 1] - w[c]);
 }
 
 /* The knots a cell's cubic depends on are c-1..c+2 where they exist.  This
@@ -322,23 +347,30 @@ static void interior_value(const oracle_grid *g, int mem, int fcol, double x,
                 acc += fabs(wx[a] * wq[b] * B[((long)ia * nqk + jb) * g->nflav + fcol]);
             }
         }
-        *S = acc;
+        /* first-order sensitivity to the rounding of t_x and t_q */
+        double rd[4];
+        for (int b = jlo; b <= jhi; ++b)
+            rd[b - jlo] = hermite_cell_dt(g->nx, g->u, B + (long)b * g->nflav + fcol, xstride, i, lx);
+        double dfx = hermite_cell(jhi - jlo + 1, sk + jlo, rd, 1, j - jlo, lq);
+        double dfq = hermite_cell_dt(jhi - jlo + 1, sk + jlo, r, 1, j - jlo, lq);
+        *S = acc + KT * (fabs(dfx) * t_cond(g->u, i, lx) + fabs(dfq) * t_cond(sk, j, lq));
     }
 }
 
 /* C-7 / C-8 switch: continuation from two anchor values at abscissa theta
  * (theta = 0 at anchor 0, 1 at anchor 1).  Log form iff both > 1e-3 (L1722). */
 static void continue_two(double f0, double S0, double f1, double S1, double theta,
-                         double *val, double *S)
+                         double theta_cond, double *val, double *S)
 {
     if (f0 > 1e-3 && f1 > 1e-3) {
         double l0 = log(f0), l1 = log(f1);
         double v = exp(l0 + theta * (l1 - l0));
         *val = v;
-        if (S) *S = fabs(v) * (fabs(1.0 - theta) * S0 / f0 + fabs(theta) * S1 / f1);
+        if (S) *S = fabs(v) * (fabs(1.0 - theta) * S0 / f0 + fabs(theta) * S1 / f1
+                               + KT * theta_cond * fabs(l1 - l0));
     } else {
         *val = f0 + theta * (f1 - f0);
-        if (S) *S = fabs(1.0 - theta) * S0 + fabs(theta) * S1;
+        if (S) *S = fabs(1.0 - theta) * S0 + fabs(theta) * S1 + KT * theta_cond * fabs(f1 - f0);
     }
 }
 
@@ -351,7 +383,7 @@ static void value_inq(const oracle_grid *g, int mem, int fcol, double x, double 
     interior_value(g, mem, fcol, g->x[0], q2, &f0, &S0);
     interior_value(g, mem, fcol, g->x[1], q2, &f1, &S1);
     double theta = (log(x) - g->u[0]) / (g->u[1] - g->u[0]);
-    continue_two(f0, S0, f1, S1, theta, val, S);
+    continue_two(f0, S0, f1, S1, theta, t_cond(g->u, 0, log(x)), val, S);
 }
 
 /* value for q2 >= Q2_min: in range, or C-8 (two highest knots, in ln Q2) */
@@ -364,7 +396,7 @@ static void value_geqmin(const oracle_grid *g, int mem, int fcol, double x, doub
     value_inq(g, mem, fcol, x, g->q2[last - 1], &g0, &S0);
     value_inq(g, mem, fcol, x, g->q2[last], &g1, &S1);
     double theta = (log(q2) - g->s[last - 1]) / (g->s[last] - g->s[last - 1]);
-    continue_two(g0, S0, g1, S1, theta, val, S);
+    continue_two(g0, S0, g1, S1, theta, t_cond(g->s, last - 1, log(q2)), val, S);
 }
 
 /* full value for a valid query: adds C-9 (eq. 3.4, limits eq. 3.5) */
@@ -481,7 +513,9 @@ int oracle_lumi(const oracle_grid *g, long long n, const double *x1,
         for (int i = 0; i < nf; ++i)
             for (int j = 0; j < nf; ++j) {
                 acc += g->C[i * nf + j] * f1[i] * f2[j];
-                sacc += fabs(g->C[i * nf + j]) * s1[i] * s2[j];
+                /* first-order propagation of the per-flavour tolerance 1e-12 |f| + 1e-14 S */
+                sacc += fabs(g->C[i * nf + j]) * (s1[i] * fabs(f2[j]) + fabs(f1[i]) * s2[j]
+                                                   + 200.0 * fabs(f1[i] * f2[j]));
             }
         out[e] = weights[e] * acc;
         if (scale) scale[e] = fabs(weights[e]) * sacc;

@@ -67,8 +67,11 @@ int oracle_locate(const oracle_grid *g, long long n, const double *x,
                   const double *q2, int *ix, int *iq, int *isub, int *region);
 
 /* C-5 ... C-11.  out is [n][npid] row-major; member may be NULL (member 0);
- * scale, if not NULL, receives [n][npid] condition scales S used by the parity
- * metric C-12 (sum of |weight*value| propagated through the extrapolation). */
+ * scale, if not NULL, receives [n][npid] condition scales used by the parity
+ * metric C-12, tol = 1e-12 |ref| + 1e-14 scale:  scale = sum |Wx_a Wq_b V_ab|
+ * (rounding of the 16-term sum) + KT (|df/dt_x| (1+|ln x|/du) + |df/dt_q|
+ * (1+|ln Q2|/ds)) (rounding of t = (ln v - ln knot)/delta, KT = 4*2^-52/1e-14),
+ * propagated to first order through the extrapolation formulas. */
 int oracle_xfxq2(const oracle_grid *g, const int *pids, int npid, long long n,
                  const double *x, const double *q2, const int *member,
                  double *out, double *scale);
@@ -77,7 +80,9 @@ int oracle_xfxq2(const oracle_grid *g, const int *pids, int npid, long long n,
 int oracle_alphas_q2(const oracle_grid *g, long long n, const double *q2,
                      double *out);
 
-/* C-L.  scale, if not NULL, receives [n] = |w| * sum_ij |C_ij| S_i S_j/(x1 x2). */
+/* C-L.  scale, if not NULL, receives [n] = |w| sum_ij |C_ij| (S1_i |f2_j| + |f1_i| S2_j +
+ * 200 |f1_i f2_j|): the per-flavour tolerance (1e-12 |f| + 1e-14 S) propagated to first order
+ * through the product, in units of 1e-14. */
 int oracle_lumi(const oracle_grid *g, long long n, const double *x1,
                 const double *x2, const double *q2, const double *weights,
                 double *out, double *scale);

@@ -77,11 +77,12 @@ __device__ __forceinline__ int find_last_le(const double *__restrict__ k, int m,
 
 __device__ __forceinline__ void hermite_weights(double t, const CellTab &c, double w[4])
 {
-    double t2 = t * t, t3 = t2 * t;
-    double h00 = 2.0 * t3 - 3.0 * t2 + 1.0;
-    double h10 = t3 - 2.0 * t2 + t;
-    double h01 = -2.0 * t3 + 3.0 * t2;
-    double h11 = t3 - t2;
+    // Hermite basis cubics in factored form: relative accuracy kept where they vanish (t -> 0, 1)
+    double omt = 1.0 - t, omt2 = omt * omt, t2 = t * t;
+    double h00 = fma(2.0, t, 1.0) * omt2;
+    double h10 = t * omt2;
+    double h01 = t2 * fma(-2.0, t, 3.0);
+    double h11 = -(t2 * omt);
     w[0] = -c.bL * h10;
     w[1] = h00 + (c.bL - c.aL) * h10 - c.aR * h11;
     w[2] = h01 + c.aL * h10 + (c.aR - c.bR) * h11;
