@@ -1,0 +1,145 @@
+// pdf_binned_host.cuh -- host side of the binned path: key geometry, work list, launch.
+#pragma once
+#include <cmath>
+#include <vector>
+
+namespace pdfg {
+
+constexpr long long kAutoMinN = 1 << 15;      // PDF_PATH_AUTO: below this the direct path is used
+
+// cell and t_q of 1.01*Q2min with the device log (C-9); res = {jg, t, in_range}
+__global__ void k_q2plus(GridDev G, double *res)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    double q = G.q2plus;
+    if (q > G.qk[G.nqtot - 1]) { res[2] = 0.0; return; }
+    int j, jg;
+    q_locate(G, q, j, jg);
+    res[0] = (double)jg;
+    res[1] = (q == G.qk[jg + 1]) ? 1.0 : (log(q) - G.cq[jg].lo_log) * G.cq[jg].inv_d;
+    res[2] = 1.0;
+}
+
+inline void binned_plan_free(BinnedPlan &p)
+{
+    cudaFree(p.d_items); cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_plus);
+    p.d_items = nullptr; p.d_lutx = p.d_lutq = nullptr; p.d_plus = nullptr; p.usable = false;
+}
+
+inline size_t binned_smem_bytes(int nx, int nqtot)
+{
+    return sizeof(double) * (nx + nqtot) + sizeof(double) * kBinWarps * 32 * kNF + sizeof(unsigned) * kBinWarps * 32 +
+           sizeof(int) * (2 * kKeysPerItem + 2) + sizeof(short) * 2 * kLutSize + 64;
+}
+
+// builds LUTs, the key geometry and the per-chunk B work list; leaves usable = false when the
+// grid does not fit the specialised path (then every call takes the direct path)
+inline int binned_plan_init(BinnedPlan &p, const GridDev &G, const std::vector<double> &xk,
+                            const std::vector<double> &qk, const std::vector<int> &qoff)
+{
+    p.usable = false;
+    const int nx = G.nx, nqt = G.nqtot;
+    if (G.nflav != kNF || G.nfp != kNFP || nx > 30000 || nqt > 30000) return 0;
+    BinDev &d = p.dev;
+    d.ncx = nx - 1; d.nqt = nqt;
+    d.k_lowx = nqt * d.ncx;
+    d.k_highq = d.k_lowx + nqt;
+    d.k_lowq = d.k_highq + d.ncx;
+    d.k_ll = d.k_lowq + d.ncx;
+    d.k_lh = d.k_ll + kCornerSub;
+    d.nkeys = d.k_lh + kCornerSub;
+
+    // search LUTs: bucket b covers ln v in [l0 + b/scale, l0 + (b+1)/scale); entry = a cell at its lower edge
+    auto make_lut = [](const std::vector<double> &k, bool last_le, double &scale, std::vector<short> &lut) {
+        const int m = (int)k.size();
+        double l0 = std::log(k.front()), l1 = std::log(k.back());
+        scale = kLutSize / (l1 - l0) * (1.0 - 1e-12);
+        lut.resize(kLutSize);
+        int c = 0;
+        for (int b = 0; b < kLutSize; ++b) {
+            double edge = std::exp(l0 + b / scale);
+            int lim = last_le ? m - 1 : m - 2;
+            while (c < lim && k[c + 1] <= edge) ++c;
+            lut[b] = (short)c;
+        }
+    };
+    std::vector<short> lx, lq;
+    make_lut(xk, false, d.lutx_scale, lx);
+    make_lut(qk, true, d.lutq_scale, lq);
+
+    std::vector<BinItem> items;
+    auto add_groups = [&](int k0, int k1, int per) {
+        for (int k = k0; k < k1; k += per) items.push_back({k, k + per < k1 ? k + per : k1});
+    };
+    add_groups(d.k_ll, d.k_ll + kCornerSub, 1);            // heaviest math first (longest-first scheduling)
+    add_groups(d.k_lh, d.k_lh + kCornerSub, 1);
+    add_groups(d.k_lowx, d.k_lowx + nqt, 8);
+    add_groups(d.k_lowq, d.k_lowq + d.ncx, kKeysPerItem);
+    add_groups(d.k_highq, d.k_highq + d.ncx, kKeysPerItem);
+    add_groups(0, d.k_lowx, kKeysPerItem);
+    for (int o = 0; o < kOvfItems; ++o) items.push_back({-(o + 1), 0});
+    d.nitems = (int)items.size();
+
+    if (cudaMalloc((void **)&p.d_items, sizeof(BinItem) * items.size()) != cudaSuccess) return PDF_ENOMEM;
+    if (cudaMalloc((void **)&p.d_lutx, sizeof(short) * kLutSize) != cudaSuccess) return PDF_ENOMEM;
+    if (cudaMalloc((void **)&p.d_lutq, sizeof(short) * kLutSize) != cudaSuccess) return PDF_ENOMEM;
+    if (cudaMalloc((void **)&p.d_plus, sizeof(double) * 4) != cudaSuccess) return PDF_ENOMEM;
+    cudaMemcpy(p.d_items, items.data(), sizeof(BinItem) * items.size(), cudaMemcpyHostToDevice);
+    cudaMemcpy(p.d_lutx, lx.data(), sizeof(short) * kLutSize, cudaMemcpyHostToDevice);
+    cudaMemcpy(p.d_lutq, lq.data(), sizeof(short) * kLutSize, cudaMemcpyHostToDevice);
+    k_q2plus<<<1, 32>>>(G, p.d_plus);
+    double res[3] = {0, 0, 0};
+    if (cudaMemcpy(res, p.d_plus, sizeof res, cudaMemcpyDeviceToHost) != cudaSuccess) return PDF_ECUDA;
+    if (res[2] != 1.0) return 0;                           // 1.01*Q2min beyond the grid: direct path only
+    d.jgplus = (int)res[0]; d.tqplus = res[1];
+    d.items = p.d_items; d.lutx = p.d_lutx; d.lutq = p.d_lutq;
+
+    size_t smem = binned_smem_bytes(nx, nqt);
+    if (smem > 100 * 1024) return 0;
+    cudaFuncSetAttribute(k_pdf_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    int per_sm = 0, dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_pdf_stream, kBinThreads, smem) != cudaSuccess || per_sm < 1)
+        return 0;
+    p.max_ctas = per_sm * sms;
+    (void)qoff;
+    p.usable = true;
+    return 0;
+}
+
+inline bool binned_qualifies(const BinnedPlan &p, const ColMap &, const int *member) { return p.usable && !member; }
+inline bool binned_lumi_qualifies(const BinnedPlan &) { return false; }
+
+// one memset + one persistent kernel for the whole call
+template <typename Scope>
+inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm, long long n, const double *x,
+                        const double *q2, double *out, long long ld, void *ws, size_t ws_bytes, long long chunk_opt,
+                        cudaStream_t s)
+{
+    if (binned_workspace_bytes(p, n, chunk_opt) > ws_bytes) return PDF_EWORKSPACE;
+    StreamArgs A;
+    A.G = G; A.B = p.dev; A.cm = cm;
+    A.chunk = binned_chunk(p, n, chunk_opt);
+    A.cap = binned_cap(A.chunk);
+    binned_carve(p, ws, A.chunk, A.cap, A.W);
+    A.x = x; A.q2 = q2; A.out = out; A.n = n; A.ld = ld;
+    A.nchunks = (int)((n + A.chunk - 1) / A.chunk);
+    A.ta = (int)(A.chunk / kTileA);
+    A.identity = cm.n == kNF;
+    for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
+    size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts + ovf_count
+    if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
+    unsigned long long tickets = (unsigned long long)A.nchunks * (A.ta + p.dev.nitems);
+    unsigned grid = (unsigned)(tickets < (unsigned long long)p.max_ctas ? tickets : p.max_ctas);
+    {
+        Scope sc(s, "k_pdf_stream");
+        k_pdf_stream<<<grid, kBinThreads, binned_smem_bytes(G.nx, G.nqtot), s>>>(A);
+    }
+    return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
+}
+
+inline int binned_lumi(const GridDev &, const BinnedPlan &, long long, const double *, const double *, const double *,
+                       const double *, double *, void *, size_t, long long, cudaStream_t) { return PDF_EINVAL; }
+
+}  // namespace pdfg

@@ -101,6 +101,7 @@ void free_grid(pdf_grid *g)
     cudaFree(g->d_xk); cudaFree(g->d_qk); cudaFree(g->d_uk); cudaFree(g->d_sk); cudaFree(g->d_V);
     cudaFree(g->d_sub_of); cudaFree(g->d_qoff); cudaFree(g->d_cx); cudaFree(g->d_cq); cudaFree(g->d_ca);
     cudaFree(g->d_ak); cudaFree(g->d_alk); cudaFree(g->d_av); cudaFree(g->d_C); cudaFree(g->d_err);
+    binned_plan_free(g->bplan);
     for (auto &s : g->stage) {
         cudaFree(s.in); cudaFree(s.out); cudaFree(s.ws);
         if (s.stream) cudaStreamDestroy(s.stream);
@@ -240,7 +241,8 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
     d.V = g->d_V; d.memstride = (size_t)tot * nx * nfp;
     d.q2plus = 1.01 * q2_knots[0];
     d.na = 0; d.alphas_mode = PDF_ALPHAS_FREEZE; d.C = nullptr; d.err_count = g->d_err;
-    binned_plan_init(g->bplan, nx, nsub, g->qoff.data(), nflav, nmem);
+    rc = binned_plan_init(g->bplan, g->d, g->xk, g->qk, g->qoff);
+    if (rc != PDF_OK) { free_grid(g); return rc; }
     *out = g;
     return PDF_OK;
 }

@@ -41,13 +41,14 @@ int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, cons
     if (n == 0) return PDF_OK;
     if (!x || !q2 || !out) return PDF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
-    bool want_binned = g->path == PDF_PATH_BINNED ||
-                       (g->path == PDF_PATH_AUTO && g->ws && binned_qualifies(g->bplan, cm, member, n));
+    bool ok_binned = binned_qualifies(g->bplan, cm, member);
+    bool want_binned = (g->path == PDF_PATH_BINNED) ||
+                       (g->path == PDF_PATH_AUTO && g->ws && ok_binned && n >= kAutoMinN &&
+                        g->ws_bytes >= pdf_workspace_bytes(g, n));
     if (want_binned) {
-        if (!binned_qualifies(g->bplan, cm, member, n)) return PDF_EINVAL;
-        size_t need = pdf_workspace_bytes(g, n);
-        if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
-        return binned_xfxq2(g->d, g->bplan, cm, n, x, q2, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
+        if (!ok_binned) return PDF_EINVAL;
+        if (!g->ws || g->ws_bytes < pdf_workspace_bytes(g, n)) return PDF_EWORKSPACE;
+        return binned_xfxq2<LaunchScope>(g->d, g->bplan, cm, n, x, q2, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
     }
     return launch_direct(g, cm, n, x, q2, member, out, ld_out, s);
 }
@@ -90,14 +91,11 @@ int pdf_lumi(const pdf_grid *g, long long n, const double *x1, const double *x2,
     if (n == 0) return PDF_OK;
     if (!x1 || !x2 || !q2 || !weights || !out) return PDF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
-    bool want_binned = g->path == PDF_PATH_BINNED ||
-                       (g->path == PDF_PATH_AUTO && g->ws && binned_lumi_qualifies(g->bplan, n));
-    if (want_binned) {
-        if (!binned_lumi_qualifies(g->bplan, n)) return PDF_EINVAL;
-        size_t need = pdf_workspace_bytes(g, n);
-        if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
+    bool want_binned = binned_lumi_qualifies(g->bplan) &&
+                       (g->path == PDF_PATH_BINNED || (g->path == PDF_PATH_AUTO && g->ws && n >= kAutoMinN &&
+                                                       g->ws_bytes >= pdf_workspace_bytes(g, n)));
+    if (want_binned)
         return binned_lumi(g->d, g->bplan, n, x1, x2, q2, weights, out, g->ws, g->ws_bytes, g->chunk, s);
-    }
     const long long slice = 1LL << 30;
     for (long long off = 0; off < n; off += slice) {
         long long m = n - off < slice ? n - off : slice;

@@ -13,7 +13,7 @@ from parity import assert_values, value_errors
 
 pytestmark = pytest.mark.gpu
 
-PATHS = ["direct", "auto"]
+PATHS = ["direct", "binned"]
 
 
 @pytest.fixture(scope="module")
@@ -25,8 +25,9 @@ def B():
 
 
 def gpu_grid(B, spec, path="direct", n=0):
-    g = B.PdfGrid.from_spec(spec, workspace_for=n if path != "direct" else 0)
-    g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_DIRECT if path == "direct" else B.PDF_PATH_AUTO)
+    g = B.PdfGrid.from_spec(spec, workspace_for=max(n, 1) if path != "direct" else 0)
+    g.pdf_grid_set_option(B.PDF_OPT_PATH, {"direct": B.PDF_PATH_DIRECT, "binned": B.PDF_PATH_BINNED,
+                                           "auto": B.PDF_PATH_AUTO}[path])
     return g
 
 
@@ -243,7 +244,9 @@ def test_host_calls_match_device_calls(B, oracle_mod):
     out_h = torch.empty((n, 11), dtype=torch.float64).pin_memory()
     g.pdf_xfxq2_host(spec.pids, x.pin_memory(), q.pin_memory(), out_h)
     out_d = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda()).cpu()
-    assert torch.equal(torch.nan_to_num(out_h, nan=-1.0), torch.nan_to_num(out_d, nan=-1.0))
+    # same kernels either way; only the chunking differs (overflow entries may take the generic order)
+    assert torch.equal(torch.isnan(out_h), torch.isnan(out_d))
+    assert torch.allclose(torch.nan_to_num(out_h), torch.nan_to_num(out_d), rtol=1e-13, atol=1e-300)
     a_h = torch.empty(n, dtype=torch.float64)
     g.pdf_alphas_q2_host(q, a_h)
     assert torch.equal(a_h, g.pdf_alphas_q2(q.cuda()).cpu())
@@ -265,3 +268,32 @@ def test_missing_state_and_workspace_errors(B):
     if g.pdf_workspace_bytes(4) > 0:
         with pytest.raises(B.PdfGridError):
             g.pdf_xfxq2(spec.pids, q * 0.1, q * 10)
+
+
+def test_binned_ring_reuse_and_overflow(B, oracle_mod):
+    """the persistent kernel's chunk ring (many small chunks) and the overflow list (queries piled
+    into a handful of cells so that bins exceed their capacity)"""
+    spec = synth.grid_c1()
+    og = make_oracle_grid(oracle_mod, spec)
+    g = B.PdfGrid.from_spec(spec)
+    g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_BINNED)
+    g.pdf_grid_set_option(B.PDF_OPT_CHUNK, 4096)
+    n = 150_001                                   # 37 chunks through a ring of 3
+    g.attach_workspace(n)
+    x, q = synth.queries_c2(spec, n, seed=31)
+    ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), want_scale=True)
+    for _ in range(2):                            # second call: control block re-initialised
+        out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda()).cpu().numpy()
+        assert_values(out, ref, S, "ring")
+    # skew: everything inside 3 x-cells and 2 Q2-cells, plus one corner class
+    g.pdf_grid_set_option(B.PDF_OPT_CHUNK, 1 << 16)
+    n = 200_000
+    g.attach_workspace(n)
+    gen = torch.Generator().manual_seed(5)
+    xs = torch.exp(torch.rand(n, generator=gen, dtype=torch.float64) * 0.3 + math.log(1e-3))
+    qs = torch.exp(torch.rand(n, generator=gen, dtype=torch.float64) * 0.9 + math.log(100.0))
+    xs[:20_000] = 1e-11
+    qs[:20_000] = 0.3
+    ref, S = og.xfxq2(spec.pids, xs.numpy(), qs.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, xs.cuda(), qs.cuda()).cpu().numpy()
+    assert_values(out, ref, S, "skew")
