@@ -118,7 +118,7 @@ def test_scan_lines_and_knots(B, oracle_mod, path):
     Xk, Qk = knot_neighbour_queries(spec)
     x = np.concatenate([X.numpy(), Xk])
     q = np.concatenate([Q.numpy(), Qk])
-    g = gpu_grid(B, spec, path, len(x))
+    g = gpu_grid(B, spec, path, max(len(x), 196 * 54))
     ref, S = og.xfxq2(spec.pids, x, q, want_scale=True)
     out = g.pdf_xfxq2(spec.pids, torch.tensor(x).cuda(), torch.tensor(q).cuda()).cpu().numpy()
     assert_values(out, ref, S, "scan")
