@@ -1,27 +1,35 @@
-// pdf_binned.cuh -- the binned, warp-coherent evaluation path (PDF_PATH_BINNED).
+// pdf_binned.cuh -- the binned, warp-coherent evaluation path (PDF_PATH_BINNED), version 2.
 //
-// Why: a query needs a 4x4 stencil x 11 flavours = 1408 B of grid data.  With unsorted queries
-// every lane gathers its own stencil and the L1/L2 request rate, not HBM or the FP64 pipe, bounds
-// the kernel (the direct path sits at ~1 % of the HBM roofline).  Here queries are first binned
-// by cell, so that the 32 lanes of a warp share ONE stencil: each 16-byte load of grid data is a
-// single broadcast wavefront that serves 32 queries.
+// Why: a query needs a 4x4 stencil x 11 flavours = 1408 B of grid data.  Gathered per lane that
+// is >= 12 clk/query/SM of L1 / shared-memory bandwidth, 2.5x the HBM and FP64 budgets, so the
+// lanes of a warp must share a cell and take the stencil as BROADCAST operands from shared memory
+// (LDS.128 with one address: 1.5 clk).  With ~10^4 cells that needs a sort domain of >= 10^5
+// queries, which no CTA holds on chip: queries are binned through L2 in chunks.
 //
-// How (B200-first): ONE persistent kernel per call, one CTA slot per SM x occupancy, pulling
-// work items from a global ticket counter.  The n queries are cut in chunks small enough that a
-// chunk's bins (32 B/query) and its scattered output rows stay in the 126 MB L2, so HBM sees
-// ~16 B/query in and 88 B/query out and nothing else.  Two item kinds alternate in ticket order
-//      A(c):  read x,q2 of a tile of chunk c (coalesced), classify, locate the cell, compute
-//             t_x,t_q (the two logs), claim a slot in the cell's bin (L2 atomic), write payload
-//      B(c):  for a group of 32 cells: warps take batches of 32 payloads of one cell, build the
-//             Hermite weights, run the 16-node x 11-flavour FMA sum with broadcast loads,
-//             transpose through shared memory and write whole 88-byte rows
-// in the order A(0) A(1) B(0) A(2) B(1) ...  B(c) waits (acquire-spin on a counter) until every
-// tile of A(c) has been released; by ticket order those tiles were claimed a whole stage earlier,
-// so the wait is normally zero and can never deadlock (all CTAs are co-resident; a ticket only
-// ever waits on lower tickets).  Bins live in a ring of R chunk slots.
-// Extrapolation classes (SURVEY a-5) get their own keys, so a warp is class-uniform.
-// Queries that do not fit their bin (capacity CAP per chunk) go to an overflow list that the
-// generic per-thread code evaluates; correctness never depends on the distribution.
+// What the machine dictates (measured on this B200):
+//   * one global atomic + one scattered store per query costs a whole roofline budget
+//       -> A items sort their tile by COARSE key (the x-cell) in shared memory, reserve one run
+//          per (tile, key) with a single global atomic, and store each 32-byte payload as one
+//          whole sector (STG.256);
+//   * unaligned 88-byte rows scattered into untouched memory reach 0.9 TB/s (partial sectors)
+//       -> A items first ZERO-FILL the output rows of their tile with coalesced stores; the later
+//          scattered row stores of B then merge into valid L2-resident sectors (2.7 ms -> in
+//          budget), and every line still leaves L2 for HBM once.
+//
+// How: ONE persistent kernel per call, CTAs pull tickets in the order
+//      A(0) | A(1) B(0) | A(2) B(1) | ... | B(last)
+//   A(c), one item per 2048 queries of chunk c: read x,q2 (coalesced), classify, locate the cell,
+//      t_x,t_q (the two logs), coarse/fine key, tile-local counting sort by coarse key, payload
+//      stores; zero-fill of the tile's output rows.
+//   B(c), one item per coarse key: copy the key's payloads and its 4 grid columns (4 x nq x 96 B)
+//      to shared memory, counting-sort by FINE key (the Q2 cell or the extrapolation class), then
+//      warps take batches of <= 32 same-cell queries: Hermite weights, 16-node x 11-flavour FMA
+//      sum with broadcast LDS.128, rows transposed through shared memory and stored.
+// B(c) waits (acquire-spin) until every tile of A(c) has been released; by ticket order those
+// tiles were claimed a whole stage earlier, so the wait is normally zero and cannot deadlock (all
+// CTAs are co-resident; a ticket only waits on lower tickets).  Bins live in a ring of kRing chunk
+// slots.  Queries that do not fit their bin (capacity per chunk and key) go to an overflow list
+// that the generic per-thread code evaluates: correctness never depends on the distribution.
 #pragma once
 #include "pdf_common.cuh"
 #include "pdf_generic.cuh"
@@ -32,30 +40,28 @@ constexpr int kBinThreads = 256;              // CTA size of the persistent kern
 constexpr int kBinWarps = kBinThreads / 32;
 constexpr int kTileQ = 8;                     // queries per thread in an A item
 constexpr int kTileA = kBinThreads * kTileQ;  // 2048 queries per A item
-constexpr int kKeysPerItem = 32;              // keys per B item (one per lane in the prologue scan)
-constexpr int kOvfItems = 8;                  // B items per chunk that drain the overflow list
+constexpr int kOvfItems = 4;                  // B items per chunk that drain the overflow list
 constexpr int kRing = 3;                      // chunk slots in flight
-constexpr int kCornerSub = 4;                 // sub-keys of each corner class (spreads heavy math)
+constexpr int kLowXSplit = 16;                // coarse keys of the low-x classes (spreads their 2.5 %)
 constexpr int kLutSize = 1024;                // search-acceleration buckets per axis
 constexpr int kNF = 11, kNFP = 12;            // the fast path is specialised for 11 flavours (pad 12)
+constexpr int kMaxCK = 1024;                  // coarse keys (x cells + kLowXSplit) the path supports
+constexpr int kMaxFK = 96;                    // fine keys (Q2 knots + 2)
+constexpr int kMaxCap = 2048;                 // payloads of one (chunk, coarse key) held in shared memory
 
 struct __align__(32) Payload {                // one sector
     double a, b;                              // class-dependent abscissae (t_x,t_q / theta / r)
     unsigned idx;                             // query index inside its chunk
-    unsigned pad0;
-    double pad1;
+    unsigned fk;                              // fine key
+    double pad;
 };
 
-struct BinItem { int key_begin, key_end; };  // key_begin < 0: overflow item number -key_begin-1
-
-// geometry of the key space and the work list; host copy in BinnedPlan, device copy in BinDev
+// geometry of the key space; host copy in BinnedPlan, device copy passed by value
 struct BinDev {
-    int ncx, nqt, nkeys;
-    int k_lowx, k_highq, k_lowq, k_ll, k_lh;  // first key of each class (interior starts at 0)
+    int ncx, nqt, nck, nfk;                   // x cells, Q2 knots, coarse keys, fine keys
     int jgplus;                               // cell (global lower-knot index) of 1.01*Q2min
     double tqplus;                            // and its t_q  (C-9)
     int nitems;                               // B items per chunk, overflow items included
-    const BinItem *items;                     // [nitems]
     const short *lutx, *lutq;                 // [kLutSize] start guesses of the knot search
     double lutx_scale, lutq_scale;            // buckets per unit of ln x / ln Q2
 };
@@ -63,19 +69,18 @@ struct BinDev {
 struct BinnedPlan {
     bool usable = false;
     BinDev dev{};
-    BinItem *d_items = nullptr;
     short *d_lutx = nullptr, *d_lutq = nullptr;
     double *d_plus = nullptr;                 // scratch of k_q2plus
     int max_ctas = 0;                         // co-resident CTAs of the persistent kernel
-    long long default_chunk = 1 << 19;
+    long long default_chunk = 1 << 18;
 };
 
 struct BinWorkspace {                         // carved out of the caller's workspace
-    unsigned long long *ctrl;                 // [0] ticket, [1] error count; then per ring slot: a_done, b_done
-    unsigned *counts;                         // [kRing][nkeys]
+    unsigned long long *ctrl;                 // [0] ticket; then per ring slot: a_done, b_fin, b_done
+    unsigned *counts;                         // [kRing][nck]
     unsigned *ovf_count;                      // [kRing]
-    Payload *bins;                            // [kRing][nkeys][cap]
-    Payload *ovf;                             // [kRing][chunk]
+    Payload *bins;                            // [kRing][nck][cap]
+    Payload *ovf;                             // [kRing][chunk]  (raw x, q2)
 };
 
 inline long long binned_chunk(const BinnedPlan &p, long long n, long long chunk_opt)
@@ -87,13 +92,14 @@ inline long long binned_chunk(const BinnedPlan &p, long long n, long long chunk_
     return c < need ? c : need;
 }
 
-inline int binned_cap(long long chunk)
+// bin capacity per (chunk, coarse key): a uniform cloud puts chunk/ncx queries on an x cell
+// (1344 at 256k and 195 cells); 1.125x that + 96 (~ +7 sigma) keeps overflow to skewed inputs
+inline int binned_cap(const BinnedPlan &p, long long chunk)
 {
-    // bin capacity per chunk: a uniform cloud puts ~chunk/9000 queries in a cell of the LHAPDF-shaped
-    // grid (58 at 512k); 4x that (min 32, max 256) keeps overflow to genuinely skewed inputs
-    long long c = chunk / 2048;
-    if (c < 32) c = 32;
-    if (c > 256) c = 256;
+    long long c = chunk / (p.dev.ncx > 0 ? p.dev.ncx : 1);
+    c = c + c / 8 + 96;
+    c = (c + 31) / 32 * 32;
+    if (c > kMaxCap) c = kMaxCap;
     return (int)c;
 }
 
@@ -103,11 +109,11 @@ inline size_t binned_workspace_bytes(const BinnedPlan &p, long long n, long long
 {
     if (!p.usable) return 0;
     long long chunk = binned_chunk(p, n, chunk_opt);
-    int cap = binned_cap(chunk);
+    int cap = binned_cap(p, chunk);
     size_t b = 4096;                                                    // ctrl
-    b += align_up(sizeof(unsigned) * (size_t)kRing * p.dev.nkeys, 256);
+    b += align_up(sizeof(unsigned) * (size_t)kRing * p.dev.nck, 256);
     b += 256;                                                           // ovf_count
-    b += align_up(sizeof(Payload) * (size_t)kRing * p.dev.nkeys * cap, 256);
+    b += align_up(sizeof(Payload) * (size_t)kRing * p.dev.nck * cap, 256);
     b += align_up(sizeof(Payload) * (size_t)kRing * chunk, 256);
     return b + 256;
 }
@@ -116,9 +122,9 @@ inline void binned_carve(const BinnedPlan &p, void *ws, long long chunk, int cap
 {
     char *c = (char *)align_up((size_t)ws, 256);
     w.ctrl = (unsigned long long *)c; c += 4096;
-    w.counts = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)kRing * p.dev.nkeys, 256);
+    w.counts = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)kRing * p.dev.nck, 256);
     w.ovf_count = (unsigned *)c; c += 256;
-    w.bins = (Payload *)c; c += align_up(sizeof(Payload) * (size_t)kRing * p.dev.nkeys * cap, 256);
+    w.bins = (Payload *)c; c += align_up(sizeof(Payload) * (size_t)kRing * p.dev.nck * cap, 256);
     w.ovf = (Payload *)c;
     (void)chunk;
 }

@@ -1,14 +1,25 @@
-// pdf_binned_eval.cuh -- B items (warp-coherent evaluation) and the persistent kernel itself.
+// pdf_binned_eval.cuh -- B items (warp-coherent evaluation from shared memory) and the
+// persistent kernel itself.
 #pragma once
 
 namespace pdfg {
 
-// acc[f] += w * V[node][f] for the 11 flavours of one node row (12 doubles, 16-byte aligned).
-// Every lane passes the SAME address: each 16-byte load is one broadcast wavefront for 32 queries.
-__device__ __forceinline__ void node_fma(const double *__restrict__ p, double w, double acc[kNF])
+// The 4 grid columns of a coarse key, staged in shared memory as sV[jg][slot a][12 doubles]:
+// the 4 x-nodes of a Q2 row are 384 contiguous bytes.  Every lane of a warp passes the SAME
+// address: each LDS.128 is one broadcast (1.5 clk) that serves 32 queries.
+// sV is addressed in the shared window (32-bit address) with explicit ld.shared: the compiler
+// cannot prove the address space of a pointer that travels through a struct
+__device__ __forceinline__ double2 lds_d2(unsigned addr)
 {
-    double2 v0 = ldg_nc_d2(p), v1 = ldg_nc_d2(p + 2), v2 = ldg_nc_d2(p + 4);
-    double2 v3 = ldg_nc_d2(p + 6), v4 = ldg_nc_d2(p + 8), v5 = ldg_nc_d2(p + 10);
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+
+__device__ __forceinline__ void node_fma_s(unsigned p, double w, double acc[kNF])
+{
+    double2 v0 = lds_d2(p), v1 = lds_d2(p + 16), v2 = lds_d2(p + 32), v3 = lds_d2(p + 48), v4 = lds_d2(p + 64),
+            v5 = lds_d2(p + 80);
     acc[0] = fma(w, v0.x, acc[0]); acc[1] = fma(w, v0.y, acc[1]);
     acc[2] = fma(w, v1.x, acc[2]); acc[3] = fma(w, v1.y, acc[3]);
     acc[4] = fma(w, v2.x, acc[4]); acc[5] = fma(w, v2.y, acc[5]);
@@ -17,108 +28,109 @@ __device__ __forceinline__ void node_fma(const double *__restrict__ p, double w,
     acc[10] = fma(w, v5.x, acc[10]);
 }
 
-__device__ __forceinline__ const double *node_ptr(const GridDev &G, int jrow, int icol)
+__device__ __forceinline__ unsigned snode(unsigned sV, int jrow, int slot)
 {
-    return G.V + ((size_t)jrow * G.nx + icol) * kNFP;
+    return sV + (unsigned)((jrow * 4 + slot) * kNFP * 8);
 }
 
 struct AxisNodes { int n[4]; };
-__device__ __forceinline__ AxisNodes x_nodes(const GridDev &G, int i)
-{
-    AxisNodes a; a.n[0] = i > 0 ? i - 1 : i; a.n[1] = i; a.n[2] = i + 1; a.n[3] = i + 2 < G.nx ? i + 2 : i + 1;
-    return a;
-}
 __device__ __forceinline__ AxisNodes q_nodes(const CellTab &c, int jg)
 {
     AxisNodes a; a.n[0] = (c.aL == 1.0) ? jg : jg - 1; a.n[1] = jg; a.n[2] = jg + 1; a.n[3] = (c.aR == 1.0) ? jg + 1 : jg + 2;
     return a;
 }
 
-// C-6: 16-node tensor sum in cell (i, jg)
-__device__ __forceinline__ void eval_interior(const GridDev &G, int i, int jg, double tx, double tq, double acc[kNF])
+__device__ __forceinline__ void zero_acc(double acc[kNF])
+{
+#pragma unroll
+    for (int f = 0; f < kNF; ++f) acc[f] = 0.0;
+}
+
+// C-6: 16-node tensor sum in cell (i, jg); the x-nodes i-1..i+2 (clamped) sit in slots 0..3
+__device__ __forceinline__ void eval_interior_s(const GridDev &G, unsigned sV, int i, int jg, double tx, double tq,
+                                                double acc[kNF])
 {
     CellTab cq = G.cq[jg];
     double wx[4], wq[4];
     hermite_weights(tx, G.cx[i], wx);
     hermite_weights(tq, cq, wq);
-    AxisNodes xn = x_nodes(G, i), qn = q_nodes(cq, jg);
-#pragma unroll
-    for (int f = 0; f < kNF; ++f) acc[f] = 0.0;
+    AxisNodes qn = q_nodes(cq, jg);
+    zero_acc(acc);
 #pragma unroll
     for (int b = 0; b < 4; ++b)
 #pragma unroll
-        for (int a = 0; a < 4; ++a) node_fma(node_ptr(G, qn.n[b], xn.n[a]), wq[b] * wx[a], acc);
+        for (int a = 0; a < 4; ++a) node_fma_s(snode(sV, qn.n[b], a), wq[b] * wx[a], acc);
 }
 
-// sum_b wq[b] V[col][rows of cell jg]  (x fixed on a knot column)
-__device__ __forceinline__ void eval_column(const GridDev &G, int col, int jg, double tq, double acc[kNF])
+// sum_b wq[b] V[slot][rows of cell jg]  (x fixed on a knot column)
+__device__ __forceinline__ void eval_column_s(const GridDev &G, unsigned sV, int slot, int jg, double tq, double acc[kNF])
 {
     CellTab cq = G.cq[jg];
     double wq[4];
     hermite_weights(tq, cq, wq);
     AxisNodes qn = q_nodes(cq, jg);
+    zero_acc(acc);
 #pragma unroll
-    for (int f = 0; f < kNF; ++f) acc[f] = 0.0;
-#pragma unroll
-    for (int b = 0; b < 4; ++b) node_fma(node_ptr(G, qn.n[b], col), wq[b], acc);
+    for (int b = 0; b < 4; ++b) node_fma_s(snode(sV, qn.n[b], slot), wq[b], acc);
 }
 
-// sum_a wx[a] V[cols of cell i][row]  (Q2 fixed on a knot row)
-__device__ __forceinline__ void eval_row(const GridDev &G, int i, int jrow, double tx, double acc[kNF])
+// sum_a wx[a] V[slots of cell i][row]  (Q2 fixed on a knot row)
+__device__ __forceinline__ void eval_row_s(const GridDev &G, unsigned sV, int i, int jrow, double tx, double acc[kNF])
 {
     double wx[4];
     hermite_weights(tx, G.cx[i], wx);
-    AxisNodes xn = x_nodes(G, i);
+    zero_acc(acc);
 #pragma unroll
-    for (int f = 0; f < kNF; ++f) acc[f] = 0.0;
-#pragma unroll
-    for (int a = 0; a < 4; ++a) node_fma(node_ptr(G, jrow, xn.n[a]), wx[a], acc);
+    for (int a = 0; a < 4; ++a) node_fma_s(snode(sV, jrow, a), wx[a], acc);
 }
 
-__device__ __forceinline__ void load_node(const GridDev &G, int jrow, int icol, double acc[kNF])
+__device__ __forceinline__ void load_node_s(unsigned sV, int jrow, int slot, double acc[kNF])
 {
-#pragma unroll
-    for (int f = 0; f < kNF; ++f) acc[f] = 0.0;
-    node_fma(node_ptr(G, jrow, icol), 1.0, acc);
+    zero_acc(acc);
+    node_fma_s(snode(sV, jrow, slot), 1.0, acc);
 }
 
-// class dispatch: key -> values of the 11 flavours for payload (a, b).  Warp-uniform branches.
-__device__ __noinline__ void eval_extrap(const GridDev &G, const BinDev &B, int key, double pa, double pb, double acc[kNF])
+// extrapolation classes (a-5).  Warp-uniform branches: a batch holds one (coarse, fine) key.
+// In an in-range-x unit the slots hold the x-nodes of cell i; in a low-x unit slot 0 / 1 hold
+// the knot columns X_0 / X_1 (C-7).
+__device__ __noinline__ void eval_extrap_s(const GridDev &G, const BinDev &B, unsigned sV, bool lowx_unit, int i,
+                                           int fk, double pa, double pb, double acc[kNF])
 {
     double e0[kNF], e1[kNF];
-    int last = G.nqtot - 1;
-    if (key >= B.k_lh) {                                   // low-x & high-Q (L1744): x rule, then Q rule
-        double e2[kNF], e3[kNF];
-        load_node(G, last - 1, 0, e0); load_node(G, last - 1, 1, e1);
-        load_node(G, last, 0, e2); load_node(G, last, 1, e3);
+    const int last = G.nqtot - 1;
+    if (!lowx_unit) {
+        if (fk == B.nqt) {                                 // low-Q (C-9): pa = t_x, pb = r
+            eval_row_s(G, sV, i, 0, pa, e0);
+            eval_interior_s(G, sV, i, B.jgplus, pa, B.tqplus, e1);
 #pragma unroll
-        for (int f = 0; f < kNF; ++f)
-            acc[f] = continue_two(continue_two(e0[f], e1[f], pa), continue_two(e2[f], e3[f], pa), pb);
-    } else if (key >= B.k_ll) {                            // low-x & low-Q
+            for (int f = 0; f < kNF; ++f) acc[f] = lowq_continue(e0[f], e1[f], pb);
+        } else {                                           // high-Q (C-8): pa = t_x, pb = theta_q
+            eval_row_s(G, sV, i, last - 1, pa, e0);
+            eval_row_s(G, sV, i, last, pa, e1);
+#pragma unroll
+            for (int f = 0; f < kNF; ++f) acc[f] = continue_two(e0[f], e1[f], pb);
+        }
+        return;
+    }
+    if (fk < B.nqt) {                                      // low-x (C-7): pa = theta_x, pb = t_q
+        eval_column_s(G, sV, 0, fk, pb, e0);
+        eval_column_s(G, sV, 1, fk, pb, e1);
+#pragma unroll
+        for (int f = 0; f < kNF; ++f) acc[f] = continue_two(e0[f], e1[f], pa);
+    } else if (fk == B.nqt) {                              // low-x & low-Q (L1744): x rule, then Q rule
         double e2[kNF], e3[kNF];
-        load_node(G, 0, 0, e0); load_node(G, 0, 1, e1);
-        eval_column(G, 0, B.jgplus, B.tqplus, e2); eval_column(G, 1, B.jgplus, B.tqplus, e3);
+        load_node_s(sV, 0, 0, e0); load_node_s(sV, 0, 1, e1);
+        eval_column_s(G, sV, 0, B.jgplus, B.tqplus, e2); eval_column_s(G, sV, 1, B.jgplus, B.tqplus, e3);
 #pragma unroll
         for (int f = 0; f < kNF; ++f)
             acc[f] = lowq_continue(continue_two(e0[f], e1[f], pa), continue_two(e2[f], e3[f], pa), pb);
-    } else if (key >= B.k_lowq) {                          // low-Q (C-9): pa = t_x, pb = r
-        int i = key - B.k_lowq;
-        eval_row(G, i, 0, pa, e0);
-        eval_interior(G, i, B.jgplus, pa, B.tqplus, e1);
+    } else {                                               // low-x & high-Q
+        double e2[kNF], e3[kNF];
+        load_node_s(sV, last - 1, 0, e0); load_node_s(sV, last - 1, 1, e1);
+        load_node_s(sV, last, 0, e2); load_node_s(sV, last, 1, e3);
 #pragma unroll
-        for (int f = 0; f < kNF; ++f) acc[f] = lowq_continue(e0[f], e1[f], pb);
-    } else if (key >= B.k_highq) {                         // high-Q (C-8): pa = t_x, pb = theta_q
-        int i = key - B.k_highq;
-        eval_row(G, i, last - 1, pa, e0);
-        eval_row(G, i, last, pa, e1);
-#pragma unroll
-        for (int f = 0; f < kNF; ++f) acc[f] = continue_two(e0[f], e1[f], pb);
-    } else {                                               // low-x (C-7): pa = theta_x, pb = t_q
-        int jg = key - B.k_lowx;
-        eval_column(G, 0, jg, pb, e0);
-        eval_column(G, 1, jg, pb, e1);
-#pragma unroll
-        for (int f = 0; f < kNF; ++f) acc[f] = continue_two(e0[f], e1[f], pa);
+        for (int f = 0; f < kNF; ++f)
+            acc[f] = continue_two(continue_two(e0[f], e1[f], pa), continue_two(e2[f], e3[f], pa), pb);
     }
 }
 
@@ -141,57 +153,106 @@ __device__ __noinline__ void ovf_item(const StreamArgs &A, int slot, long long c
 }
 
 struct BSmem {
+    uint4 *sP;            // [cap] payloads (2 x uint4 each)
+    double *sV;           // [nqt][4][12]
     double *stage;        // [kBinWarps][32*kNF]
     unsigned *sidx;       // [kBinWarps][32]
-    int *bstart;          // [kKeysPerItem+1]
-    int *cnt;             // [kKeysPerItem]
+    int *fcnt;            // [nfk]
+    int *foff;            // [nfk+1]
+    int *bstart;          // [nfk+1]
+    unsigned short *order;// [cap]
 };
 
+// ---- B item: one coarse key of one chunk ------------------------------------------------------
 __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int slot, long long chunk_base, int item)
 {
     const BinDev &B = A.B;
-    BinItem it = B.items[item];
-    if (it.key_begin < 0) { ovf_item(A, slot, chunk_base, -it.key_begin - 1); return; }
-    unsigned *counts = A.W.counts + (size_t)slot * B.nkeys;
-    const Payload *bins = A.W.bins + (size_t)slot * B.nkeys * A.cap;
-    const int nk = it.key_end - it.key_begin;
+    const GridDev &G = A.G;
+    if (item >= B.nck) { ovf_item(A, slot, chunk_base, item - B.nck); return; }
+    const int ck = item;
+    unsigned *counts = A.W.counts + (size_t)slot * B.nck;
+    unsigned cnt_u = __ldcg(counts + ck);
+    if (cnt_u == 0u) return;                               // uniform over the CTA
+    const int cnt = cnt_u > (unsigned)A.cap ? A.cap : (int)cnt_u;
+    const uint4 *bin = reinterpret_cast<const uint4 *>(A.W.bins + ((size_t)slot * B.nck + ck) * A.cap);
+    const bool lowx_unit = ck >= B.ncx;
+    const int i = lowx_unit ? 0 : ck;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (warp == 0) {                                       // batches per key, prefix-summed
-        unsigned c = lane < nk ? __ldcg(counts + it.key_begin + lane) : 0u;
-        if (c > (unsigned)A.cap) c = A.cap;
-        int nb = (int)((c + 31) >> 5), incl = nb;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += v; }
-        if (lane < nk) { S.cnt[lane] = (int)c; S.bstart[lane + 1] = incl; }
-        if (lane == 0) S.bstart[0] = 0;
+
+    // stage payloads (coalesced) and the key's 4 grid columns
+    for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) S.sP[e] = __ldcg(bin + e);
+    {
+        int c0, c1, c2, c3;
+        if (lowx_unit) { c0 = 0; c1 = 1; c2 = 0; c3 = 1; }
+        else { c0 = i > 0 ? i - 1 : i; c1 = i; c2 = i + 1; c3 = i + 2 < G.nx ? i + 2 : i + 1; }
+        const double2 *V2 = reinterpret_cast<const double2 *>(G.V);
+        double2 *sV2 = reinterpret_cast<double2 *>(S.sV);
+        const int tot = G.nqtot * 24;                      // double2 units: rows x 4 slots x 6
+        for (int e = threadIdx.x; e < tot; e += kBinThreads) {
+            int jg = e / 24, r = e - jg * 24, a = r / 6, p = r - a * 6;
+            int col = a == 0 ? c0 : a == 1 ? c1 : a == 2 ? c2 : c3;
+            sV2[e] = __ldg(V2 + ((size_t)jg * G.nx + col) * 6 + p);
+        }
+    }
+    for (int k = threadIdx.x; k < B.nfk; k += kBinThreads) S.fcnt[k] = 0;
+    __syncthreads();
+    // counting sort by fine key: rank kept in the payload's spare word
+    for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
+        uint4 w1 = S.sP[2 * e + 1];                        // {idx, fk, pad, pad}
+        int r = atomicAdd(S.fcnt + w1.y, 1);
+        w1.z = (unsigned)r;
+        S.sP[2 * e + 1] = w1;
     }
     __syncthreads();
-    const int total = S.bstart[nk];
+    if (warp == 0) {                                       // exclusive scans: slots and 32-query batches per key
+        int carry_o = 0, carry_b = 0;
+        for (int k0 = 0; k0 < B.nfk; k0 += 32) {
+            int k = k0 + lane;
+            int c = k < B.nfk ? S.fcnt[k] : 0;
+            int nb = (c + 31) >> 5;
+            int so = c, sb = nb;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                int vo = __shfl_up_sync(0xffffffffu, so, d), vb = __shfl_up_sync(0xffffffffu, sb, d);
+                if (lane >= d) { so += vo; sb += vb; }
+            }
+            if (k < B.nfk) { S.foff[k] = carry_o + so - c; S.bstart[k] = carry_b + sb - nb; }
+            carry_o += __shfl_sync(0xffffffffu, so, 31);
+            carry_b += __shfl_sync(0xffffffffu, sb, 31);
+        }
+        if (lane == 0) { S.foff[B.nfk] = carry_o; S.bstart[B.nfk] = carry_b; }
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
+        uint4 w1 = S.sP[2 * e + 1];
+        S.order[S.foff[w1.y] + (int)w1.z] = (unsigned short)e;
+    }
+    __syncthreads();
+
+    const int total = S.bstart[B.nfk];
+    const unsigned sVa = (unsigned)__cvta_generic_to_shared(S.sV);
     double *stage = S.stage + warp * (32 * kNF);
     unsigned *sidx = S.sidx + warp * 32;
     int k = 0;
     for (int fb = warp; fb < total; fb += kBinWarps) {
-        while (S.bstart[k + 1] <= fb) ++k;
-        const int key = it.key_begin + k, cnt = S.cnt[k];
-        const int lslot = (fb - S.bstart[k]) * 32 + lane;
-        const bool active = lslot < cnt;
-        const int nact = min(32, cnt - (fb - S.bstart[k]) * 32);
+        while (S.bstart[k + 1] <= fb) ++k;                 // fine key of this batch (monotone in fb)
+        const int fk = k, kcnt = S.fcnt[k];
+        const int first = (fb - S.bstart[k]) * 32;
+        const int nact = min(32, kcnt - first);
+        const bool active = lane < nact;
         double pa = 0.0, pb = 0.0;
         unsigned idx = 0;
         if (active) {
-            const Payload *src = bins + (size_t)key * A.cap + lslot;
-            double2 ab = __ldcg(reinterpret_cast<const double2 *>(src));
-            uint2 ii = __ldcg(reinterpret_cast<const uint2 *>(src) + 2);
-            pa = ab.x; pb = ab.y; idx = ii.x;
+            int e = S.order[S.foff[k] + first + lane];
+            uint4 w0 = S.sP[2 * e], w1 = S.sP[2 * e + 1];
+            pa = __hiloint2double((int)w0.y, (int)w0.x);
+            pb = __hiloint2double((int)w0.w, (int)w0.z);
+            idx = w1.x;
         }
         double acc[kNF];
-        if (key < B.k_lowx) {
-            int jg = key / B.ncx, i = key - jg * B.ncx;
-            eval_interior(A.G, i, jg, pa, pb, acc);
-        } else {
-            eval_extrap(A.G, B, key, pa, pb, acc);
-        }
-        // transpose through shared memory so that whole 88-byte rows leave in coalesced stores
+        if (!lowx_unit && fk < B.nqt) eval_interior_s(G, sVa, i, fk, pa, pb, acc);
+        else eval_extrap_s(G, B, sVa, lowx_unit, i, fk, pa, pb, acc);
+        // transpose through shared memory so that whole rows leave in contiguous pieces
 #pragma unroll
         for (int f = 0; f < kNF; ++f) stage[lane * kNF + f] = acc[f];
         sidx[lane] = idx;
@@ -216,21 +277,33 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
         __syncwarp();
     }
     __syncthreads();
-    if (threadIdx.x < nk) counts[it.key_begin + threadIdx.x] = 0u;   // bins are empty again for the ring
+    if (threadIdx.x == 0) counts[ck] = 0u;                 // the bin is empty again for the ring
 }
 
 // ---- the persistent kernel -----------------------------------------------------------------------
+// dynamic shared memory: [knots | LUTs | item region]; the item region is used by A items as
+// (cnt, base) and by B items as (payloads, columns, stage, sort tables)
+__host__ __device__ inline size_t bsmem_item_bytes(int nqt, int nck, int nfk, int cap)
+{
+    size_t b = (size_t)cap * 32;                                        // sP
+    b += (size_t)nqt * 4 * kNFP * sizeof(double);                       // sV
+    b += (size_t)kBinWarps * 32 * kNF * sizeof(double);                 // stage
+    b += (size_t)kBinWarps * 32 * sizeof(unsigned);                     // sidx
+    b += (size_t)(3 * nfk + 4) * sizeof(int);                           // fcnt, foff, bstart
+    b += ((size_t)cap * sizeof(unsigned short) + 15) / 16 * 16;         // order
+    size_t a = (size_t)2 * nck * sizeof(unsigned);                      // A items: cnt, base
+    return (b > a ? b : a) + 32;
+}
+
 __global__ void __launch_bounds__(kBinThreads, 2) k_pdf_stream(const __grid_constant__ StreamArgs A)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(32) unsigned char smem_raw[];
     double *s_xk = reinterpret_cast<double *>(smem_raw);
     double *s_qk = s_xk + A.G.nx;
-    double *s_stage = s_qk + A.G.nqtot;
-    unsigned *s_idx = reinterpret_cast<unsigned *>(s_stage + kBinWarps * 32 * kNF);
-    int *s_bstart = reinterpret_cast<int *>(s_idx + kBinWarps * 32);
-    int *s_cnt = s_bstart + kKeysPerItem + 1;
-    short *s_lutx = reinterpret_cast<short *>(s_cnt + kKeysPerItem + 1);
+    short *s_lutx = reinterpret_cast<short *>(s_qk + A.G.nqtot);
     short *s_lutq = s_lutx + kLutSize;
+    unsigned char *region = reinterpret_cast<unsigned char *>(s_lutq + kLutSize);
+    region = reinterpret_cast<unsigned char *>((reinterpret_cast<size_t>(region) + 31) & ~(size_t)31);
     __shared__ unsigned long long s_ticket;
 
     for (int i = threadIdx.x; i < A.G.nx; i += kBinThreads) s_xk[i] = A.G.xk[i];
@@ -238,7 +311,18 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_pdf_stream(const __grid_cons
     for (int i = threadIdx.x; i < kLutSize; i += kBinThreads) { s_lutx[i] = A.B.lutx[i]; s_lutq[i] = A.B.lutq[i]; }
     __syncthreads();
     SmemTables T{s_xk, s_qk, s_lutx, s_lutq};
-    BSmem S{s_stage, s_idx, s_bstart, s_cnt};
+    ASmem SA;
+    SA.cnt = reinterpret_cast<unsigned *>(region);
+    SA.base = SA.cnt + A.B.nck;
+    BSmem SB;
+    SB.sP = reinterpret_cast<uint4 *>(region);
+    SB.sV = reinterpret_cast<double *>(region + (size_t)A.cap * 32);
+    SB.stage = SB.sV + (size_t)A.G.nqtot * 4 * kNFP;
+    SB.sidx = reinterpret_cast<unsigned *>(SB.stage + kBinWarps * 32 * kNF);
+    SB.fcnt = reinterpret_cast<int *>(SB.sidx + kBinWarps * 32);
+    SB.foff = SB.fcnt + A.B.nfk + 1;
+    SB.bstart = SB.foff + A.B.nfk + 1;
+    SB.order = reinterpret_cast<unsigned short *>(SB.bstart + A.B.nfk + 2);
 
     unsigned long long *ctrl = A.W.ctrl;
     const unsigned long long TA = A.ta, TB = A.B.nitems, per = TA + TB;
@@ -266,14 +350,14 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_pdf_stream(const __grid_cons
         if (isA) {
             if (threadIdx.x == 0 && gen > 0) wait_counter(b_done, gen * TB);   // ring slot drained
             __syncthreads();
-            a_item(A, T, slot, chunk_base, sub, &err_local);
+            a_item(A, T, SA, slot, chunk_base, sub, &err_local);
             __threadfence();
             __syncthreads();
             if (threadIdx.x == 0) atomicAdd(a_done, 1ULL);
         } else {
             if (threadIdx.x == 0) wait_counter(a_done, (gen + 1) * TA);        // every tile of A(c) released
             __syncthreads();
-            b_item(A, S, slot, chunk_base, sub);
+            b_item(A, SB, slot, chunk_base, sub);
             __threadfence();
             __syncthreads();
             if (threadIdx.x == 0) {

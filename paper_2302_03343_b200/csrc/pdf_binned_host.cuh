@@ -22,32 +22,29 @@ __global__ void k_q2plus(GridDev G, double *res)
 
 inline void binned_plan_free(BinnedPlan &p)
 {
-    cudaFree(p.d_items); cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_plus);
-    p.d_items = nullptr; p.d_lutx = p.d_lutq = nullptr; p.d_plus = nullptr; p.usable = false;
+    cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_plus);
+    p.d_lutx = p.d_lutq = nullptr; p.d_plus = nullptr; p.usable = false;
 }
 
-inline size_t binned_smem_bytes(int nx, int nqtot)
+inline size_t binned_smem_bytes(int nx, int nqtot, int nck, int nfk, int cap)
 {
-    return sizeof(double) * (nx + nqtot) + sizeof(double) * kBinWarps * 32 * kNF + sizeof(unsigned) * kBinWarps * 32 +
-           sizeof(int) * (2 * kKeysPerItem + 2) + sizeof(short) * 2 * kLutSize + 64;
+    return sizeof(double) * (nx + nqtot) + sizeof(short) * 2 * kLutSize + 64 + bsmem_item_bytes(nqtot, nck, nfk, cap);
 }
 
-// builds LUTs, the key geometry and the per-chunk B work list; leaves usable = false when the
-// grid does not fit the specialised path (then every call takes the direct path)
+// builds LUTs and the key geometry; leaves usable = false when the grid does not fit the
+// specialised path (then every call takes the direct path)
 inline int binned_plan_init(BinnedPlan &p, const GridDev &G, const std::vector<double> &xk,
                             const std::vector<double> &qk, const std::vector<int> &qoff)
 {
     p.usable = false;
     const int nx = G.nx, nqt = G.nqtot;
-    if (G.nflav != kNF || G.nfp != kNFP || nx > 30000 || nqt > 30000) return 0;
+    if (G.nflav != kNF || G.nfp != kNFP || G.nmem != 1) return 0;
+    if (nx - 1 + kLowXSplit > kMaxCK || nqt + 2 > kMaxFK || nx < 2) return 0;
     BinDev &d = p.dev;
     d.ncx = nx - 1; d.nqt = nqt;
-    d.k_lowx = nqt * d.ncx;
-    d.k_highq = d.k_lowx + nqt;
-    d.k_lowq = d.k_highq + d.ncx;
-    d.k_ll = d.k_lowq + d.ncx;
-    d.k_lh = d.k_ll + kCornerSub;
-    d.nkeys = d.k_lh + kCornerSub;
+    d.nck = d.ncx + kLowXSplit;
+    d.nfk = nqt + 2;
+    d.nitems = d.nck + kOvfItems;
 
     // search LUTs: bucket b covers ln v in [l0 + b/scale, l0 + (b+1)/scale); entry = a cell at its lower edge
     auto make_lut = [](const std::vector<double> &k, bool last_le, double &scale, std::vector<short> &lut) {
@@ -67,24 +64,9 @@ inline int binned_plan_init(BinnedPlan &p, const GridDev &G, const std::vector<d
     make_lut(xk, false, d.lutx_scale, lx);
     make_lut(qk, true, d.lutq_scale, lq);
 
-    std::vector<BinItem> items;
-    auto add_groups = [&](int k0, int k1, int per) {
-        for (int k = k0; k < k1; k += per) items.push_back({k, k + per < k1 ? k + per : k1});
-    };
-    add_groups(d.k_ll, d.k_ll + kCornerSub, 1);            // heaviest math first (longest-first scheduling)
-    add_groups(d.k_lh, d.k_lh + kCornerSub, 1);
-    add_groups(d.k_lowx, d.k_lowx + nqt, 8);
-    add_groups(d.k_lowq, d.k_lowq + d.ncx, kKeysPerItem);
-    add_groups(d.k_highq, d.k_highq + d.ncx, kKeysPerItem);
-    add_groups(0, d.k_lowx, kKeysPerItem);
-    for (int o = 0; o < kOvfItems; ++o) items.push_back({-(o + 1), 0});
-    d.nitems = (int)items.size();
-
-    if (cudaMalloc((void **)&p.d_items, sizeof(BinItem) * items.size()) != cudaSuccess) return PDF_ENOMEM;
     if (cudaMalloc((void **)&p.d_lutx, sizeof(short) * kLutSize) != cudaSuccess) return PDF_ENOMEM;
     if (cudaMalloc((void **)&p.d_lutq, sizeof(short) * kLutSize) != cudaSuccess) return PDF_ENOMEM;
     if (cudaMalloc((void **)&p.d_plus, sizeof(double) * 4) != cudaSuccess) return PDF_ENOMEM;
-    cudaMemcpy(p.d_items, items.data(), sizeof(BinItem) * items.size(), cudaMemcpyHostToDevice);
     cudaMemcpy(p.d_lutx, lx.data(), sizeof(short) * kLutSize, cudaMemcpyHostToDevice);
     cudaMemcpy(p.d_lutq, lq.data(), sizeof(short) * kLutSize, cudaMemcpyHostToDevice);
     k_q2plus<<<1, 32>>>(G, p.d_plus);
@@ -92,17 +74,12 @@ inline int binned_plan_init(BinnedPlan &p, const GridDev &G, const std::vector<d
     if (cudaMemcpy(res, p.d_plus, sizeof res, cudaMemcpyDeviceToHost) != cudaSuccess) return PDF_ECUDA;
     if (res[2] != 1.0) return 0;                           // 1.01*Q2min beyond the grid: direct path only
     d.jgplus = (int)res[0]; d.tqplus = res[1];
-    d.items = p.d_items; d.lutx = p.d_lutx; d.lutq = p.d_lutq;
+    d.lutx = p.d_lutx; d.lutq = p.d_lutq;
 
-    size_t smem = binned_smem_bytes(nx, nqt);
-    if (smem > 100 * 1024) return 0;
-    cudaFuncSetAttribute(k_pdf_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    int per_sm = 0, dev = 0, sms = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_pdf_stream, kBinThreads, smem) != cudaSuccess || per_sm < 1)
-        return 0;
-    p.max_ctas = per_sm * sms;
+    // largest shared-memory footprint (cap = kMaxCap) must fit one CTA; the launch computes the real one
+    size_t smem_max = binned_smem_bytes(nx, nqt, d.nck, d.nfk, kMaxCap);
+    if (smem_max > 200 * 1024) return 0;
+    if (cudaFuncSetAttribute(k_pdf_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max) != cudaSuccess) return 0;
     (void)qoff;
     p.usable = true;
     return 0;
@@ -121,20 +98,28 @@ inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm,
     StreamArgs A;
     A.G = G; A.B = p.dev; A.cm = cm;
     A.chunk = binned_chunk(p, n, chunk_opt);
-    A.cap = binned_cap(A.chunk);
+    A.cap = binned_cap(p, A.chunk);
     binned_carve(p, ws, A.chunk, A.cap, A.W);
     A.x = x; A.q2 = q2; A.out = out; A.n = n; A.ld = ld;
     A.nchunks = (int)((n + A.chunk - 1) / A.chunk);
     A.ta = (int)(A.chunk / kTileA);
     A.identity = cm.n == kNF;
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
+    A.zfill = (ld == cm.n) ? 1 : 0;
     size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts + ovf_count
     if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
+    size_t smem = binned_smem_bytes(G.nx, G.nqtot, p.dev.nck, p.dev.nfk, A.cap);
+    int per_sm = 0, dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_pdf_stream, kBinThreads, smem) != cudaSuccess || per_sm < 1)
+        return PDF_ECUDA;
+    unsigned long long max_ctas = (unsigned long long)per_sm * sms;         // all CTAs must be co-resident
     unsigned long long tickets = (unsigned long long)A.nchunks * (A.ta + p.dev.nitems);
-    unsigned grid = (unsigned)(tickets < (unsigned long long)p.max_ctas ? tickets : p.max_ctas);
+    unsigned grid = (unsigned)(tickets < max_ctas ? tickets : max_ctas);
     {
         Scope sc(s, "k_pdf_stream");
-        k_pdf_stream<<<grid, kBinThreads, binned_smem_bytes(G.nx, G.nqtot), s>>>(A);
+        k_pdf_stream<<<grid, kBinThreads, smem, s>>>(A);
     }
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }

@@ -1,4 +1,5 @@
-// pdf_binned_kernel.cuh -- device code of the persistent binned kernel (see pdf_binned.cuh).
+// pdf_binned_kernel.cuh -- device code of the persistent binned kernel: helpers and A items
+// (see pdf_binned.cuh for the design).
 #pragma once
 
 namespace pdfg {
@@ -12,8 +13,9 @@ struct StreamArgs {
     double *out;
     long long n, ld;
     long long chunk;           // queries per chunk (multiple of kTileA)
-    int nchunks, ta, cap;      // chunks, A items per chunk, bin capacity
+    int nchunks, ta, cap;      // chunks, A items per chunk, bin capacity per (chunk, coarse key)
     int identity;              // 1: requested columns == the grid's 11 columns in order
+    int zfill;                 // 1: rows are contiguous (ld == npid): A items zero-fill their tile of `out`
 };
 
 // ---- small device helpers ----------------------------------------------------------------------
@@ -33,9 +35,11 @@ __device__ __forceinline__ void wait_counter(const unsigned long long *p, unsign
     }
 }
 
-__device__ __forceinline__ double2 ldg_nc_d2(const double *p)
+// one payload = one 32-byte sector, stored whole (STG.256): never a partial-sector write
+__device__ __forceinline__ void store_payload(Payload *dst, double a, double b, unsigned idx, unsigned fk)
 {
-    return __ldg(reinterpret_cast<const double2 *>(p));
+    double w2 = __hiloint2double((int)fk, (int)idx);       // low word idx, high word fk
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(dst), "d"(a), "d"(b), "d"(w2), "d"(0.0) : "memory");
 }
 
 // knot search from a LUT guess; exact for any knots (walks to the C-4 cell from wherever it starts)
@@ -54,49 +58,71 @@ __device__ __forceinline__ int search_last_le(const double *__restrict__ k, int 
     return g;
 }
 
-// ---- A item: classify, locate, t_x / t_q, bin ---------------------------------------------------
-// smem: raw knots and LUTs staged once per CTA
+// shared memory of the persistent kernel: tables staged once per CTA + a region that A and B
+// items use in turn
 struct SmemTables {
     const double *xk, *qk;
     const short *lutx, *lutq;
 };
+struct ASmem {
+    unsigned *cnt;        // [nck] queries of this tile per coarse key
+    unsigned *base;       // [nck] first slot of the tile's run in the key's bin
+};
 
-__device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T, int slot, long long chunk_base,
-                                       int tile, unsigned long long *err_local)
+// zero-fill rows [r0, r1) of `out` (contiguous rows, ld doubles each) with coalesced stores, so
+// that the scattered row stores of B land in valid, L2-resident sectors
+__device__ __forceinline__ void zero_fill_rows(double *out, long long ld, long long r0, long long r1)
+{
+    double *p = out + r0 * ld, *e = out + r1 * ld;
+    if (p >= e) return;
+    if ((reinterpret_cast<size_t>(p) & 8) != 0) { if (threadIdx.x == 0) *p = 0.0; ++p; }
+    long long n2 = (e - p) >> 1;
+    double2 *p2 = reinterpret_cast<double2 *>(p);
+    for (long long k = threadIdx.x; k < n2; k += kBinThreads) p2[k] = make_double2(0.0, 0.0);
+    if (((e - p) & 1) && threadIdx.x == 0) e[-1] = 0.0;
+}
+
+// ---- A item: classify, locate, t_x / t_q, tile-local sort by coarse key, payload stores ---------
+__device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T, const ASmem &S, int slot,
+                                       long long chunk_base, int tile, unsigned long long *err_local)
 {
     const GridDev &G = A.G;
     const BinDev &B = A.B;
-    unsigned *counts = A.W.counts + (size_t)slot * B.nkeys;
-    Payload *bins = A.W.bins + (size_t)slot * B.nkeys * A.cap;
+    unsigned *counts = A.W.counts + (size_t)slot * B.nck;
+    Payload *bins = A.W.bins + (size_t)slot * B.nck * A.cap;
     Payload *ovf = A.W.ovf + (size_t)slot * A.chunk;
     unsigned *ovf_count = A.W.ovf_count + slot;
     const double xmin = T.xk[0], xmax = T.xk[G.nx - 1], qmin = T.qk[0], qmax = T.qk[G.nqtot - 1];
     const double u0 = __ldg(G.uk), s0 = __ldg(G.sk);
 
+    for (int k = threadIdx.x; k < B.nck; k += kBinThreads) S.cnt[k] = 0u;
+
+    const long long t0 = chunk_base + (long long)tile * kTileA;
+    long long t1 = t0 + kTileA;
+    if (t1 > A.n) t1 = A.n;
+    if (t1 > chunk_base + A.chunk) t1 = chunk_base + A.chunk;
     double xv[kTileQ], qv[kTileQ];
-    long long e0 = chunk_base + (long long)tile * kTileA + threadIdx.x;
+    const long long e0 = t0 + threadIdx.x;
 #pragma unroll
     for (int q = 0; q < kTileQ; ++q) {
         long long e = e0 + q * kBinThreads;
-        bool in = e < A.n && e < chunk_base + A.chunk;
+        bool in = e < t1;
         xv[q] = in ? __ldcs(A.x + e) : -1.0;      // streaming: read once
         qv[q] = in ? __ldcs(A.q2 + e) : -1.0;
     }
-    int key[kTileQ];
-    Payload pl[kTileQ];
+    if (A.zfill) zero_fill_rows(A.out, A.ld, t0, t1);
+    __syncthreads();
+
+    int ck[kTileQ];
+    unsigned fkv[kTileQ], rank[kTileQ];
+    double pa[kTileQ], pb[kTileQ];
 #pragma unroll
     for (int q = 0; q < kTileQ; ++q) {
         long long e = e0 + q * kBinThreads;
-        bool in = e < A.n && e < chunk_base + A.chunk;
         double x = xv[q], q2 = qv[q];
-        key[q] = -1;
-        if (!in) continue;
-        unsigned idx = (unsigned)(e - chunk_base);
-        pl[q].idx = idx; pl[q].pad0 = 0; pl[q].pad1 = 0.0;
-        if (!(finite_pos(x) && finite_pos(q2)) || x > xmax) {      // C-10
-            key[q] = -2;
-            continue;
-        }
+        ck[q] = -1; rank[q] = 0; fkv[q] = 0; pa[q] = 0.0; pb[q] = 0.0;
+        if (e >= t1) continue;
+        if (!(finite_pos(x) && finite_pos(q2)) || x > xmax) { ck[q] = -2; continue; }       // C-10
         bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
         double lx = log(x), lq = log(q2);
         int i = 0, jg = 0;
@@ -127,29 +153,31 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         } else {
             tb = q2 / qmin;                                        // r (C-9)
         }
-        int kk;
-        if (lowx) kk = lowq ? B.k_ll + (int)(idx & (kCornerSub - 1))
-                   : highq ? B.k_lh + (int)(idx & (kCornerSub - 1)) : B.k_lowx + jg;
-        else kk = lowq ? B.k_lowq + i : highq ? B.k_highq + i : jg * B.ncx + i;
-        key[q] = kk;
-        pl[q].a = ta; pl[q].b = tb;
+        unsigned idx = (unsigned)(e - chunk_base);
+        ck[q] = lowx ? B.ncx + (int)(idx & (kLowXSplit - 1)) : i;
+        fkv[q] = lowq ? (unsigned)B.nqt : highq ? (unsigned)B.nqt + 1u : (unsigned)jg;
+        pa[q] = ta; pb[q] = tb;
+        rank[q] = atomicAdd(S.cnt + ck[q], 1u);
     }
-    unsigned slotv[kTileQ];
-#pragma unroll
-    for (int q = 0; q < kTileQ; ++q) slotv[q] = key[q] >= 0 ? atomicAdd(counts + key[q], 1u) : 0u;
+    __syncthreads();
+    for (int k = threadIdx.x; k < B.nck; k += kBinThreads) {       // one global atomic per (tile, key)
+        unsigned c = S.cnt[k];
+        S.base[k] = c ? atomicAdd(counts + k, c) : 0u;
+    }
+    __syncthreads();
 #pragma unroll
     for (int q = 0; q < kTileQ; ++q) {
-        if (key[q] >= 0) {
-            Payload *dst;
-            if (slotv[q] < (unsigned)A.cap) dst = bins + (size_t)key[q] * A.cap + slotv[q];
+        long long e = e0 + q * kBinThreads;
+        if (ck[q] >= 0) {
+            unsigned idx = (unsigned)(e - chunk_base);
+            unsigned pos = S.base[ck[q]] + rank[q];
+            if (pos < (unsigned)A.cap) store_payload(bins + (size_t)ck[q] * A.cap + pos, pa[q], pb[q], idx, fkv[q]);
             else {                                                 // bin full: raw query to the overflow list
                 unsigned o = atomicAdd(ovf_count, 1u);
-                dst = ovf + o;
-                pl[q].a = xv[q]; pl[q].b = qv[q];
+                store_payload(ovf + o, xv[q], qv[q], idx, 0u);
             }
-            *dst = pl[q];
-        } else if (key[q] == -2) {
-            double *o = A.out + (chunk_base + pl[q].idx) * A.ld;
+        } else if (ck[q] == -2) {
+            double *o = A.out + e * A.ld;
             for (int p = 0; p < A.cm.n; ++p) o[p] = qnan();
             ++*err_local;
         }
