@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--e2e-n", type=int, default=0, help="0 = same as --n")
     ap.add_argument("--cpu-sample", type=int, default=10_000_000)
     ap.add_argument("--path", default="auto", choices=["auto", "direct", "binned"])
+    ap.add_argument("--chunk", type=int, default=0, help="binned-path chunk size (0 = library default)")
     ap.add_argument("--skip-extras", action="store_true", help="only the headline step (no lumi/members/e2e/cpu)")
     return ap.parse_args()
 
@@ -212,6 +213,9 @@ def run_ours(args):
     n = args.n
     g = binding.PdfGrid.from_spec(spec, workspace_for=0 if args.path == "direct" else n)
     g.pdf_grid_set_option(binding.PDF_OPT_PATH, pathopt)
+    if args.chunk:
+        g.pdf_grid_set_option(binding.PDF_OPT_CHUNK, args.chunk)
+        g.attach_workspace(n)
     x, q2 = synth.queries_c2(spec, n, seed=synth.BASE_SEED + 2 + 1000 * rank, device="cuda")
     out = torch.empty((n, 11), dtype=torch.float64, device="cuda")
     aout = torch.empty(n, dtype=torch.float64, device="cuda")

@@ -16,9 +16,9 @@
 //          scattered row stores of B then merge into valid L2-resident sectors (2.7 ms -> in
 //          budget), and every line still leaves L2 for HBM once.
 //
-// How: ONE persistent kernel per call, CTAs pull tickets in the order
+// How: ONE persistent kernel per call, CTAs pull tickets in the order (lag kLag = 1)
 //      A(0) | A(1) B(0) | A(2) B(1) | ... | B(last)
-//   A(c), one item per 2048 queries of chunk c: read x,q2 (coalesced), classify, locate the cell,
+//   A(c), one item per 1024 queries of chunk c: read x,q2 (coalesced), classify, locate the cell,
 //      t_x,t_q (the two logs), coarse/fine key, tile-local counting sort by coarse key, payload
 //      stores; zero-fill of the tile's output rows.
 //   B(c), one item per coarse key: copy the key's payloads and its 4 grid columns (4 x nq x 96 B)
@@ -38,11 +38,18 @@ namespace pdfg {
 
 constexpr int kBinThreads = 256;              // CTA size of the persistent kernel
 constexpr int kBinWarps = kBinThreads / 32;
-constexpr int kTileQ = 8;                     // queries per thread in an A item
-constexpr int kTileA = kBinThreads * kTileQ;  // 2048 queries per A item
+#ifndef PDF_TILEQ
+#define PDF_TILEQ 4
+#endif
+#ifndef PDF_LAG
+#define PDF_LAG 1
+#endif
+constexpr int kTileQ = PDF_TILEQ;                     // queries per thread in an A item
+constexpr int kTileA = kBinThreads * kTileQ;  // 1024 queries per A item
 constexpr int kOvfItems = 4;                  // B items per chunk that drain the overflow list
-constexpr int kRing = 3;                      // chunk slots in flight
-constexpr int kLowXSplit = 16;                // coarse keys of the low-x classes (spreads their 2.5 %)
+constexpr int kLag = PDF_LAG;                       // B(c) tickets follow A(c) tickets by this many rounds
+constexpr int kRing = kLag + 2;               // chunk slots in flight
+constexpr int kLowXSplit = 16;                // coarse keys of the low-x classes: bands of Q2 cells
 constexpr int kLutSize = 1024;                // search-acceleration buckets per axis
 constexpr int kNF = 11, kNFP = 12;            // the fast path is specialised for 11 flavours (pad 12)
 constexpr int kMaxCK = 1024;                  // coarse keys (x cells + kLowXSplit) the path supports

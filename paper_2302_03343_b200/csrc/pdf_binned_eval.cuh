@@ -102,8 +102,9 @@ __device__ __noinline__ void eval_extrap_s(const GridDev &G, const BinDev &B, un
         if (fk == B.nqt) {                                 // low-Q (C-9): pa = t_x, pb = r
             eval_row_s(G, sV, i, 0, pa, e0);
             eval_interior_s(G, sV, i, B.jgplus, pa, B.tqplus, e1);
+            const double lnr = log(pb);
 #pragma unroll
-            for (int f = 0; f < kNF; ++f) acc[f] = lowq_continue(e0[f], e1[f], pb);
+            for (int f = 0; f < kNF; ++f) acc[f] = lowq_continue_ln(e0[f], e1[f], pb, lnr);
         } else {                                           // high-Q (C-8): pa = t_x, pb = theta_q
             eval_row_s(G, sV, i, last - 1, pa, e0);
             eval_row_s(G, sV, i, last, pa, e1);
@@ -119,11 +120,12 @@ __device__ __noinline__ void eval_extrap_s(const GridDev &G, const BinDev &B, un
         for (int f = 0; f < kNF; ++f) acc[f] = continue_two(e0[f], e1[f], pa);
     } else if (fk == B.nqt) {                              // low-x & low-Q (L1744): x rule, then Q rule
         double e2[kNF], e3[kNF];
+        const double lnr = log(pb);
         load_node_s(sV, 0, 0, e0); load_node_s(sV, 0, 1, e1);
         eval_column_s(G, sV, 0, B.jgplus, B.tqplus, e2); eval_column_s(G, sV, 1, B.jgplus, B.tqplus, e3);
 #pragma unroll
         for (int f = 0; f < kNF; ++f)
-            acc[f] = lowq_continue(continue_two(e0[f], e1[f], pa), continue_two(e2[f], e3[f], pa), pb);
+            acc[f] = lowq_continue_ln(continue_two(e0[f], e1[f], pa), continue_two(e2[f], e3[f], pa), pb, lnr);
     } else {                                               // low-x & high-Q
         double e2[kNF], e3[kNF];
         load_node_s(sV, last - 1, 0, e0); load_node_s(sV, last - 1, 1, e1);
@@ -156,10 +158,11 @@ struct BSmem {
     uint4 *sP;            // [cap] payloads (2 x uint4 each)
     double *sV;           // [nqt][4][12]
     double *stage;        // [kBinWarps][32*kNF]
-    unsigned *sidx;       // [kBinWarps][32]
+    unsigned long long *sptr; // [kBinWarps][32] output row pointers of the staged batch
     int *fcnt;            // [nfk]
     int *foff;            // [nfk+1]
     int *bstart;          // [nfk+1]
+    int *next;            // [1] batch queue of the item
     unsigned short *order;// [cap]
 };
 
@@ -178,37 +181,46 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
     const bool lowx_unit = ck >= B.ncx;
     const int i = lowx_unit ? 0 : ck;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned sPa = (unsigned)__cvta_generic_to_shared(S.sP), sVa = (unsigned)__cvta_generic_to_shared(S.sV);
+    const unsigned fcnt = (unsigned)__cvta_generic_to_shared(S.fcnt), foff = (unsigned)__cvta_generic_to_shared(S.foff);
+    const unsigned bstart = (unsigned)__cvta_generic_to_shared(S.bstart), order = (unsigned)__cvta_generic_to_shared(S.order);
+    const unsigned nexta = (unsigned)__cvta_generic_to_shared(S.next);
+    const unsigned stage = (unsigned)__cvta_generic_to_shared(S.stage) + (unsigned)warp * (32 * kNF * 8);
+    const unsigned sptr = (unsigned)__cvta_generic_to_shared(S.sptr) + (unsigned)warp * (32 * 8);
 
     // stage payloads (coalesced) and the key's 4 grid columns
-    for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) S.sP[e] = __ldcg(bin + e);
+    for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) {
+        uint4 v = __ldcg(bin + e);
+        sts_v4u32(sPa + 16u * e, v.x, v.y, v.z, v.w);
+    }
     {
         int c0, c1, c2, c3;
         if (lowx_unit) { c0 = 0; c1 = 1; c2 = 0; c3 = 1; }
         else { c0 = i > 0 ? i - 1 : i; c1 = i; c2 = i + 1; c3 = i + 2 < G.nx ? i + 2 : i + 1; }
         const double2 *V2 = reinterpret_cast<const double2 *>(G.V);
-        double2 *sV2 = reinterpret_cast<double2 *>(S.sV);
         const int tot = G.nqtot * 24;                      // double2 units: rows x 4 slots x 6
         for (int e = threadIdx.x; e < tot; e += kBinThreads) {
             int jg = e / 24, r = e - jg * 24, a = r / 6, p = r - a * 6;
             int col = a == 0 ? c0 : a == 1 ? c1 : a == 2 ? c2 : c3;
-            sV2[e] = __ldg(V2 + ((size_t)jg * G.nx + col) * 6 + p);
+            double2 v = __ldg(V2 + ((size_t)jg * G.nx + col) * 6 + p);
+            sts_v2f64(sVa + 16u * e, v.x, v.y);
         }
     }
-    for (int k = threadIdx.x; k < B.nfk; k += kBinThreads) S.fcnt[k] = 0;
+    for (int k = threadIdx.x; k < B.nfk; k += kBinThreads) sts_u32(fcnt + 4u * k, 0u);
+    if (threadIdx.x == 0) sts_u32(nexta, 0u);
     __syncthreads();
     // counting sort by fine key: rank kept in the payload's spare word
     for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
-        uint4 w1 = S.sP[2 * e + 1];                        // {idx, fk, pad, pad}
-        int r = atomicAdd(S.fcnt + w1.y, 1);
-        w1.z = (unsigned)r;
-        S.sP[2 * e + 1] = w1;
+        unsigned fk = lds_u32(sPa + 32u * e + 20u);
+        unsigned r = atoms_add(fcnt + 4u * fk, 1u);
+        sts_u32(sPa + 32u * e + 24u, r);
     }
     __syncthreads();
     if (warp == 0) {                                       // exclusive scans: slots and 32-query batches per key
         int carry_o = 0, carry_b = 0;
         for (int k0 = 0; k0 < B.nfk; k0 += 32) {
             int k = k0 + lane;
-            int c = k < B.nfk ? S.fcnt[k] : 0;
+            int c = k < B.nfk ? (int)lds_u32(fcnt + 4u * k) : 0;
             int nb = (c + 31) >> 5;
             int so = c, sb = nb;
 #pragma unroll
@@ -216,46 +228,56 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
                 int vo = __shfl_up_sync(0xffffffffu, so, d), vb = __shfl_up_sync(0xffffffffu, sb, d);
                 if (lane >= d) { so += vo; sb += vb; }
             }
-            if (k < B.nfk) { S.foff[k] = carry_o + so - c; S.bstart[k] = carry_b + sb - nb; }
+            if (k < B.nfk) { sts_u32(foff + 4u * k, (unsigned)(carry_o + so - c)); sts_u32(bstart + 4u * k, (unsigned)(carry_b + sb - nb)); }
             carry_o += __shfl_sync(0xffffffffu, so, 31);
             carry_b += __shfl_sync(0xffffffffu, sb, 31);
         }
-        if (lane == 0) { S.foff[B.nfk] = carry_o; S.bstart[B.nfk] = carry_b; }
+        if (lane == 0) { sts_u32(foff + 4u * B.nfk, (unsigned)carry_o); sts_u32(bstart + 4u * B.nfk, (unsigned)carry_b); }
     }
     __syncthreads();
     for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
-        uint4 w1 = S.sP[2 * e + 1];
-        S.order[S.foff[w1.y] + (int)w1.z] = (unsigned short)e;
+        uint2 w = make_uint2(lds_u32(sPa + 32u * e + 20u), lds_u32(sPa + 32u * e + 24u));
+        unsigned pos = lds_u32(foff + 4u * w.x) + w.y;
+        asm volatile("st.shared.u16 [%0], %1;" ::"r"(order + 2u * pos), "h"((unsigned short)e) : "memory");
     }
     __syncthreads();
 
-    const int total = S.bstart[B.nfk];
-    const unsigned sVa = (unsigned)__cvta_generic_to_shared(S.sV);
-    double *stage = S.stage + warp * (32 * kNF);
-    unsigned *sidx = S.sidx + warp * 32;
-    int k = 0;
-    for (int fb = warp; fb < total; fb += kBinWarps) {
-        while (S.bstart[k + 1] <= fb) ++k;                 // fine key of this batch (monotone in fb)
-        const int fk = k, kcnt = S.fcnt[k];
-        const int first = (fb - S.bstart[k]) * 32;
+    const int total = (int)lds_u32(bstart + 4u * B.nfk);
+    for (;;) {
+        int fb = 0;
+        if (lane == 0) fb = (int)atoms_add(nexta, 1u);     // batches are handed out dynamically,
+        fb = __shfl_sync(0xffffffffu, fb, 0);              // last keys first: the extrapolation classes
+        if (fb >= total) break;                            // (long, few lanes) must not form the tail
+        fb = total - 1 - fb;
+        int lo = 0, hi = B.nfk;                            // largest k with bstart[k] <= fb
+        while (hi - lo > 1) {
+            int mid = (lo + hi) >> 1;
+            if ((int)lds_u32(bstart + 4u * mid) <= fb) lo = mid; else hi = mid;
+        }
+        const int fk = lo, kcnt = (int)lds_u32(fcnt + 4u * fk);
+        const int first = (fb - (int)lds_u32(bstart + 4u * fk)) * 32;
         const int nact = min(32, kcnt - first);
         const bool active = lane < nact;
         double pa = 0.0, pb = 0.0;
         unsigned idx = 0;
         if (active) {
-            int e = S.order[S.foff[k] + first + lane];
-            uint4 w0 = S.sP[2 * e], w1 = S.sP[2 * e + 1];
-            pa = __hiloint2double((int)w0.y, (int)w0.x);
-            pb = __hiloint2double((int)w0.w, (int)w0.z);
-            idx = w1.x;
+            unsigned short e16;
+            asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(order + 2u * (lds_u32(foff + 4u * fk) + first + lane)));
+            const unsigned pe = sPa + 32u * e16;
+            double2 ab = lds_v2f64(pe);
+            pa = ab.x; pb = ab.y;
+            idx = lds_u32(pe + 16u);
         }
         double acc[kNF];
         if (!lowx_unit && fk < B.nqt) eval_interior_s(G, sVa, i, fk, pa, pb, acc);
         else eval_extrap_s(G, B, sVa, lowx_unit, i, fk, pa, pb, acc);
         // transpose through shared memory so that whole rows leave in contiguous pieces
 #pragma unroll
-        for (int f = 0; f < kNF; ++f) stage[lane * kNF + f] = acc[f];
-        sidx[lane] = idx;
+        for (int f = 0; f < kNF; ++f) sts_f64(stage + 8u * (lane * kNF + f), acc[f]);
+        {
+            unsigned long long rp = reinterpret_cast<unsigned long long>(A.out + (chunk_base + idx) * A.ld);
+            asm volatile("st.shared.u64 [%0], %1;" ::"r"(sptr + 8u * lane), "l"(rp) : "memory");
+        }
         __syncwarp();
         if (A.identity) {
             const int tot = nact * kNF;
@@ -263,15 +285,19 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
             for (int itx = 0; itx < kNF; ++itx) {
                 int e = itx * 32 + lane;
                 if (e < tot) {
-                    int r = e / kNF, p = e - r * kNF;
-                    A.out[(chunk_base + sidx[r]) * A.ld + p] = stage[e];
+                    int r = (e * 745) >> 13, p = e - r * kNF;          // e / 11 for e < 352
+                    unsigned long long rp;
+                    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(rp) : "r"(sptr + 8u * r));
+                    reinterpret_cast<double *>(rp)[p] = lds_f64(stage + 8u * e);
                 }
             }
         } else {
             const int np = A.cm.n, tot = nact * np;
             for (int e = lane; e < tot; e += 32) {
                 int r = e / np, p = e - r * np, c = A.cm.col[p];
-                A.out[(chunk_base + sidx[r]) * A.ld + p] = c < 0 ? 0.0 : stage[r * kNF + c];
+                unsigned long long rp;
+                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(rp) : "r"(sptr + 8u * r));
+                reinterpret_cast<double *>(rp)[p] = c < 0 ? 0.0 : lds_f64(stage + 8u * (r * kNF + c));
             }
         }
         __syncwarp();
@@ -288,10 +314,10 @@ __host__ __device__ inline size_t bsmem_item_bytes(int nqt, int nck, int nfk, in
     size_t b = (size_t)cap * 32;                                        // sP
     b += (size_t)nqt * 4 * kNFP * sizeof(double);                       // sV
     b += (size_t)kBinWarps * 32 * kNF * sizeof(double);                 // stage
-    b += (size_t)kBinWarps * 32 * sizeof(unsigned);                     // sidx
-    b += (size_t)(3 * nfk + 4) * sizeof(int);                           // fcnt, foff, bstart
+    b += (size_t)kBinWarps * 32 * sizeof(unsigned long long);           // sptr
+    b += (size_t)(3 * nfk + 8) * sizeof(int);                           // fcnt, foff, bstart, next
     b += ((size_t)cap * sizeof(unsigned short) + 15) / 16 * 16;         // order
-    size_t a = (size_t)2 * nck * sizeof(unsigned);                      // A items: cnt, base
+    size_t a = (size_t)kTileA * 32 + (size_t)2 * nck * sizeof(unsigned); // A items: payloads, cnt, base
     return (b > a ? b : a) + 32;
 }
 
@@ -312,36 +338,54 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_pdf_stream(const __grid_cons
     __syncthreads();
     SmemTables T{s_xk, s_qk, s_lutx, s_lutq};
     ASmem SA;
-    SA.cnt = reinterpret_cast<unsigned *>(region);
+    SA.pay = reinterpret_cast<uint4 *>(region);
+    SA.cnt = reinterpret_cast<unsigned *>(region + (size_t)kTileA * 32);
     SA.base = SA.cnt + A.B.nck;
     BSmem SB;
     SB.sP = reinterpret_cast<uint4 *>(region);
     SB.sV = reinterpret_cast<double *>(region + (size_t)A.cap * 32);
     SB.stage = SB.sV + (size_t)A.G.nqtot * 4 * kNFP;
-    SB.sidx = reinterpret_cast<unsigned *>(SB.stage + kBinWarps * 32 * kNF);
-    SB.fcnt = reinterpret_cast<int *>(SB.sidx + kBinWarps * 32);
+    SB.sptr = reinterpret_cast<unsigned long long *>(SB.stage + kBinWarps * 32 * kNF);
+    SB.fcnt = reinterpret_cast<int *>(SB.sptr + kBinWarps * 32);
     SB.foff = SB.fcnt + A.B.nfk + 1;
     SB.bstart = SB.foff + A.B.nfk + 1;
-    SB.order = reinterpret_cast<unsigned short *>(SB.bstart + A.B.nfk + 2);
+    SB.next = SB.bstart + A.B.nfk + 2;
+    SB.order = reinterpret_cast<unsigned short *>(SB.next + 2);
 
     unsigned long long *ctrl = A.W.ctrl;
     const unsigned long long TA = A.ta, TB = A.B.nitems, per = TA + TB;
     const unsigned long long total = (unsigned long long)A.nchunks * per;
     unsigned long long err_local = 0;
 
+    // the next ticket is fetched while the current item runs (a global atomic is ~1 us)
+    unsigned long long next_t = 0;
+    if (threadIdx.x == 0) next_t = atomicAdd(ctrl, 1ULL);
     for (;;) {
-        if (threadIdx.x == 0) s_ticket = atomicAdd(ctrl, 1ULL);
+        if (threadIdx.x == 0) s_ticket = next_t;
         __syncthreads();
         const unsigned long long t = s_ticket;
         __syncthreads();
         if (t >= total) break;
-        // ticket order: A(0) | A(1) B(0) | A(2) B(1) | ... | B(last)
+        if (threadIdx.x == 0) next_t = atomicAdd(ctrl, 1ULL);      // consumed at the top of the next round
+        // ticket order, lag L = kLag rounds:  round r = [A(r) tiles | B(r-L) items]; B(c) is handed out
+        // L rounds after A(c), so its tiles were claimed >= L waves earlier and the wait below is ~never taken
         bool isA; long long c; int sub;
-        if (t < TA) { isA = true; c = 0; sub = (int)t; }
-        else {
-            unsigned long long tp = t - TA, round = 1 + tp / per, w = tp % per;
-            if ((long long)round < A.nchunks) { isA = w < TA; c = isA ? (long long)round : (long long)round - 1; sub = (int)(isA ? w : w - TA); }
-            else { isA = false; c = A.nchunks - 1; sub = (int)w; if (w >= TB) continue; }
+        {
+            const unsigned long long RA = (unsigned long long)(A.nchunks < kLag ? A.nchunks : kLag);   // A-only rounds
+            const unsigned long long F = (unsigned long long)A.nchunks - RA;                             // full rounds
+            if (t < RA * TA) { isA = true; c = (long long)(t / TA); sub = (int)(t % TA); }
+            else {
+                unsigned long long tp = t - RA * TA;
+                if (tp < F * per) {
+                    unsigned long long round = RA + tp / per, w = tp % per;
+                    isA = w < TA;
+                    c = isA ? (long long)round : (long long)(round - RA);
+                    sub = (int)(isA ? w : w - TA);
+                } else {
+                    unsigned long long tq = tp - F * per;
+                    isA = false; c = (long long)(F + tq / TB); sub = (int)(tq % TB);
+                }
+            }
         }
         const int slot = (int)(c % kRing);
         const unsigned long long gen = (unsigned long long)(c / kRing);

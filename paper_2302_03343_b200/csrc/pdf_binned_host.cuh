@@ -106,6 +106,9 @@ inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm,
     A.identity = cm.n == kNF;
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
     A.zfill = (ld == cm.n) ? 1 : 0;
+#ifdef PDF_NOZFILL
+    A.zfill = 0;
+#endif
     size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts + ovf_count
     if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
     size_t smem = binned_smem_bytes(G.nx, G.nqtot, p.dev.nck, p.dev.nfk, A.cap);

@@ -64,25 +64,69 @@ struct SmemTables {
     const double *xk, *qk;
     const short *lutx, *lutq;
 };
-struct ASmem {
-    unsigned *cnt;        // [nck] queries of this tile per coarse key
-    unsigned *base;       // [nck] first slot of the tile's run in the key's bin
-};
+// explicit shared-window accessors (32-bit addresses): the compiler cannot prove the address space
+// of pointers that travel through structs and would emit generic loads
+__device__ __forceinline__ double lds_f64(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+__device__ __forceinline__ unsigned lds_u32(unsigned a) { unsigned v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ int lds_s16(unsigned a) { short v; asm volatile("ld.shared.s16 %0, [%1];" : "=h"(v) : "r"(a)); return (int)v; }
+__device__ __forceinline__ double2 lds_v2f64(unsigned a)
+{
+    double2 v; asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a)); return v;
+}
+__device__ __forceinline__ uint4 lds_v4u32(unsigned a)
+{
+    uint4 v; asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v;
+}
+__device__ __forceinline__ void sts_u32(unsigned a, unsigned v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts_f64(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ void sts_v2f64(unsigned a, double x, double y)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(a), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void sts_v4u32(unsigned a, unsigned x, unsigned y, unsigned z, unsigned w)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ unsigned atoms_add(unsigned a, unsigned v)
+{
+    unsigned r; asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
+}
 
 // zero-fill rows [r0, r1) of `out` (contiguous rows, ld doubles each) with coalesced stores, so
-// that the scattered row stores of B land in valid, L2-resident sectors
-__device__ __forceinline__ void zero_fill_rows(double *out, long long ld, long long r0, long long r1)
+// that the scattered row stores of B land in valid, L2-resident sectors.  The work is cut in
+// `nslice` slices that the A loop issues between queries: the stores drain under the logarithms.
+struct ZeroFill {
+    double2 *p2; long long n2; double *head, *tail;
+};
+__device__ __forceinline__ ZeroFill zero_fill_plan(double *out, long long ld, long long r0, long long r1)
 {
+    ZeroFill z{nullptr, 0, nullptr, nullptr};
     double *p = out + r0 * ld, *e = out + r1 * ld;
-    if (p >= e) return;
-    if ((reinterpret_cast<size_t>(p) & 8) != 0) { if (threadIdx.x == 0) *p = 0.0; ++p; }
-    long long n2 = (e - p) >> 1;
-    double2 *p2 = reinterpret_cast<double2 *>(p);
-    for (long long k = threadIdx.x; k < n2; k += kBinThreads) p2[k] = make_double2(0.0, 0.0);
-    if (((e - p) & 1) && threadIdx.x == 0) e[-1] = 0.0;
+    if (p >= e) return z;
+    if ((reinterpret_cast<size_t>(p) & 8) != 0) { z.head = p; ++p; }
+    z.n2 = (e - p) >> 1;
+    z.p2 = reinterpret_cast<double2 *>(p);
+    if ((e - p) & 1) z.tail = e - 1;
+    return z;
+}
+__device__ __forceinline__ void zero_fill_slice(const ZeroFill &z, int slice, int nslice)
+{
+    const long long per = (z.n2 + nslice - 1) / nslice;
+    long long k0 = per * slice, k1 = k0 + per;
+    if (k1 > z.n2) k1 = z.n2;
+    for (long long k = k0 + threadIdx.x; k < k1; k += kBinThreads) z.p2[k] = make_double2(0.0, 0.0);
+    if (slice == 0 && threadIdx.x == 0) { if (z.head) *z.head = 0.0; if (z.tail) *z.tail = 0.0; }
 }
 
 // ---- A item: classify, locate, t_x / t_q, tile-local sort by coarse key, payload stores ---------
+// Per query only (x, q2) live in registers across the loop; the payload (a, b, idx, fk) and the
+// (coarse key, rank) pair are parked in shared memory until the tile's runs have been reserved.
+struct ASmem {
+    unsigned *cnt;        // [nck] queries of this tile per coarse key
+    unsigned *base;       // [nck] first slot of the tile's run in the key's bin
+    uint4 *pay;           // [kTileA][2] payloads in query order; .w of the second word = ck<<16 | rank
+};
+
 __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T, const ASmem &S, int slot,
                                        long long chunk_base, int tile, unsigned long long *err_local)
 {
@@ -92,94 +136,106 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
     Payload *bins = A.W.bins + (size_t)slot * B.nck * A.cap;
     Payload *ovf = A.W.ovf + (size_t)slot * A.chunk;
     unsigned *ovf_count = A.W.ovf_count + slot;
-    const double xmin = T.xk[0], xmax = T.xk[G.nx - 1], qmin = T.qk[0], qmax = T.qk[G.nqtot - 1];
+    const unsigned s_xk = (unsigned)__cvta_generic_to_shared(T.xk), s_qk = (unsigned)__cvta_generic_to_shared(T.qk);
+    const unsigned s_lx = (unsigned)__cvta_generic_to_shared(T.lutx), s_lq = (unsigned)__cvta_generic_to_shared(T.lutq);
+    const unsigned s_cnt = (unsigned)__cvta_generic_to_shared(S.cnt), s_base = (unsigned)__cvta_generic_to_shared(S.base);
+    const unsigned s_pay = (unsigned)__cvta_generic_to_shared(S.pay);
+    const int nx = G.nx, nqt = G.nqtot;
+    const double xmin = lds_f64(s_xk), xmax = lds_f64(s_xk + 8u * (nx - 1));
+    const double qmin = lds_f64(s_qk), qmax = lds_f64(s_qk + 8u * (nqt - 1));
     const double u0 = __ldg(G.uk), s0 = __ldg(G.sk);
 
-    for (int k = threadIdx.x; k < B.nck; k += kBinThreads) S.cnt[k] = 0u;
+    for (int k = threadIdx.x; k < B.nck; k += kBinThreads) sts_u32(s_cnt + 4u * k, 0u);
 
     const long long t0 = chunk_base + (long long)tile * kTileA;
     long long t1 = t0 + kTileA;
     if (t1 > A.n) t1 = A.n;
     if (t1 > chunk_base + A.chunk) t1 = chunk_base + A.chunk;
-    double xv[kTileQ], qv[kTileQ];
-    const long long e0 = t0 + threadIdx.x;
-#pragma unroll
-    for (int q = 0; q < kTileQ; ++q) {
-        long long e = e0 + q * kBinThreads;
-        bool in = e < t1;
-        xv[q] = in ? __ldcs(A.x + e) : -1.0;      // streaming: read once
-        qv[q] = in ? __ldcs(A.q2 + e) : -1.0;
-    }
-    if (A.zfill) zero_fill_rows(A.out, A.ld, t0, t1);
+    ZeroFill zf = zero_fill_plan(A.out, A.ld, t0, A.zfill ? t1 : t0);
     __syncthreads();
 
-    int ck[kTileQ];
-    unsigned fkv[kTileQ], rank[kTileQ];
-    double pa[kTileQ], pb[kTileQ];
-#pragma unroll
+    // rolled loop (small code, no register arrays); the next query's inputs are fetched one round ahead
+    double xn = -1.0, qn = -1.0;
+    if (t0 + threadIdx.x < t1) { xn = __ldcs(A.x + t0 + threadIdx.x); qn = __ldcs(A.q2 + t0 + threadIdx.x); }
+#pragma unroll 1
     for (int q = 0; q < kTileQ; ++q) {
-        long long e = e0 + q * kBinThreads;
-        double x = xv[q], q2 = qv[q];
-        ck[q] = -1; rank[q] = 0; fkv[q] = 0; pa[q] = 0.0; pb[q] = 0.0;
-        if (e >= t1) continue;
-        if (!(finite_pos(x) && finite_pos(q2)) || x > xmax) { ck[q] = -2; continue; }       // C-10
-        bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
-        double lx = log(x), lq = log(q2);
-        int i = 0, jg = 0;
-        double ta, tb;
-        if (!lowx) {
-            int b = (int)((lx - u0) * B.lutx_scale);
-            b = b < 0 ? 0 : (b >= kLutSize ? kLutSize - 1 : b);
-            i = search_cell(T.xk, G.nx, x, T.lutx[b]);
-            CellTab c = G.cx[i];
-            ta = (x == T.xk[i + 1]) ? 1.0 : (lx - c.lo_log) * c.inv_d;
-        } else {
-            ta = (lx - u0) / (__ldg(G.uk + 1) - u0);              // theta_x (C-7)
+        const int ql = q * kBinThreads + threadIdx.x;             // query index inside the tile
+        const long long e = t0 + ql;
+        const double x = xn, q2 = qn;
+        if (q + 1 < kTileQ && e + kBinThreads < t1) { xn = __ldcs(A.x + e + kBinThreads); qn = __ldcs(A.q2 + e + kBinThreads); }
+        zero_fill_slice(zf, q, kTileQ);
+        unsigned tag = 0xffffffffu;                                // not a query
+        double ta = 0.0, tb = 0.0;
+        unsigned fk = 0;
+        if (e < t1) {
+            if (!(finite_pos(x) && finite_pos(q2)) || x > xmax) tag = 0xfffffffeu;      // C-10
+            else {
+                const bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
+                const double lx = log(x), lq = log(q2);
+                int i = 0, jg = 0;
+                if (!lowx) {
+                    int b = (int)((lx - u0) * B.lutx_scale);
+                    b = b < 0 ? 0 : (b >= kLutSize ? kLutSize - 1 : b);
+                    int c = lds_s16(s_lx + 2u * b);
+                    while (c > 0 && lds_f64(s_xk + 8u * c) > x) --c;
+                    while (c < nx - 2 && lds_f64(s_xk + 8u * (c + 1)) <= x) ++c;
+                    i = c;
+                    const double2 ci = __ldg(reinterpret_cast<const double2 *>(G.cx + i));   // lo_log, inv_d
+                    ta = (x == lds_f64(s_xk + 8u * (i + 1))) ? 1.0 : (lx - ci.x) * ci.y;
+                } else {
+                    ta = (lx - u0) / (__ldg(G.uk + 1) - u0);      // theta_x (C-7)
+                }
+                if (!lowq && !highq) {
+                    int b = (int)((lq - s0) * B.lutq_scale);
+                    b = b < 0 ? 0 : (b >= kLutSize ? kLutSize - 1 : b);
+                    int g = lds_s16(s_lq + 2u * b);
+                    while (g > 0 && lds_f64(s_qk + 8u * g) > q2) --g;
+                    while (g < nqt - 1 && lds_f64(s_qk + 8u * (g + 1)) <= q2) ++g;
+                    jg = g - (int)__ldg(G.cell_adj + g);           // last knot of a sub-grid -> its last cell
+                    const double2 cj = __ldg(reinterpret_cast<const double2 *>(G.cq + jg));
+                    tb = (q2 == lds_f64(s_qk + 8u * (jg + 1))) ? 1.0 : (lq - cj.x) * cj.y;
+                } else if (highq) {
+                    tb = (lq - __ldg(G.sk + nqt - 2)) / (__ldg(G.sk + nqt - 1) - __ldg(G.sk + nqt - 2));   // theta_q (C-8)
+                } else {
+                    tb = q2 / qmin;                                // r (C-9)
+                }
+                fk = lowq ? (unsigned)nqt : highq ? (unsigned)nqt + 1u : (unsigned)jg;
+                // low-x classes: one coarse key per band of Q2 cells, so that their batches fill up
+                const unsigned band = lowq ? 0u : highq ? (unsigned)(kLowXSplit - 1) : (unsigned)(jg * kLowXSplit) / (unsigned)nqt;
+                const unsigned ck = lowx ? (unsigned)B.ncx + band : (unsigned)i;
+                const unsigned rank = atoms_add(s_cnt + 4u * ck, 1u);
+                tag = (ck << 16) | rank;
+            }
         }
-        if (!lowq && !highq) {
-            int b = (int)((lq - s0) * B.lutq_scale);
-            b = b < 0 ? 0 : (b >= kLutSize ? kLutSize - 1 : b);
-            int g = search_last_le(T.qk, G.nqtot, q2, T.lutq[b]);
-            int k = __ldg(G.sub_of + g);
-            int q0 = __ldg(G.qoff + k), q1 = __ldg(G.qoff + k + 1);
-            int j = g - q0;
-            if (j > q1 - q0 - 2) j = q1 - q0 - 2;
-            jg = q0 + j;
-            CellTab c = G.cq[jg];
-            tb = (q2 == T.qk[jg + 1]) ? 1.0 : (lq - c.lo_log) * c.inv_d;
-        } else if (highq) {
-            int last = G.nqtot - 1;
-            tb = (lq - __ldg(G.sk + last - 1)) / (__ldg(G.sk + last) - __ldg(G.sk + last - 1));   // theta_q (C-8)
-        } else {
-            tb = q2 / qmin;                                        // r (C-9)
-        }
-        unsigned idx = (unsigned)(e - chunk_base);
-        ck[q] = lowx ? B.ncx + (int)(idx & (kLowXSplit - 1)) : i;
-        fkv[q] = lowq ? (unsigned)B.nqt : highq ? (unsigned)B.nqt + 1u : (unsigned)jg;
-        pa[q] = ta; pb[q] = tb;
-        rank[q] = atomicAdd(S.cnt + ck[q], 1u);
+        const unsigned pa = s_pay + 32u * ql;
+        sts_v2f64(pa, ta, tb);
+        sts_v4u32(pa + 16u, (unsigned)(e - chunk_base), fk, 0u, tag);
     }
     __syncthreads();
     for (int k = threadIdx.x; k < B.nck; k += kBinThreads) {       // one global atomic per (tile, key)
-        unsigned c = S.cnt[k];
-        S.base[k] = c ? atomicAdd(counts + k, c) : 0u;
+        unsigned c = lds_u32(s_cnt + 4u * k);
+        sts_u32(s_base + 4u * k, c ? atomicAdd(counts + k, c) : 0u);
     }
     __syncthreads();
-#pragma unroll
+#pragma unroll 1
     for (int q = 0; q < kTileQ; ++q) {
-        long long e = e0 + q * kBinThreads;
-        if (ck[q] >= 0) {
-            unsigned idx = (unsigned)(e - chunk_base);
-            unsigned pos = S.base[ck[q]] + rank[q];
-            if (pos < (unsigned)A.cap) store_payload(bins + (size_t)ck[q] * A.cap + pos, pa[q], pb[q], idx, fkv[q]);
-            else {                                                 // bin full: raw query to the overflow list
-                unsigned o = atomicAdd(ovf_count, 1u);
-                store_payload(ovf + o, xv[q], qv[q], idx, 0u);
-            }
-        } else if (ck[q] == -2) {
-            double *o = A.out + e * A.ld;
+        const int ql = q * kBinThreads + threadIdx.x;
+        const unsigned pa = s_pay + 32u * ql;
+        const uint4 w1 = lds_v4u32(pa + 16u);
+        if (w1.w == 0xffffffffu) continue;
+        if (w1.w == 0xfffffffeu) {
+            double *o = A.out + (t0 + ql) * A.ld;
             for (int p = 0; p < A.cm.n; ++p) o[p] = qnan();
             ++*err_local;
+            continue;
+        }
+        const double2 ab = lds_v2f64(pa);
+        const unsigned ck = w1.w >> 16, rank = w1.w & 0xffffu;
+        const unsigned pos = lds_u32(s_base + 4u * ck) + rank;
+        if (pos < (unsigned)A.cap) store_payload(bins + (size_t)ck * A.cap + pos, ab.x, ab.y, w1.x, w1.y);
+        else {                                                     // bin full: raw query to the overflow list
+            unsigned o = atomicAdd(ovf_count, 1u);
+            store_payload(ovf + o, __ldg(A.x + t0 + ql), __ldg(A.q2 + t0 + ql), w1.x, 0u);
         }
     }
 }

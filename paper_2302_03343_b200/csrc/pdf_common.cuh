@@ -31,6 +31,7 @@ struct GridDev {
     const double *uk, *sk;        // ln knots (device log: the same routine the queries go through)
     const int *sub_of;            // [nqtot] sub-grid of global knot jg
     const int *qoff;              // [nsub+1]
+    const int *cell_adj;          // [nqtot] 1 on the last knot of a sub-grid (it belongs to the cell below), else 0
     const CellTab *cx;            // [nx-1]
     const CellTab *cq;            // [nqtot], entry jg valid when jg is not the last knot of its sub-grid
     const double *V;
@@ -188,6 +189,14 @@ __device__ __forceinline__ double lowq_continue(double fmin, double fplus, doubl
     double gamma = 1.0;
     if (fmin > 1e-5) gamma = fmax(-2.5, (fplus - fmin) / (0.01 * fmin));
     return fmin * pow(r, (gamma - 1.0) * r + 1.0);
+}
+
+// the same with ln r shared by the 11 flavours of a query: r^e = exp(e ln r) (binned path)
+__device__ __forceinline__ double lowq_continue_ln(double fmin, double fplus, double r, double lnr)
+{
+    double gamma = 1.0;
+    if (fmin > 1e-5) gamma = fmax(-2.5, (fplus - fmin) / (0.01 * fmin));
+    return fmin * exp(((gamma - 1.0) * r + 1.0) * lnr);
 }
 
 // C-6 as a 16-term tensor sum for one flavour column

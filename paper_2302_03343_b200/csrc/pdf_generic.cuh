@@ -103,33 +103,46 @@ k_xfxq2_direct(GridDev G, ColMap cm, long long n, const double *__restrict__ x,
 }
 
 // ---- a-6: alpha_s ----------------------------------------------------------------------------
+// knots, values and per-cell constants staged in shared memory; 4 independent queries per thread
+// and round so that the log / search / Hermite chains of different queries overlap
+constexpr int kAlphasIlp = 4;
+
+__device__ __forceinline__ double alphas_one(const GridDev &G, const double *ak, const double *av, const CellTab *ct,
+                                             double q)
+{
+    const int m = G.na;
+    if (!finite_pos(q)) return qnan();
+    if (q > ak[m - 1]) return av[m - 1];
+    if (q < ak[0])        // L1835 constant (default) or L1746 logarithmic-gradient continuation
+        return G.alphas_mode ? av[0] * pow(q / ak[0], log(av[1] / av[0]) / log(ak[1] / ak[0])) : av[0];
+    int c = find_cell(ak, m, q);
+    CellTab t4 = ct[c];
+    double t = (q == ak[c + 1]) ? 1.0 : (log(q) - t4.lo_log) * t4.inv_d;
+    double w[4];
+    hermite_weights(t, t4, w);
+    int i0 = c > 0 ? c - 1 : c, i3 = c + 2 < m ? c + 2 : c + 1;
+    return fma(w[0], av[i0], fma(w[1], av[c], fma(w[2], av[c + 1], w[3] * av[i3])));
+}
+
 __global__ void __launch_bounds__(256)
 k_alphas(GridDev G, long long n, const double *__restrict__ q2, double *__restrict__ out)
 {
-    extern __shared__ double sm[];
+    extern __shared__ __align__(16) double sm[];
     double *ak = sm;                 // [na] raw knots
     double *av = sm + G.na;          // [na] values
+    CellTab *ct = reinterpret_cast<CellTab *>(sm + 2 * G.na);   // [na-1]
     for (int i = threadIdx.x; i < G.na; i += blockDim.x) { ak[i] = G.ak[i]; av[i] = G.av[i]; }
+    for (int i = threadIdx.x; i < G.na - 1; i += blockDim.x) ct[i] = G.ca[i];
     __syncthreads();
-    long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
-        double q = q2[e];
-        double v;
-        int m = G.na;
-        if (!finite_pos(q)) v = qnan();
-        else if (q > ak[m - 1]) v = av[m - 1];
-        else if (q < ak[0])   // L1835 constant (default) or L1746 logarithmic-gradient continuation
-            v = G.alphas_mode ? av[0] * pow(q / ak[0], log(av[1] / av[0]) / log(ak[1] / ak[0])) : av[0];
-        else {
-            int c = find_cell(ak, m, q);
-            CellTab ct = G.ca[c];
-            double t = (q == ak[c + 1]) ? 1.0 : (log(q) - ct.lo_log) * ct.inv_d;
-            double w[4];
-            hermite_weights(t, ct, w);
-            int i0 = c > 0 ? c - 1 : c, i3 = c + 2 < m ? c + 2 : c + 1;
-            v = fma(w[0], av[i0], fma(w[1], av[c], fma(w[2], av[c + 1], w[3] * av[i3])));
-        }
-        out[e] = v;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long e0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; e0 < n; e0 += stride * kAlphasIlp) {
+        double q[kAlphasIlp], v[kAlphasIlp];
+#pragma unroll
+        for (int k = 0; k < kAlphasIlp; ++k) { long long e = e0 + k * stride; q[k] = e < n ? __ldcs(q2 + e) : 1.0; }
+#pragma unroll
+        for (int k = 0; k < kAlphasIlp; ++k) v[k] = alphas_one(G, ak, av, ct, q[k]);
+#pragma unroll
+        for (int k = 0; k < kAlphasIlp; ++k) { long long e = e0 + k * stride; if (e < n) __stcs(out + e, v[k]); }
     }
 }
 

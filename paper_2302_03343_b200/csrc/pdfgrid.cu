@@ -73,7 +73,7 @@ struct pdf_grid {
     std::vector<int> nq, qoff, pids;
     // owned device allocations
     double *d_xk = nullptr, *d_qk = nullptr, *d_uk = nullptr, *d_sk = nullptr, *d_V = nullptr;
-    int *d_sub_of = nullptr, *d_qoff = nullptr;
+    int *d_sub_of = nullptr, *d_qoff = nullptr, *d_cell_adj = nullptr;
     CellTab *d_cx = nullptr, *d_cq = nullptr, *d_ca = nullptr;
     double *d_ak = nullptr, *d_alk = nullptr, *d_av = nullptr, *d_C = nullptr;
     unsigned long long *d_err = nullptr;
@@ -99,7 +99,7 @@ void free_grid(pdf_grid *g)
 {
     if (!g) return;
     cudaFree(g->d_xk); cudaFree(g->d_qk); cudaFree(g->d_uk); cudaFree(g->d_sk); cudaFree(g->d_V);
-    cudaFree(g->d_sub_of); cudaFree(g->d_qoff); cudaFree(g->d_cx); cudaFree(g->d_cq); cudaFree(g->d_ca);
+    cudaFree(g->d_sub_of); cudaFree(g->d_qoff); cudaFree(g->d_cell_adj); cudaFree(g->d_cx); cudaFree(g->d_cq); cudaFree(g->d_ca);
     cudaFree(g->d_ak); cudaFree(g->d_alk); cudaFree(g->d_av); cudaFree(g->d_C); cudaFree(g->d_err);
     binned_plan_free(g->bplan);
     for (auto &s : g->stage) {
@@ -188,11 +188,11 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
     g->nq.assign(nq, nq + nsub);
     g->pids.assign(flavour_pids, flavour_pids + nflav);
     g->qoff.resize(nsub + 1);
-    std::vector<int> sub_of(tot);
+    std::vector<int> sub_of(tot), cell_adj(tot);
     g->qoff[0] = 0;
     for (int k = 0; k < nsub; ++k) {
         g->qoff[k + 1] = g->qoff[k] + nq[k];
-        for (int j = 0; j < nq[k]; ++j) sub_of[g->qoff[k] + j] = k;
+        for (int j = 0; j < nq[k]; ++j) { sub_of[g->qoff[k] + j] = k; cell_adj[g->qoff[k] + j] = (j == nq[k] - 1) ? 1 : 0; }
     }
     int nfp = (nflav + 1) & ~1;                       // even: 16-byte vector loads of a node row
     size_t vdev = (size_t)nmem * tot * nx * nfp;
@@ -201,7 +201,7 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
 #define TRYC(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { rc = cuda_fail(e__, #call); free_grid(g); return rc; } } while (0)
     TRY(dev_alloc(&g->d_xk, nx)); TRY(dev_alloc(&g->d_uk, nx));
     TRY(dev_alloc(&g->d_qk, tot)); TRY(dev_alloc(&g->d_sk, tot));
-    TRY(dev_alloc(&g->d_sub_of, tot)); TRY(dev_alloc(&g->d_qoff, nsub + 1));
+    TRY(dev_alloc(&g->d_sub_of, tot)); TRY(dev_alloc(&g->d_qoff, nsub + 1)); TRY(dev_alloc(&g->d_cell_adj, tot));
     TRY(dev_alloc(&g->d_cx, nx)); TRY(dev_alloc(&g->d_cq, tot));
     TRY(dev_alloc(&g->d_V, vdev)); TRY(dev_alloc(&g->d_err, 1));
     double *d_src = nullptr;
@@ -209,6 +209,7 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
     TRYC(cudaMemcpy(g->d_xk, x_knots, sizeof(double) * nx, cudaMemcpyHostToDevice));
     TRYC(cudaMemcpy(g->d_qk, q2_knots, sizeof(double) * tot, cudaMemcpyHostToDevice));
     TRYC(cudaMemcpy(g->d_sub_of, sub_of.data(), sizeof(int) * tot, cudaMemcpyHostToDevice));
+    TRYC(cudaMemcpy(g->d_cell_adj, cell_adj.data(), sizeof(int) * tot, cudaMemcpyHostToDevice));
     TRYC(cudaMemcpy(g->d_qoff, g->qoff.data(), sizeof(int) * (nsub + 1), cudaMemcpyHostToDevice));
     TRYC(cudaMemcpy(d_src, values, sizeof(double) * per_mem * nmem, cudaMemcpyHostToDevice));
     TRYC(cudaMemset(g->d_err, 0, sizeof(unsigned long long)));
@@ -237,7 +238,7 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
     GridDev &d = g->d;
     d.nx = nx; d.nsub = nsub; d.nflav = nflav; d.nfp = nfp; d.nmem = nmem; d.nqtot = tot;
     d.xk = g->d_xk; d.qk = g->d_qk; d.uk = g->d_uk; d.sk = g->d_sk;
-    d.sub_of = g->d_sub_of; d.qoff = g->d_qoff; d.cx = g->d_cx; d.cq = g->d_cq;
+    d.sub_of = g->d_sub_of; d.qoff = g->d_qoff; d.cell_adj = g->d_cell_adj; d.cx = g->d_cx; d.cq = g->d_cq;
     d.V = g->d_V; d.memstride = (size_t)tot * nx * nfp;
     d.q2plus = 1.01 * q2_knots[0];
     d.na = 0; d.alphas_mode = PDF_ALPHAS_FREEZE; d.C = nullptr; d.err_count = g->d_err;

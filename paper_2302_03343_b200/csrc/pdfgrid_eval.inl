@@ -75,9 +75,11 @@ int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out,
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device);
     long long want = (n + 255) / 256;
-    unsigned grid = (unsigned)(want < (long long)sms * 16 ? want : (long long)sms * 16);
+    unsigned grid = (unsigned)(want < (long long)sms * 8 ? want : (long long)sms * 8);
     LaunchScope a(s, "k_alphas");
-    k_alphas<<<grid, 256, sizeof(double) * 2 * g->d.na, s>>>(g->d, n, q2, out);
+    size_t smem = sizeof(double) * 2 * g->d.na + sizeof(CellTab) * g->d.na;
+    if (smem > 48 * 1024) return PDF_EINVAL;
+    k_alphas<<<grid, 256, smem, s>>>(g->d, n, q2, out);
     CK(cudaGetLastError());
     return PDF_OK;
 }
