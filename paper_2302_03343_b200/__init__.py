@@ -5,4 +5,4 @@
 ``paper_2302_03343_b200.binding`` thin ctypes binding of libpdfgrid.so (loaded lazily;
                                   raises if the CUDA library is missing - no CPU fallback)
 """
-__all__ = ["synth", "binding"]
+__all__ = ["synth", "binding", "shard"]

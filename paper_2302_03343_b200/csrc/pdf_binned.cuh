@@ -41,14 +41,20 @@ constexpr int kBinWarps = kBinThreads / 32;
 #ifndef PDF_TILEQ
 #define PDF_TILEQ 4
 #endif
+#ifndef PDF_MINB
+#define PDF_MINB 2
+#endif
 #ifndef PDF_LAG
-#define PDF_LAG 1
+#define PDF_LAG 3
 #endif
 constexpr int kTileQ = PDF_TILEQ;                     // queries per thread in an A item
 constexpr int kTileA = kBinThreads * kTileQ;  // 1024 queries per A item
 constexpr int kOvfItems = 4;                  // B items per chunk that drain the overflow list
 constexpr int kLag = PDF_LAG;                       // B(c) tickets follow A(c) tickets by this many rounds
-constexpr int kRing = kLag + 2;               // chunk slots in flight
+#ifndef PDF_RING_EXTRA
+#define PDF_RING_EXTRA 4
+#endif
+constexpr int kRing = kLag + PDF_RING_EXTRA;  // chunk slots in flight: A(c) reuses the slot of B(c-kRing), issued >= 2 rounds earlier
 constexpr int kLowXSplit = 16;                // coarse keys of the low-x classes: bands of Q2 cells
 constexpr int kLutSize = 1024;                // search-acceleration buckets per axis
 constexpr int kNF = 11, kNFP = 12;            // the fast path is specialised for 11 flavours (pad 12)

@@ -154,11 +154,41 @@ __device__ __noinline__ void ovf_item(const StreamArgs &A, int slot, long long c
     }
 }
 
+// ---- interior cells on the FP64 tensor pipe (DMMA m8n8k4) ---------------------------------------
+// A batch is one cell: out[q][f] = sum_n W[q][n] V[n][f] is a (queries x 16 nodes) x (16 nodes x 11
+// flavours) contraction.  As mma.sync.m8n8k4 tiles (8 queries x 8 flavours, k = 4 nodes) the cell's
+// values are read ONCE per batch, 8 doubles per lane, instead of 192 broadcast doubles per lane;
+// DMMA runs on the same FP64 pipe as DFMA, so this buys operand traffic and
+// instruction count, not flops.  Lane (g = lane/4, t = lane%4) serves query g of the 8-query tile.
+// Step r of 4 uses Q2-row (t ^ r) and x-node t:  A[g][t] = wq_g[t^r] wx_g[t],  B[t][n] = V[row t^r][node t][n].
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// node weight number t of the 1-D Hermite operator in the factored form
+//   w_t = (1-s)^2 (c0 + c1 s) + s^2 (c2 + c3 (1-s))        (same weights as hermite_weights)
+struct WCoef { double c0, c1, c2, c3; };
+__device__ __forceinline__ WCoef weight_coef(const CellTab &c, int t)
+{
+    WCoef w;
+    w.c0 = t == 1 ? 1.0 : 0.0;
+    w.c1 = t == 0 ? -c.bL : t == 1 ? 2.0 + c.bL - c.aL : t == 2 ? c.aL : 0.0;
+    w.c2 = t == 2 ? 1.0 : 0.0;
+    w.c3 = t == 1 ? c.aR : t == 2 ? 2.0 - c.aR + c.bR : t == 3 ? -c.bR : 0.0;
+    return w;
+}
+__device__ __forceinline__ double weight_eval(const WCoef &w, double s)
+{
+    double om = 1.0 - s, om2 = om * om, s2 = s * s;
+    return fma(om2, fma(w.c1, s, w.c0), s2 * fma(w.c3, om, w.c2));
+}
+
 struct BSmem {
     uint4 *sP;            // [cap] payloads (2 x uint4 each)
     double *sV;           // [nqt][4][12]
-    double *stage;        // [kBinWarps][32*kNF]
-    unsigned long long *sptr; // [kBinWarps][32] output row pointers of the staged batch
+    unsigned char *bkey;  // [cap/32 + nfk] fine key of every 32-query batch
     int *fcnt;            // [nfk]
     int *foff;            // [nfk+1]
     int *bstart;          // [nfk+1]
@@ -185,8 +215,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
     const unsigned fcnt = (unsigned)__cvta_generic_to_shared(S.fcnt), foff = (unsigned)__cvta_generic_to_shared(S.foff);
     const unsigned bstart = (unsigned)__cvta_generic_to_shared(S.bstart), order = (unsigned)__cvta_generic_to_shared(S.order);
     const unsigned nexta = (unsigned)__cvta_generic_to_shared(S.next);
-    const unsigned stage = (unsigned)__cvta_generic_to_shared(S.stage) + (unsigned)warp * (32 * kNF * 8);
-    const unsigned sptr = (unsigned)__cvta_generic_to_shared(S.sptr) + (unsigned)warp * (32 * 8);
+    const unsigned bkey = (unsigned)__cvta_generic_to_shared(S.bkey);
 
     // stage payloads (coalesced) and the key's 4 grid columns
     for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) {
@@ -233,6 +262,11 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
             carry_b += __shfl_sync(0xffffffffu, sb, 31);
         }
         if (lane == 0) { sts_u32(foff + 4u * B.nfk, (unsigned)carry_o); sts_u32(bstart + 4u * B.nfk, (unsigned)carry_b); }
+        __syncwarp();
+        for (int k = lane; k < B.nfk; k += 32) {           // batch -> fine key table
+            const int b0 = (int)lds_u32(bstart + 4u * k), b1 = (int)lds_u32(bstart + 4u * (k + 1));
+            for (int bb = b0; bb < b1; ++bb) asm volatile("st.shared.u8 [%0], %1;" ::"r"(bkey + (unsigned)bb), "r"(k) : "memory");
+        }
     }
     __syncthreads();
     for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
@@ -243,61 +277,102 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
     __syncthreads();
 
     const int total = (int)lds_u32(bstart + 4u * B.nfk);
+    const WCoef kx = weight_coef(G.cx[i], lane & 3);       // x-axis weight of this lane's node, fixed for the unit
     for (;;) {
         int fb = 0;
         if (lane == 0) fb = (int)atoms_add(nexta, 1u);     // batches are handed out dynamically,
         fb = __shfl_sync(0xffffffffu, fb, 0);              // last keys first: the extrapolation classes
         if (fb >= total) break;                            // (long, few lanes) must not form the tail
         fb = total - 1 - fb;
-        int lo = 0, hi = B.nfk;                            // largest k with bstart[k] <= fb
-        while (hi - lo > 1) {
-            int mid = (lo + hi) >> 1;
-            if ((int)lds_u32(bstart + 4u * mid) <= fb) lo = mid; else hi = mid;
-        }
-        const int fk = lo, kcnt = (int)lds_u32(fcnt + 4u * fk);
+        int fk;
+        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(fk) : "r"(bkey + (unsigned)fb));
+        const int kcnt = (int)lds_u32(fcnt + 4u * fk);
         const int first = (fb - (int)lds_u32(bstart + 4u * fk)) * 32;
         const int nact = min(32, kcnt - first);
+        const unsigned ord0 = order + 2u * (lds_u32(foff + 4u * fk) + first);
+        if (!lowx_unit && fk < B.nqt) {
+            // ---- interior cell (i, fk): DMMA tiles of 8 queries ----
+            const int g = lane >> 2, t = lane & 3;
+            const CellTab cq = G.cq[fk];
+            const WCoef kq = weight_coef(cq, t);
+            const AxisNodes qn = q_nodes(cq, fk);
+            double b0[4], b1[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int tr = t ^ r;
+                const int row = tr == 0 ? qn.n[0] : tr == 1 ? qn.n[1] : tr == 2 ? qn.n[2] : qn.n[3];
+                const unsigned pn = snode(sVa, row, t);
+                b0[r] = lds_f64(pn + 8u * g);
+                b1[r] = g < 4 ? lds_f64(pn + 8u * (8 + g)) : 0.0;
+            }
+            for (int m0 = 0; m0 < nact; m0 += 8) {
+                const int qi = m0 + g;
+                const bool valid = qi < nact;
+                double tx = 0.0, tq = 0.0;
+                unsigned idx = 0;
+                if (valid) {
+                    unsigned short e16;
+                    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * qi));
+                    const unsigned pe = sPa + 32u * e16;
+                    const double2 ab = lds_v2f64(pe);
+                    tx = ab.x; tq = ab.y;
+                    idx = lds_u32(pe + 16u);
+                }
+                const double wx = valid ? weight_eval(kx, tx) : 0.0;
+                const double wq0 = weight_eval(kq, tq);
+                const double wq1 = __shfl_xor_sync(0xffffffffu, wq0, 1);
+                const double wq2 = __shfl_xor_sync(0xffffffffu, wq0, 2);
+                const double wq3 = __shfl_xor_sync(0xffffffffu, wq0, 3);
+                double d00 = 0.0, d01 = 0.0, d10 = 0.0, d11 = 0.0;
+                const double a0 = wq0 * wx, a1 = wq1 * wx, a2 = wq2 * wx, a3 = wq3 * wx;
+                dmma884(d00, d01, a0, b0[0]); dmma884(d10, d11, a0, b1[0]);
+                dmma884(d00, d01, a1, b0[1]); dmma884(d10, d11, a1, b1[1]);
+                dmma884(d00, d01, a2, b0[2]); dmma884(d10, d11, a2, b1[2]);
+                dmma884(d00, d01, a3, b0[3]); dmma884(d10, d11, a3, b1[3]);
+                if (valid) {                               // lane holds flavours 2t, 2t+1, 8+2t, 9+2t of its query
+                    double *rp = A.out + (chunk_base + idx) * A.ld;
+                    if (A.identity) {
+                        rp[2 * t] = d00; rp[2 * t + 1] = d01;
+                        if (t < 2) rp[8 + 2 * t] = d10;
+                        if (t == 0) rp[9] = d11;
+                    } else {
+                        for (int p = 0; p < A.cm.n; ++p) {
+                            const int c = A.cm.col[p];
+                            if (c < 0) { if (t == 0) rp[p] = 0.0; continue; }
+                            if (((c & 7) >> 1) == t) rp[p] = (c & 8) ? ((c & 1) ? d11 : d10) : ((c & 1) ? d01 : d00);
+                        }
+                    }
+                }
+            }
+            continue;
+        }
+        // ---- extrapolation classes: one query per lane, broadcast operands ----
         const bool active = lane < nact;
         double pa = 0.0, pb = 0.0;
         unsigned idx = 0;
         if (active) {
             unsigned short e16;
-            asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(order + 2u * (lds_u32(foff + 4u * fk) + first + lane)));
+            asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * lane));
             const unsigned pe = sPa + 32u * e16;
             double2 ab = lds_v2f64(pe);
             pa = ab.x; pb = ab.y;
             idx = lds_u32(pe + 16u);
         }
         double acc[kNF];
-        if (!lowx_unit && fk < B.nqt) eval_interior_s(G, sVa, i, fk, pa, pb, acc);
-        else eval_extrap_s(G, B, sVa, lowx_unit, i, fk, pa, pb, acc);
-        // transpose through shared memory so that whole rows leave in contiguous pieces
+        eval_extrap_s(G, B, sVa, lowx_unit, i, fk, pa, pb, acc);
+        if (active) {                                      // 5 % of the queries: one row per lane
+            double *rp = A.out + (chunk_base + idx) * A.ld;
+            if (A.identity) {
 #pragma unroll
-        for (int f = 0; f < kNF; ++f) sts_f64(stage + 8u * (lane * kNF + f), acc[f]);
-        {
-            unsigned long long rp = reinterpret_cast<unsigned long long>(A.out + (chunk_base + idx) * A.ld);
-            asm volatile("st.shared.u64 [%0], %1;" ::"r"(sptr + 8u * lane), "l"(rp) : "memory");
-        }
-        __syncwarp();
-        if (A.identity) {
-            const int tot = nact * kNF;
+                for (int f = 0; f < kNF; ++f) rp[f] = acc[f];
+            } else {
+                for (int p = 0; p < A.cm.n; ++p) {
+                    const int c = A.cm.col[p];
+                    double v = 0.0;
 #pragma unroll
-            for (int itx = 0; itx < kNF; ++itx) {
-                int e = itx * 32 + lane;
-                if (e < tot) {
-                    int r = (e * 745) >> 13, p = e - r * kNF;          // e / 11 for e < 352
-                    unsigned long long rp;
-                    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(rp) : "r"(sptr + 8u * r));
-                    reinterpret_cast<double *>(rp)[p] = lds_f64(stage + 8u * e);
+                    for (int f = 0; f < kNF; ++f) v = c == f ? acc[f] : v;
+                    rp[p] = v;
                 }
-            }
-        } else {
-            const int np = A.cm.n, tot = nact * np;
-            for (int e = lane; e < tot; e += 32) {
-                int r = e / np, p = e - r * np, c = A.cm.col[p];
-                unsigned long long rp;
-                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(rp) : "r"(sptr + 8u * r));
-                reinterpret_cast<double *>(rp)[p] = c < 0 ? 0.0 : lds_f64(stage + 8u * (r * kNF + c));
             }
         }
         __syncwarp();
@@ -313,15 +388,14 @@ __host__ __device__ inline size_t bsmem_item_bytes(int nqt, int nck, int nfk, in
 {
     size_t b = (size_t)cap * 32;                                        // sP
     b += (size_t)nqt * 4 * kNFP * sizeof(double);                       // sV
-    b += (size_t)kBinWarps * 32 * kNF * sizeof(double);                 // stage
-    b += (size_t)kBinWarps * 32 * sizeof(unsigned long long);           // sptr
+    b += ((size_t)(cap / 32 + nfk) + 15) / 16 * 16;                     // bkey
     b += (size_t)(3 * nfk + 8) * sizeof(int);                           // fcnt, foff, bstart, next
     b += ((size_t)cap * sizeof(unsigned short) + 15) / 16 * 16;         // order
     size_t a = (size_t)kTileA * 32 + (size_t)2 * nck * sizeof(unsigned); // A items: payloads, cnt, base
     return (b > a ? b : a) + 32;
 }
 
-__global__ void __launch_bounds__(kBinThreads, 2) k_pdf_stream(const __grid_constant__ StreamArgs A)
+__global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __grid_constant__ StreamArgs A)
 {
     extern __shared__ __align__(32) unsigned char smem_raw[];
     double *s_xk = reinterpret_cast<double *>(smem_raw);
@@ -344,13 +418,12 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_pdf_stream(const __grid_cons
     BSmem SB;
     SB.sP = reinterpret_cast<uint4 *>(region);
     SB.sV = reinterpret_cast<double *>(region + (size_t)A.cap * 32);
-    SB.stage = SB.sV + (size_t)A.G.nqtot * 4 * kNFP;
-    SB.sptr = reinterpret_cast<unsigned long long *>(SB.stage + kBinWarps * 32 * kNF);
-    SB.fcnt = reinterpret_cast<int *>(SB.sptr + kBinWarps * 32);
+    SB.fcnt = reinterpret_cast<int *>(SB.sV + (size_t)A.G.nqtot * 4 * kNFP);
     SB.foff = SB.fcnt + A.B.nfk + 1;
     SB.bstart = SB.foff + A.B.nfk + 1;
     SB.next = SB.bstart + A.B.nfk + 2;
     SB.order = reinterpret_cast<unsigned short *>(SB.next + 2);
+    SB.bkey = reinterpret_cast<unsigned char *>(SB.order + ((A.cap + 7) & ~7));
 
     unsigned long long *ctrl = A.W.ctrl;
     const unsigned long long TA = A.ta, TB = A.B.nitems, per = TA + TB;

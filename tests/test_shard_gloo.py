@@ -1,0 +1,61 @@
+"""N > 1 host logic on CPU: two gloo ranks shard a query range, evaluate their shares with the
+oracle and the concatenation equals the single-rank result; the job time is the max over ranks."""
+import os
+import socket
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2302_03343_b200 import shard, synth
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, n, outdir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle
+    oracle.build()
+    spec = synth.grid_c0()
+    x, q = synth.queries_inside(spec, n, seed=123, strict=True)
+    lo, hi = shard.shard_range(n, rank, world)
+    og = oracle.OracleGrid(spec.x_knots.numpy(), [t.numpy() for t in spec.q2_subgrids], spec.values.numpy(), spec.pids)
+    part = og.xfxq2(spec.pids, x[lo:hi].numpy(), q[lo:hi].numpy())
+    np.save(os.path.join(outdir, f"part{rank}.npy"), part)
+    ranges = [None] * world
+    dist.all_gather_object(ranges, (lo, hi))
+    tmax = shard.max_over_ranks(dist, 1.0 + rank)
+    if rank == 0:
+        np.save(os.path.join(outdir, "meta.npy"), np.array([r for ab in ranges for r in ab] + [tmax]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_ranks_tile_the_queries(tmp_path, oracle_mod):
+    n, world = 20_001, 2
+    mp.spawn(_worker, args=(world, _free_port(), n, str(tmp_path)), nprocs=world, join=True)
+    meta = np.load(tmp_path / "meta.npy")
+    assert list(meta[:4]) == [0, 10_001, 10_001, n] and meta[4] == 2.0
+    spec = synth.grid_c0()
+    x, q = synth.queries_inside(spec, n, seed=123, strict=True)
+    og = oracle_mod.OracleGrid(spec.x_knots.numpy(), [t.numpy() for t in spec.q2_subgrids], spec.values.numpy(), spec.pids)
+    full = og.xfxq2(spec.pids, x.numpy(), q.numpy())
+    got = np.concatenate([np.load(tmp_path / f"part{r}.npy") for r in range(world)])
+    assert np.array_equal(full, got)
+
+
+def test_shard_range_properties():
+    for n in (0, 1, 7, 100, 1_000_003):
+        for world in (1, 2, 3, 8):
+            edges = [shard.shard_range(n, r, world) for r in range(world)]
+            assert edges[0][0] == 0 and edges[-1][1] == n
+            assert all(edges[r][1] == edges[r + 1][0] for r in range(world - 1))
+            sizes = [b - a for a, b in edges]
+            assert max(sizes) - min(sizes) <= 1
