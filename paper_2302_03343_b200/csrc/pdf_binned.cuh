@@ -105,14 +105,24 @@ inline long long binned_chunk(const BinnedPlan &p, long long n, long long chunk_
     return c < need ? c : need;
 }
 
-// bin capacity per (chunk, coarse key): a uniform cloud puts chunk/ncx queries on an x cell
-// (1344 at 256k and 195 cells); 1.125x that + 96 (~ +7 sigma) keeps overflow to skewed inputs
-inline int binned_cap(const BinnedPlan &p, long long chunk)
+// shared-memory segment of a B item: a uniform cloud puts chunk/ncx queries on an x cell (1344 at
+// 256k and 195 cells); 1.125x that + 96 (~ +7 sigma) lets such a bin go through in one segment
+inline int binned_scap(const BinnedPlan &p, long long chunk)
 {
     long long c = chunk / (p.dev.ncx > 0 ? p.dev.ncx : 1);
     c = c + c / 8 + 96;
     c = (c + 31) / 32 * 32;
     if (c > kMaxCap) c = kMaxCap;
+    return (int)c;
+}
+// bin capacity in the workspace: 4x the uniform share, so that narrower clouds (configs[4] covers
+// 2/3 of the x range; VEGAS-like peaks) still bin; beyond it queries overflow to the generic path
+inline int binned_cap(const BinnedPlan &p, long long chunk)
+{
+    long long c = 4 * (chunk / (p.dev.ncx > 0 ? p.dev.ncx : 1)) + 256;
+    c = (c + 31) / 32 * 32;
+    if (c > chunk) c = chunk;
+    if (c < binned_scap(p, chunk)) c = binned_scap(p, chunk);
     return (int)c;
 }
 

@@ -206,7 +206,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
     unsigned *counts = A.W.counts + (size_t)slot * B.nck;
     unsigned cnt_u = __ldcg(counts + ck);
     if (cnt_u == 0u) return;                               // uniform over the CTA
-    const int cnt = cnt_u > (unsigned)A.cap ? A.cap : (int)cnt_u;
+    const int cnt_all = cnt_u > (unsigned)A.cap ? A.cap : (int)cnt_u;
     const uint4 *bin = reinterpret_cast<const uint4 *>(A.W.bins + ((size_t)slot * B.nck + ck) * A.cap);
     const bool lowx_unit = ck >= B.ncx;
     const int i = lowx_unit ? 0 : ck;
@@ -217,11 +217,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
     const unsigned nexta = (unsigned)__cvta_generic_to_shared(S.next);
     const unsigned bkey = (unsigned)__cvta_generic_to_shared(S.bkey);
 
-    // stage payloads (coalesced) and the key's 4 grid columns
-    for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) {
-        uint4 v = __ldcg(bin + e);
-        sts_v4u32(sPa + 16u * e, v.x, v.y, v.z, v.w);
-    }
+    // stage the key's 4 grid columns once
     {
         int c0, c1, c2, c3;
         if (lowx_unit) { c0 = 0; c1 = 1; c2 = 0; c3 = 1; }
@@ -234,6 +230,14 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
             double2 v = __ldg(V2 + ((size_t)jg * G.nx + col) * 6 + p);
             sts_v2f64(sVa + 16u * e, v.x, v.y);
         }
+    }
+    // the bin is processed in segments of at most A.scap payloads (what fits in shared memory)
+    for (int s0 = 0; s0 < cnt_all; s0 += A.scap) {
+    const int cnt = min(A.scap, cnt_all - s0);
+    if (s0) __syncthreads();                               // the previous segment's batches are done
+    for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) {
+        uint4 v = __ldcg(bin + 2 * s0 + e);
+        sts_v4u32(sPa + 16u * e, v.x, v.y, v.z, v.w);
     }
     for (int k = threadIdx.x; k < B.nfk; k += kBinThreads) sts_u32(fcnt + 4u * k, 0u);
     if (threadIdx.x == 0) sts_u32(nexta, 0u);
@@ -377,6 +381,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
         }
         __syncwarp();
     }
+    }   // segments
     __syncthreads();
     if (threadIdx.x == 0) counts[ck] = 0u;                 // the bin is empty again for the ring
 }
@@ -417,13 +422,13 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
     SA.base = SA.cnt + A.B.nck;
     BSmem SB;
     SB.sP = reinterpret_cast<uint4 *>(region);
-    SB.sV = reinterpret_cast<double *>(region + (size_t)A.cap * 32);
+    SB.sV = reinterpret_cast<double *>(region + (size_t)A.scap * 32);
     SB.fcnt = reinterpret_cast<int *>(SB.sV + (size_t)A.G.nqtot * 4 * kNFP);
     SB.foff = SB.fcnt + A.B.nfk + 1;
     SB.bstart = SB.foff + A.B.nfk + 1;
     SB.next = SB.bstart + A.B.nfk + 2;
     SB.order = reinterpret_cast<unsigned short *>(SB.next + 2);
-    SB.bkey = reinterpret_cast<unsigned char *>(SB.order + ((A.cap + 7) & ~7));
+    SB.bkey = reinterpret_cast<unsigned char *>(SB.order + ((A.scap + 7) & ~7));
 
     unsigned long long *ctrl = A.W.ctrl;
     const unsigned long long TA = A.ta, TB = A.B.nitems, per = TA + TB;

@@ -86,19 +86,61 @@ inline int binned_plan_init(BinnedPlan &p, const GridDev &G, const std::vector<d
 }
 
 inline bool binned_qualifies(const BinnedPlan &p, const ColMap &, const int *member) { return p.usable && !member; }
-inline bool binned_lumi_qualifies(const BinnedPlan &) { return false; }
+// ---- luminosity on top of the binned path ------------------------------------------------------
+// pdf_lumi in slices of kLumiSlice events: xf(x1,Q2) and xf(x2,Q2) of the slice by two runs of the
+// persistent binned kernel into two scratch arrays, then k_lumi_combine reduces the 11 x 11 coupling
+// per event in registers.  The per-flavour values of a slice make one round trip through the
+// scratch (L2 / HBM); the fused single-kernel form is k_lumi_direct (PDF_PATH_DIRECT).
+constexpr long long kLumiSlice = 1 << 20;
+
+struct CouplingParam { double c[kNF * kNF]; };            // passed by value: constant-bank operands
+
+__global__ void __launch_bounds__(256)
+k_lumi_combine(const __grid_constant__ CouplingParam C, long long n, const double *__restrict__ f1,
+               const double *__restrict__ f2, const double *__restrict__ x1, const double *__restrict__ x2,
+               const double *__restrict__ w, double *__restrict__ out, unsigned long long *err_count)
+{
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const double a = __ldcs(x1 + e), b = __ldcs(x2 + e);
+    double h[kNF];
+    const double inv_b = 1.0 / b, inv_a = 1.0 / a;
+#pragma unroll
+    for (int j = 0; j < kNF; ++j) h[j] = __ldcs(f2 + e * kNF + j) * inv_b;
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < kNF; ++i) {
+        double row = 0.0;
+#pragma unroll
+        for (int j = 0; j < kNF; ++j) row = fma(C.c[i * kNF + j], h[j], row);
+        acc = fma(__ldcs(f1 + e * kNF + i) * inv_a, row, acc);
+    }
+    const double v = __ldcs(w + e) * acc;
+    if (!(finite_pos(a) && finite_pos(b)) || v != v) {
+        // an invalid parton made its whole row NaN (C-10); the event counts once
+        if (isnan(__ldcs(f1 + e * kNF)) || isnan(__ldcs(f2 + e * kNF))) { atomicAdd(err_count, 1ULL); out[e] = qnan(); return; }
+    }
+    out[e] = v;
+}
+
+inline bool binned_lumi_qualifies(const BinnedPlan &p) { return p.usable; }
+inline size_t binned_lumi_scratch_bytes(const BinnedPlan &p)
+{
+    return p.usable ? (size_t)2 * kLumiSlice * kNF * sizeof(double) + 512 : 0;
+}
 
 // one memset + one persistent kernel for the whole call
 template <typename Scope>
 inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm, long long n, const double *x,
                         const double *q2, double *out, long long ld, void *ws, size_t ws_bytes, long long chunk_opt,
-                        cudaStream_t s)
+                        cudaStream_t s, int count_err = 1)
 {
     if (binned_workspace_bytes(p, n, chunk_opt) > ws_bytes) return PDF_EWORKSPACE;
     StreamArgs A;
     A.G = G; A.B = p.dev; A.cm = cm;
     A.chunk = binned_chunk(p, n, chunk_opt);
     A.cap = binned_cap(p, A.chunk);
+    A.scap = binned_scap(p, A.chunk);
     binned_carve(p, ws, A.chunk, A.cap, A.W);
     A.x = x; A.q2 = q2; A.out = out; A.n = n; A.ld = ld;
     A.nchunks = (int)((n + A.chunk - 1) / A.chunk);
@@ -106,12 +148,13 @@ inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm,
     A.identity = cm.n == kNF;
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
     A.zfill = (ld == cm.n) ? 1 : 0;
+    A.count_err = count_err;
 #ifdef PDF_NOZFILL
     A.zfill = 0;
 #endif
     size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts + ovf_count
     if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
-    size_t smem = binned_smem_bytes(G.nx, G.nqtot, p.dev.nck, p.dev.nfk, A.cap);
+    size_t smem = binned_smem_bytes(G.nx, G.nqtot, p.dev.nck, p.dev.nfk, A.scap);
     int per_sm = 0, dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -127,7 +170,33 @@ inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm,
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }
 
-inline int binned_lumi(const GridDev &, const BinnedPlan &, long long, const double *, const double *, const double *,
-                       const double *, double *, void *, size_t, long long, cudaStream_t) { return PDF_EINVAL; }
+template <typename Scope>
+inline int binned_lumi(const GridDev &G, const BinnedPlan &p, const double *hostC, long long n, const double *x1,
+                       const double *x2, const double *q2, const double *w, double *out, void *ws, size_t ws_bytes,
+                       long long chunk_opt, cudaStream_t s)
+{
+    const long long slice = n < kLumiSlice ? n : kLumiSlice;
+    const size_t ws_x = binned_workspace_bytes(p, slice, chunk_opt);
+    if (ws_x + binned_lumi_scratch_bytes(p) > ws_bytes) return PDF_EWORKSPACE;
+    double *f1 = reinterpret_cast<double *>(align_up((size_t)ws + ws_x, 256));
+    double *f2 = f1 + kLumiSlice * kNF;
+    ColMap cm; cm.n = kNF;
+    for (int f = 0; f < kNF; ++f) cm.col[f] = f;
+    CouplingParam C;
+    for (int k = 0; k < kNF * kNF; ++k) C.c[k] = hostC[k];
+    for (long long off = 0; off < n; off += slice) {
+        const long long m = n - off < slice ? n - off : slice;
+        int rc = binned_xfxq2<Scope>(G, p, cm, m, x1 + off, q2 + off, f1, kNF, ws, ws_x, chunk_opt, s, 0);
+        if (rc) return rc;
+        rc = binned_xfxq2<Scope>(G, p, cm, m, x2 + off, q2 + off, f2, kNF, ws, ws_x, chunk_opt, s, 0);
+        if (rc) return rc;
+        {
+            Scope sc(s, "k_lumi_combine");
+            k_lumi_combine<<<(unsigned)((m + 255) / 256), 256, 0, s>>>(C, m, f1, f2, x1 + off, x2 + off, w + off, out + off,
+                                                                      G.err_count);
+        }
+    }
+    return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
+}
 
 }  // namespace pdfg

@@ -14,8 +14,10 @@ struct StreamArgs {
     long long n, ld;
     long long chunk;           // queries per chunk (multiple of kTileA)
     int nchunks, ta, cap;      // chunks, A items per chunk, bin capacity per (chunk, coarse key)
+    int scap;                  // payloads a B item holds in shared memory at a time (segment size)
     int identity;              // 1: requested columns == the grid's 11 columns in order
     int zfill;                 // 1: rows are contiguous (ld == npid): A items zero-fill their tile of `out`
+    int count_err;             // 1: invalid queries bump the grid's error counter (0 inside pdf_lumi)
 };
 
 // ---- small device helpers ----------------------------------------------------------------------
@@ -226,7 +228,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         if (w1.w == 0xfffffffeu) {
             double *o = A.out + (t0 + ql) * A.ld;
             for (int p = 0; p < A.cm.n; ++p) o[p] = qnan();
-            ++*err_local;
+            if (A.count_err) ++*err_local;
             continue;
         }
         const double2 ab = lds_v2f64(pa);

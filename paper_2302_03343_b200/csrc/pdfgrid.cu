@@ -77,7 +77,7 @@ struct pdf_grid {
     CellTab *d_cx = nullptr, *d_cq = nullptr, *d_ca = nullptr;
     double *d_ak = nullptr, *d_alk = nullptr, *d_av = nullptr, *d_C = nullptr;
     unsigned long long *d_err = nullptr;
-    std::vector<double> h_av, h_ak;
+    std::vector<double> h_av, h_ak, h_C;
     // caller-owned workspace of the binned path
     void *ws = nullptr; size_t ws_bytes = 0;
     int path = PDF_PATH_AUTO;
@@ -283,6 +283,7 @@ int pdf_grid_set_coupling(pdf_grid *g, const double *C)
     if (!g->d_C) { int rc = dev_alloc(&g->d_C, n); if (rc) return rc; }
     CK(cudaMemcpy(g->d_C, C, sizeof(double) * n, cudaMemcpyHostToDevice));
     g->d.C = g->d_C;
+    g->h_C.assign(C, C + n);
     return PDF_OK;
 }
 

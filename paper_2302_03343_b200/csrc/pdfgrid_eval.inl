@@ -62,7 +62,9 @@ int pdf_xfxq2(const pdf_grid *g, const int *pids, int npid, long long n, const d
 size_t pdf_workspace_bytes(const pdf_grid *g, long long n)
 {
     if (!g || n < 0) return 0;
-    return binned_workspace_bytes(g->bplan, n, g->chunk);
+    size_t b = binned_workspace_bytes(g->bplan, n, g->chunk);
+    if (b && g->d.C) b += binned_lumi_scratch_bytes(g->bplan) + 256;    // pdf_lumi slices (only once a coupling is set)
+    return b;
 }
 
 int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out, void *stream)
@@ -97,7 +99,7 @@ int pdf_lumi(const pdf_grid *g, long long n, const double *x1, const double *x2,
                        (g->path == PDF_PATH_BINNED || (g->path == PDF_PATH_AUTO && g->ws && n >= kAutoMinN &&
                                                        g->ws_bytes >= pdf_workspace_bytes(g, n)));
     if (want_binned)
-        return binned_lumi(g->d, g->bplan, n, x1, x2, q2, weights, out, g->ws, g->ws_bytes, g->chunk, s);
+        return binned_lumi<LaunchScope>(g->d, g->bplan, g->h_C.data(), n, x1, x2, q2, weights, out, g->ws, g->ws_bytes, g->chunk, s);
     const long long slice = 1LL << 30;
     for (long long off = 0; off < n; off += slice) {
         long long m = n - off < slice ? n - off : slice;
