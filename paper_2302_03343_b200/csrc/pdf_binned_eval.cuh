@@ -12,7 +12,7 @@ namespace pdfg {
 __device__ __forceinline__ double2 lds_d2(unsigned addr)
 {
     double2 v;
-    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
     return v;
 }
 
@@ -139,7 +139,7 @@ __device__ __noinline__ void eval_extrap_s(const GridDev &G, const BinDev &B, un
 // overflow list: raw queries evaluated by the generic per-thread code (rare; register-capped)
 __device__ __noinline__ void ovf_item(const StreamArgs &A, int slot, long long chunk_base, int part)
 {
-    unsigned cnt = __ldcg(A.W.ovf_count + slot);
+    unsigned cnt = ld_acquire_u32(A.W.ovf_count + slot);
     const Payload *ovf = A.W.ovf + (size_t)slot * A.chunk;
     for (unsigned e = part * kBinThreads + threadIdx.x; e < cnt; e += kOvfItems * kBinThreads) {
         double2 ab = __ldcg(reinterpret_cast<const double2 *>(ovf + e));
@@ -204,8 +204,14 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
     if (item >= B.nck) { ovf_item(A, slot, chunk_base, item - B.nck); return; }
     const int ck = item;
     unsigned *counts = A.W.counts + (size_t)slot * B.nck;
-    unsigned cnt_u = __ldcg(counts + ck);
-    if (cnt_u == 0u) return;                               // uniform over the CTA
+    // one thread reads the count and the CTA takes that value: every later branch and barrier count
+    // of the item depends on it, so it must be the same in all 256 threads
+    const unsigned nexta0 = (unsigned)__cvta_generic_to_shared(S.next);
+    if (threadIdx.x == 0) sts_u32(nexta0 + 4u, ld_acquire_u32(counts + ck));
+    cta_sync();
+    const unsigned cnt_u = lds_u32(nexta0 + 4u);
+    cta_sync();
+    if (cnt_u == 0u) return;
     const int cnt_all = cnt_u > (unsigned)A.cap ? A.cap : (int)cnt_u;
     const uint4 *bin = reinterpret_cast<const uint4 *>(A.W.bins + ((size_t)slot * B.nck + ck) * A.cap);
     const bool lowx_unit = ck >= B.ncx;
@@ -234,21 +240,22 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
     // the bin is processed in segments of at most A.scap payloads (what fits in shared memory)
     for (int s0 = 0; s0 < cnt_all; s0 += A.scap) {
     const int cnt = min(A.scap, cnt_all - s0);
-    if (s0) __syncthreads();                               // the previous segment's batches are done
+    if (s0) cta_sync();                               // the previous segment's batches are done
     for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) {
         uint4 v = __ldcg(bin + 2 * s0 + e);
         sts_v4u32(sPa + 16u * e, v.x, v.y, v.z, v.w);
     }
     for (int k = threadIdx.x; k < B.nfk; k += kBinThreads) sts_u32(fcnt + 4u * k, 0u);
     if (threadIdx.x == 0) sts_u32(nexta, 0u);
-    __syncthreads();
+    cta_sync();
     // counting sort by fine key: rank kept in the payload's spare word
     for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
         unsigned fk = lds_u32(sPa + 32u * e + 20u);
+        PDF_ASSERT(fk < (unsigned)B.nfk);
         unsigned r = atoms_add(fcnt + 4u * fk, 1u);
         sts_u32(sPa + 32u * e + 24u, r);
     }
-    __syncthreads();
+    cta_sync();
     if (warp == 0) {                                       // exclusive scans: slots and 32-query batches per key
         int carry_o = 0, carry_b = 0;
         for (int k0 = 0; k0 < B.nfk; k0 += 32) {
@@ -272,13 +279,14 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
             for (int bb = b0; bb < b1; ++bb) asm volatile("st.shared.u8 [%0], %1;" ::"r"(bkey + (unsigned)bb), "r"(k) : "memory");
         }
     }
-    __syncthreads();
+    cta_sync();
     for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
         uint2 w = make_uint2(lds_u32(sPa + 32u * e + 20u), lds_u32(sPa + 32u * e + 24u));
         unsigned pos = lds_u32(foff + 4u * w.x) + w.y;
+        PDF_ASSERT(w.x < (unsigned)B.nfk && pos < (unsigned)cnt);
         asm volatile("st.shared.u16 [%0], %1;" ::"r"(order + 2u * pos), "h"((unsigned short)e) : "memory");
     }
-    __syncthreads();
+    cta_sync();
 
     const int total = (int)lds_u32(bstart + 4u * B.nfk);
     const WCoef kx = weight_coef(G.cx[i], lane & 3);       // x-axis weight of this lane's node, fixed for the unit
@@ -289,8 +297,9 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
         if (fb >= total) break;                            // (long, few lanes) must not form the tail
         fb = total - 1 - fb;
         int fk;
-        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(fk) : "r"(bkey + (unsigned)fb));
+        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(fk) : "r"(bkey + (unsigned)fb) : "memory");
         const int kcnt = (int)lds_u32(fcnt + 4u * fk);
+        PDF_ASSERT(fk >= 0 && fk < B.nfk && fb >= 0 && fb < A.scap / 32 + B.nfk);
         const int first = (fb - (int)lds_u32(bstart + 4u * fk)) * 32;
         const int nact = min(32, kcnt - first);
         const unsigned ord0 = order + 2u * (lds_u32(foff + 4u * fk) + first);
@@ -316,7 +325,8 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
                 unsigned idx = 0;
                 if (valid) {
                     unsigned short e16;
-                    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * qi));
+                    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * qi) : "memory");
+                    PDF_ASSERT(e16 < cnt);
                     const unsigned pe = sPa + 32u * e16;
                     const double2 ab = lds_v2f64(pe);
                     tx = ab.x; tq = ab.y;
@@ -334,6 +344,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
                 dmma884(d00, d01, a2, b0[2]); dmma884(d10, d11, a2, b1[2]);
                 dmma884(d00, d01, a3, b0[3]); dmma884(d10, d11, a3, b1[3]);
                 if (valid) {                               // lane holds flavours 2t, 2t+1, 8+2t, 9+2t of its query
+                    PDF_ASSERT(chunk_base + idx < A.n);
                     double *rp = A.out + (chunk_base + idx) * A.ld;
                     if (A.identity) {
                         rp[2 * t] = d00; rp[2 * t + 1] = d01;
@@ -356,7 +367,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
         unsigned idx = 0;
         if (active) {
             unsigned short e16;
-            asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * lane));
+            asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * lane) : "memory");
             const unsigned pe = sPa + 32u * e16;
             double2 ab = lds_v2f64(pe);
             pa = ab.x; pb = ab.y;
@@ -382,7 +393,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
         __syncwarp();
     }
     }   // segments
-    __syncthreads();
+    cta_sync();
     if (threadIdx.x == 0) counts[ck] = 0u;                 // the bin is empty again for the ring
 }
 
@@ -414,7 +425,7 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
     for (int i = threadIdx.x; i < A.G.nx; i += kBinThreads) s_xk[i] = A.G.xk[i];
     for (int i = threadIdx.x; i < A.G.nqtot; i += kBinThreads) s_qk[i] = A.G.qk[i];
     for (int i = threadIdx.x; i < kLutSize; i += kBinThreads) { s_lutx[i] = A.B.lutx[i]; s_lutq[i] = A.B.lutq[i]; }
-    __syncthreads();
+    cta_sync();
     SmemTables T{s_xk, s_qk, s_lutx, s_lutq};
     ASmem SA;
     SA.pay = reinterpret_cast<uint4 *>(region);
@@ -440,9 +451,9 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
     if (threadIdx.x == 0) next_t = atomicAdd(ctrl, 1ULL);
     for (;;) {
         if (threadIdx.x == 0) s_ticket = next_t;
-        __syncthreads();
+        cta_sync();
         const unsigned long long t = s_ticket;
-        __syncthreads();
+        cta_sync();
         if (t >= total) break;
         if (threadIdx.x == 0) next_t = atomicAdd(ctrl, 1ULL);      // consumed at the top of the next round
         // ticket order, lag L = kLag rounds:  round r = [A(r) tiles | B(r-L) items]; B(c) is handed out
@@ -470,18 +481,20 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
         unsigned long long *a_done = ctrl + 8 + slot * 4, *b_fin = a_done + 1, *b_done = a_done + 2;
         const long long chunk_base = c * A.chunk;
         if (isA) {
-            if (threadIdx.x == 0 && gen > 0) wait_counter(b_done, gen * TB);   // ring slot drained
-            __syncthreads();
+            // the whole warp polls (same address): a lane that spins alone would reach the barrier
+            // below apart from its warp, and bar.sync counts such a warp twice
+            if (threadIdx.x < 32 && gen > 0) wait_counter(b_done, gen * TB);   // ring slot drained
+            cta_sync();
             a_item(A, T, SA, slot, chunk_base, sub, &err_local);
             __threadfence();
-            __syncthreads();
+            cta_sync();
             if (threadIdx.x == 0) atomicAdd(a_done, 1ULL);
         } else {
-            if (threadIdx.x == 0) wait_counter(a_done, (gen + 1) * TA);        // every tile of A(c) released
-            __syncthreads();
+            if (threadIdx.x < 32) wait_counter(a_done, (gen + 1) * TA);        // every tile of A(c) released
+            cta_sync();
             b_item(A, SB, slot, chunk_base, sub);
             __threadfence();
-            __syncthreads();
+            cta_sync();
             if (threadIdx.x == 0) {
                 unsigned long long old = atomicAdd(b_fin, 1ULL);
                 if (old + 1 == (gen + 1) * TB) {                               // last item of the chunk

@@ -2,7 +2,17 @@
 // (see pdf_binned.cuh for the design).
 #pragma once
 
+#ifdef PDF_CHECKS
+#include <assert.h>
+#endif
+
 namespace pdfg {
+
+#ifdef PDF_CHECKS
+#define PDF_ASSERT(c) assert(c)
+#else
+#define PDF_ASSERT(c) ((void)0)
+#endif
 
 struct StreamArgs {
     GridDev G;
@@ -21,17 +31,48 @@ struct StreamArgs {
 };
 
 // ---- small device helpers ----------------------------------------------------------------------
+// CTA barrier of this kernel.  The shared-memory traffic around it is issued through inline PTX
+// (st.shared / atom.shared / ld.shared with explicit shared-window addresses); without the block
+// fence a warp was observed to read counters after the barrier that the other warps' atom.shared
+// had not finished updating (cold launches, 80-register builds).  The fence makes every prior
+// shared-memory operation of the warp performed before it arrives; cost: one MEMBAR.CTA.
+__device__ __forceinline__ void cta_sync()
+{
+    __threadfence_block();
+    __syncwarp();
+    __syncthreads();
+}
+
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p)
 {
     unsigned long long v;
+#ifdef PDF_RELAXED_POLL
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+#else
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+#endif
     return v;
 }
 
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
+{
+    unsigned v;
+#ifdef PDF_RELAXED_POLL
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+#else
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+#endif
+    return v;
+}
+
+// called by all 32 lanes of one warp (converged): lane 0's view decides, so the warp leaves the loop together
 __device__ __forceinline__ void wait_counter(const unsigned long long *p, unsigned long long target)
 {
     unsigned ns = 32;
-    while (ld_acquire_u64(p) < target) {
+    for (;;) {
+        unsigned long long v = ld_acquire_u64(p);
+        v = __shfl_sync(0xffffffffu, v, 0);
+        if (v >= target) break;
         __nanosleep(ns);
         if (ns < 1024) ns <<= 1;
     }
@@ -68,16 +109,16 @@ struct SmemTables {
 };
 // explicit shared-window accessors (32-bit addresses): the compiler cannot prove the address space
 // of pointers that travel through structs and would emit generic loads
-__device__ __forceinline__ double lds_f64(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
-__device__ __forceinline__ unsigned lds_u32(unsigned a) { unsigned v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
-__device__ __forceinline__ int lds_s16(unsigned a) { short v; asm volatile("ld.shared.s16 %0, [%1];" : "=h"(v) : "r"(a)); return (int)v; }
+__device__ __forceinline__ double lds_f64(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ unsigned lds_u32(unsigned a) { unsigned v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ int lds_s16(unsigned a) { short v; asm volatile("ld.shared.s16 %0, [%1];" : "=h"(v) : "r"(a) : "memory"); return (int)v; }
 __device__ __forceinline__ double2 lds_v2f64(unsigned a)
 {
-    double2 v; asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a)); return v;
+    double2 v; asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a) : "memory"); return v;
 }
 __device__ __forceinline__ uint4 lds_v4u32(unsigned a)
 {
-    uint4 v; asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v;
+    uint4 v; asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory"); return v;
 }
 __device__ __forceinline__ void sts_u32(unsigned a, unsigned v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 __device__ __forceinline__ void sts_f64(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
@@ -154,7 +195,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
     if (t1 > A.n) t1 = A.n;
     if (t1 > chunk_base + A.chunk) t1 = chunk_base + A.chunk;
     ZeroFill zf = zero_fill_plan(A.out, A.ld, t0, A.zfill ? t1 : t0);
-    __syncthreads();
+    cta_sync();
 
     // rolled loop (small code, no register arrays); the next query's inputs are fetched one round ahead
     double xn = -1.0, qn = -1.0;
@@ -202,9 +243,10 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
                     tb = q2 / qmin;                                // r (C-9)
                 }
                 fk = lowq ? (unsigned)nqt : highq ? (unsigned)nqt + 1u : (unsigned)jg;
-                // low-x classes: one coarse key per band of Q2 cells, so that their batches fill up
-                const unsigned band = lowq ? 0u : highq ? (unsigned)(kLowXSplit - 1) : (unsigned)(jg * kLowXSplit) / (unsigned)nqt;
-                const unsigned ck = lowx ? (unsigned)B.ncx + band : (unsigned)i;
+                unsigned ck = (unsigned)i;
+                if (lowx)       // low-x classes: one coarse key per band of Q2 cells, so that their batches fill up
+                    ck = (unsigned)B.ncx + (lowq ? 0u : highq ? (unsigned)(kLowXSplit - 1) : (unsigned)(jg * kLowXSplit) / (unsigned)nqt);
+                PDF_ASSERT(ck < (unsigned)B.nck && fk < (unsigned)B.nfk);
                 const unsigned rank = atoms_add(s_cnt + 4u * ck, 1u);
                 tag = (ck << 16) | rank;
             }
@@ -213,12 +255,12 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         sts_v2f64(pa, ta, tb);
         sts_v4u32(pa + 16u, (unsigned)(e - chunk_base), fk, 0u, tag);
     }
-    __syncthreads();
+    cta_sync();
     for (int k = threadIdx.x; k < B.nck; k += kBinThreads) {       // one global atomic per (tile, key)
         unsigned c = lds_u32(s_cnt + 4u * k);
         sts_u32(s_base + 4u * k, c ? atomicAdd(counts + k, c) : 0u);
     }
-    __syncthreads();
+    cta_sync();
 #pragma unroll 1
     for (int q = 0; q < kTileQ; ++q) {
         const int ql = q * kBinThreads + threadIdx.x;
@@ -233,6 +275,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         }
         const double2 ab = lds_v2f64(pa);
         const unsigned ck = w1.w >> 16, rank = w1.w & 0xffffu;
+        PDF_ASSERT(ck < (unsigned)B.nck);
         const unsigned pos = lds_u32(s_base + 4u * ck) + rank;
         if (pos < (unsigned)A.cap) store_payload(bins + (size_t)ck * A.cap + pos, ab.x, ab.y, w1.x, w1.y);
         else {                                                     // bin full: raw query to the overflow list

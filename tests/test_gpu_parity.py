@@ -297,3 +297,16 @@ def test_binned_ring_reuse_and_overflow(B, oracle_mod):
     ref, S = og.xfxq2(spec.pids, xs.numpy(), qs.numpy(), want_scale=True)
     out = g.pdf_xfxq2(spec.pids, xs.cuda(), qs.cuda()).cpu().numpy()
     assert_values(out, ref, S, "skew")
+
+
+@pytest.mark.parametrize("n", [262_144, 1_000_003])
+def test_binned_first_calls_in_a_fresh_process(n):
+    """regression: shared-memory atomics of the binned kernel were read across a barrier before they
+    had landed, only when the pipeline's waits were really taken (first calls of a process)"""
+    import os
+    import subprocess
+    import sys
+    script = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cold_check.py")
+    for _ in range(2):
+        r = subprocess.run([sys.executable, script, str(n)], capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
