@@ -2,8 +2,8 @@
 //
 // Why: a query needs a 4x4 stencil x 11 flavours = 1408 B of grid data.  Gathered per lane that
 // is >= 12 clk/query/SM of L1 / shared-memory bandwidth, 2.5x the HBM and FP64 budgets, so the
-// lanes of a warp must share a cell and take the stencil as BROADCAST operands from shared memory
-// (LDS.128 with one address: 1.5 clk).  With ~10^4 cells that needs a sort domain of >= 10^5
+// lanes of a warp must share a cell: its values then come from shared memory as tensor-pipe
+// fragments (interior cells) or broadcast operands (LDS.128 with one address: 1.5 clk).  With ~10^4 cells that needs a sort domain of >= 10^5
 // queries, which no CTA holds on chip: queries are binned through L2 in chunks.
 //
 // What the machine dictates (measured on this B200):
@@ -16,20 +16,22 @@
 //          scattered row stores of B then merge into valid L2-resident sectors (2.7 ms -> in
 //          budget), and every line still leaves L2 for HBM once.
 //
-// How: ONE persistent kernel per call, CTAs pull tickets in the order (lag kLag = 1)
-//      A(0) | A(1) B(0) | A(2) B(1) | ... | B(last)
+// How: ONE persistent kernel per call, CTAs pull tickets in the order (lag kLag = 3 rounds)
+//      round r = [ A(r) tiles | B(r-3) items ]
 //   A(c), one item per 1024 queries of chunk c: read x,q2 (coalesced), classify, locate the cell,
 //      t_x,t_q (the two logs), coarse/fine key, tile-local counting sort by coarse key, payload
 //      stores; zero-fill of the tile's output rows.
 //   B(c), one item per coarse key: copy the key's payloads and its 4 grid columns (4 x nq x 96 B)
 //      to shared memory, counting-sort by FINE key (the Q2 cell or the extrapolation class), then
-//      warps take batches of <= 32 same-cell queries: Hermite weights, 16-node x 11-flavour FMA
-//      sum with broadcast LDS.128, rows transposed through shared memory and stored.
-// B(c) waits (acquire-spin) until every tile of A(c) has been released; by ticket order those
-// tiles were claimed a whole stage earlier, so the wait is normally zero and cannot deadlock (all
-// CTAs are co-resident; a ticket only waits on lower tickets).  Bins live in a ring of kRing chunk
-// slots.  Queries that do not fit their bin (capacity per chunk and key) go to an overflow list
-// that the generic per-thread code evaluates: correctness never depends on the distribution.
+//      warps take batches of <= 32 same-cell queries.  Interior cells: FP64 mma.sync (DMMA m8n8k4)
+//      tiles of 8 queries x 8 flavours over the 16 nodes, rows stored straight from the accumulator
+//      fragments.  Extrapolation classes: one query per lane with broadcast LDS.128 operands.
+// B(c) waits (acquire-spin by one whole warp) until every tile of A(c) has been released; by
+// ticket order those tiles were claimed three rounds earlier, so the wait is normally zero and
+// cannot deadlock (all CTAs are co-resident; a ticket only waits on lower tickets).  Bins live in
+// a ring of kRing chunk slots.  Queries that do not fit their bin (capacity per chunk and key) go
+// to an overflow list that the generic per-thread code evaluates: correctness never depends on
+// the distribution.
 #pragma once
 #include "pdf_common.cuh"
 #include "pdf_generic.cuh"
