@@ -338,13 +338,14 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
                                 "sample": f"first {ns} queries of this run's C2 batch, xfxq2 (11 flavours) + alphas, {dt:.1f} s"}
         # sampled parity at full size, in the timed launch configuration (oracle one by one on the sample)
         import numpy as np
-        got = out_sample.cpu().numpy()
-        _, S = og.xfxq2(spec.pids, cx[:200_000], cq[:200_000], want_scale=True)
-        err = np.abs(got[:200_000] - ref[:200_000])
-        tol = 1e-12 * np.abs(ref[:200_000]) + 1e-14 * S
-        okn = ~np.isnan(ref[:200_000])
-        line["parity_sample"] = {"n": 200_000, "worst_err_over_tol": float(np.max(err[okn] / np.maximum(tol[okn], 1e-300))),
-                                 "nan_match": bool(np.array_equal(np.isnan(got[:200_000]), ~okn))}
+        np_ = min(200_000, ns)
+        got = out_sample.cpu().numpy()[:np_]
+        _, S = og.xfxq2(spec.pids, cx[:np_], cq[:np_], want_scale=True)
+        err = np.abs(got - ref[:np_])
+        tol = 1e-12 * np.abs(ref[:np_]) + 1e-14 * S
+        okn = ~np.isnan(ref[:np_])
+        line["parity_sample"] = {"n": np_, "worst_err_over_tol": float(np.max(err[okn] / np.maximum(tol[okn], 1e-300))),
+                                 "nan_match": bool(np.array_equal(np.isnan(got), ~okn))}
 
 
 def main():

@@ -91,7 +91,7 @@ inline bool binned_qualifies(const BinnedPlan &p, const ColMap &, const int *mem
 // persistent binned kernel into two scratch arrays, then k_lumi_combine reduces the 11 x 11 coupling
 // per event in registers.  The per-flavour values of a slice make one round trip through the
 // scratch (L2 / HBM); the fused single-kernel form is k_lumi_direct (PDF_PATH_DIRECT).
-constexpr long long kLumiSlice = 1 << 20;
+constexpr long long kLumiSlice = 1 << 22;
 
 struct CouplingParam { double c[kNF * kNF]; };            // passed by value: constant-bank operands
 
