@@ -28,6 +28,8 @@ if ROOT not in sys.path:
 
 METRIC = "PDF evaluations (points x flavours)/s"
 UNIT = "points*flavours/s"
+WORKLOAD = ("configs[2] (C2): 196x(6+8+40) LHAPDF-shaped grid, 11 flavours, "
+            "5% of queries extrapolated, + alpha_s over the same Q2 (60 knots)")
 BYTES_PER_QUERY = 16 + 88          # x, q2 in; 11 fp64 out
 BYTES_PER_EVENT = 32 + 8
 BYTES_PER_ALPHAS = 16
@@ -127,7 +129,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": "configs[2] (C2): LHAPDF-shaped grid, 5% extrapolated + alpha_s",
+            "data": "synthetic", "config": {"workload": WORKLOAD,
                                             "queries_per_step": n, "l2": "n/a (CPU)"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                              "sample": f"first {n} queries of the C2 recipe per step, xfxq2 (11 flavours) + alphas"},
@@ -235,8 +237,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[2] (C2): 196x(6+8+40) LHAPDF-shaped grid, 11 flavours, "
-                                   "5% of queries extrapolated, + alpha_s over the same Q2 (60 knots)",
+            "config": {"workload": WORKLOAD,
                        "queries_per_gpu_per_step": n, "path": args.path, "n_invalid": n_invalid,
                        "l2": "inputs (1.6 GB) and outputs (9.6 GB) per step exceed the 126 MB L2; no flush needed"},
             "clocks": clocks, "gpu_launches": launches, "kernels": table, "roofline": roof}
