@@ -68,8 +68,11 @@ enum { PDF_ALPHAS_FREEZE = 0, PDF_ALPHAS_LOGGRAD = 1 };
 /* evaluation strategy of pdf_xfxq2 / pdf_lumi (pdf_grid_set_option(PDF_OPT_PATH, ...)) */
 enum {
     PDF_PATH_AUTO = 0,    /* binned when a workspace is attached and the call qualifies, else direct */
-    PDF_PATH_DIRECT = 1,  /* one thread per query, stencil gathered through L1/L2                   */
-    PDF_PATH_BINNED = 2   /* queries binned by cell so that warps share one stencil (needs workspace) */
+    PDF_PATH_DIRECT = 1,  /* one thread per query, stencil gathered through L1/L2; pdf_lumi: one fused
+                             kernel, the per-flavour values never leave the registers               */
+    PDF_PATH_BINNED = 2   /* queries binned by cell so that warps share one stencil (needs workspace;
+                             11-flavour single-member grids, no member array); pdf_lumi: sliced binned
+                             evaluation of both partons into workspace scratch + a combine kernel     */
 };
 enum { PDF_OPT_PATH = 1, PDF_OPT_ALPHAS_MODE = 2, PDF_OPT_CHUNK = 3 };
 
@@ -95,7 +98,9 @@ int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double
 /* flavour-pair coupling C, HOST [nflav][nflav] row-major, in the grid's column order; eq. 4.1 */
 int pdf_grid_set_coupling(pdf_grid *g, const double *C);
 /* caller-owned DEVICE scratch for the binned path; must stay valid until replaced or the grid is
- * destroyed; bytes >= pdf_workspace_bytes(g, n) for the largest n it will be used with.
+ * destroyed; bytes >= pdf_workspace_bytes(g, n) for the largest n it will be used with (the
+ * figure grows by the luminosity scratch once a coupling has been set, so query it after
+ * pdf_grid_set_coupling).  The contents are scratch: one evaluation call at a time may use it.
  * dev_ptr == NULL detaches. */
 int pdf_grid_set_workspace(pdf_grid *g, void *dev_ptr, size_t bytes);
 size_t pdf_workspace_bytes(const pdf_grid *g, long long n);
