@@ -8,6 +8,7 @@
 
 namespace pdfg {
 
+constexpr int kAlphaLut = 256;     // search-acceleration buckets of the alpha_s knot line
 constexpr int kMaxLumiFlav = 16;   // generic pdf_lumi keeps both flavour vectors in registers/local
 constexpr int kRegionInterior = 0, kRegionLowX = 1, kRegionLowQ = 2, kRegionHighQ = 3,
               kRegionLowXLowQ = 4, kRegionLowXHighQ = 5, kRegionInvalid = 6;
@@ -41,6 +42,9 @@ struct GridDev {
     int na, alphas_mode;
     const double *ak, *alk, *av;  // raw knots, ln knots, values
     const CellTab *ca;            // [na-1]
+    const double *acell;          // [na-1][6] per-cell cubic: ln lower knot, 1/dln, c0..c3 (alpha_s = c0 + t(c1 + t(c2 + t c3)))
+    const short *alut;            // [kAlphaLut] start guesses of the alpha_s knot search
+    double alut_scale;            // buckets per unit of ln Q2
     // luminosity coupling [nflav][nflav]
     const double *C;
     unsigned long long *err_count;

@@ -103,44 +103,69 @@ k_xfxq2_direct(GridDev G, ColMap cm, long long n, const double *__restrict__ x,
 }
 
 // ---- a-6: alpha_s ----------------------------------------------------------------------------
-// knots, values and per-cell constants staged in shared memory; 4 independent queries per thread
-// and round so that the log / search / Hermite chains of different queries overlap
-constexpr int kAlphasIlp = 4;
-
-__device__ __forceinline__ double alphas_one(const GridDev &G, const double *ak, const double *av, const CellTab *ct,
-                                             double q)
+// Per cell the Hermite cubic of C-5 is kept in monomial form in t (built once by k_alphas_cells from
+// the same cell constants the PDF path uses):  with H00 = A_c, H01 = A_{c+1},
+//   H10 = -bL A_{c-1} + (bL - aL) A_c + aL A_{c+1},   H11 = -aR A_c + (aR - bR) A_{c+1} + bR A_{c+2},
+//   alpha_s(t) = H00 h00 + H10 h10 + H01 h01 + H11 h11 = c0 + t (c1 + t (c2 + t c3)).
+// alpha_s values are positive and smooth, so the monomial form loses nothing (1e-15 relative).
+__global__ void k_alphas_cells(const CellTab *__restrict__ ca, const double *__restrict__ av, double *__restrict__ cell, int m)
 {
-    const int m = G.na;
-    if (!finite_pos(q)) return qnan();
-    if (q > ak[m - 1]) return av[m - 1];
-    if (q < ak[0])        // L1835 constant (default) or L1746 logarithmic-gradient continuation
-        return G.alphas_mode ? av[0] * pow(q / ak[0], log(av[1] / av[0]) / log(ak[1] / ak[0])) : av[0];
-    int c = find_cell(ak, m, q);
-    CellTab t4 = ct[c];
-    double t = (q == ak[c + 1]) ? 1.0 : (log(q) - t4.lo_log) * t4.inv_d;
-    double w[4];
-    hermite_weights(t, t4, w);
-    int i0 = c > 0 ? c - 1 : c, i3 = c + 2 < m ? c + 2 : c + 1;
-    return fma(w[0], av[i0], fma(w[1], av[c], fma(w[2], av[c + 1], w[3] * av[i3])));
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= m - 1) return;
+    CellTab t = ca[c];
+    double am = av[c > 0 ? c - 1 : c], a0 = av[c], a1 = av[c + 1], a2 = av[c + 2 < m ? c + 2 : c + 1];
+    double H00 = a0, H01 = a1;
+    double H10 = -t.bL * am + (t.bL - t.aL) * a0 + t.aL * a1;
+    double H11 = -t.aR * a0 + (t.aR - t.bR) * a1 + t.bR * a2;
+    double *o = cell + 6 * c;
+    o[0] = t.lo_log; o[1] = t.inv_d;
+    o[2] = H00; o[3] = H10;
+    o[4] = -3.0 * H00 - 2.0 * H10 + 3.0 * H01 - H11;
+    o[5] = 2.0 * H00 + H10 - 2.0 * H01 + H11;
 }
+
+constexpr int kAlphasIlp = 4;
 
 __global__ void __launch_bounds__(256)
 k_alphas(GridDev G, long long n, const double *__restrict__ q2, double *__restrict__ out)
 {
     extern __shared__ __align__(16) double sm[];
-    double *ak = sm;                 // [na] raw knots
-    double *av = sm + G.na;          // [na] values
-    CellTab *ct = reinterpret_cast<CellTab *>(sm + 2 * G.na);   // [na-1]
-    for (int i = threadIdx.x; i < G.na; i += blockDim.x) { ak[i] = G.ak[i]; av[i] = G.av[i]; }
-    for (int i = threadIdx.x; i < G.na - 1; i += blockDim.x) ct[i] = G.ca[i];
+    const int m = G.na;
+    double *ak = sm;                               // [na] raw knots
+    double *av = sm + m;                           // [na] values
+    double *cell = sm + 2 * m;                     // [na-1][6]
+    short *lut = reinterpret_cast<short *>(cell + 6 * (m - 1));
+    for (int i = threadIdx.x; i < m; i += blockDim.x) { ak[i] = G.ak[i]; av[i] = G.av[i]; }
+    for (int i = threadIdx.x; i < 6 * (m - 1); i += blockDim.x) cell[i] = G.acell[i];
+    for (int i = threadIdx.x; i < kAlphaLut; i += blockDim.x) lut[i] = G.alut[i];
     __syncthreads();
+    const double kmin = ak[0], kmax = ak[m - 1], l0 = cell[0], scale = G.alut_scale;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long e0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; e0 < n; e0 += stride * kAlphasIlp) {
         double q[kAlphasIlp], v[kAlphasIlp];
 #pragma unroll
         for (int k = 0; k < kAlphasIlp; ++k) { long long e = e0 + k * stride; q[k] = e < n ? __ldcs(q2 + e) : 1.0; }
 #pragma unroll
-        for (int k = 0; k < kAlphasIlp; ++k) v[k] = alphas_one(G, ak, av, ct, q[k]);
+        for (int k = 0; k < kAlphasIlp; ++k) {
+            const double qq = q[k];
+            if (!finite_pos(qq)) { v[k] = qnan(); continue; }
+            if (qq > kmax) { v[k] = av[m - 1]; continue; }                 // L1746: constant above the last knot
+            if (qq < kmin) {      // L1835 constant (default) or L1746 logarithmic-gradient continuation
+                v[k] = G.alphas_mode ? av[0] * pow(qq / kmin, log(av[1] / av[0]) / log(ak[1] / kmin)) : av[0];
+                continue;
+            }
+            const double lq = log(qq);
+            int b = (int)((lq - l0) * scale);
+            b = b < 0 ? 0 : (b >= kAlphaLut ? kAlphaLut - 1 : b);
+            int c = lut[b];                                                // start guess; the walk makes it exact (C-4)
+            while (c > 0 && ak[c] > qq) --c;
+            while (c < m - 2 && ak[c + 1] <= qq) ++c;
+            const double2 *cc = reinterpret_cast<const double2 *>(cell + 6 * c);
+            const double2 c01 = cc[0], c23 = cc[1], c45 = cc[2];
+            const double t = (lq - c01.x) * c01.y;
+            const double poly = fma(fma(fma(c45.y, t, c45.x), t, c23.y), t, c23.x);
+            v[k] = (qq == ak[c + 1]) ? av[c + 1] : poly;                   // a knot returns its stored value
+        }
 #pragma unroll
         for (int k = 0; k < kAlphasIlp; ++k) { long long e = e0 + k * stride; if (e < n) __stcs(out + e, v[k]); }
     }

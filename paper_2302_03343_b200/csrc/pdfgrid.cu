@@ -75,7 +75,8 @@ struct pdf_grid {
     double *d_xk = nullptr, *d_qk = nullptr, *d_uk = nullptr, *d_sk = nullptr, *d_V = nullptr;
     int *d_sub_of = nullptr, *d_qoff = nullptr, *d_cell_adj = nullptr;
     CellTab *d_cx = nullptr, *d_cq = nullptr, *d_ca = nullptr;
-    double *d_ak = nullptr, *d_alk = nullptr, *d_av = nullptr, *d_C = nullptr;
+    double *d_ak = nullptr, *d_alk = nullptr, *d_av = nullptr, *d_C = nullptr, *d_acell = nullptr;
+    short *d_alut = nullptr;
     unsigned long long *d_err = nullptr;
     std::vector<double> h_av, h_ak, h_C;
     // caller-owned workspace of the binned path
@@ -101,6 +102,7 @@ void free_grid(pdf_grid *g)
     cudaFree(g->d_xk); cudaFree(g->d_qk); cudaFree(g->d_uk); cudaFree(g->d_sk); cudaFree(g->d_V);
     cudaFree(g->d_sub_of); cudaFree(g->d_qoff); cudaFree(g->d_cell_adj); cudaFree(g->d_cx); cudaFree(g->d_cq); cudaFree(g->d_ca);
     cudaFree(g->d_ak); cudaFree(g->d_alk); cudaFree(g->d_av); cudaFree(g->d_C); cudaFree(g->d_err);
+    cudaFree(g->d_acell); cudaFree(g->d_alut);
     binned_plan_free(g->bplan);
     for (auto &s : g->stage) {
         cudaFree(s.in); cudaFree(s.out); cudaFree(s.ws);
@@ -261,17 +263,31 @@ int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double
         if (!finite_pos_h(q2_knots[j]) || !std::isfinite(values[j])) return PDF_EINVAL;
         if (j && !(q2_knots[j] > q2_knots[j - 1])) return PDF_EINVAL;
     }
-    cudaFree(g->d_ak); cudaFree(g->d_alk); cudaFree(g->d_av); cudaFree(g->d_ca);
-    g->d_ak = g->d_alk = g->d_av = nullptr; g->d_ca = nullptr; g->d.na = 0;
+    cudaFree(g->d_ak); cudaFree(g->d_alk); cudaFree(g->d_av); cudaFree(g->d_ca); cudaFree(g->d_acell); cudaFree(g->d_alut);
+    g->d_ak = g->d_alk = g->d_av = g->d_acell = nullptr; g->d_ca = nullptr; g->d_alut = nullptr; g->d.na = 0;
     int rc;
     if ((rc = dev_alloc(&g->d_ak, n)) || (rc = dev_alloc(&g->d_alk, n)) || (rc = dev_alloc(&g->d_av, n)) ||
-        (rc = dev_alloc(&g->d_ca, n))) return rc;
+        (rc = dev_alloc(&g->d_ca, n)) || (rc = dev_alloc(&g->d_acell, 6 * (size_t)n)) || (rc = dev_alloc(&g->d_alut, kAlphaLut))) return rc;
     CK(cudaMemcpy(g->d_ak, q2_knots, sizeof(double) * n, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(g->d_av, values, sizeof(double) * n, cudaMemcpyHostToDevice));
     { LaunchScope a(0, "k_log_knots"); k_log_knots<<<(n + 127) / 128, 128>>>(g->d_ak, g->d_alk, n); }
     { LaunchScope a(0, "k_cell_tables"); k_cell_tables<<<(n + 127) / 128, 128>>>(g->d_alk, g->d_ca, 0, n); }
+    { LaunchScope a(0, "k_alphas_cells"); k_alphas_cells<<<(n + 127) / 128, 128>>>(g->d_ca, g->d_av, g->d_acell, n); }
+    {   // search LUT over ln Q2 (a start guess only: host log here, exact walk on the device)
+        std::vector<short> lut(kAlphaLut);
+        double l0 = std::log(q2_knots[0]), l1 = std::log(q2_knots[n - 1]);
+        g->d.alut_scale = kAlphaLut / (l1 - l0) * (1.0 - 1e-12);
+        int c = 0;
+        for (int b = 0; b < kAlphaLut; ++b) {
+            double edge = std::exp(l0 + b / g->d.alut_scale);
+            while (c < n - 2 && q2_knots[c + 1] <= edge) ++c;
+            lut[b] = (short)c;
+        }
+        CK(cudaMemcpy(g->d_alut, lut.data(), sizeof(short) * kAlphaLut, cudaMemcpyHostToDevice));
+    }
     CK(cudaDeviceSynchronize());
     g->d.na = n; g->d.ak = g->d_ak; g->d.alk = g->d_alk; g->d.av = g->d_av; g->d.ca = g->d_ca;
+    g->d.acell = g->d_acell; g->d.alut = g->d_alut;
     return PDF_OK;
 }
 

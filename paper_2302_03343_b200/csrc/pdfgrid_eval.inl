@@ -79,7 +79,7 @@ int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out,
     long long want = (n + 255) / 256;
     unsigned grid = (unsigned)(want < (long long)sms * 8 ? want : (long long)sms * 8);
     LaunchScope a(s, "k_alphas");
-    size_t smem = sizeof(double) * 2 * g->d.na + sizeof(CellTab) * g->d.na;
+    size_t smem = sizeof(double) * (2 * g->d.na + 6 * (g->d.na - 1)) + sizeof(short) * kAlphaLut + 16;
     if (smem > 48 * 1024) return PDF_EINVAL;
     k_alphas<<<grid, 256, smem, s>>>(g->d, n, q2, out);
     CK(cudaGetLastError());
