@@ -30,6 +30,9 @@ METRIC = "PDF evaluations (points x flavours)/s"
 UNIT = "points*flavours/s"
 WORKLOAD = ("configs[2] (C2): 196x(6+8+40) LHAPDF-shaped grid, 11 flavours, "
             "5% of queries extrapolated, + alpha_s over the same Q2 (60 knots)")
+# dram__bytes_read.sum + dram__bytes_write.sum of k_pdf_stream at n = 1e8 (C2), one ncu capture of this
+# command line: profiles/r1g_traffic_pdf_stream_1e8.csv; null for any other n
+NCU_TRAFFIC_BYTES_1E8 = 5426908416 + 21800476160
 BYTES_PER_QUERY = 16 + 88          # x, q2 in; 11 fp64 out
 BYTES_PER_EVENT = 32 + 8
 BYTES_PER_ALPHAS = 16
@@ -232,7 +235,9 @@ def run_ours(args):
     table = kernel_table(prof, args.steps)
     value = world * n * 11 * args.steps / secs
     xf_kernels = [k for k in table if k != "k_alphas"]
-    roof = roofline_hbm(table, xf_kernels, BYTES_PER_QUERY * n, peak_gbs, peak_src)
+    roof = roofline_hbm(table, xf_kernels, BYTES_PER_QUERY * n, peak_gbs, peak_src,
+                        traffic=NCU_TRAFFIC_BYTES_1E8 if (n == 100_000_000 and args.path != "direct") else None)
+    roof["algorithmic_bytes"] = BYTES_PER_QUERY * n
     roof["alphas"] = roofline_hbm(table, ["k_alphas"], BYTES_PER_ALPHAS * n, peak_gbs, peak_src)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True,
