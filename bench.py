@@ -281,6 +281,8 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
                                                 "nominal 64 DFMA/clk/SM x 148 SMs x 1.965 GHz x 2 = 37.2",
                                  "flops_per_event": flops_event,
                                  "hbm_frac": BYTES_PER_EVENT * nl / (lms * 1e-3) / 1e9 / peak_gbs if lms else None}}
+    lumi_sample = (x1[:50_000].cpu().numpy(), x2[:50_000].cpu().numpy(), ql[:50_000].cpu().numpy(),
+                   w[:50_000].cpu().numpy(), lout[:50_000].clone().cpu().numpy())
     del x1, x2, ql, w
 
     # ---- a-8: replica batch, configs[3] (100 members) ------------------------------------------
@@ -331,6 +333,7 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
 
     # ---- cpu_baseline: the oracle as it stands on the host cores (rank 0, N = 1 only) ----------
     if rank == 0 and world == 1:
+        import numpy as np
         import oracle
         ns = min(args.cpu_sample, n)
         og = oracle.OracleGrid(spec.x_knots.numpy(), [q.numpy() for q in spec.q2_subgrids], spec.values.numpy(), spec.pids)
@@ -344,6 +347,14 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
                                 "sample": f"first {ns} queries of this run's C2 batch, xfxq2 (11 flavours) + alphas, {dt:.1f} s"}
         # sampled parity at full size, in the timed launch configuration (oracle one by one on the sample)
         import numpy as np
+        # the same for the luminosity call (50 000 sampled events of the 1e8 launch)
+        og.set_coupling(spec.coupling.numpy())
+        lref, ls = og.lumi(*lumi_sample[:4], want_scale=True)
+        lerr = np.abs(lumi_sample[4] - lref)
+        ltol = 1e-12 * np.abs(lref) + 1e-14 * ls
+        lok = ~np.isnan(lref)
+        line["lumi"]["parity_sample"] = {"n": int(lref.size), "worst_err_over_tol": float(np.max(lerr[lok] / np.maximum(ltol[lok], 1e-300))),
+                                         "nan_match": bool(np.array_equal(np.isnan(lumi_sample[4]), ~lok))}
         np_ = min(200_000, ns)
         got = out_sample.cpu().numpy()[:np_]
         _, S = og.xfxq2(spec.pids, cx[:np_], cq[:np_], want_scale=True)
