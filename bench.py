@@ -289,7 +289,7 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
     nm = args.members_n
     if nm > 0:
         mspec = synth.grid_c1(nmem=100)
-        mg = binding.PdfGrid.from_spec(mspec)
+        mg = binding.PdfGrid.from_spec(mspec, workspace_for=nm)
         mem = synth.members(mspec, nm, device="cuda")
         secs, _, prof, launches = timed_steps(
             torch, dist, world, lambda: mg.pdf_xfxq2(mspec.pids, x[:nm], q2[:nm], out=out[:nm], member=mem), steps, warm)

@@ -157,4 +157,5 @@ inline void binned_carve(const BinnedPlan &p, void *ws, long long chunk, int cap
 }  // namespace pdfg
 
 #include "pdf_binned_kernel.cuh"
+#include "pdf_members.cuh"
 #include "pdf_binned_host.cuh"

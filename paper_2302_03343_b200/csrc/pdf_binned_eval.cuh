@@ -137,7 +137,7 @@ __device__ __noinline__ void eval_extrap_s(const GridDev &G, const BinDev &B, un
 }
 
 // overflow list: raw queries evaluated by the generic per-thread code (rare; register-capped)
-__device__ __noinline__ void ovf_item(const StreamArgs &A, int slot, long long chunk_base, int part)
+__device__ __noinline__ void ovf_item(const StreamArgs &A, const double *V, int slot, long long chunk_base, int part)
 {
     unsigned cnt = ld_acquire_u32(A.W.ovf_count + slot);
     const Payload *ovf = A.W.ovf + (size_t)slot * A.chunk;
@@ -149,7 +149,7 @@ __device__ __noinline__ void ovf_item(const StreamArgs &A, int slot, long long c
         double *o = A.out + (chunk_base + ii.x) * A.ld;
         for (int p = 0; p < A.cm.n; ++p) {
             int c = A.cm.col[p];
-            o[p] = c < 0 ? 0.0 : plan_value(A.G, A.G.V, P, c);
+            o[p] = c < 0 ? 0.0 : plan_value(A.G, V, P, c);
         }
     }
 }
@@ -197,11 +197,11 @@ struct BSmem {
 };
 
 // ---- B item: one coarse key of one chunk ------------------------------------------------------
-__device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int slot, long long chunk_base, int item)
+__device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, const double *V, int slot, long long chunk_base, int item)
 {
     const BinDev &B = A.B;
     const GridDev &G = A.G;
-    if (item >= B.nck) { ovf_item(A, slot, chunk_base, item - B.nck); return; }
+    if (item >= B.nck) { ovf_item(A, V, slot, chunk_base, item - B.nck); return; }
     const int ck = item;
     unsigned *counts = A.W.counts + (size_t)slot * B.nck;
     // one thread reads the count and the CTA takes that value: every later branch and barrier count
@@ -228,7 +228,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, int 
         int c0, c1, c2, c3;
         if (lowx_unit) { c0 = 0; c1 = 1; c2 = 0; c3 = 1; }
         else { c0 = i > 0 ? i - 1 : i; c1 = i; c2 = i + 1; c3 = i + 2 < G.nx ? i + 2 : i + 1; }
-        const double2 *V2 = reinterpret_cast<const double2 *>(G.V);
+        const double2 *V2 = reinterpret_cast<const double2 *>(V);
         const int tot = G.nqtot * 24;                      // double2 units: rows x 4 slots x 6
         for (int e = threadIdx.x; e < tot; e += kBinThreads) {
             int jg = e / 24, r = e - jg * 24, a = r / 6, p = r - a * 6;
@@ -443,7 +443,8 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
 
     unsigned long long *ctrl = A.W.ctrl;
     const unsigned long long TA = A.ta, TB = A.B.nitems, per = TA + TB;
-    const unsigned long long total = (unsigned long long)A.nchunks * per;
+    const int nchunks = A.ctab ? __ldg(A.nchunks_dev) : A.nchunks;
+    const unsigned long long total = (unsigned long long)nchunks * per;
     unsigned long long err_local = 0;
 
     // the next ticket is fetched while the current item runs (a global atomic is ~1 us)
@@ -460,8 +461,8 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
         // L rounds after A(c), so its tiles were claimed >= L waves earlier and the wait below is ~never taken
         bool isA; long long c; int sub;
         {
-            const unsigned long long RA = (unsigned long long)(A.nchunks < kLag ? A.nchunks : kLag);   // A-only rounds
-            const unsigned long long F = (unsigned long long)A.nchunks - RA;                             // full rounds
+            const unsigned long long RA = (unsigned long long)(nchunks < kLag ? nchunks : kLag);   // A-only rounds
+            const unsigned long long F = (unsigned long long)nchunks - RA;                             // full rounds
             if (t < RA * TA) { isA = true; c = (long long)(t / TA); sub = (int)(t % TA); }
             else {
                 unsigned long long tp = t - RA * TA;
@@ -479,20 +480,27 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
         const int slot = (int)(c % kRing);
         const unsigned long long gen = (unsigned long long)(c / kRing);
         unsigned long long *a_done = ctrl + 8 + slot * 4, *b_fin = a_done + 1, *b_done = a_done + 2;
-        const long long chunk_base = c * A.chunk;
+        long long chunk_base = c * A.chunk, chunk_end = chunk_base + A.chunk;
+        if (chunk_end > A.n) chunk_end = A.n;
+        const double *V = A.G.V;
+        if (A.ctab) {                                              // a-8: the chunk is a piece of one member's run
+            const int4 ce = __ldg(reinterpret_cast<const int4 *>(A.ctab) + c);
+            chunk_base = ce.x; chunk_end = (long long)ce.x + ce.y;
+            V += (size_t)ce.z * A.G.memstride;
+        }
         if (isA) {
             // the whole warp polls (same address): a lane that spins alone would reach the barrier
             // below apart from its warp, and bar.sync counts such a warp twice
             if (threadIdx.x < 32 && gen > 0) wait_counter(b_done, gen * TB);   // ring slot drained
             cta_sync();
-            a_item(A, T, SA, slot, chunk_base, sub, &err_local);
+            a_item(A, T, SA, slot, chunk_base, chunk_end, sub, &err_local);
             __threadfence();
             cta_sync();
             if (threadIdx.x == 0) atomicAdd(a_done, 1ULL);
         } else {
             if (threadIdx.x < 32) wait_counter(a_done, (gen + 1) * TA);        // every tile of A(c) released
             cta_sync();
-            b_item(A, SB, slot, chunk_base, sub);
+            b_item(A, SB, V, slot, chunk_base, sub);
             __threadfence();
             cta_sync();
             if (threadIdx.x == 0) {

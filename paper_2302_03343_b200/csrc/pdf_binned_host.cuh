@@ -6,6 +6,7 @@
 namespace pdfg {
 
 constexpr long long kAutoMinN = 1 << 15;      // PDF_PATH_AUTO: below this the direct path is used
+constexpr long long kMemberMinPer = 1 << 14;  // PDF_PATH_AUTO with member ids: queries per member below which the direct path is used
 
 // cell and t_q of 1.01*Q2min with the device log (C-9); res = {jg, t, in_range}
 __global__ void k_q2plus(GridDev G, double *res)
@@ -38,7 +39,7 @@ inline int binned_plan_init(BinnedPlan &p, const GridDev &G, const std::vector<d
 {
     p.usable = false;
     const int nx = G.nx, nqt = G.nqtot;
-    if (G.nflav != kNF || G.nfp != kNFP || G.nmem != 1) return 0;
+    if (G.nflav != kNF || G.nfp != kNFP) return 0;
     if (nx - 1 + kLowXSplit > kMaxCK || nqt + 2 > kMaxFK || nx < 2) return 0;
     BinDev &d = p.dev;
     d.ncx = nx - 1; d.nqt = nqt;
@@ -86,6 +87,10 @@ inline int binned_plan_init(BinnedPlan &p, const GridDev &G, const std::vector<d
 }
 
 inline bool binned_qualifies(const BinnedPlan &p, const ColMap &, const int *member) { return p.usable && !member; }
+inline bool binned_members_qualifies(const BinnedPlan &p, const GridDev &G, const int *member)
+{
+    return p.usable && member && G.nmem > 1 && G.nmem <= kMemMax;
+}
 // ---- luminosity on top of the binned path ------------------------------------------------------
 // pdf_lumi in slices of kLumiSlice events: xf(x1,Q2) and xf(x2,Q2) of the slice by two runs of the
 // persistent binned kernel into two scratch arrays, then k_lumi_combine reduces the 11 x 11 coupling
@@ -133,10 +138,11 @@ inline size_t binned_lumi_scratch_bytes(const BinnedPlan &p)
 template <typename Scope>
 inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm, long long n, const double *x,
                         const double *q2, double *out, long long ld, void *ws, size_t ws_bytes, long long chunk_opt,
-                        cudaStream_t s, int count_err = 1)
+                        cudaStream_t s, int count_err = 1, const int *ctab = nullptr, const int *nchunks_dev = nullptr)
 {
     if (binned_workspace_bytes(p, n, chunk_opt) > ws_bytes) return PDF_EWORKSPACE;
     StreamArgs A;
+    A.ctab = ctab; A.nchunks_dev = nchunks_dev;
     A.G = G; A.B = p.dev; A.cm = cm;
     A.chunk = binned_chunk(p, n, chunk_opt);
     A.cap = binned_cap(p, A.chunk);
@@ -161,11 +167,67 @@ inline int binned_xfxq2(const GridDev &G, const BinnedPlan &p, const ColMap &cm,
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_pdf_stream, kBinThreads, smem) != cudaSuccess || per_sm < 1)
         return PDF_ECUDA;
     unsigned long long max_ctas = (unsigned long long)per_sm * sms;         // all CTAs must be co-resident
-    unsigned long long tickets = (unsigned long long)A.nchunks * (A.ta + p.dev.nitems);
+    // with a chunk table the chunk count is on the device: the launch takes its upper bound
+    const long long nch = ctab ? member_max_chunks(n, A.chunk, G.nmem) : (long long)A.nchunks;
+    unsigned long long tickets = (unsigned long long)nch * (A.ta + p.dev.nitems);
     unsigned grid = (unsigned)(tickets < max_ctas ? tickets : max_ctas);
     {
         Scope sc(s, "k_pdf_stream");
         k_pdf_stream<<<grid, kBinThreads, smem, s>>>(A);
+    }
+    return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
+}
+
+// a-8 on the binned path (pdf_members.cuh): per slice, partition by member, one persistent-kernel
+// run over the chunk table into the sorted scratch rows, gather back to query order
+inline size_t binned_members_bytes(const BinnedPlan &p, const GridDev &G, long long n, long long chunk_opt, int npid)
+{
+    if (!p.usable || G.nmem < 2 || G.nmem > kMemMax) return 0;
+    const long long slice = member_slice(n);
+    const long long chunk = binned_chunk(p, slice, chunk_opt);
+    return binned_workspace_bytes(p, slice, chunk_opt) + member_scratch_bytes(slice, chunk, G.nmem, npid) + 256;
+}
+
+template <typename Scope>
+inline int binned_members(const GridDev &G, const BinnedPlan &p, const ColMap &cm, long long n, const double *x,
+                          const double *q2, const int *member, double *out, long long ld, void *ws, size_t ws_bytes,
+                          long long chunk_opt, cudaStream_t s)
+{
+    if (binned_members_bytes(p, G, n, chunk_opt, cm.n) > ws_bytes) return PDF_EWORKSPACE;
+    const long long slice = member_slice(n);
+    const long long chunk = binned_chunk(p, slice, chunk_opt);
+    const size_t ws_x = binned_workspace_bytes(p, slice, chunk_opt);
+    MemberWs M;
+    member_carve((char *)ws + ws_x, slice, chunk, G.nmem, M);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const size_t hsm = sizeof(unsigned) * (size_t)G.nmem;
+    for (long long off = 0; off < n; off += slice) {
+        const long long m = n - off < slice ? n - off : slice;
+        if (cudaMemsetAsync(M.hist, 0, hsm, s) != cudaSuccess) return PDF_ECUDA;
+        {
+            Scope sc(s, "k_member_hist");
+            long long want = (m + 2047) / 2048;
+            k_member_hist<<<(unsigned)(want < sms * 8 ? want : sms * 8), 256, hsm, s>>>(member + off, m, G.nmem, M.hist);
+        }
+        {
+            Scope sc(s, "k_member_plan");
+            k_member_plan<<<1, 256, hsm, s>>>(M.hist, G.nmem, (int)chunk, M.cursor, M.ctab, M.nchunks);
+        }
+        {
+            Scope sc(s, "k_member_scatter");
+            k_member_scatter<<<(unsigned)((m + 256 * kMemTileQ - 1) / (256 * kMemTileQ)), 256, 2 * hsm, s>>>(
+                x + off, q2 + off, member + off, m, G.nmem, M.cursor, M.xs, M.q2s, M.inv);
+        }
+        int rc = binned_xfxq2<Scope>(G, p, cm, m, M.xs, M.q2s, M.tmp, cm.n, ws, ws_x, chunk_opt, s, 1, M.ctab, M.nchunks);
+        if (rc) return rc;
+        {
+            Scope sc(s, "k_member_gather");
+            long long want = (m + 255) / 256;
+            k_member_gather<<<(unsigned)(want < sms * 16 ? want : sms * 16), 256, 0, s>>>(M.tmp, M.inv, m, cm.n, out + off * ld, ld,
+                                                                                       G.err_count);
+        }
     }
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }

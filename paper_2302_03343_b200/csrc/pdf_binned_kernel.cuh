@@ -28,6 +28,11 @@ struct StreamArgs {
     int identity;              // 1: requested columns == the grid's 11 columns in order
     int zfill;                 // 1: rows are contiguous (ld == npid): A items zero-fill their tile of `out`
     int count_err;             // 1: invalid queries bump the grid's error counter (0 inside pdf_lumi)
+    // member axis (a-8, pdf_members.cuh): the queries arrive sorted by member and every chunk lies
+    // inside one member's run; ctab[c] = {first query, queries, member, 0}, *nchunks_dev chunks.
+    // Null for the plain path (chunk c = queries [c*chunk, (c+1)*chunk), member 0).
+    const int *ctab;
+    const int *nchunks_dev;
 };
 
 // ---- small device helpers ----------------------------------------------------------------------
@@ -171,7 +176,7 @@ struct ASmem {
 };
 
 __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T, const ASmem &S, int slot,
-                                       long long chunk_base, int tile, unsigned long long *err_local)
+                                       long long chunk_base, long long chunk_end, int tile, unsigned long long *err_local)
 {
     const GridDev &G = A.G;
     const BinDev &B = A.B;
@@ -192,8 +197,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
 
     const long long t0 = chunk_base + (long long)tile * kTileA;
     long long t1 = t0 + kTileA;
-    if (t1 > A.n) t1 = A.n;
-    if (t1 > chunk_base + A.chunk) t1 = chunk_base + A.chunk;
+    if (t1 > chunk_end) t1 = chunk_end;
     ZeroFill zf = zero_fill_plan(A.out, A.ld, t0, A.zfill ? t1 : t0);
     cta_sync();
 

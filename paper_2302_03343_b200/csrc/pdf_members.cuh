@@ -1,0 +1,180 @@
+// pdf_members.cuh -- a-8, the member axis on the binned path (configs[3]: 100 replica grids, one
+// member id per query).
+//
+// All members share the knots, so cell search, t_x / t_q and the node weights do not depend on
+// the member; only the values do.  With ~10^6 (member, cell) pairs no chunk of 2^18 queries is
+// cell-coherent, so the queries of a slice (<= 2^25) are first partitioned by member:
+//   k_member_hist     histogram of the member ids of the slice (shared-memory counters per CTA)
+//   k_member_plan     exclusive scan -> first slot of every member; chunk table: every member's run
+//                     is cut in equal pieces of <= chunk queries {first, count, member}
+//   k_member_scatter  x, q2 -> xs, q2s in member order; inv[i] = slot of query i.  A CTA ranks its
+//                     2048 queries per member in shared memory and reserves its runs with one
+//                     global atomic per (CTA, member): ~20 consecutive slots per run
+//   k_pdf_stream      the persistent binned kernel over the chunk table: chunk c evaluates against
+//                     V + member(c) * memstride and writes rows in SORTED order to tmp
+//   k_member_gather   out[i][:] = tmp[inv[i]][:] (coalesced writes, row-granular reads); queries
+//                     with a member id outside [0, nmem) get a NaN row and count as errors (C-10)
+// The order of the queries inside a member's run is whatever the atomics gave: every row depends on
+// its own query only, so the result does not.
+#pragma once
+
+namespace pdfg {
+
+constexpr long long kMemSlice = 1 << 25;      // queries partitioned at a time (scratch: 108 B per query of a slice)
+constexpr int kMemMax = 4096;                 // members the shared-memory histograms hold
+constexpr int kMemTileQ = 8;                  // queries per thread of k_member_scatter
+constexpr unsigned kNoSlot = 0xffffffffu;
+
+struct MemberWs {
+    unsigned *hist;       // [nmem]
+    unsigned *cursor;     // [nmem] next free slot of every member's run
+    int *nchunks;         // [1]
+    int *ctab;            // [max_chunks][4]
+    unsigned *inv;        // [slice]
+    double *xs, *q2s;     // [slice]
+    double *tmp;          // [slice][npid]
+};
+
+// slices of equal length for a call of n queries
+inline long long member_slice(long long n)
+{
+    const long long ns = (n + kMemSlice - 1) / kMemSlice;
+    long long sl = ns ? (n + ns - 1) / ns : 0;
+    sl = (sl + 2047) / 2048 * 2048;
+    return sl < n ? sl : n;
+}
+
+inline long long member_max_chunks(long long slice, long long chunk, int nmem) { return (slice + chunk - 1) / chunk + nmem; }
+
+inline size_t member_scratch_bytes(long long slice, long long chunk, int nmem, int npid)
+{
+    size_t b = 3 * align_up(sizeof(unsigned) * (size_t)nmem + 16, 256);
+    b += align_up(sizeof(int) * 4 * (size_t)member_max_chunks(slice, chunk, nmem), 256);
+    b += align_up(sizeof(unsigned) * (size_t)slice, 256);
+    b += 2 * align_up(sizeof(double) * (size_t)slice, 256);
+    b += align_up(sizeof(double) * (size_t)slice * npid, 256);
+    return b + 256;
+}
+
+inline void member_carve(void *p, long long slice, long long chunk, int nmem, MemberWs &w)
+{
+    char *c = (char *)align_up((size_t)p, 256);
+    const size_t hb = align_up(sizeof(unsigned) * (size_t)nmem + 16, 256);
+    w.hist = (unsigned *)c; c += hb;
+    w.cursor = (unsigned *)c; c += hb;
+    w.nchunks = (int *)c; c += hb;
+    w.ctab = (int *)c; c += align_up(sizeof(int) * 4 * (size_t)member_max_chunks(slice, chunk, nmem), 256);
+    w.inv = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)slice, 256);
+    w.xs = (double *)c; c += align_up(sizeof(double) * (size_t)slice, 256);
+    w.q2s = (double *)c; c += align_up(sizeof(double) * (size_t)slice, 256);
+    w.tmp = (double *)c;
+}
+
+__global__ void __launch_bounds__(256)
+k_member_hist(const int *__restrict__ member, long long n, int nmem, unsigned *__restrict__ hist)
+{
+    extern __shared__ unsigned s_h[];
+    for (int k = threadIdx.x; k < nmem; k += blockDim.x) s_h[k] = 0u;
+    __syncthreads();
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+        const int m = __ldcs(member + e);
+        if (m >= 0 && m < nmem) atomicAdd(s_h + m, 1u);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nmem; k += blockDim.x) {
+        const unsigned c = s_h[k];
+        if (c) atomicAdd(hist + k, c);
+    }
+}
+
+// one CTA: scan of the histogram and the chunk table (a few hundred entries)
+__global__ void __launch_bounds__(256)
+k_member_plan(const unsigned *__restrict__ hist, int nmem, int chunk, unsigned *__restrict__ cursor,
+              int *__restrict__ ctab, int *__restrict__ nchunks)
+{
+    extern __shared__ unsigned s_h[];
+    for (int k = threadIdx.x; k < nmem; k += blockDim.x) s_h[k] = hist[k];
+    __syncthreads();
+    if (threadIdx.x) return;
+    unsigned start = 0;
+    int nc = 0;
+    for (int m = 0; m < nmem; ++m) {
+        const unsigned cnt = s_h[m];
+        cursor[m] = start;
+        const unsigned pieces = (cnt + (unsigned)chunk - 1) / (unsigned)chunk;
+        unsigned step = pieces ? (cnt + pieces - 1) / pieces : 0u;     // equal pieces, whole A tiles (chunk is a multiple)
+        step = (step + kTileA - 1) / kTileA * kTileA;
+        for (unsigned o = 0; o < cnt; o += step) {
+            const unsigned len = cnt - o < step ? cnt - o : step;
+            reinterpret_cast<int4 *>(ctab)[nc++] = make_int4((int)(start + o), (int)len, m, 0);
+        }
+        start += cnt;
+    }
+    *nchunks = nc;
+}
+
+__global__ void __launch_bounds__(256)
+k_member_scatter(const double *__restrict__ x, const double *__restrict__ q2, const int *__restrict__ member,
+                 long long n, int nmem, unsigned *__restrict__ cursor, double *__restrict__ xs,
+                 double *__restrict__ q2s, unsigned *__restrict__ inv)
+{
+    extern __shared__ unsigned s_c[];             // [nmem] counts, then [nmem] bases
+    unsigned *s_b = s_c + nmem;
+    for (int k = threadIdx.x; k < nmem; k += 256) s_c[k] = 0u;
+    __syncthreads();
+    const long long t0 = (long long)blockIdx.x * (256 * kMemTileQ);
+    unsigned tag[kMemTileQ];                      // member << 12 | rank inside the CTA's tile
+#pragma unroll
+    for (int q = 0; q < kMemTileQ; ++q) {
+        const long long e = t0 + q * 256 + threadIdx.x;
+        tag[q] = kNoSlot;
+        if (e < n) {
+            const int m = __ldcs(member + e);
+            if (m >= 0 && m < nmem) tag[q] = ((unsigned)m << 12) | atomicAdd(s_c + m, 1u);
+        }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nmem; k += 256) {
+        const unsigned c = s_c[k];
+        s_b[k] = c ? atomicAdd(cursor + k, c) : 0u;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < kMemTileQ; ++q) {
+        const long long e = t0 + q * 256 + threadIdx.x;
+        if (e >= n) continue;
+        unsigned pos = kNoSlot;
+        if (tag[q] != kNoSlot) {
+            pos = s_b[tag[q] >> 12] + (tag[q] & 0xfffu);
+            xs[pos] = __ldcs(x + e);
+            q2s[pos] = __ldcs(q2 + e);
+        }
+        inv[e] = pos;
+    }
+}
+
+// out[i][p] = tmp[inv[i]][p]; a thread per output element, so that writes are coalesced and the
+// npid doubles of a row are read by adjacent lanes
+__global__ void __launch_bounds__(256)
+k_member_gather(const double *__restrict__ tmp, const unsigned *__restrict__ inv, long long n, int npid,
+                double *__restrict__ out, long long ld, unsigned long long *err_count)
+{
+    unsigned long long bad = 0;
+    const unsigned per = 256u * (unsigned)npid;                       // elements of 256 rows
+    for (long long r0 = (long long)blockIdx.x * 256; r0 < n; r0 += (long long)gridDim.x * 256) {
+        const unsigned rows = n - r0 < 256 ? (unsigned)(n - r0) : 256u;
+        const unsigned lim = rows * (unsigned)npid;
+        for (unsigned kk = threadIdx.x; kk < per; kk += 256u) {
+            if (kk >= lim) break;
+            const unsigned il = kk / (unsigned)npid, p = kk - il * (unsigned)npid;
+            const unsigned pos = __ldg(inv + r0 + il);
+            double v;
+            if (pos == kNoSlot) { v = qnan(); bad += p == 0u; }
+            else v = __ldcs(tmp + (size_t)pos * npid + p);
+            __stcs(out + (r0 + il) * ld + p, v);
+        }
+    }
+    if (bad) atomicAdd(err_count, bad);
+}
+
+}  // namespace pdfg

@@ -41,6 +41,16 @@ int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, cons
     if (n == 0) return PDF_OK;
     if (!x || !q2 || !out) return PDF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
+    // a-8: per-query member ids on the binned path (partition by member first, pdf_members.cuh)
+    if (binned_members_qualifies(g->bplan, g->d, member) && npid <= g->d.nflav) {
+        const size_t need = binned_members_bytes(g->bplan, g->d, n, g->chunk, npid);
+        if (g->path == PDF_PATH_BINNED) {
+            if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
+            return binned_members<LaunchScope>(g->d, g->bplan, cm, n, x, q2, member, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
+        }
+        if (g->path == PDF_PATH_AUTO && g->ws && g->ws_bytes >= need && n >= kMemberMinPer * g->d.nmem)
+            return binned_members<LaunchScope>(g->d, g->bplan, cm, n, x, q2, member, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
+    }
     bool ok_binned = binned_qualifies(g->bplan, cm, member);
     bool want_binned = (g->path == PDF_PATH_BINNED) ||
                        (g->path == PDF_PATH_AUTO && g->ws && ok_binned && n >= kAutoMinN &&
@@ -64,6 +74,10 @@ size_t pdf_workspace_bytes(const pdf_grid *g, long long n)
     if (!g || n < 0) return 0;
     size_t b = binned_workspace_bytes(g->bplan, n, g->chunk);
     if (b && g->d.C) b += binned_lumi_scratch_bytes(g->bplan) + 256;    // pdf_lumi slices (only once a coupling is set)
+    if (g->d.nmem > 1) {                                                // a-8: member partition scratch (all flavours)
+        size_t m = binned_members_bytes(g->bplan, g->d, n, g->chunk, g->d.nflav);
+        if (m > b) b = m;
+    }
     return b;
 }
 

@@ -130,22 +130,45 @@ def test_scan_lines_and_knots(B, oracle_mod, path):
         assert torch.equal(got, want)
 
 
-def test_c3_members_parity(B, oracle_mod):
-    """configs[3]: replica batch, per-query member index (20 members here; the 100-member grid runs in bench)"""
+@pytest.mark.parametrize("path", PATHS)
+def test_c3_members_parity(B, oracle_mod, path):
+    """configs[3]: replica batch, per-query member index (20 members here; the 100-member grid runs in bench).
+    Queries as configs[2] (5 % extrapolated), so every class crosses the member axis; on the binned
+    path they are partitioned by member first (pdf_members.cuh)"""
     spec = synth.grid_c1(nmem=20)
-    n = 400_000
-    x, q = synth.queries_inside(spec, n, synth.BASE_SEED + 13)
+    n = 400_037
+    x, q = synth.queries_c2(spec, n, synth.BASE_SEED + 13)
     mem = synth.members(spec, n)
-    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec)
+    mem[:3000] = 7                       # an uneven histogram: one member's run spans two chunks below
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
     ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), member=mem.numpy(), want_scale=True)
     out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda(), member=mem.cuda()).cpu().numpy()
     assert_values(out, ref, S, "c3")
-    bad = mem.clone()
+    assert g.pdf_error_count() == 0
+    # invalid member ids, invalid x, and both at once: NaN rows, each query counted once
+    bad, xb = mem.clone(), x.clone()
     bad[:5] = 20
     bad[5:9] = -1
-    out = g.pdf_xfxq2(spec.pids, x[:100].cuda(), q[:100].cuda(), member=bad[:100].cuda()).cpu().numpy()
-    assert np.all(np.isnan(out[:9])) and not np.any(np.isnan(out[9:]))
-    assert g.pdf_error_count() == 9
+    xb[7:12] = 2.0
+    m = 50_000
+    out = g.pdf_xfxq2(spec.pids, xb[:m].cuda(), q[:m].cuda(), member=bad[:m].cuda()).cpu().numpy()
+    assert np.all(np.isnan(out[:12])) and not np.any(np.isnan(out[12:]))
+    assert g.pdf_error_count() == 12
+    assert_values(out[12:], ref[12:m], S[12:m], "c3 after bad rows")
+    # a pid subset with an unknown pid, padded rows; small chunks so that runs span several chunks
+    if path == "binned":
+        g.pdf_grid_set_option(B.PDF_OPT_CHUNK, 8192)
+    pids = [21, 2, 99, -3]
+    o = torch.full((m, 6), -7.0, dtype=torch.float64, device="cuda")
+    g.pdf_xfxq2(pids, x[:m].cuda(), q[:m].cuda(), out=o, member=mem[:m].cuda(), ld_out=6)
+    o = o.cpu().numpy()
+    cols = [spec.pids.index(21), spec.pids.index(2), None, spec.pids.index(-3)]
+    for k, c in enumerate(cols):
+        if c is None:
+            assert np.all(o[:, k] == 0.0)
+        else:
+            assert_values(o[:, k], ref[:m, c], S[:m, c], f"c3 pid {pids[k]}")
+    assert np.all(o[:, 4:] == -7.0)
 
 
 @pytest.mark.parametrize("path", PATHS)
