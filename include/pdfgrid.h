@@ -71,7 +71,8 @@ enum {
     PDF_PATH_DIRECT = 1,  /* one thread per query, stencil gathered through L1/L2; pdf_lumi: one fused
                              kernel, the per-flavour values never leave the registers               */
     PDF_PATH_BINNED = 2   /* queries binned by cell so that warps share one stencil (needs workspace;
-                             11-flavour single-member grids, no member array); pdf_lumi: sliced binned
+                             11-flavour grids); with a member array the queries are first partitioned
+                             by member (<= 4096 members, npid <= nflav); pdf_lumi: sliced binned
                              evaluation of both partons into workspace scratch + a combine kernel     */
 };
 enum { PDF_OPT_PATH = 1, PDF_OPT_ALPHAS_MODE = 2, PDF_OPT_CHUNK = 3 };
@@ -100,7 +101,8 @@ int pdf_grid_set_coupling(pdf_grid *g, const double *C);
 /* caller-owned DEVICE scratch for the binned path; must stay valid until replaced or the grid is
  * destroyed; bytes >= pdf_workspace_bytes(g, n) for the largest n it will be used with (the
  * figure grows by the luminosity scratch once a coupling has been set, so query it after
- * pdf_grid_set_coupling).  The contents are scratch: one evaluation call at a time may use it.
+ * pdf_grid_set_coupling; for a grid with nmem > 1 it includes the member-partition scratch,
+ * 108 bytes per query up to 2^25 queries).  The contents are scratch: one evaluation call at a time may use it.
  * dev_ptr == NULL detaches. */
 int pdf_grid_set_workspace(pdf_grid *g, void *dev_ptr, size_t bytes);
 size_t pdf_workspace_bytes(const pdf_grid *g, long long n);
