@@ -57,7 +57,10 @@ constexpr int kLag = PDF_LAG;                       // B(c) tickets follow A(c) 
 #define PDF_RING_EXTRA 4
 #endif
 constexpr int kRing = kLag + PDF_RING_EXTRA;  // chunk slots in flight: A(c) reuses the slot of B(c-kRing), issued >= 2 rounds earlier
-constexpr int kLowXSplit = 16;                // coarse keys of the low-x classes: bands of Q2 cells
+constexpr int kLowXBands = 16;                // coarse keys of low-x queries with Q2 inside: bands of Q2 cells
+constexpr int kCornerSplit = 8;               // coarse keys per corner class (low-x and low-Q / high-Q): their rows cost
+                                              // ~100 transcendental calls, one item of 650 of them held its ring slot 130 us
+constexpr int kLowXSplit = kLowXBands + 2 * kCornerSplit;
 constexpr int kLutSize = 1024;                // search-acceleration buckets per axis
 constexpr int kNF = 11, kNFP = 12;            // the fast path is specialised for 11 flavours (pad 12)
 constexpr int kMaxCK = 1024;                  // coarse keys (x cells + kLowXSplit) the path supports

@@ -185,15 +185,22 @@ __device__ __forceinline__ double weight_eval(const WCoef &w, double s)
     return fma(om2, fma(w.c1, s, w.c0), s2 * fma(w.c3, om, w.c2));
 }
 
-struct BSmem {
-    uint4 *sP;            // [cap] payloads (2 x uint4 each)
-    double *sV;           // [nqt][4][12]
-    unsigned char *bkey;  // [cap/32 + nfk] fine key of every 32-query batch
-    int *fcnt;            // [nfk]
-    int *foff;            // [nfk+1]
-    int *bstart;          // [nfk+1]
-    int *next;            // [1] batch queue of the item
-    unsigned short *order;// [cap]
+// 16-byte asynchronous copy global -> shared through L2 (LDGSTS): bins are written by other SMs
+__device__ __forceinline__ void cp_async16(unsigned saddr, const void *g)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+struct BSmem {            // 32-bit shared-window addresses
+    unsigned sP;          // uint4 [cap][2] payloads
+    unsigned sV;          // double [nqt][4][12]
+    unsigned bkey;        // u8 [cap/32 + nfk] fine key of every 32-query batch
+    unsigned fcnt;        // int [nfk]
+    unsigned foff;        // int [nfk+1]
+    unsigned bstart;      // int [nfk+1]
+    unsigned next;        // int [2] batch queue of the item; the item's count
+    unsigned order;       // u16 [cap]
 };
 
 // ---- B item: one coarse key of one chunk ------------------------------------------------------
@@ -202,28 +209,17 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
     const BinDev &B = A.B;
     const GridDev &G = A.G;
     if (item >= B.nck) { ovf_item(A, V, slot, chunk_base, item - B.nck); return; }
-    const int ck = item;
+    const int ck = B.nck - 1 - item;                       // low-x keys first: the long items must not end the round
+    PH_DECL;
     unsigned *counts = A.W.counts + (size_t)slot * B.nck;
-    // one thread reads the count and the CTA takes that value: every later branch and barrier count
-    // of the item depends on it, so it must be the same in all 256 threads
-    const unsigned nexta0 = (unsigned)__cvta_generic_to_shared(S.next);
-    if (threadIdx.x == 0) sts_u32(nexta0 + 4u, ld_acquire_u32(counts + ck));
-    cta_sync();
-    const unsigned cnt_u = lds_u32(nexta0 + 4u);
-    cta_sync();
-    if (cnt_u == 0u) return;
-    const int cnt_all = cnt_u > (unsigned)A.cap ? A.cap : (int)cnt_u;
-    const uint4 *bin = reinterpret_cast<const uint4 *>(A.W.bins + ((size_t)slot * B.nck + ck) * A.cap);
     const bool lowx_unit = ck >= B.ncx;
     const int i = lowx_unit ? 0 : ck;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned sPa = (unsigned)__cvta_generic_to_shared(S.sP), sVa = (unsigned)__cvta_generic_to_shared(S.sV);
-    const unsigned fcnt = (unsigned)__cvta_generic_to_shared(S.fcnt), foff = (unsigned)__cvta_generic_to_shared(S.foff);
-    const unsigned bstart = (unsigned)__cvta_generic_to_shared(S.bstart), order = (unsigned)__cvta_generic_to_shared(S.order);
-    const unsigned nexta = (unsigned)__cvta_generic_to_shared(S.next);
-    const unsigned bkey = (unsigned)__cvta_generic_to_shared(S.bkey);
+    const unsigned sPa = S.sP, sVa = S.sV, fcnt = S.fcnt, foff = S.foff, bstart = S.bstart, order = S.order;
+    const unsigned nexta = S.next, bkey = S.bkey;
 
-    // stage the key's 4 grid columns once
+    // stage the key's 4 grid columns: asynchronous copies (no registers, all in flight at once) that
+    // run under the count read below
     {
         int c0, c1, c2, c3;
         if (lowx_unit) { c0 = 0; c1 = 1; c2 = 0; c3 = 1; }
@@ -233,21 +229,29 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         for (int e = threadIdx.x; e < tot; e += kBinThreads) {
             int jg = e / 24, r = e - jg * 24, a = r / 6, p = r - a * 6;
             int col = a == 0 ? c0 : a == 1 ? c1 : a == 2 ? c2 : c3;
-            double2 v = __ldg(V2 + ((size_t)jg * G.nx + col) * 6 + p);
-            sts_v2f64(sVa + 16u * e, v.x, v.y);
+            cp_async16(sVa + 16u * e, V2 + ((size_t)jg * G.nx + col) * 6 + p);
         }
     }
+    // one thread reads the count and the CTA takes that value: every later branch and barrier count
+    // of the item depends on it, so it must be the same in all 256 threads
+    if (threadIdx.x == 0) sts_u32(nexta + 4u, ld_acquire_u32(counts + ck));
+    cta_sync();
+    const unsigned cnt_u = lds_u32(nexta + 4u);
+    cta_sync();
+    PH(0);
+    if (cnt_u == 0u) { cp_async_wait_all(); cta_sync(); return; }
+    const int cnt_all = cnt_u > (unsigned)A.cap ? A.cap : (int)cnt_u;
+    const char *bin = reinterpret_cast<const char *>(A.W.bins + ((size_t)slot * B.nck + ck) * A.cap);
     // the bin is processed in segments of at most A.scap payloads (what fits in shared memory)
     for (int s0 = 0; s0 < cnt_all; s0 += A.scap) {
     const int cnt = min(A.scap, cnt_all - s0);
     if (s0) cta_sync();                               // the previous segment's batches are done
-    for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) {
-        uint4 v = __ldcg(bin + 2 * s0 + e);
-        sts_v4u32(sPa + 16u * e, v.x, v.y, v.z, v.w);
-    }
+    for (int e = threadIdx.x; e < cnt * 2; e += kBinThreads) cp_async16(sPa + 16u * e, bin + 16 * (size_t)(2 * s0 + e));
+    cp_async_wait_all();
     for (int k = threadIdx.x; k < B.nfk; k += kBinThreads) sts_u32(fcnt + 4u * k, 0u);
     if (threadIdx.x == 0) sts_u32(nexta, 0u);
     cta_sync();
+    PH(1);
     // counting sort by fine key: rank kept in the payload's spare word
     for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
         unsigned fk = lds_u32(sPa + 32u * e + 20u);
@@ -256,6 +260,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         sts_u32(sPa + 32u * e + 24u, r);
     }
     cta_sync();
+    PH(2);
     if (warp == 0) {                                       // exclusive scans: slots and 32-query batches per key
         int carry_o = 0, carry_b = 0;
         for (int k0 = 0; k0 < B.nfk; k0 += 32) {
@@ -280,6 +285,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         }
     }
     cta_sync();
+    PH(3);
     for (int e = threadIdx.x; e < cnt; e += kBinThreads) {
         uint2 w = make_uint2(lds_u32(sPa + 32u * e + 20u), lds_u32(sPa + 32u * e + 24u));
         unsigned pos = lds_u32(foff + 4u * w.x) + w.y;
@@ -287,6 +293,7 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         asm volatile("st.shared.u16 [%0], %1;" ::"r"(order + 2u * pos), "h"((unsigned short)e) : "memory");
     }
     cta_sync();
+    PH(4);
 
     const int total = (int)lds_u32(bstart + 4u * B.nfk);
     const WCoef kx = weight_coef(G.cx[i], lane & 3);       // x-axis weight of this lane's node, fixed for the unit
@@ -392,6 +399,10 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         }
         __syncwarp();
     }
+    if (threadIdx.x == 0) { PH(5); }
+    __syncwarp();
+    cta_sync();
+    PH(6);
     }   // segments
     cta_sync();
     if (threadIdx.x == 0) counts[ck] = 0u;                 // the bin is empty again for the ring
@@ -426,20 +437,8 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
     for (int i = threadIdx.x; i < A.G.nqtot; i += kBinThreads) s_qk[i] = A.G.qk[i];
     for (int i = threadIdx.x; i < kLutSize; i += kBinThreads) { s_lutx[i] = A.B.lutx[i]; s_lutq[i] = A.B.lutq[i]; }
     cta_sync();
-    SmemTables T{s_xk, s_qk, s_lutx, s_lutq};
-    ASmem SA;
-    SA.pay = reinterpret_cast<uint4 *>(region);
-    SA.cnt = reinterpret_cast<unsigned *>(region + (size_t)kTileA * 32);
-    SA.base = SA.cnt + A.B.nck;
-    BSmem SB;
-    SB.sP = reinterpret_cast<uint4 *>(region);
-    SB.sV = reinterpret_cast<double *>(region + (size_t)A.scap * 32);
-    SB.fcnt = reinterpret_cast<int *>(SB.sV + (size_t)A.G.nqtot * 4 * kNFP);
-    SB.foff = SB.fcnt + A.B.nfk + 1;
-    SB.bstart = SB.foff + A.B.nfk + 1;
-    SB.next = SB.bstart + A.B.nfk + 2;
-    SB.order = reinterpret_cast<unsigned short *>(SB.next + 2);
-    SB.bkey = reinterpret_cast<unsigned char *>(SB.order + ((A.scap + 7) & ~7));
+    const unsigned region_a = (unsigned)__cvta_generic_to_shared(region);   // everything below derives from this one address
+    const unsigned tables_a = (unsigned)__cvta_generic_to_shared(smem_raw);
 
     unsigned long long *ctrl = A.W.ctrl;
     const unsigned long long TA = A.ta, TB = A.B.nitems, per = TA + TB;
@@ -491,18 +490,58 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
         if (isA) {
             // the whole warp polls (same address): a lane that spins alone would reach the barrier
             // below apart from its warp, and bar.sync counts such a warp twice
+            PH_DECL;
+#ifdef PDF_PHASES
+            if (threadIdx.x == 0 && gen > 0 && ld_acquire_u64(b_done) < gen * TB) atomicAdd(A.W.ctrl + 256 + 14, 1ULL);
+            if (threadIdx.x == 0) atomicAdd(A.W.ctrl + 256 + 15, 1ULL);
+#endif
             if (threadIdx.x < 32 && gen > 0) wait_counter(b_done, gen * TB);   // ring slot drained
+            PH(11);
             cta_sync();
+            PH(12);
+            SmemTables T;
+            T.xk = tables_a; T.qk = T.xk + 8u * A.G.nx; T.lutx = T.qk + 8u * A.G.nqtot; T.lutq = T.lutx + 2u * kLutSize;
+            ASmem SA;
+            SA.pay = region_a; SA.cnt = region_a + (unsigned)kTileA * 32u; SA.base = SA.cnt + 4u * A.B.nck;
             a_item(A, T, SA, slot, chunk_base, chunk_end, sub, &err_local);
+#ifdef PDF_PHASES
+            ph_t = clock64();
+#endif
             __threadfence();
             cta_sync();
+            PH(20);
             if (threadIdx.x == 0) atomicAdd(a_done, 1ULL);
         } else {
+            PH_DECL;
             if (threadIdx.x < 32) wait_counter(a_done, (gen + 1) * TA);        // every tile of A(c) released
             cta_sync();
+            PH(13);
+#ifdef PDF_PHASES
+            long long bt0 = clock64();
+#endif
+            BSmem SB;
+            SB.sP = region_a;
+            SB.sV = region_a + (unsigned)A.scap * 32u;
+            SB.fcnt = SB.sV + (unsigned)A.G.nqtot * (4u * kNFP * 8u);
+            SB.foff = SB.fcnt + 4u * (A.B.nfk + 1);
+            SB.bstart = SB.foff + 4u * (A.B.nfk + 1);
+            SB.next = SB.bstart + 4u * (A.B.nfk + 2);
+            SB.order = SB.next + 8u;
+            SB.bkey = SB.order + 2u * ((A.scap + 7) & ~7);
             b_item(A, SB, V, slot, chunk_base, sub);
+#ifdef PDF_PHASES
+            if (threadIdx.x == 0) {
+                unsigned long long dt = (unsigned long long)(clock64() - bt0);
+                atomicMax(A.W.ctrl + 256 + 16, dt);
+                if (dt > 100000ULL) atomicAdd(A.W.ctrl + 256 + 17, 1ULL);
+                if (dt > 200000ULL) atomicAdd(A.W.ctrl + 256 + 18, 1ULL);
+                if (dt > 200000ULL) A.W.ctrl[256 + 19] = (unsigned long long)sub;
+            }
+            ph_t = clock64();
+#endif
             __threadfence();
             cta_sync();
+            PH(7);
             if (threadIdx.x == 0) {
                 unsigned long long old = atomicAdd(b_fin, 1ULL);
                 if (old + 1 == (gen + 1) * TB) {                               // last item of the chunk

@@ -14,6 +14,15 @@ namespace pdfg {
 #define PDF_ASSERT(c) ((void)0)
 #endif
 
+// phase clocks of thread 0 (development builds only, -DPDF_PHASES): ctrl[256 + k] += cycles
+#ifdef PDF_PHASES
+#define PH_DECL long long ph_t = clock64()
+#define PH(k) do { if (threadIdx.x == 0) { long long ph_n = clock64(); atomicAdd(A.W.ctrl + 256 + (k), (unsigned long long)(ph_n - ph_t)); ph_t = ph_n; } } while (0)
+#else
+#define PH_DECL ((void)0)
+#define PH(k) ((void)0)
+#endif
+
 struct StreamArgs {
     GridDev G;
     BinDev B;
@@ -108,9 +117,9 @@ __device__ __forceinline__ int search_last_le(const double *__restrict__ k, int 
 
 // shared memory of the persistent kernel: tables staged once per CTA + a region that A and B
 // items use in turn
-struct SmemTables {
-    const double *xk, *qk;
-    const short *lutx, *lutq;
+struct SmemTables {       // 32-bit shared-window addresses
+    unsigned xk, qk;
+    unsigned lutx, lutq;
 };
 // explicit shared-window accessors (32-bit addresses): the compiler cannot prove the address space
 // of pointers that travel through structs and would emit generic loads
@@ -169,10 +178,10 @@ __device__ __forceinline__ void zero_fill_slice(const ZeroFill &z, int slice, in
 // ---- A item: classify, locate, t_x / t_q, tile-local sort by coarse key, payload stores ---------
 // Per query only (x, q2) live in registers across the loop; the payload (a, b, idx, fk) and the
 // (coarse key, rank) pair are parked in shared memory until the tile's runs have been reserved.
-struct ASmem {
-    unsigned *cnt;        // [nck] queries of this tile per coarse key
-    unsigned *base;       // [nck] first slot of the tile's run in the key's bin
-    uint4 *pay;           // [kTileA][2] payloads in query order; .w of the second word = ck<<16 | rank
+struct ASmem {            // 32-bit shared-window addresses
+    unsigned cnt;         // unsigned [nck] queries of this tile per coarse key
+    unsigned base;        // unsigned [nck] first slot of the tile's run in the key's bin
+    unsigned pay;         // uint4 [kTileA][2] payloads in query order; .w of the second word = ck<<16 | rank
 };
 
 __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T, const ASmem &S, int slot,
@@ -184,15 +193,14 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
     Payload *bins = A.W.bins + (size_t)slot * B.nck * A.cap;
     Payload *ovf = A.W.ovf + (size_t)slot * A.chunk;
     unsigned *ovf_count = A.W.ovf_count + slot;
-    const unsigned s_xk = (unsigned)__cvta_generic_to_shared(T.xk), s_qk = (unsigned)__cvta_generic_to_shared(T.qk);
-    const unsigned s_lx = (unsigned)__cvta_generic_to_shared(T.lutx), s_lq = (unsigned)__cvta_generic_to_shared(T.lutq);
-    const unsigned s_cnt = (unsigned)__cvta_generic_to_shared(S.cnt), s_base = (unsigned)__cvta_generic_to_shared(S.base);
-    const unsigned s_pay = (unsigned)__cvta_generic_to_shared(S.pay);
+    const unsigned s_xk = T.xk, s_qk = T.qk, s_lx = T.lutx, s_lq = T.lutq;
+    const unsigned s_cnt = S.cnt, s_base = S.base, s_pay = S.pay;
     const int nx = G.nx, nqt = G.nqtot;
     const double xmin = lds_f64(s_xk), xmax = lds_f64(s_xk + 8u * (nx - 1));
     const double qmin = lds_f64(s_qk), qmax = lds_f64(s_qk + 8u * (nqt - 1));
     const double u0 = __ldg(G.uk), s0 = __ldg(G.sk);
 
+    PH_DECL;
     for (int k = threadIdx.x; k < B.nck; k += kBinThreads) sts_u32(s_cnt + 4u * k, 0u);
 
     const long long t0 = chunk_base + (long long)tile * kTileA;
@@ -248,8 +256,11 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
                 }
                 fk = lowq ? (unsigned)nqt : highq ? (unsigned)nqt + 1u : (unsigned)jg;
                 unsigned ck = (unsigned)i;
-                if (lowx)       // low-x classes: one coarse key per band of Q2 cells, so that their batches fill up
-                    ck = (unsigned)B.ncx + (lowq ? 0u : highq ? (unsigned)(kLowXSplit - 1) : (unsigned)(jg * kLowXSplit) / (unsigned)nqt);
+                if (lowx)       // low-x classes: one coarse key per band of Q2 cells, so that their batches fill up;
+                                // the corners, whose rows are the most expensive, are dealt over kCornerSplit keys each
+                    ck = (unsigned)B.ncx + (lowq ? (unsigned)kLowXBands + (threadIdx.x & (kCornerSplit - 1))
+                                                 : highq ? (unsigned)(kLowXBands + kCornerSplit) + (threadIdx.x & (kCornerSplit - 1))
+                                                         : (unsigned)(jg * kLowXBands) / (unsigned)nqt);
                 PDF_ASSERT(ck < (unsigned)B.nck && fk < (unsigned)B.nfk);
                 const unsigned rank = atoms_add(s_cnt + 4u * ck, 1u);
                 tag = (ck << 16) | rank;
@@ -260,11 +271,13 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         sts_v4u32(pa + 16u, (unsigned)(e - chunk_base), fk, 0u, tag);
     }
     cta_sync();
+    PH(8);
     for (int k = threadIdx.x; k < B.nck; k += kBinThreads) {       // one global atomic per (tile, key)
         unsigned c = lds_u32(s_cnt + 4u * k);
         sts_u32(s_base + 4u * k, c ? atomicAdd(counts + k, c) : 0u);
     }
     cta_sync();
+    PH(9);
 #pragma unroll 1
     for (int q = 0; q < kTileQ; ++q) {
         const int ql = q * kBinThreads + threadIdx.x;
@@ -287,6 +300,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
             store_payload(ovf + o, __ldg(A.x + t0 + ql), __ldg(A.q2 + t0 + ql), w1.x, 0u);
         }
     }
+    PH(10);
 }
 
 }  // namespace pdfg
