@@ -204,11 +204,18 @@ struct BSmem {            // 32-bit shared-window addresses
 };
 
 // ---- B item: one coarse key of one chunk ------------------------------------------------------
-__device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, const double *V, int slot, long long chunk_base, int item)
+__device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, const double *V, int slot, long long chunk_base, int item,
+                                       const unsigned long long *a_done, unsigned long long a_target)
 {
     const BinDev &B = A.B;
     const GridDev &G = A.G;
-    if (item >= B.nck) { ovf_item(A, V, slot, chunk_base, item - B.nck); return; }
+    // every tile of A(c) must have been released; one whole warp polls (see a_item)
+    if (item >= B.nck) {
+        if (threadIdx.x < 32) wait_counter(a_done, a_target);
+        cta_sync();
+        ovf_item(A, V, slot, chunk_base, item - B.nck);
+        return;
+    }
     const int ck = B.nck - 1 - item;                       // low-x keys first: the long items must not end the round
     PH_DECL;
     unsigned *counts = A.W.counts + (size_t)slot * B.nck;
@@ -234,10 +241,12 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
     }
     // one thread reads the count and the CTA takes that value: every later branch and barrier count
     // of the item depends on it, so it must be the same in all 256 threads
-    if (threadIdx.x == 0) sts_u32(nexta + 4u, ld_acquire_u32(counts + ck));
+    if (threadIdx.x < 32) {
+        wait_counter(a_done, a_target);
+        if (threadIdx.x == 0) sts_u32(nexta + 4u, ld_acquire_u32(counts + ck));
+    }
     cta_sync();
-    const unsigned cnt_u = lds_u32(nexta + 4u);
-    cta_sync();
+    const unsigned cnt_u = lds_u32(nexta + 4u);                // not written again before the item's last barrier
     PH(0);
     if (cnt_u == 0u) { cp_async_wait_all(); cta_sync(); return; }
     const int cnt_all = cnt_u > (unsigned)A.cap ? A.cap : (int)cnt_u;
@@ -488,22 +497,15 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
             V += (size_t)ce.z * A.G.memstride;
         }
         if (isA) {
-            // the whole warp polls (same address): a lane that spins alone would reach the barrier
-            // below apart from its warp, and bar.sync counts such a warp twice
-            PH_DECL;
+            // (the wait for the ring slot is inside the item, under its loads)
 #ifdef PDF_PHASES
-            if (threadIdx.x == 0 && gen > 0 && ld_acquire_u64(b_done) < gen * TB) atomicAdd(A.W.ctrl + 256 + 14, 1ULL);
-            if (threadIdx.x == 0) atomicAdd(A.W.ctrl + 256 + 15, 1ULL);
+            long long ph_t;
 #endif
-            if (threadIdx.x < 32 && gen > 0) wait_counter(b_done, gen * TB);   // ring slot drained
-            PH(11);
-            cta_sync();
-            PH(12);
             SmemTables T;
             T.xk = tables_a; T.qk = T.xk + 8u * A.G.nx; T.lutx = T.qk + 8u * A.G.nqtot; T.lutq = T.lutx + 2u * kLutSize;
             ASmem SA;
             SA.pay = region_a; SA.cnt = region_a + (unsigned)kTileA * 32u; SA.base = SA.cnt + 4u * A.B.nck;
-            a_item(A, T, SA, slot, chunk_base, chunk_end, sub, &err_local);
+            a_item(A, T, SA, slot, chunk_base, chunk_end, sub, &err_local, b_done, gen * TB);
 #ifdef PDF_PHASES
             ph_t = clock64();
 #endif
@@ -512,10 +514,6 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
             PH(20);
             if (threadIdx.x == 0) atomicAdd(a_done, 1ULL);
         } else {
-            PH_DECL;
-            if (threadIdx.x < 32) wait_counter(a_done, (gen + 1) * TA);        // every tile of A(c) released
-            cta_sync();
-            PH(13);
 #ifdef PDF_PHASES
             long long bt0 = clock64();
 #endif
@@ -528,7 +526,7 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
             SB.next = SB.bstart + 4u * (A.B.nfk + 2);
             SB.order = SB.next + 8u;
             SB.bkey = SB.order + 2u * ((A.scap + 7) & ~7);
-            b_item(A, SB, V, slot, chunk_base, sub);
+            b_item(A, SB, V, slot, chunk_base, sub, a_done, (gen + 1) * TA);
 #ifdef PDF_PHASES
             if (threadIdx.x == 0) {
                 unsigned long long dt = (unsigned long long)(clock64() - bt0);
@@ -537,7 +535,7 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
                 if (dt > 200000ULL) atomicAdd(A.W.ctrl + 256 + 18, 1ULL);
                 if (dt > 200000ULL) A.W.ctrl[256 + 19] = (unsigned long long)sub;
             }
-            ph_t = clock64();
+            long long ph_t = clock64();
 #endif
             __threadfence();
             cta_sync();

@@ -185,7 +185,8 @@ struct ASmem {            // 32-bit shared-window addresses
 };
 
 __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T, const ASmem &S, int slot,
-                                       long long chunk_base, long long chunk_end, int tile, unsigned long long *err_local)
+                                       long long chunk_base, long long chunk_end, int tile, unsigned long long *err_local,
+                                       const unsigned long long *ring_free, unsigned long long ring_target)
 {
     const GridDev &G = A.G;
     const BinDev &B = A.B;
@@ -209,67 +210,165 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
     ZeroFill zf = zero_fill_plan(A.out, A.ld, t0, A.zfill ? t1 : t0);
     cta_sync();
 
-    // rolled loop (small code, no register arrays); the next query's inputs are fetched one round ahead
-    double xn = -1.0, qn = -1.0;
-    if (t0 + threadIdx.x < t1) { xn = __ldcs(A.x + t0 + threadIdx.x); qn = __ldcs(A.q2 + t0 + threadIdx.x); }
-#pragma unroll 1
+    // The thread's kTileQ queries go through the steps together, so that the independent loads and
+    // logarithms of one step overlap (the shared-memory accessors are ordered asm statements: only
+    // what is issued before the first use runs concurrently).
+    double xv[kTileQ], qv[kTileQ], lx[kTileQ], lq[kTileQ];
+    int gi[kTileQ], gj[kTileQ];
+    unsigned st[kTileQ];                                           // 0: not a query, 1: invalid, 2: valid
+#pragma unroll
     for (int q = 0; q < kTileQ; ++q) {
-        const int ql = q * kBinThreads + threadIdx.x;             // query index inside the tile
-        const long long e = t0 + ql;
-        const double x = xn, q2 = qn;
-        if (q + 1 < kTileQ && e + kBinThreads < t1) { xn = __ldcs(A.x + e + kBinThreads); qn = __ldcs(A.q2 + e + kBinThreads); }
-        zero_fill_slice(zf, q, kTileQ);
-        unsigned tag = 0xffffffffu;                                // not a query
-        double ta = 0.0, tb = 0.0;
-        unsigned fk = 0;
-        if (e < t1) {
-            if (!(finite_pos(x) && finite_pos(q2)) || x > xmax) tag = 0xfffffffeu;      // C-10
-            else {
-                const bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
-                const double lx = log(x), lq = log(q2);
-                int i = 0, jg = 0;
-                if (!lowx) {
-                    int b = (int)((lx - u0) * B.lutx_scale);
-                    b = b < 0 ? 0 : (b >= kLutSize ? kLutSize - 1 : b);
-                    int c = lds_s16(s_lx + 2u * b);
+        const long long e = t0 + q * kBinThreads + threadIdx.x;
+        xv[q] = 1.0; qv[q] = 1.0;
+        if (e < t1) { xv[q] = __ldcs(A.x + e); qv[q] = __ldcs(A.q2 + e); }
+    }
+    PH(21);
+    // The ring slot must have been drained by B(c - kRing) before this tile touches its bins (after the
+    // next barrier); polled here, under the loads.  The whole warp polls (same address): a lane that
+    // spins alone would reach the barrier apart from its warp, and bar.sync counts such a warp twice.
+    if (threadIdx.x < 32 && ring_target) wait_counter(ring_free, ring_target);
+    PH(11);
+    zero_fill_slice(zf, 0, 4);
+    PH(22);
+#pragma unroll
+    for (int q = 0; q < kTileQ; ++q) {
+        const long long e = t0 + q * kBinThreads + threadIdx.x;
+        st[q] = e < t1 ? ((!(finite_pos(xv[q]) && finite_pos(qv[q])) || xv[q] > xmax) ? 1u : 2u) : 0u;   // C-10
+        lx[q] = 0.0; lq[q] = 0.0;
+        if (st[q] == 2u) { lx[q] = log(xv[q]); lq[q] = log(qv[q]); }
+    }
+    PH(23);
+    zero_fill_slice(zf, 1, 4);
+    PH(22);
+    // start guesses of both searches (buckets clamped: always a valid table entry)
+#pragma unroll
+    for (int q = 0; q < kTileQ; ++q) {
+        int bx = (int)((lx[q] - u0) * B.lutx_scale), bq = (int)((lq[q] - s0) * B.lutq_scale);
+        bx = bx < 0 ? 0 : (bx >= kLutSize ? kLutSize - 1 : bx);
+        bq = bq < 0 ? 0 : (bq >= kLutSize ? kLutSize - 1 : bq);
+        gi[q] = lds_s16(s_lx + 2u * bx);
+        gj[q] = lds_s16(s_lq + 2u * bq);
+    }
+    // The guess is the cell at the lower edge of the bucket and buckets are finer than cells, so the
+    // query lies <= 1 knot (x) or <= 2 knots (Q2: a threshold is two equal knots) above it: branch-free
+    // steps on knots loaded together, a check of the C-4 condition on the raw values, and the exact
+    // walk only where the check fails (coarser tables, rounding of the bucket index).
+    {
+        double xa[kTileQ], xb[kTileQ], xc[kTileQ], qa[kTileQ], qb[kTileQ], qc[kTileQ], qd[kTileQ];
+#pragma unroll
+        for (int q = 0; q < kTileQ; ++q) {
+            const int c = gi[q], g = gj[q];
+            xa[q] = lds_f64(s_xk + 8u * c);
+            xb[q] = lds_f64(s_xk + 8u * min(c + 1, nx - 1));
+            xc[q] = lds_f64(s_xk + 8u * min(c + 2, nx - 1));
+            qa[q] = lds_f64(s_qk + 8u * g);
+            qb[q] = lds_f64(s_qk + 8u * min(g + 1, nqt - 1));
+            qc[q] = lds_f64(s_qk + 8u * min(g + 2, nqt - 1));
+            qd[q] = lds_f64(s_qk + 8u * min(g + 3, nqt - 1));
+        }
+        bool fix = false;
+#pragma unroll
+        for (int q = 0; q < kTileQ; ++q) {
+            const double x = xv[q], q2 = qv[q];
+            int c = gi[q];
+            const bool ux = c < nx - 2 && xb[q] <= x;              // x cells: [0, nx-2]
+            c += ux;
+            const double xlo = ux ? xb[q] : xa[q], xhi = ux ? xc[q] : xb[q];
+            const bool okx = xlo <= x && (c >= nx - 2 || x < xhi);
+            gi[q] = c;
+            int g = gj[q];                                         // last knot <= q2: [0, nqt-1]
+            const bool u1 = g < nqt - 1 && qb[q] <= q2;
+            g += u1;
+            double lo = u1 ? qb[q] : qa[q], hi = u1 ? qc[q] : qb[q];
+            const double nx2 = u1 ? qd[q] : qc[q];
+            const bool u2 = g < nqt - 1 && hi <= q2;
+            g += u2;
+            lo = u2 ? hi : lo; hi = u2 ? nx2 : hi;
+            const bool okq = lo <= q2 && (g >= nqt - 1 || q2 < hi);
+            gj[q] = g;
+            fix |= st[q] == 2u && ((!(x < xmin) && !okx) || (!(q2 < qmin) && !okq));
+        }
+        if (fix) {
+#pragma unroll
+            for (int q = 0; q < kTileQ; ++q) {
+                const double x = xv[q], q2 = qv[q];
+                if (st[q] != 2u) continue;
+                if (!(x < xmin)) {
+                    int c = gi[q];
                     while (c > 0 && lds_f64(s_xk + 8u * c) > x) --c;
                     while (c < nx - 2 && lds_f64(s_xk + 8u * (c + 1)) <= x) ++c;
-                    i = c;
-                    const double2 ci = __ldg(reinterpret_cast<const double2 *>(G.cx + i));   // lo_log, inv_d
-                    ta = (x == lds_f64(s_xk + 8u * (i + 1))) ? 1.0 : (lx - ci.x) * ci.y;
-                } else {
-                    ta = (lx - u0) / (__ldg(G.uk + 1) - u0);      // theta_x (C-7)
+                    gi[q] = c;
                 }
-                if (!lowq && !highq) {
-                    int b = (int)((lq - s0) * B.lutq_scale);
-                    b = b < 0 ? 0 : (b >= kLutSize ? kLutSize - 1 : b);
-                    int g = lds_s16(s_lq + 2u * b);
+                if (!(q2 < qmin)) {
+                    int g = gj[q];
                     while (g > 0 && lds_f64(s_qk + 8u * g) > q2) --g;
                     while (g < nqt - 1 && lds_f64(s_qk + 8u * (g + 1)) <= q2) ++g;
-                    jg = g - (int)__ldg(G.cell_adj + g);           // last knot of a sub-grid -> its last cell
-                    const double2 cj = __ldg(reinterpret_cast<const double2 *>(G.cq + jg));
-                    tb = (q2 == lds_f64(s_qk + 8u * (jg + 1))) ? 1.0 : (lq - cj.x) * cj.y;
-                } else if (highq) {
-                    tb = (lq - __ldg(G.sk + nqt - 2)) / (__ldg(G.sk + nqt - 1) - __ldg(G.sk + nqt - 2));   // theta_q (C-8)
-                } else {
-                    tb = q2 / qmin;                                // r (C-9)
+                    gj[q] = g;
                 }
-                fk = lowq ? (unsigned)nqt : highq ? (unsigned)nqt + 1u : (unsigned)jg;
-                unsigned ck = (unsigned)i;
-                if (lowx)       // low-x classes: one coarse key per band of Q2 cells, so that their batches fill up;
-                                // the corners, whose rows are the most expensive, are dealt over kCornerSplit keys each
-                    ck = (unsigned)B.ncx + (lowq ? (unsigned)kLowXBands + (threadIdx.x & (kCornerSplit - 1))
-                                                 : highq ? (unsigned)(kLowXBands + kCornerSplit) + (threadIdx.x & (kCornerSplit - 1))
-                                                         : (unsigned)(jg * kLowXBands) / (unsigned)nqt);
-                PDF_ASSERT(ck < (unsigned)B.nck && fk < (unsigned)B.nfk);
-                const unsigned rank = atoms_add(s_cnt + 4u * ck, 1u);
-                tag = (ck << 16) | rank;
             }
         }
-        const unsigned pa = s_pay + 32u * ql;
-        sts_v2f64(pa, ta, tb);
-        sts_v4u32(pa + 16u, (unsigned)(e - chunk_base), fk, 0u, tag);
     }
+    PH(24);
+    zero_fill_slice(zf, 2, 4);
+    PH(22);
+    // cell constants (L1-resident tables) and the knots above, all in flight
+    {
+        int adj[kTileQ];
+#pragma unroll
+        for (int q = 0; q < kTileQ; ++q) adj[q] = (int)__ldg(G.cell_adj + gj[q]);   // last knot of a sub-grid -> its last cell
+        double2 ci[kTileQ], cj[kTileQ];
+        double kx1[kTileQ], kq1[kTileQ];
+#pragma unroll
+        for (int q = 0; q < kTileQ; ++q) {
+            gj[q] -= adj[q];
+            ci[q] = __ldg(reinterpret_cast<const double2 *>(G.cx + gi[q]));          // lo_log, inv_d
+            cj[q] = __ldg(reinterpret_cast<const double2 *>(G.cq + gj[q]));
+            kx1[q] = lds_f64(s_xk + 8u * (gi[q] + 1));
+            kq1[q] = lds_f64(s_qk + 8u * (gj[q] + 1));
+        }
+        // the extrapolation abscissae through reciprocals (one division each per item instead of per query)
+        const double inv_du0 = 1.0 / (__ldg(G.uk + 1) - u0);
+        const double sA = __ldg(G.sk + nqt - 2), inv_ds = 1.0 / (__ldg(G.sk + nqt - 1) - sA), inv_qmin = 1.0 / qmin;
+#pragma unroll
+        for (int q = 0; q < kTileQ; ++q) {
+            const double x = xv[q], q2 = qv[q];
+            const bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
+            const double ta = lowx ? (lx[q] - u0) * inv_du0                           // theta_x (C-7)
+                                   : (x == kx1[q]) ? 1.0 : (lx[q] - ci[q].x) * ci[q].y;
+            const double tb = lowq ? q2 * inv_qmin                                    // r (C-9)
+                            : highq ? (lq[q] - sA) * inv_ds                           // theta_q (C-8)
+                                    : (q2 == kq1[q]) ? 1.0 : (lq[q] - cj[q].x) * cj[q].y;
+            lx[q] = ta; lq[q] = tb;
+        }
+    }
+    PH(25);
+    zero_fill_slice(zf, 3, 4);
+    PH(22);
+#pragma unroll
+    for (int q = 0; q < kTileQ; ++q) {
+        const int ql = q * kBinThreads + threadIdx.x;             // query index inside the tile
+        const double x = xv[q], q2 = qv[q];
+        const bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
+        unsigned tag = st[q] == 0u ? 0xffffffffu : 0xfffffffeu;
+        unsigned fk = 0;
+        if (st[q] == 2u) {
+            const int jg = gj[q];
+            fk = lowq ? (unsigned)nqt : highq ? (unsigned)nqt + 1u : (unsigned)jg;
+            unsigned ck = (unsigned)gi[q];
+            if (lowx)       // low-x classes: one coarse key per band of Q2 cells, so that their batches fill up;
+                            // the corners, whose rows are the most expensive, are dealt over kCornerSplit keys each
+                ck = (unsigned)B.ncx + (lowq ? (unsigned)kLowXBands + (threadIdx.x & (kCornerSplit - 1))
+                                             : highq ? (unsigned)(kLowXBands + kCornerSplit) + (threadIdx.x & (kCornerSplit - 1))
+                                                     : (unsigned)(jg * kLowXBands) / (unsigned)nqt);
+            PDF_ASSERT(ck < (unsigned)B.nck && fk < (unsigned)B.nfk);
+            const unsigned rank = atoms_add(s_cnt + 4u * ck, 1u);
+            tag = (ck << 16) | rank;
+        }
+        const unsigned pa = s_pay + 32u * ql;
+        sts_v2f64(pa, lx[q], lq[q]);
+        sts_v4u32(pa + 16u, (unsigned)(t0 + ql - chunk_base), fk, 0u, tag);
+    }
+    PH(26);
     cta_sync();
     PH(8);
     for (int k = threadIdx.x; k < B.nck; k += kBinThreads) {       // one global atomic per (tile, key)
