@@ -334,19 +334,36 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
                 b0[r] = lds_f64(pn + 8u * g);
                 b1[r] = g < 4 ? lds_f64(pn + 8u * (8 + g)) : 0.0;
             }
+            // the next tile's abscissae are fetched (two dependent shared-memory loads) under this tile's arithmetic
+            double txn = 0.0, tqn = 0.0;
+            unsigned idxn = 0;
+            bool vn = g < nact;
+            if (vn) {
+                unsigned short e16;
+                asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * g) : "memory");
+                PDF_ASSERT(e16 < cnt);
+                const unsigned pe = sPa + 32u * e16;
+                const double2 ab = lds_v2f64(pe);
+                txn = ab.x; tqn = ab.y;
+                idxn = lds_u32(pe + 16u);
+            }
             for (int m0 = 0; m0 < nact; m0 += 8) {
-                const int qi = m0 + g;
-                const bool valid = qi < nact;
-                double tx = 0.0, tq = 0.0;
-                unsigned idx = 0;
-                if (valid) {
-                    unsigned short e16;
-                    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * qi) : "memory");
-                    PDF_ASSERT(e16 < cnt);
-                    const unsigned pe = sPa + 32u * e16;
-                    const double2 ab = lds_v2f64(pe);
-                    tx = ab.x; tq = ab.y;
-                    idx = lds_u32(pe + 16u);
+                const bool valid = vn;
+                const double tx = txn, tq = tqn;
+                const unsigned idx = idxn;
+                {
+                    const int qi = m0 + 8 + g;
+                    vn = qi < nact;
+                    txn = 0.0; tqn = 0.0;
+                    if (vn) {
+                        unsigned short e16;
+                        asm volatile("ld.shared.u16 %0, [%1];" : "=h"(e16) : "r"(ord0 + 2u * qi) : "memory");
+                        PDF_ASSERT(e16 < cnt);
+                        const unsigned pe = sPa + 32u * e16;
+                        const double2 ab = lds_v2f64(pe);
+                        txn = ab.x; tqn = ab.y;
+                        idxn = lds_u32(pe + 16u);
+                    }
                 }
                 const double wx = valid ? weight_eval(kx, tx) : 0.0;
                 const double wq0 = weight_eval(kq, tq);
