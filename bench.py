@@ -31,8 +31,8 @@ UNIT = "points*flavours/s"
 WORKLOAD = ("configs[2] (C2): 196x(6+8+40) LHAPDF-shaped grid, 11 flavours, "
             "5% of queries extrapolated, + alpha_s over the same Q2 (60 knots)")
 # dram__bytes_read.sum + dram__bytes_write.sum of k_pdf_stream at n = 1e8 (C2), one ncu capture of this
-# command line: profiles/r1g_traffic_pdf_stream_1e8.csv; null for any other n
-NCU_TRAFFIC_BYTES_1E8 = 5426908416 + 21800476160
+# command line: profiles/r1h_traffic_pdf_stream_1e8.csv; null for any other n
+NCU_TRAFFIC_BYTES_1E8 = 5404000768 + 22269288192
 BYTES_PER_QUERY = 16 + 88          # x, q2 in; 11 fp64 out
 BYTES_PER_EVENT = 32 + 8
 BYTES_PER_ALPHAS = 16
@@ -294,7 +294,12 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
         secs, _, prof, launches = timed_steps(
             torch, dist, world, lambda: mg.pdf_xfxq2(mspec.pids, x[:nm], q2[:nm], out=out[:nm], member=mem), steps, warm)
         line["members"] = {"value": world * nm * 11 * steps / secs, "unit": UNIT, "ms_per_step": secs / steps * 1e3,
-                           "queries_per_gpu_per_step": nm, "nmem": 100, "kernels": kernel_table(prof, steps)}
+                           "queries_per_gpu_per_step": nm, "nmem": 100, "kernels": kernel_table(prof, steps),
+                           "roofline": {"bound": "hbm", "achieved": (BYTES_PER_QUERY + 4) * nm / (secs / steps) / 1e9,
+                                        "peak": peak_gbs, "unit": "GB/s",
+                                        "frac": (BYTES_PER_QUERY + 4) * nm / (secs / steps) / 1e9 / peak_gbs,
+                                        "traffic": None, "peak_source": peak_src,
+                                        "note": "whole call (partition + binned kernel + gather), 108 algorithmic B/query"}}
         mg.close()
         del mem
 

@@ -18,7 +18,8 @@
 //
 // How: ONE persistent kernel per call, CTAs pull tickets in the order (lag kLag = 3 rounds)
 //      round r = [ A(r) tiles | B(r-3) items ]
-//   A(c), one item per 1024 queries of chunk c: read x,q2 (coalesced), classify, locate the cell,
+//   A(c), one item per 1024 queries of chunk c: read x,q2 (coalesced), classify, locate the cell (a thread
+//      takes its 4 queries through the steps together, so that loads and logarithms overlap),
 //      t_x,t_q (the two logs), coarse/fine key, tile-local counting sort by coarse key, payload
 //      stores; zero-fill of the tile's output rows.
 //   B(c), one item per coarse key: copy the key's payloads and its 4 grid columns (4 x nq x 96 B)
