@@ -100,8 +100,8 @@ int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double
 int pdf_grid_set_coupling(pdf_grid *g, const double *C);
 /* caller-owned DEVICE scratch for the binned path; must stay valid until replaced or the grid is
  * destroyed; bytes >= pdf_workspace_bytes(g, n) for the largest n it will be used with (the
- * figure grows by the luminosity scratch once a coupling has been set, so query it after
- * pdf_grid_set_coupling; for a grid with nmem > 1 it includes the member-partition scratch,
+ * figure grows by the luminosity scratch (176 bytes per event, up to 2^24 events) once a coupling
+ * has been set, so query it after pdf_grid_set_coupling; for a grid with nmem > 1 it includes the member-partition scratch,
  * 108 bytes per query up to 2^25 queries).  The contents are scratch: one evaluation call at a time may use it.
  * dev_ptr == NULL detaches. */
 int pdf_grid_set_workspace(pdf_grid *g, void *dev_ptr, size_t bytes);

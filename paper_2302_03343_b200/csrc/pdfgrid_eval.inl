@@ -52,12 +52,12 @@ int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, cons
             return binned_members<LaunchScope>(g->d, g->bplan, cm, n, x, q2, member, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
     }
     bool ok_binned = binned_qualifies(g->bplan, cm, member);
+    const size_t need = binned_workspace_bytes(g->bplan, n, g->chunk);      // what THIS call uses of the workspace
     bool want_binned = (g->path == PDF_PATH_BINNED) ||
-                       (g->path == PDF_PATH_AUTO && g->ws && ok_binned && n >= kAutoMinN &&
-                        g->ws_bytes >= pdf_workspace_bytes(g, n));
+                       (g->path == PDF_PATH_AUTO && g->ws && ok_binned && n >= kAutoMinN && g->ws_bytes >= need);
     if (want_binned) {
         if (!ok_binned) return PDF_EINVAL;
-        if (!g->ws || g->ws_bytes < pdf_workspace_bytes(g, n)) return PDF_EWORKSPACE;
+        if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
         return binned_xfxq2<LaunchScope>(g->d, g->bplan, cm, n, x, q2, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
     }
     return launch_direct(g, cm, n, x, q2, member, out, ld_out, s);
@@ -73,7 +73,7 @@ size_t pdf_workspace_bytes(const pdf_grid *g, long long n)
 {
     if (!g || n < 0) return 0;
     size_t b = binned_workspace_bytes(g->bplan, n, g->chunk);
-    if (b && g->d.C) b += binned_lumi_scratch_bytes(g->bplan) + 256;    // pdf_lumi slices (only once a coupling is set)
+    if (b && g->d.C) b += binned_lumi_scratch_bytes(g->bplan, n) + 256;    // pdf_lumi slices (only once a coupling is set)
     if (g->d.nmem > 1) {                                                // a-8: member partition scratch (all flavours)
         size_t m = binned_members_bytes(g->bplan, g->d, n, g->chunk, g->d.nflav);
         if (m > b) b = m;
@@ -109,9 +109,11 @@ int pdf_lumi(const pdf_grid *g, long long n, const double *x1, const double *x2,
     if (n == 0) return PDF_OK;
     if (!x1 || !x2 || !q2 || !weights || !out) return PDF_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
+    const size_t need = binned_workspace_bytes(g->bplan, n < kLumiSlice ? n : kLumiSlice, g->chunk) +
+                        binned_lumi_scratch_bytes(g->bplan, n) + 256;
     bool want_binned = binned_lumi_qualifies(g->bplan) &&
                        (g->path == PDF_PATH_BINNED || (g->path == PDF_PATH_AUTO && g->ws && n >= kAutoMinN &&
-                                                       g->ws_bytes >= pdf_workspace_bytes(g, n)));
+                                                       g->ws_bytes >= need));
     if (want_binned)
         return binned_lumi<LaunchScope>(g->d, g->bplan, g->h_C.data(), n, x1, x2, q2, weights, out, g->ws, g->ws_bytes, g->chunk, s);
     const long long slice = 1LL << 30;
