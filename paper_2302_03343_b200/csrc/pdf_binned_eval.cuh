@@ -324,12 +324,12 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
             const int g = lane >> 2, t = lane & 3;
             const CellTab cq = G.cq[fk];
             const WCoef kq = weight_coef(cq, t);
-            const AxisNodes qn = q_nodes(cq, fk);
+            const int edge_lo = cq.aL == 1.0 ? 1 : 0, edge_hi = cq.aR == 1.0 ? 1 : 0;   // one-sided ends of a sub-grid (q_nodes)
             double b0[4], b1[4];
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
                 const int tr = t ^ r;
-                const int row = tr == 0 ? qn.n[0] : tr == 1 ? qn.n[1] : tr == 2 ? qn.n[2] : qn.n[3];
+                const int row = fk - 1 + tr + (tr == 0 ? edge_lo : 0) - (tr == 3 ? edge_hi : 0);
                 const unsigned pn = snode(sVa, row, t);
                 b0[r] = lds_f64(pn + 8u * g);
                 b1[r] = g < 4 ? lds_f64(pn + 8u * (8 + g)) : 0.0;
