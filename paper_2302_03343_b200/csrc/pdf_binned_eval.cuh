@@ -195,7 +195,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 struct BSmem {            // 32-bit shared-window addresses
     unsigned sP;          // uint4 [cap][2] payloads
     unsigned sV;          // double [nqt][4][12]
-    unsigned bkey;        // u8 [cap/32 + nfk] fine key of every 32-query batch
+    unsigned bkey;        // u32 [cap/32 + nfk] descriptor of every 32-query batch: fine key | queries << 8 | first slot in `order` << 16
     unsigned fcnt;        // int [nfk]
     unsigned foff;        // int [nfk+1]
     unsigned bstart;      // int [nfk+1]
@@ -288,9 +288,13 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         }
         if (lane == 0) { sts_u32(foff + 4u * B.nfk, (unsigned)carry_o); sts_u32(bstart + 4u * B.nfk, (unsigned)carry_b); }
         __syncwarp();
-        for (int k = lane; k < B.nfk; k += 32) {           // batch -> fine key table
+        for (int k = lane; k < B.nfk; k += 32) {           // batch descriptors
             const int b0 = (int)lds_u32(bstart + 4u * k), b1 = (int)lds_u32(bstart + 4u * (k + 1));
-            for (int bb = b0; bb < b1; ++bb) asm volatile("st.shared.u8 [%0], %1;" ::"r"(bkey + (unsigned)bb), "r"(k) : "memory");
+            const int c = (int)lds_u32(fcnt + 4u * k), fo = (int)lds_u32(foff + 4u * k);
+            for (int bb = b0; bb < b1; ++bb) {
+                const int first = (bb - b0) * 32;
+                sts_u32(bkey + 4u * (unsigned)bb, (unsigned)k | ((unsigned)min(32, c - first) << 8) | ((unsigned)(fo + first) << 16));
+            }
         }
     }
     cta_sync();
@@ -312,13 +316,10 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         fb = __shfl_sync(0xffffffffu, fb, 0);              // last keys first: the extrapolation classes
         if (fb >= total) break;                            // (long, few lanes) must not form the tail
         fb = total - 1 - fb;
-        int fk;
-        asm volatile("ld.shared.u8 %0, [%1];" : "=r"(fk) : "r"(bkey + (unsigned)fb) : "memory");
-        const int kcnt = (int)lds_u32(fcnt + 4u * fk);
-        PDF_ASSERT(fk >= 0 && fk < B.nfk && fb >= 0 && fb < A.scap / 32 + B.nfk);
-        const int first = (fb - (int)lds_u32(bstart + 4u * fk)) * 32;
-        const int nact = min(32, kcnt - first);
-        const unsigned ord0 = order + 2u * (lds_u32(foff + 4u * fk) + first);
+        const unsigned desc = lds_u32(bkey + 4u * (unsigned)fb);
+        const int fk = (int)(desc & 0xffu), nact = (int)((desc >> 8) & 0x3fu);
+        PDF_ASSERT(fk < B.nfk && fb >= 0 && fb < A.scap / 32 + B.nfk && nact >= 1 && nact <= 32);
+        const unsigned ord0 = order + 2u * (desc >> 16);
         if (!lowx_unit && fk < B.nqt) {
             // ---- interior cell (i, fk): DMMA tiles of 8 queries ----
             const int g = lane >> 2, t = lane & 3;
@@ -441,7 +442,7 @@ __host__ __device__ inline size_t bsmem_item_bytes(int nqt, int nck, int nfk, in
 {
     size_t b = (size_t)cap * 32;                                        // sP
     b += (size_t)nqt * 4 * kNFP * sizeof(double);                       // sV
-    b += ((size_t)(cap / 32 + nfk) + 15) / 16 * 16;                     // bkey
+    b += ((size_t)(cap / 32 + nfk) * 4 + 15) / 16 * 16;                 // bkey (batch descriptors)
     b += (size_t)(3 * nfk + 8) * sizeof(int);                           // fcnt, foff, bstart, next
     b += ((size_t)cap * sizeof(unsigned short) + 15) / 16 * 16;         // order
     size_t a = (size_t)kTileA * 32 + (size_t)2 * nck * sizeof(unsigned); // A items: payloads, cnt, base
