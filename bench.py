@@ -300,6 +300,8 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
                                         "frac": (BYTES_PER_QUERY + 4) * nm / (secs / steps) / 1e9 / peak_gbs,
                                         "traffic": None, "peak_source": peak_src,
                                         "note": "whole call (partition + binned kernel + gather), 108 algorithmic B/query"}}
+        members_sample = (mspec, x[:50_000].cpu().numpy(), q2[:50_000].cpu().numpy(), mem[:50_000].cpu().numpy(),
+                          out[:50_000].clone().cpu().numpy())
         mg.close()
         del mem
 
@@ -360,6 +362,16 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
         lok = ~np.isnan(lref)
         line["lumi"]["parity_sample"] = {"n": int(lref.size), "worst_err_over_tol": float(np.max(lerr[lok] / np.maximum(ltol[lok], 1e-300))),
                                          "nan_match": bool(np.array_equal(np.isnan(lumi_sample[4]), ~lok))}
+        # and for the replica batch (50 000 sampled queries of the timed launch, 100 members)
+        if nm > 0:
+            ms_, mx, mq, mm, mgot = members_sample
+            mog = oracle.OracleGrid(ms_.x_knots.numpy(), [q.numpy() for q in ms_.q2_subgrids], ms_.values.numpy(), ms_.pids,
+                                    nmem=ms_.nmem)
+            mref, mS = mog.xfxq2(ms_.pids, mx, mq, member=mm, want_scale=True)
+            mok = ~np.isnan(mref)
+            mtol = 1e-12 * np.abs(mref) + 1e-14 * mS
+            line["members"]["parity_sample"] = {"n": int(mx.size), "worst_err_over_tol": float(np.max(np.abs(mgot - mref)[mok] / np.maximum(mtol[mok], 1e-300))),
+                                                "nan_match": bool(np.array_equal(np.isnan(mgot), ~mok))}
         np_ = min(200_000, ns)
         got = out_sample.cpu().numpy()[:np_]
         _, S = og.xfxq2(spec.pids, cx[:np_], cq[:np_], want_scale=True)
