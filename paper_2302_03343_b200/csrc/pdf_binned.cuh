@@ -91,7 +91,8 @@ struct BinnedPlan {
     short *d_lutx = nullptr, *d_lutq = nullptr;
     double *d_plus = nullptr;                 // scratch of k_q2plus
     int max_ctas = 0;                         // co-resident CTAs of the persistent kernel
-    long long default_chunk = 1 << 18;
+    long long default_chunk = 352 * 1024;     // measured (C2, n = 1e8): 192k 12.2, 256k 11.2, 320k 11.1, 352k 10.95, 384k 11.1 ms;
+                                              // 352k/195 cells + 4.6 sigma is what one shared-memory segment (kMaxCap) holds
 };
 
 struct BinWorkspace {                         // carved out of the caller's workspace
@@ -112,7 +113,8 @@ inline long long binned_chunk(const BinnedPlan &p, long long n, long long chunk_
 }
 
 // shared-memory segment of a B item: a uniform cloud puts chunk/ncx queries on an x cell (1344 at
-// 256k and 195 cells); 1.125x that + 96 (~ +7 sigma) lets such a bin go through in one segment
+// 256k and 195 cells, 1848 at the default 352k); 1.125x that + 96, capped at kMaxCap, lets such a bin go
+// through in one segment
 inline int binned_scap(const BinnedPlan &p, long long chunk)
 {
     long long c = chunk / (p.dev.ncx > 0 ? p.dev.ncx : 1);

@@ -2,7 +2,7 @@
 // member id per query).
 //
 // All members share the knots, so cell search, t_x / t_q and the node weights do not depend on
-// the member; only the values do.  With ~10^6 (member, cell) pairs no chunk of 2^18 queries is
+// the member; only the values do.  With ~10^6 (member, cell) pairs no chunk of 3.6e5 queries is
 // cell-coherent, so the queries of a slice (<= 2^25) are first partitioned by member:
 //   k_member_hist     histogram of the member ids of the slice (shared-memory counters per CTA)
 //   k_member_plan     exclusive scan -> first slot of every member; chunk table: every member's run
