@@ -46,7 +46,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=100_000_000, help="queries per GPU and step")
     ap.add_argument("--lumi-n", type=int, default=100_000_000)
-    ap.add_argument("--members-n", type=int, default=20_000_000)
+    ap.add_argument("--members-n", type=int, default=100_000_000)
     ap.add_argument("--e2e-n", type=int, default=0, help="0 = same as --n")
     ap.add_argument("--cpu-sample", type=int, default=10_000_000)
     ap.add_argument("--path", default="auto", choices=["auto", "direct", "binned"])
