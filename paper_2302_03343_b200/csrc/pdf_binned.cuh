@@ -134,7 +134,7 @@ inline int binned_cap(const BinnedPlan &p, long long chunk)
     return (int)c;
 }
 
-inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+__host__ __device__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 inline size_t binned_workspace_bytes(const BinnedPlan &p, long long n, long long chunk_opt)
 {

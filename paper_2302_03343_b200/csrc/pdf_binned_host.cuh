@@ -205,6 +205,8 @@ inline int binned_members(const GridDev &G, const BinnedPlan &p, const ColMap &c
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const size_t hsm = sizeof(unsigned) * (size_t)G.nmem;
+    if (cudaFuncSetAttribute(k_member_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)member_scatter_smem(G.nmem)) != cudaSuccess)
+        return PDF_ECUDA;
     for (long long off = 0; off < n; off += slice) {
         const long long m = n - off < slice ? n - off : slice;
         if (cudaMemsetAsync(M.hist, 0, hsm, s) != cudaSuccess) return PDF_ECUDA;
@@ -219,7 +221,7 @@ inline int binned_members(const GridDev &G, const BinnedPlan &p, const ColMap &c
         }
         {
             Scope sc(s, "k_member_scatter");
-            k_member_scatter<<<(unsigned)((m + 256 * kMemTileQ - 1) / (256 * kMemTileQ)), 256, 2 * hsm, s>>>(
+            k_member_scatter<<<(unsigned)((m + kMemScatThreads * kMemTileQ - 1) / (kMemScatThreads * kMemTileQ)), kMemScatThreads, member_scatter_smem(G.nmem), s>>>(
                 x + off, q2 + off, member + off, m, G.nmem, M.cursor, M.xs, M.q2s, M.inv);
         }
         int rc = binned_xfxq2<Scope>(G, p, cm, m, M.xs, M.q2s, M.tmp, cm.n, ws, ws_x, chunk_opt, s, 1, M.ctab, M.nchunks);

@@ -8,8 +8,9 @@
 //   k_member_plan     exclusive scan -> first slot of every member; chunk table: every member's run
 //                     is cut in equal pieces of <= chunk queries {first, count, member}
 //   k_member_scatter  x, q2 -> xs, q2s in member order; inv[i] = slot of query i.  A CTA ranks its
-//                     2048 queries per member in shared memory and reserves its runs with one
-//                     global atomic per (CTA, member): ~20 consecutive slots per run
+//                     4096 queries per member in shared memory, reserves its runs with one global
+//                     atomic per (CTA, member), sorts the tile in shared memory and writes the runs out
+//                     in slot order (~40 consecutive slots per run at 100 members)
 //   k_pdf_stream      the persistent binned kernel over the chunk table: chunk c evaluates against
 //                     V + member(c) * memstride and writes rows in SORTED order to tmp
 //   k_member_gather   out[i][:] = tmp[inv[i]][:] (coalesced writes, row-granular reads); queries
@@ -23,6 +24,7 @@ namespace pdfg {
 constexpr long long kMemSlice = 1 << 25;      // queries partitioned at a time (scratch: 108 B per query of a slice)
 constexpr int kMemMax = 4096;                 // members the shared-memory histograms hold
 constexpr int kMemTileQ = 8;                  // queries per thread of k_member_scatter
+constexpr int kMemScatThreads = 512;          // its CTA: 4096 queries, sorted by member in shared memory before they leave
 constexpr unsigned kNoSlot = 0xffffffffu;
 
 struct MemberWs {
@@ -113,43 +115,90 @@ k_member_plan(const unsigned *__restrict__ hist, int nmem, int chunk, unsigned *
     *nchunks = nc;
 }
 
-__global__ void __launch_bounds__(256)
+// shared memory of k_member_scatter: 3 counter arrays, warp totals, then the tile sorted by member
+inline size_t member_scatter_smem(int nmem)
+{
+    return align_up(sizeof(unsigned) * 3 * (size_t)nmem + 256, 16) + (size_t)kMemScatThreads * kMemTileQ * (8 + 8 + 2);
+}
+
+__global__ void __launch_bounds__(kMemScatThreads)
 k_member_scatter(const double *__restrict__ x, const double *__restrict__ q2, const int *__restrict__ member,
                  long long n, int nmem, unsigned *__restrict__ cursor, double *__restrict__ xs,
                  double *__restrict__ q2s, unsigned *__restrict__ inv)
 {
-    extern __shared__ unsigned s_c[];             // [nmem] counts, then [nmem] bases
-    unsigned *s_b = s_c + nmem;
-    for (int k = threadIdx.x; k < nmem; k += 256) s_c[k] = 0u;
+    constexpr int T = kMemScatThreads, TILE = T * kMemTileQ;
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    unsigned *s_c = reinterpret_cast<unsigned *>(s_raw);          // [nmem] queries of the tile per member
+    unsigned *s_b = s_c + nmem;                                   // [nmem] first global slot of the tile's run
+    unsigned *s_l = s_b + nmem;                                   // [nmem] first slot of the run inside the sorted tile
+    unsigned *s_w = s_l + nmem;                                   // [T/32 + 1] scan scratch
+    double *sx = reinterpret_cast<double *>(s_raw + align_up(sizeof(unsigned) * 3 * (size_t)nmem + 256, 16));
+    double *sq = sx + TILE;
+    unsigned short *sm = reinterpret_cast<unsigned short *>(sq + TILE);
+    for (int k = threadIdx.x; k < nmem; k += T) s_c[k] = 0u;
     __syncthreads();
-    const long long t0 = (long long)blockIdx.x * (256 * kMemTileQ);
-    unsigned tag[kMemTileQ];                      // member << 12 | rank inside the CTA's tile
+    const long long t0 = (long long)blockIdx.x * TILE;
+    unsigned tag[kMemTileQ];                      // member << 16 | rank inside the CTA's tile
+    double xv[kMemTileQ], qv[kMemTileQ];
 #pragma unroll
     for (int q = 0; q < kMemTileQ; ++q) {
-        const long long e = t0 + q * 256 + threadIdx.x;
+        const long long e = t0 + q * T + threadIdx.x;
         tag[q] = kNoSlot;
+        xv[q] = 0.0; qv[q] = 0.0;
         if (e < n) {
             const int m = __ldcs(member + e);
-            if (m >= 0 && m < nmem) tag[q] = ((unsigned)m << 12) | atomicAdd(s_c + m, 1u);
+            xv[q] = __ldcs(x + e); qv[q] = __ldcs(q2 + e);
+            if (m >= 0 && m < nmem) tag[q] = ((unsigned)m << 16) | atomicAdd(s_c + m, 1u);
         }
     }
     __syncthreads();
-    for (int k = threadIdx.x; k < nmem; k += 256) {
+    // one global atomic per (CTA, member); exclusive scan of the counts = the runs inside the sorted tile
+    for (int k = threadIdx.x; k < nmem; k += T) {
         const unsigned c = s_c[k];
         s_b[k] = c ? atomicAdd(cursor + k, c) : 0u;
     }
+    {
+        const int per = (nmem + T - 1) / T, b0 = threadIdx.x * per;
+        unsigned sum = 0;
+        for (int i = 0; i < per; ++i) if (b0 + i < nmem) sum += s_c[b0 + i];
+        unsigned inc = sum;
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { unsigned v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        if (lane == 31) s_w[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            unsigned w = lane < T / 32 ? s_w[lane] : 0u, wi = w;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { unsigned v = __shfl_up_sync(0xffffffffu, wi, d); if (lane >= d) wi += v; }
+            if (lane < T / 32) s_w[lane] = wi - w;
+            if (lane == 31) s_w[T / 32] = wi;                     // valid queries of the tile
+        }
+        __syncthreads();
+        unsigned run = s_w[warp] + inc - sum;
+        for (int i = 0; i < per; ++i) if (b0 + i < nmem) { s_l[b0 + i] = run; run += s_c[b0 + i]; }
+    }
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < kMemTileQ; ++q) {
-        const long long e = t0 + q * 256 + threadIdx.x;
+        const long long e = t0 + q * T + threadIdx.x;
         if (e >= n) continue;
         unsigned pos = kNoSlot;
         if (tag[q] != kNoSlot) {
-            pos = s_b[tag[q] >> 12] + (tag[q] & 0xfffu);
-            xs[pos] = __ldcs(x + e);
-            q2s[pos] = __ldcs(q2 + e);
+            const unsigned m = tag[q] >> 16, rank = tag[q] & 0xffffu;
+            const unsigned l = s_l[m] + rank;
+            sx[l] = xv[q]; sq[l] = qv[q]; sm[l] = (unsigned short)m;
+            pos = s_b[m] + rank;
         }
         inv[e] = pos;
+    }
+    __syncthreads();
+    // the sorted tile leaves in slot order: consecutive threads write consecutive slots of a run
+    const unsigned total = s_w[T / 32];
+    for (unsigned j = threadIdx.x; j < total; j += T) {
+        const unsigned m = sm[j], g = s_b[m] + (j - s_l[m]);
+        xs[g] = sx[j];
+        q2s[g] = sq[j];
     }
 }
 
@@ -159,19 +208,30 @@ __global__ void __launch_bounds__(256)
 k_member_gather(const double *__restrict__ tmp, const unsigned *__restrict__ inv, long long n, int npid,
                 double *__restrict__ out, long long ld, unsigned long long *err_count)
 {
+    constexpr int U = 4;                                              // row reads in flight per thread (latency-bound gather)
     unsigned long long bad = 0;
     const unsigned per = 256u * (unsigned)npid;                       // elements of 256 rows
     for (long long r0 = (long long)blockIdx.x * 256; r0 < n; r0 += (long long)gridDim.x * 256) {
         const unsigned rows = n - r0 < 256 ? (unsigned)(n - r0) : 256u;
         const unsigned lim = rows * (unsigned)npid;
-        for (unsigned kk = threadIdx.x; kk < per; kk += 256u) {
-            if (kk >= lim) break;
-            const unsigned il = kk / (unsigned)npid, p = kk - il * (unsigned)npid;
-            const unsigned pos = __ldg(inv + r0 + il);
-            double v;
-            if (pos == kNoSlot) { v = qnan(); bad += p == 0u; }
-            else v = __ldcs(tmp + (size_t)pos * npid + p);
-            __stcs(out + (r0 + il) * ld + p, v);
+        for (unsigned k0 = threadIdx.x; k0 < per; k0 += 256u * U) {
+            unsigned il[U], p[U], pos[U];
+            double v[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const unsigned kk = k0 + 256u * u;
+                il[u] = kk / (unsigned)npid; p[u] = kk - il[u] * (unsigned)npid;
+                pos[u] = kk < lim ? __ldg(inv + r0 + il[u]) : kNoSlot;
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) v[u] = pos[u] != kNoSlot ? __ldcs(tmp + (size_t)pos[u] * npid + p[u]) : qnan();
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const unsigned kk = k0 + 256u * u;
+                if (kk >= lim) continue;
+                bad += (pos[u] == kNoSlot && p[u] == 0u) ? 1u : 0u;
+                __stcs(out + (r0 + il[u]) * ld + p[u], v[u]);
+            }
         }
     }
     if (bad) atomicAdd(err_count, bad);
