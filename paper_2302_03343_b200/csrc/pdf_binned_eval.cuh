@@ -527,10 +527,11 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
 #ifdef PDF_PHASES
             ph_t = clock64();
 #endif
-            __threadfence();
+            // release: the barrier orders every thread's stores before thread 0's gpu-scope fence, and the
+            // fence is cumulative (the pattern of a grid-wide barrier: bar.sync; one thread fences and signals)
             cta_sync();
             PH(20);
-            if (threadIdx.x == 0) atomicAdd(a_done, 1ULL);
+            if (threadIdx.x == 0) { __threadfence(); atomicAdd(a_done, 1ULL); }
         } else {
 #ifdef PDF_PHASES
             long long bt0 = clock64();
@@ -555,10 +556,10 @@ __global__ void __launch_bounds__(kBinThreads, PDF_MINB) k_pdf_stream(const __gr
             }
             long long ph_t = clock64();
 #endif
-            __threadfence();
             cta_sync();
             PH(7);
             if (threadIdx.x == 0) {
+                __threadfence();
                 unsigned long long old = atomicAdd(b_fin, 1ULL);
                 if (old + 1 == (gen + 1) * TB) {                               // last item of the chunk
                     A.W.ovf_count[slot] = 0u;
