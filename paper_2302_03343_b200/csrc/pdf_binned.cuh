@@ -18,8 +18,8 @@
 //
 // How: ONE persistent kernel per call, CTAs pull tickets in the order (lag kLag = 3 rounds)
 //      round r = [ A(r) tiles | B(r-3) items ]
-//   A(c), one item per 1024 queries of chunk c: read x,q2 (coalesced), classify, locate the cell (a thread
-//      takes its 4 queries through the steps together, so that loads and logarithms overlap),
+//   A(c), one item per 2048 queries of chunk c: read x,q2 (coalesced), classify, locate the cell (a thread
+//      takes its queries through the steps in groups of 2, so that loads and logarithms overlap),
 //      t_x,t_q (the two logs), coarse/fine key, tile-local counting sort by coarse key, payload
 //      stores; zero-fill of the tile's output rows.
 //   B(c), one item per coarse key: copy the key's payloads and its 4 grid columns (4 x nq x 96 B)
@@ -42,7 +42,7 @@ namespace pdfg {
 constexpr int kBinThreads = 256;              // CTA size of the persistent kernel
 constexpr int kBinWarps = kBinThreads / 32;
 #ifndef PDF_TILEQ
-#define PDF_TILEQ 4
+#define PDF_TILEQ 8
 #endif
 #ifndef PDF_MINB
 #define PDF_MINB 2
@@ -51,7 +51,7 @@ constexpr int kBinWarps = kBinThreads / 32;
 #define PDF_LAG 3
 #endif
 constexpr int kTileQ = PDF_TILEQ;                     // queries per thread in an A item
-constexpr int kTileA = kBinThreads * kTileQ;  // 1024 queries per A item
+constexpr int kTileA = kBinThreads * kTileQ;  // 2048 queries per A item (1024: 10.76, 1536: 10.26, 2048: 10.22, 3072: 10.21 ms)
 constexpr int kOvfItems = 4;                  // B items per chunk that drain the overflow list
 constexpr int kLag = PDF_LAG;                       // B(c) tickets follow A(c) tickets by this many rounds
 #ifndef PDF_RING_EXTRA

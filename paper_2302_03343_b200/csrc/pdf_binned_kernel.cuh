@@ -178,6 +178,13 @@ __device__ __forceinline__ void zero_fill_slice(const ZeroFill &z, int slice, in
 // ---- A item: classify, locate, t_x / t_q, tile-local sort by coarse key, payload stores ---------
 // Per query only (x, q2) live in registers across the loop; the payload (a, b, idx, fk) and the
 // (coarse key, rank) pair are parked in shared memory until the tile's runs have been reserved.
+#ifndef PDF_AGRP
+#define PDF_AGRP 2
+#endif
+constexpr int kGrp = PDF_AGRP;         // queries of a thread that go through the A item's steps together
+                                       // (1024-query tiles: 1: 11.67, 2: 10.93, 4: 10.77 ms; 2048-query tiles: 2: 10.22, 4: 10.54 ms)
+static_assert(kTileQ % kGrp == 0, "kTileQ must be a multiple of kGrp");
+
 struct ASmem {            // 32-bit shared-window addresses
     unsigned cnt;         // unsigned [nck] queries of this tile per coarse key
     unsigned base;        // unsigned [nck] first slot of the tile's run in the key's bin
@@ -213,12 +220,15 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
     // The thread's kTileQ queries go through the steps together, so that the independent loads and
     // logarithms of one step overlap (the shared-memory accessors are ordered asm statements: only
     // what is issued before the first use runs concurrently).
-    double xv[kTileQ], qv[kTileQ], lx[kTileQ], lq[kTileQ];
-    int gi[kTileQ], gj[kTileQ];
-    unsigned st[kTileQ];                                           // 0: not a query, 1: invalid, 2: valid
+    // in groups of kGrp (a rolled loop over the groups keeps the code small)
+#pragma unroll 1
+    for (int g0 = 0; g0 < kTileQ; g0 += kGrp) {
+    double xv[kGrp], qv[kGrp], lx[kGrp], lq[kGrp];
+    int gi[kGrp], gj[kGrp];
+    unsigned st[kGrp];                                           // 0: not a query, 1: invalid, 2: valid
 #pragma unroll
-    for (int q = 0; q < kTileQ; ++q) {
-        const long long e = t0 + q * kBinThreads + threadIdx.x;
+    for (int q = 0; q < kGrp; ++q) {
+        const long long e = t0 + (g0 + q) * kBinThreads + threadIdx.x;
         xv[q] = 1.0; qv[q] = 1.0;
         if (e < t1) { xv[q] = __ldcs(A.x + e); qv[q] = __ldcs(A.q2 + e); }
     }
@@ -226,23 +236,23 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
     // The ring slot must have been drained by B(c - kRing) before this tile touches its bins (after the
     // next barrier); polled here, under the loads.  The whole warp polls (same address): a lane that
     // spins alone would reach the barrier apart from its warp, and bar.sync counts such a warp twice.
-    if (threadIdx.x < 32 && ring_target) wait_counter(ring_free, ring_target);
+    if (g0 == 0 && threadIdx.x < 32 && ring_target) wait_counter(ring_free, ring_target);
     PH(11);
-    zero_fill_slice(zf, 0, 4);
+    zero_fill_slice(zf, (g0 / kGrp) * 4 + 0, 4 * (kTileQ / kGrp));
     PH(22);
 #pragma unroll
-    for (int q = 0; q < kTileQ; ++q) {
-        const long long e = t0 + q * kBinThreads + threadIdx.x;
+    for (int q = 0; q < kGrp; ++q) {
+        const long long e = t0 + (g0 + q) * kBinThreads + threadIdx.x;
         st[q] = e < t1 ? ((!(finite_pos(xv[q]) && finite_pos(qv[q])) || xv[q] > xmax) ? 1u : 2u) : 0u;   // C-10
         lx[q] = 0.0; lq[q] = 0.0;
         if (st[q] == 2u) { lx[q] = log(xv[q]); lq[q] = log(qv[q]); }
     }
     PH(23);
-    zero_fill_slice(zf, 1, 4);
+    zero_fill_slice(zf, (g0 / kGrp) * 4 + 1, 4 * (kTileQ / kGrp));
     PH(22);
     // start guesses of both searches (buckets clamped: always a valid table entry)
 #pragma unroll
-    for (int q = 0; q < kTileQ; ++q) {
+    for (int q = 0; q < kGrp; ++q) {
         int bx = (int)((lx[q] - u0) * B.lutx_scale), bq = (int)((lq[q] - s0) * B.lutq_scale);
         bx = bx < 0 ? 0 : (bx >= kLutSize ? kLutSize - 1 : bx);
         bq = bq < 0 ? 0 : (bq >= kLutSize ? kLutSize - 1 : bq);
@@ -254,9 +264,9 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
     // steps on knots loaded together, a check of the C-4 condition on the raw values, and the exact
     // walk only where the check fails (coarser tables, rounding of the bucket index).
     {
-        double xa[kTileQ], xb[kTileQ], xc[kTileQ], qa[kTileQ], qb[kTileQ], qc[kTileQ], qd[kTileQ];
+        double xa[kGrp], xb[kGrp], xc[kGrp], qa[kGrp], qb[kGrp], qc[kGrp], qd[kGrp];
 #pragma unroll
-        for (int q = 0; q < kTileQ; ++q) {
+        for (int q = 0; q < kGrp; ++q) {
             const int c = gi[q], g = gj[q];
             xa[q] = lds_f64(s_xk + 8u * c);
             xb[q] = lds_f64(s_xk + 8u * min(c + 1, nx - 1));
@@ -268,7 +278,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         }
         bool fix = false;
 #pragma unroll
-        for (int q = 0; q < kTileQ; ++q) {
+        for (int q = 0; q < kGrp; ++q) {
             const double x = xv[q], q2 = qv[q];
             int c = gi[q];
             const bool ux = c < nx - 2 && xb[q] <= x;              // x cells: [0, nx-2]
@@ -290,7 +300,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         }
         if (fix) {
 #pragma unroll
-            for (int q = 0; q < kTileQ; ++q) {
+            for (int q = 0; q < kGrp; ++q) {
                 const double x = xv[q], q2 = qv[q];
                 if (st[q] != 2u) continue;
                 if (!(x < xmin)) {
@@ -309,17 +319,17 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         }
     }
     PH(24);
-    zero_fill_slice(zf, 2, 4);
+    zero_fill_slice(zf, (g0 / kGrp) * 4 + 2, 4 * (kTileQ / kGrp));
     PH(22);
     // cell constants (L1-resident tables) and the knots above, all in flight
     {
-        int adj[kTileQ];
+        int adj[kGrp];
 #pragma unroll
-        for (int q = 0; q < kTileQ; ++q) adj[q] = (int)__ldg(G.cell_adj + gj[q]);   // last knot of a sub-grid -> its last cell
-        double2 ci[kTileQ], cj[kTileQ];
-        double kx1[kTileQ], kq1[kTileQ];
+        for (int q = 0; q < kGrp; ++q) adj[q] = (int)__ldg(G.cell_adj + gj[q]);   // last knot of a sub-grid -> its last cell
+        double2 ci[kGrp], cj[kGrp];
+        double kx1[kGrp], kq1[kGrp];
 #pragma unroll
-        for (int q = 0; q < kTileQ; ++q) {
+        for (int q = 0; q < kGrp; ++q) {
             gj[q] -= adj[q];
             ci[q] = __ldg(reinterpret_cast<const double2 *>(G.cx + gi[q]));          // lo_log, inv_d
             cj[q] = __ldg(reinterpret_cast<const double2 *>(G.cq + gj[q]));
@@ -330,7 +340,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         const double inv_du0 = 1.0 / (__ldg(G.uk + 1) - u0);
         const double sA = __ldg(G.sk + nqt - 2), inv_ds = 1.0 / (__ldg(G.sk + nqt - 1) - sA), inv_qmin = 1.0 / qmin;
 #pragma unroll
-        for (int q = 0; q < kTileQ; ++q) {
+        for (int q = 0; q < kGrp; ++q) {
             const double x = xv[q], q2 = qv[q];
             const bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
             const double ta = lowx ? (lx[q] - u0) * inv_du0                           // theta_x (C-7)
@@ -342,11 +352,11 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         }
     }
     PH(25);
-    zero_fill_slice(zf, 3, 4);
+    zero_fill_slice(zf, (g0 / kGrp) * 4 + 3, 4 * (kTileQ / kGrp));
     PH(22);
 #pragma unroll
-    for (int q = 0; q < kTileQ; ++q) {
-        const int ql = q * kBinThreads + threadIdx.x;             // query index inside the tile
+    for (int q = 0; q < kGrp; ++q) {
+        const int ql = (g0 + q) * kBinThreads + threadIdx.x;             // query index inside the tile
         const double x = xv[q], q2 = qv[q];
         const bool lowx = x < xmin, lowq = q2 < qmin, highq = q2 > qmax;
         unsigned tag = st[q] == 0u ? 0xffffffffu : 0xfffffffeu;
@@ -367,6 +377,7 @@ __device__ __forceinline__ void a_item(const StreamArgs &A, const SmemTables &T,
         const unsigned pa = s_pay + 32u * ql;
         sts_v2f64(pa, lx[q], lq[q]);
         sts_v4u32(pa + 16u, (unsigned)(t0 + ql - chunk_base), fk, 0u, tag);
+    }
     }
     PH(26);
     cta_sync();
