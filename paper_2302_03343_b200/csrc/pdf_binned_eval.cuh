@@ -192,10 +192,18 @@ __device__ __forceinline__ void cp_async16(unsigned saddr, const void *g)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// queries per batch of an interior cell = 1 << kCellBatchShift (a batch is a loop over 8-query DMMA
+// tiles; its prologue -- cell constants, node rows, the cell's 8 values per lane -- is paid once)
+#ifndef PDF_CELLBATCH_SHIFT
+#define PDF_CELLBATCH_SHIFT 6
+#endif
+constexpr int kCellBatchShift = PDF_CELLBATCH_SHIFT;
+static_assert(kCellBatchShift >= 5 && kCellBatchShift <= 7, "batch descriptor holds <= 255 queries");
+
 struct BSmem {            // 32-bit shared-window addresses
     unsigned sP;          // uint4 [cap][2] payloads
     unsigned sV;          // double [nqt][4][12]
-    unsigned bkey;        // u32 [cap/32 + nfk] descriptor of every 32-query batch: fine key | queries << 8 | first slot in `order` << 16
+    unsigned bkey;        // u32 [cap/32 + nfk] descriptor of every batch (<= 32 queries, interior cells <= 1 << kCellBatchShift): fine key | queries << 8 | first slot in `order` << 16
     unsigned fcnt;        // int [nfk]
     unsigned foff;        // int [nfk+1]
     unsigned bstart;      // int [nfk+1]
@@ -275,7 +283,8 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         for (int k0 = 0; k0 < B.nfk; k0 += 32) {
             int k = k0 + lane;
             int c = k < B.nfk ? (int)lds_u32(fcnt + 4u * k) : 0;
-            int nb = (c + 31) >> 5;
+            const int bsh = (!lowx_unit && k < B.nqt) ? kCellBatchShift : 5;   // interior cells: DMMA tiles, longer batches
+            int nb = (c + (1 << bsh) - 1) >> bsh;
             int so = c, sb = nb;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
@@ -291,9 +300,10 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         for (int k = lane; k < B.nfk; k += 32) {           // batch descriptors
             const int b0 = (int)lds_u32(bstart + 4u * k), b1 = (int)lds_u32(bstart + 4u * (k + 1));
             const int c = (int)lds_u32(fcnt + 4u * k), fo = (int)lds_u32(foff + 4u * k);
+            const int bmax = 1 << ((!lowx_unit && k < B.nqt) ? kCellBatchShift : 5);
             for (int bb = b0; bb < b1; ++bb) {
-                const int first = (bb - b0) * 32;
-                sts_u32(bkey + 4u * (unsigned)bb, (unsigned)k | ((unsigned)min(32, c - first) << 8) | ((unsigned)(fo + first) << 16));
+                const int first = (bb - b0) * bmax;
+                sts_u32(bkey + 4u * (unsigned)bb, (unsigned)k | ((unsigned)min(bmax, c - first) << 8) | ((unsigned)(fo + first) << 16));
             }
         }
     }
@@ -317,8 +327,8 @@ __device__ __forceinline__ void b_item(const StreamArgs &A, const BSmem &S, cons
         if (fb >= total) break;                            // (long, few lanes) must not form the tail
         fb = total - 1 - fb;
         const unsigned desc = lds_u32(bkey + 4u * (unsigned)fb);
-        const int fk = (int)(desc & 0xffu), nact = (int)((desc >> 8) & 0x3fu);
-        PDF_ASSERT(fk < B.nfk && fb >= 0 && fb < A.scap / 32 + B.nfk && nact >= 1 && nact <= 32);
+        const int fk = (int)(desc & 0xffu), nact = (int)((desc >> 8) & 0xffu);
+        PDF_ASSERT(fk < B.nfk && fb >= 0 && fb < A.scap / 32 + B.nfk && nact >= 1 && nact <= (1 << kCellBatchShift));
         const unsigned ord0 = order + 2u * (desc >> 16);
         if (!lowx_unit && fk < B.nqt) {
             // ---- interior cell (i, fk): DMMA tiles of 8 queries ----
