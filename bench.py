@@ -31,8 +31,8 @@ UNIT = "points*flavours/s"
 WORKLOAD = ("configs[2] (C2): 196x(6+8+40) LHAPDF-shaped grid, 11 flavours, "
             "5% of queries extrapolated, + alpha_s over the same Q2 (60 knots)")
 # dram__bytes_read.sum + dram__bytes_write.sum of k_pdf_stream at n = 1e8 (C2), one ncu capture of this
-# command line: profiles/r1h_traffic_pdf_stream_1e8.csv; null for any other n
-NCU_TRAFFIC_BYTES_1E8 = 5870010624 + 22529576192
+# command line: profiles/r1i_traffic_pdf_stream_1e8.csv; null for any other n
+NCU_TRAFFIC_BYTES_1E8 = 5887876352 + 22069447424
 BYTES_PER_QUERY = 16 + 88          # x, q2 in; 11 fp64 out
 BYTES_PER_EVENT = 32 + 8
 BYTES_PER_ALPHAS = 16
