@@ -33,6 +33,9 @@ WORKLOAD = ("configs[2] (C2): 196x(6+8+40) LHAPDF-shaped grid, 11 flavours, "
 # dram__bytes_read.sum + dram__bytes_write.sum of k_pdf_stream at n = 1e8 (C2), one ncu capture of this
 # command line: profiles/r1i_traffic_pdf_stream_1e8.csv; null for any other n
 NCU_TRAFFIC_BYTES_1E8 = 5887876352 + 22069447424
+# PAPER.md Table 3.3 (L1896-1905), seconds: N_rep -> (LHAPDF CPU, PDFFlow GPU, PDFFlow CPU) on the thesis's system P1
+PAPER_TABLE33 = {10: (0.08, 0.07, 0.05), 50: (0.41, 0.35, 0.28), 100: (0.83, 0.69, 0.56),
+                 200: (1.87, 1.46, 1.12), 300: (2.85, 1.29, 1.79), 400: (3.63, 1.69, 2.12)}
 BYTES_PER_QUERY = 16 + 88          # x, q2 in; 11 fp64 out
 BYTES_PER_EVENT = 32 + 8
 BYTES_PER_ALPHAS = 16
@@ -51,6 +54,7 @@ def parse_args():
     ap.add_argument("--cpu-sample", type=int, default=10_000_000)
     ap.add_argument("--path", default="auto", choices=["auto", "direct", "binned"])
     ap.add_argument("--chunk", type=int, default=0, help="binned-path chunk size (0 = library default)")
+    ap.add_argument("--table33-reps", type=int, default=10, help="timed calls per N_rep of the Table 3.3 leg (0 = skip)")
     ap.add_argument("--skip-extras", action="store_true", help="only the headline step (no lumi/members/e2e/cpu)")
     return ap.parse_args()
 
@@ -305,6 +309,47 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
         mg.close()
         del mem
 
+    # ---- NEXT-3: Table 3.3 workload: 11 flavours x 2415 x-points x N_rep members ----
+    # One pdf_xfxq2_ex call per N_rep (member-major queries, fixed Q2).  Each call is timed alone with CUDA
+    # events after an L2 flush (the whole problem would otherwise sit in the 126 MB L2 between repeats).
+    table33_sample = None
+    if args.table33_reps > 0 and rank == 0:
+        tspec = synth.grid_c1(nmem=max(synth.TABLE33_NREP))
+        tg = binding.PdfGrid.from_spec(tspec)
+        flush = torch.empty(32 * 1024 * 1024, dtype=torch.float64, device="cuda")          # 256 MB > L2
+        rows = []
+        for nrep in synth.TABLE33_NREP:
+            tx, tq, tm = synth.queries_table33(nrep, device="cuda")
+            tout = out[: tx.numel()]
+            for _ in range(3):
+                tg.pdf_xfxq2(tspec.pids, tx, tq, out=tout, member=tm)
+            ms = []
+            for _ in range(args.table33_reps):
+                flush.zero_()
+                ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                ea.record()
+                tg.pdf_xfxq2(tspec.pids, tx, tq, out=tout, member=tm)
+                eb.record()
+                torch.cuda.synchronize()
+                ms.append(ea.elapsed_time(eb))
+            ms.sort()
+            med = ms[len(ms) // 2]
+            paper = PAPER_TABLE33[nrep]
+            rows.append({"nrep": nrep, "queries": int(tx.numel()), "ms_median": med, "ms_min": ms[0],
+                         "value": tx.numel() * 11 / (med * 1e-3), "unit": UNIT,
+                         "paper_seconds": {"lhapdf_cpu": paper[0], "pdfflow_gpu": paper[1], "pdfflow_cpu": paper[2]}})
+            if nrep == max(synth.TABLE33_NREP):
+                pick = torch.arange(0, tx.numel(), 31, device="cuda")[:30_000]
+                table33_sample = (tspec, tx[pick].cpu().numpy(), tq[pick].cpu().numpy(), tm[pick].cpu().numpy(),
+                                  tout[pick].clone().cpu().numpy())
+        line["table33"] = {"workload": "Table 3.3: 11 flavours x 2415 fixed x-points x N_rep members at Q2 = 1.65^2 GeV2, "
+                                       "C1-shaped 400-member grid (lognormal member noise), member-major queries",
+                           "timing": f"median of {args.table33_reps} single calls, CUDA events, 256 MB L2 flush before each",
+                           "rows": rows,
+                           "paper_hardware": "system P1: i9-9980XE; TITAN V / RTX 2080 Ti (PAPER.md Table 3.2, 3.3): context, not a target"}
+        tg.close()
+        del flush
+
     # ---- e2e: host buffers through pdf_xfxq2_host / pdf_alphas_q2_host -------------------------
     ne = args.e2e_n or n
     try:
@@ -372,6 +417,15 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
             mtol = 1e-12 * np.abs(mref) + 1e-14 * mS
             line["members"]["parity_sample"] = {"n": int(mx.size), "worst_err_over_tol": float(np.max(np.abs(mgot - mref)[mok] / np.maximum(mtol[mok], 1e-300))),
                                                 "nan_match": bool(np.array_equal(np.isnan(mgot), ~mok))}
+        # and for the Table 3.3 workload (30 000 sampled rows of the N_rep = 400 call)
+        if table33_sample is not None:
+            ts_, tx_, tq_, tm_, tgot = table33_sample
+            tog = oracle.OracleGrid(ts_.x_knots.numpy(), [q.numpy() for q in ts_.q2_subgrids], ts_.values.numpy(), ts_.pids,
+                                    nmem=ts_.nmem)
+            tref, tS = tog.xfxq2(ts_.pids, tx_, tq_, member=tm_, want_scale=True)
+            ttol = 1e-12 * np.abs(tref) + 1e-14 * tS
+            line["table33"]["parity_sample"] = {"n": int(tx_.size), "worst_err_over_tol": float(np.max(np.abs(tgot - tref) / np.maximum(ttol, 1e-300))),
+                                                "nan_match": bool(not np.isnan(tgot).any() and not np.isnan(tref).any())}
         np_ = min(200_000, ns)
         got = out_sample.cpu().numpy()[:np_]
         _, S = og.xfxq2(spec.pids, cx[:np_], cq[:np_], want_scale=True)

@@ -39,7 +39,10 @@
 
 namespace pdfg {
 
-constexpr int kBinThreads = 256;              // CTA size of the persistent kernel
+#ifndef PDF_BINTHREADS
+#define PDF_BINTHREADS 256
+#endif
+constexpr int kBinThreads = PDF_BINTHREADS;   // CTA size of the persistent kernel
 constexpr int kBinWarps = kBinThreads / 32;
 #ifndef PDF_TILEQ
 #define PDF_TILEQ 8
@@ -66,7 +69,10 @@ constexpr int kLutSize = 1024;                // search-acceleration buckets per
 constexpr int kNF = 11, kNFP = 12;            // the fast path is specialised for 11 flavours (pad 12)
 constexpr int kMaxCK = 1024;                  // coarse keys (x cells + kLowXSplit) the path supports
 constexpr int kMaxFK = 96;                    // fine keys (Q2 knots + 2)
-constexpr int kMaxCap = 2048;                 // payloads of one (chunk, coarse key) held in shared memory
+#ifndef PDF_MAXCAP
+#define PDF_MAXCAP 2048
+#endif
+constexpr int kMaxCap = PDF_MAXCAP;                 // payloads of one (chunk, coarse key) held in shared memory
 
 struct __align__(32) Payload {                // one sector
     double a, b;                              // class-dependent abscissae (t_x,t_q / theta / r)

@@ -223,6 +223,33 @@ def events_c4(n: int, seed: int = BASE_SEED + 4, device="cpu"):
     return x1, x2, q2, w
 
 
+# ---- NEXT-3: the multi-member workload of Table 3.3 ---------------------------
+TABLE33_NX = 2415                 # "a grid of 2415 points in x" (Table 3.3 caption)
+TABLE33_NREP = (10, 50, 100, 200, 300, 400)
+TABLE33_Q2 = 1.65 ** 2            # the thesis gives no scale: FastKernel tables take the PDFs at the fit's
+                                  # initial scale, Q0 = 1.65 GeV for NNPDF3.1 (reading)
+
+
+def xgrid_table33() -> torch.Tensor:
+    """2415 fixed x-points shaped like a FastKernel x-grid: log-spaced in [1e-7, 0.1), then
+    linear in [0.1, 1).  Deterministic (no seed): the workload is structured, not sampled."""
+    nlog = TABLE33_NX // 2
+    nlin = TABLE33_NX - nlog
+    lo = _geomspace(1e-7, 0.1, nlog + 1)[:-1]
+    hi = torch.linspace(0.1, 1.0, nlin + 1, dtype=torch.float64)[:-1]
+    return torch.cat([lo, hi]).contiguous()
+
+
+def queries_table33(nrep: int, device="cpu"):
+    """member-major (member, x-point) queries: every member is evaluated on the same x-grid at
+    one fixed Q2 (all 11 flavours are requested by the caller).  Returns x, q2, member."""
+    xg = xgrid_table33().to(device)
+    x = xg.repeat(nrep)
+    q2 = torch.full((nrep * TABLE33_NX,), TABLE33_Q2, dtype=torch.float64, device=device)
+    mem = torch.arange(nrep, dtype=torch.int32, device=device).repeat_interleave(TABLE33_NX)
+    return x.contiguous(), q2, mem.contiguous()
+
+
 def scan_lines(spec: GridSpec, npts: int = 400):
     """The thesis' accuracy-scan pattern (Fig. 3.5 caption, L1846): vary x at
     several fixed Q, and Q at several fixed x."""

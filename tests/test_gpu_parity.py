@@ -333,3 +333,23 @@ def test_binned_first_calls_in_a_fresh_process(n):
     for _ in range(2):
         r = subprocess.run([sys.executable, script, str(n)], capture_output=True, text=True, timeout=600)
         assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+
+
+@pytest.mark.parametrize("path", ["direct", "auto"])
+def test_table33_workload_parity(B, oracle_mod, path):
+    """NEXT-3, the multi-member workload of Table 3.3: all 11 flavours on the fixed
+    2415-point x-grid at one Q2 for every member (50 members here; bench.py times N_rep = 10 ... 400).
+    Every row against the oracle, the cell indices bit-exact; all members of an x-point share one cell."""
+    nrep = 50
+    spec = synth.grid_c1(nmem=nrep)
+    x, q, mem = synth.queries_table33(nrep)
+    n = x.numel()
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), member=mem.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda(), member=mem.cuda()).cpu().numpy()
+    assert out.shape == (nrep * synth.TABLE33_NX, 11)
+    assert_values(out, ref, S, "table33")
+    assert g.pdf_error_count() == 0
+    check_locate(B, og, g, x.numpy()[: synth.TABLE33_NX], q.numpy()[: synth.TABLE33_NX])
+    # members differ (lognormal noise), so a wrong member stride cannot pass: rows of two members at one x-point
+    assert not np.allclose(out[: synth.TABLE33_NX], out[synth.TABLE33_NX: 2 * synth.TABLE33_NX], rtol=1e-6, atol=0)

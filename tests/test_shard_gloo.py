@@ -59,3 +59,19 @@ def test_shard_range_properties():
             assert all(edges[r][1] == edges[r + 1][0] for r in range(world - 1))
             sizes = [b - a for a, b in edges]
             assert max(sizes) - min(sizes) <= 1
+
+
+def test_table33_generator_shape():
+    """NEXT-3 input recipe (Table 3.3): 2415 increasing x-points inside the C1 grid, member-major, one Q2"""
+    import torch
+    from paper_2302_03343_b200 import synth
+    xg = synth.xgrid_table33()
+    assert xg.numel() == synth.TABLE33_NX == 2415 and bool((xg[1:] > xg[:-1]).all())
+    spec = synth.grid_c1()
+    assert float(xg[0]) >= float(spec.x_knots[0]) and float(xg[-1]) < float(spec.x_knots[-1])
+    assert float(spec.q2_subgrids[1][0]) < synth.TABLE33_Q2 < float(spec.q2_subgrids[1][-1])
+    x, q2, mem = synth.queries_table33(3)
+    assert x.numel() == q2.numel() == mem.numel() == 3 * 2415
+    assert torch.equal(x[:2415], xg) and torch.equal(x[2415:4830], xg)
+    assert torch.equal(mem, torch.arange(3, dtype=torch.int32).repeat_interleave(2415))
+    assert bool((q2 == synth.TABLE33_Q2).all())
