@@ -333,10 +333,30 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
                 torch.cuda.synchronize()
                 ms.append(ea.elapsed_time(eb))
             ms.sort()
+            med_ex = ms[len(ms) // 2]
+            # the structured entry point: the same rows from the 2415 points and the member count
+            xg, qg = tx[: synth.TABLE33_NX], tq[: synth.TABLE33_NX]
+            tout3 = tout.view(nrep, synth.TABLE33_NX, 11)
+            for _ in range(3):
+                tg.pdf_xfxq2_xgrid(tspec.pids, xg, qg, nrep, out=tout3)
+            ms = []
+            for _ in range(args.table33_reps):
+                flush.zero_()
+                ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                ea.record()
+                tg.pdf_xfxq2_xgrid(tspec.pids, xg, qg, nrep, out=tout3)
+                eb.record()
+                torch.cuda.synchronize()
+                ms.append(ea.elapsed_time(eb))
+            ms.sort()
             med = ms[len(ms) // 2]
             paper = PAPER_TABLE33[nrep]
+            t33_bytes = tx.numel() * 88 + nrep * 4 * 196 * 96 + synth.TABLE33_NX * 16   # rows out + the 4 Q2 rows of every member in
             rows.append({"nrep": nrep, "queries": int(tx.numel()), "ms_median": med, "ms_min": ms[0],
+                         "ms_median_xfxq2_ex": med_ex,
                          "value": tx.numel() * 11 / (med * 1e-3), "unit": UNIT,
+                         "roofline": {"bound": "hbm", "achieved": t33_bytes / (med * 1e-3) / 1e9, "peak": peak_gbs, "unit": "GB/s",
+                                      "frac": t33_bytes / (med * 1e-3) / 1e9 / peak_gbs, "traffic": None, "peak_source": peak_src},
                          "paper_seconds": {"lhapdf_cpu": paper[0], "pdfflow_gpu": paper[1], "pdfflow_cpu": paper[2]}})
             if nrep == max(synth.TABLE33_NREP):
                 pick = torch.arange(0, tx.numel(), 31, device="cuda")[:30_000]
@@ -345,6 +365,7 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
         line["table33"] = {"workload": "Table 3.3: 11 flavours x 2415 fixed x-points x N_rep members at Q2 = 1.65^2 GeV2, "
                                        "C1-shaped 400-member grid (lognormal member noise), member-major queries",
                            "timing": f"median of {args.table33_reps} single calls, CUDA events, 256 MB L2 flush before each",
+                           "api": "pdf_xfxq2_xgrid (ms_median, value, roofline); pdf_xfxq2_ex on the member-major expansion (ms_median_xfxq2_ex)",
                            "rows": rows,
                            "paper_hardware": "system P1: i9-9980XE; TITAN V / RTX 2080 Ti (PAPER.md Table 3.2, 3.3): context, not a target"}
         tg.close()

@@ -120,6 +120,19 @@ int pdf_xfxq2(const pdf_grid *g, const int *pids, int npid, long long n, const d
 int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
                  const double *q2, const int *member, double *out, long long ld_out, void *stream);
 
+/* NEXT-3, multi-member evaluation on one shared list of points ("load multiple members of
+ * a PDF set at once ... PDFs evaluated in a grid of x points"; the workload of Table 3.3):
+ *   out[(r * npts + p) * ld_out + k] = xf_{pids[k]}(member members[r]; x[p], q2[p]),  r < nrep, p < npts.
+ * pids HOST [npid]; x, q2 DEVICE [npts]; members DEVICE int32 [nrep] or NULL (= 0 .. nrep-1); out DEVICE
+ * [nrep][npts][ld_out], ld_out >= npid; caller-owned, nothing is allocated.  Same values as pdf_xfxq2_ex
+ * on the member-major expansion of the points (bit-identical to its direct path); validity, cell search
+ * and node weights are computed once per point.  A point outside the domain, or a member id outside
+ * [0, nmem), gives a quiet-NaN row and one error count per (point, member).  npts == 0 or nrep == 0 is a
+ * no-op.  Enqueues one kernel on `stream`; PDF_EINVAL on bad arguments. */
+int pdf_xfxq2_xgrid(const pdf_grid *g, const int *pids, int npid, long long npts, const double *x,
+                    const double *q2, int nrep, const int *members, double *out, long long ld_out,
+                    void *stream);
+
 /* a-6: alpha_s(Q2); q2, out DEVICE [n].  PDF_ESTATE if no alpha_s knots were set. */
 int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out, void *stream);
 

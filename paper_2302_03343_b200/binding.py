@@ -28,7 +28,7 @@ PDF_ALPHAS_FREEZE, PDF_ALPHAS_LOGGRAD = 0, 1
 SYMBOLS = (
     "pdf_grid_create", "pdf_grid_destroy", "pdf_grid_set_alphas", "pdf_grid_set_coupling",
     "pdf_grid_set_workspace", "pdf_workspace_bytes", "pdf_grid_set_option", "pdf_grid_limits",
-    "pdf_xfxq2", "pdf_xfxq2_ex", "pdf_alphas_q2", "pdf_lumi", "pdf_locate", "pdf_error_count",
+    "pdf_xfxq2", "pdf_xfxq2_ex", "pdf_xfxq2_xgrid", "pdf_alphas_q2", "pdf_lumi", "pdf_locate", "pdf_error_count",
     "pdf_xfxq2_host", "pdf_alphas_q2_host", "pdf_lumi_host", "pdf_status_string",
     "pdf_last_cuda_error", "pdf_launch_count", "pdf_profile_enable", "pdf_profile_read",
     "pdf_measure_fp64_tflops",
@@ -63,6 +63,7 @@ def lib():
     L.pdf_grid_limits.argtypes = [vp, dp, dp, dp, dp]
     L.pdf_xfxq2.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp]
     L.pdf_xfxq2_ex.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp, ll, vp]
+    L.pdf_xfxq2_xgrid.argtypes = [vp, ip, C.c_int, ll, vp, vp, C.c_int, vp, vp, ll, vp]
     L.pdf_alphas_q2.argtypes = [vp, ll, vp, vp, vp]
     L.pdf_lumi.argtypes = [vp, ll, vp, vp, vp, vp, vp, vp]
     L.pdf_locate.argtypes = [vp, ll, vp, vp, vp, vp, vp, vp, vp]
@@ -234,6 +235,23 @@ class PdfGrid:
             mp = _dev(member, torch.int32, "member") if member is not None else None
             rc = lib().pdf_xfxq2_ex(self._h, _iptr(pid), pid.numel(), n, xp, qp, mp, op, ld, _stream_ptr(stream))
         _check(rc, "pdf_xfxq2")
+        return out
+
+    def pdf_xfxq2_xgrid(self, pids, x: torch.Tensor, q2: torch.Tensor, nrep: int,
+                        members: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
+                        ld_out: Optional[int] = None, stream=None):
+        """out[r, p, k] = xf_{pids[k]}(member members[r] (default r); x[p], q2[p]): every member on one shared point list"""
+        pid = _hi(list(pids))
+        npts = x.numel()
+        ld = ld_out or pid.numel()
+        if out is None:
+            out = torch.empty((nrep, npts, ld), dtype=torch.float64, device=x.device)
+        xp, qp, op = _dev(x, torch.float64, "x"), _dev(q2, torch.float64, "q2"), _dev(out, torch.float64, "out")
+        if q2.numel() != npts or out.numel() < nrep * npts * ld or (members is not None and members.numel() != nrep):
+            raise PdfGridError("size mismatch")
+        mp = _dev(members, torch.int32, "members") if members is not None else None
+        _check(lib().pdf_xfxq2_xgrid(self._h, _iptr(pid), pid.numel(), npts, xp, qp, nrep, mp, op, ld, _stream_ptr(stream)),
+               "pdf_xfxq2_xgrid")
         return out
 
     def pdf_alphas_q2(self, q2: torch.Tensor, out: Optional[torch.Tensor] = None, stream=None):

@@ -102,6 +102,147 @@ k_xfxq2_direct(GridDev G, ColMap cm, long long n, const double *__restrict__ x,
     }
 }
 
+// ---- NEXT-3: multi-member evaluation on one shared list of points (Table 3.3) ----
+// out[(r * npts + p) * ld + k] = xf_{pids[k]}(member members[r]; x[p], q2[p]).  A thread owns one point:
+// validity, search and the 2 x 4 node weights are done ONCE and reused for every member of its slice
+// (blockIdx.y strides over the member list); the direct kernel repeats them per (point, member).
+// For the 11-flavour layout (rows of 12 doubles) the stencil is read row-wise, 6 x LDG.128 per node, in
+// the summation order of stencil_col (x-sum, then Q2-sum), so the rows are bit-identical to
+// k_xfxq2_direct's.  Points are in increasing x in the paper's workload, so the lanes of a warp share
+// cells and the loads coalesce to a few L1 wavefronts.  With contiguous rows (ld == npid == 11) a warp's
+// 32 rows (requested columns = the 11 value columns in order) are transposed through shared memory and
+// leave as 11 coalesced 256-byte stores (a lane writing its own row would touch 32 sectors per
+// instruction).  Extrapolated points and other layouts take plan_value column by column.
+// Measured (Table 3.3 shape, N_rep = 400): 0.092 ms against 0.169 ms for the direct kernel; what bounds it is
+// the L1 request path (96 LDG.128 per (point, member), 4-5 distinct rows per warp instruction): the next
+// step is one read of a (member, cell) stencil shared by the cell's points.
+constexpr int kXgridThreads = 128;
+
+// an extrapolated point of the 11-flavour layout: full plan, column by column (rare; kept out of line so
+// that its registers do not weigh on the interior path)
+__device__ __noinline__ void xgrid_slow_row(const GridDev &G, const double *Vm, double xv, double qv, double *dst)
+{
+    QueryPlan P;
+    make_plan(G, xv, qv, P);
+    for (int f = 0; f < 11; ++f) dst[f] = plan_value(G, Vm, P, f);
+}
+
+__global__ void __launch_bounds__(kXgridThreads, 4)
+k_xfxq2_xgrid(const __grid_constant__ GridDev G, const __grid_constant__ ColMap cm, long long npts, const double *__restrict__ x, const double *__restrict__ q2,
+              int nrep, const int *__restrict__ members, double *__restrict__ out, long long ld, int fast11, int coalesce)
+{
+    __shared__ double stage[kXgridThreads / 32][32 * 11];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long p = (long long)blockIdx.x * kXgridThreads + threadIdx.x;
+    const long long p0 = p - lane;                             // first point of the warp
+    const bool live = p < npts;
+    double xv = 1.0, qv = 1.0;
+    if (live) { xv = x[p]; qv = q2[p]; }
+    const bool valid = live && classify(G, xv, qv) != kRegionInvalid;
+    // only the interior plan (2 x 4 node indices and weights) stays in registers across the member loop;
+    // the rare extrapolated point rebuilds its full plan per member
+    Point1D X0, Q0;
+    bool interior = false;
+    if (valid) {
+        QueryPlan P;
+        make_plan(G, xv, qv, P);
+        interior = !P.X.low && !P.lowq && !P.Q.high;
+        X0 = P.X.p0; Q0 = P.Q.p0;
+    }
+    const int rows_w = (int)((npts - p0) < 32 ? (npts - p0) : 32);   // rows of this warp (warp-uniform; <= 0: none)
+    unsigned long long errs = 0;
+    for (int r = blockIdx.y; r < nrep; r += gridDim.y) {
+        const int mem = members ? __ldg(members + r) : r;
+        const bool ok = valid && mem >= 0 && mem < G.nmem;
+        if (fast11) {
+            double *srow = &stage[warp][lane * 11];               // every row goes through shared memory
+            // A member's rows are touched by this CTA only, once, so every stencil load would start a DRAM
+            // round trip in the thread's critical path: the NEXT member's 16 rows are requested now (both ends
+            // of a 96-byte row, which may straddle two lines), under this member's arithmetic.
+            if (interior && r + (int)gridDim.y < nrep) {
+                const int mn = members ? __ldg(members + r + gridDim.y) : r + (int)gridDim.y;
+                if (mn >= 0 && mn < G.nmem) {
+                    const double *Vn = G.V + (size_t)mn * G.memstride;
+#pragma unroll
+                    for (int b = 0; b < 4; ++b)
+#pragma unroll
+                        for (int a = 0; a < 4; ++a) {
+                            const double *row = Vn + ((size_t)Q0.idx[b] * G.nx + X0.idx[a]) * 12;
+                            asm volatile("prefetch.global.L1 [%0];" ::"l"(row));
+                            asm volatile("prefetch.global.L1 [%0];" ::"l"(row + 11));
+                        }
+                }
+            }
+            __syncwarp();
+            if (ok && interior) {
+                const double *Vm = G.V + (size_t)mem * G.memstride;
+                double acc[11];
+#pragma unroll
+                for (int f = 0; f < 11; ++f) acc[f] = 0.0;
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    double rb[11];
+#pragma unroll
+                    for (int f = 0; f < 11; ++f) rb[f] = 0.0;
+                    const double *qrow = Vm + (size_t)Q0.idx[b] * G.nx * 12;
+#pragma unroll
+                    for (int a = 0; a < 4; ++a) {
+                        const double2 *row = reinterpret_cast<const double2 *>(qrow + (size_t)X0.idx[a] * 12);
+                        const double w = X0.w[a];
+                        const double2 v0 = __ldg(row), v1 = __ldg(row + 1), v2 = __ldg(row + 2), v3 = __ldg(row + 3),
+                                      v4 = __ldg(row + 4), v5 = __ldg(row + 5);
+                        rb[0] = fma(w, v0.x, rb[0]); rb[1] = fma(w, v0.y, rb[1]);
+                        rb[2] = fma(w, v1.x, rb[2]); rb[3] = fma(w, v1.y, rb[3]);
+                        rb[4] = fma(w, v2.x, rb[4]); rb[5] = fma(w, v2.y, rb[5]);
+                        rb[6] = fma(w, v3.x, rb[6]); rb[7] = fma(w, v3.y, rb[7]);
+                        rb[8] = fma(w, v4.x, rb[8]); rb[9] = fma(w, v4.y, rb[9]);
+                        rb[10] = fma(w, v5.x, rb[10]);
+                    }
+                    const double wq = Q0.w[b];
+#pragma unroll
+                    for (int f = 0; f < 11; ++f) acc[f] = fma(wq, rb[f], acc[f]);
+                }
+#pragma unroll
+                for (int f = 0; f < 11; ++f) srow[f] = acc[f];
+            } else if (ok) {
+                xgrid_slow_row(G, G.V + (size_t)mem * G.memstride, xv, qv, srow);
+            } else {
+#pragma unroll
+                for (int f = 0; f < 11; ++f) srow[f] = qnan();
+                if (live) ++errs;
+            }
+            __syncwarp();
+            double *o = out + ((long long)r * npts + p0) * ld;     // the warp's first row for this member
+            if (coalesce) {
+                const int tot = rows_w * 11;
+#pragma unroll
+                for (int k = 0; k < 11; ++k) {
+                    const int e = k * 32 + lane;
+                    if (e < tot) o[e] = stage[warp][e];
+                }
+            } else if (live) {
+                double *orow = o + (long long)lane * ld;
+                for (int k = 0; k < cm.n; ++k) {
+                    const int c = cm.col[k];
+                    orow[k] = !ok ? qnan() : (c < 0 ? 0.0 : srow[c]);      // an invalid row is NaN in every requested column
+                }
+            }
+        } else if (live) {                                         // any other layout: column by column
+            double *orow = out + ((long long)r * npts + p) * ld;
+            if (ok) {
+                const double *Vm = G.V + (size_t)mem * G.memstride;
+                QueryPlan P;
+                make_plan(G, xv, qv, P);
+                for (int k = 0; k < cm.n; ++k) { const int c = cm.col[k]; orow[k] = c < 0 ? 0.0 : plan_value(G, Vm, P, c); }
+            } else {
+                for (int k = 0; k < cm.n; ++k) orow[k] = qnan();
+                ++errs;
+            }
+        }
+    }
+    if (errs) atomicAdd(G.err_count, errs);
+}
+
 // ---- a-6: alpha_s ----------------------------------------------------------------------------
 // Per cell the Hermite cubic of C-5 is kept in monomial form in t (built once by k_alphas_cells from
 // the same cell constants the PDF path uses):  with H00 = A_c, H01 = A_{c+1},

@@ -69,6 +69,37 @@ int pdf_xfxq2(const pdf_grid *g, const int *pids, int npid, long long n, const d
     return pdf_xfxq2_ex(g, pids, npid, n, x, q2, nullptr, out, npid, stream);
 }
 
+int pdf_xfxq2_xgrid(const pdf_grid *g, const int *pids, int npid, long long npts, const double *x, const double *q2,
+                    int nrep, const int *members, double *out, long long ld_out, void *stream)
+{
+    if (!g || npts < 0 || nrep < 0 || ld_out < npid) return PDF_EINVAL;
+    ColMap cm;
+    int rc = build_colmap(g, pids, npid, cm);
+    if (rc) return rc;
+    if (npts == 0 || nrep == 0) return PDF_OK;
+    if (!x || !q2 || !out) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device);
+    const long long bx = (npts + kXgridThreads - 1) / kXgridThreads;
+    if (bx > 0x7fffffffLL) return PDF_EINVAL;
+    // member slices: one wave of co-resident CTAs (4 per SM at 128 registers), at most one slice per member
+    long long by = ((long long)sms * 4) / bx;
+    if (by > nrep) by = nrep;
+    if (by > 65535) by = 65535;
+    if (by < 1) by = 1;
+    // the row-wise path: 11 value columns in rows of 12 doubles; the coalesced store also needs contiguous
+    // rows and the identity column map
+    const int fast11 = g->d.nflav == 11 && g->d.nfp == 12;
+    bool ident = fast11 && ld_out == 11 && cm.n == 11;
+    for (int k = 0; ident && k < 11; ++k) ident = cm.col[k] == k;
+    LaunchScope a(s, "k_xfxq2_xgrid");
+    k_xfxq2_xgrid<<<dim3((unsigned)bx, (unsigned)by), kXgridThreads, 0, s>>>(g->d, cm, npts, x, q2, nrep, members, out,
+                                                                              ld_out, fast11, ident ? 1 : 0);
+    CK(cudaGetLastError());
+    return PDF_OK;
+}
+
 size_t pdf_workspace_bytes(const pdf_grid *g, long long n)
 {
     if (!g || n < 0) return 0;

@@ -353,3 +353,59 @@ def test_table33_workload_parity(B, oracle_mod, path):
     check_locate(B, og, g, x.numpy()[: synth.TABLE33_NX], q.numpy()[: synth.TABLE33_NX])
     # members differ (lognormal noise), so a wrong member stride cannot pass: rows of two members at one x-point
     assert not np.allclose(out[: synth.TABLE33_NX], out[synth.TABLE33_NX: 2 * synth.TABLE33_NX], rtol=1e-6, atol=0)
+
+
+def test_xgrid_matches_member_major_calls(B, oracle_mod):
+    """pdf_xfxq2_xgrid (NEXT-3): every member on one shared point list == pdf_xfxq2_ex on the member-major
+    expansion, bit for bit against its direct path, and within tolerance of the oracle."""
+    nrep = 23
+    spec = synth.grid_c1(nmem=nrep)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, "direct")
+    xg = synth.xgrid_table33()
+    npts = xg.numel()
+    q = torch.full((npts,), synth.TABLE33_Q2, dtype=torch.float64)
+    x, qq, mem = synth.queries_table33(nrep)
+    want = g.pdf_xfxq2(spec.pids, x.cuda(), qq.cuda(), member=mem.cuda()).cpu()
+    got = g.pdf_xfxq2_xgrid(spec.pids, xg.cuda(), q.cuda(), nrep).cpu()
+    assert got.shape == (nrep, npts, 11)
+    assert torch.equal(got.reshape(-1, 11), want)
+    ref, S = og.xfxq2(spec.pids, x.numpy(), qq.numpy(), member=mem.numpy(), want_scale=True)
+    assert_values(got.reshape(-1, 11).numpy(), ref, S, "xgrid")
+    assert g.pdf_error_count() == 0
+
+
+def test_xgrid_edge_cases(B, oracle_mod):
+    """ragged point count, extrapolated and invalid points, a member list with repeats and a bad id, a pid
+    subset with an unknown pid, padded rows; error count = invalid (point, member) pairs"""
+    spec = synth.grid_c1(nmem=7)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, "direct")
+    npts = 1000 + 13
+    x, q = synth.queries_c2(spec, npts, synth.BASE_SEED + 77)        # 5 % extrapolated, all classes
+    x[5] = 2.0                                                        # x > x_max: invalid
+    x[600] = float("nan")
+    members = torch.tensor([3, 0, 6, 3, 7, 1], dtype=torch.int32)     # 7 is out of range
+    nrep = members.numel()
+    pids = [21, 2, 99, -5]
+    out = torch.full((nrep, npts, 6), -7.0, dtype=torch.float64, device="cuda")
+    g.pdf_xfxq2_xgrid(pids, x.cuda(), q.cuda(), nrep, members=members.cuda(), out=out, ld_out=6)
+    out = out.cpu().numpy()
+    assert np.all(out[:, :, 4:] == -7.0)                              # padding untouched
+    n_bad = 0
+    for r, m in enumerate(members.tolist()):
+        if m >= spec.nmem:
+            assert np.isnan(out[r, :, :4]).all()
+            n_bad += npts
+            continue
+        ref, S = og.xfxq2(pids, x.numpy(), q.numpy(), member=np.full(npts, m, dtype=np.int32), want_scale=True)
+        assert_values(out[r, :, :4], ref, S, f"xgrid edge member {m}")
+        assert np.all(out[r, ~np.isnan(ref[:, 0]), 2] == 0.0)         # unknown pid -> 0.0
+        n_bad += int(np.isnan(ref[:, 0]).sum())
+    assert g.pdf_error_count() == n_bad
+    # all 11 flavours, contiguous rows (the coalesced store path) on the same ragged, mixed point list
+    got = g.pdf_xfxq2_xgrid(spec.pids, x.cuda(), q.cuda(), 7).cpu().numpy()
+    for m in range(7):
+        ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), member=np.full(npts, m, dtype=np.int32), want_scale=True)
+        assert_values(got[m], ref, S, f"xgrid full member {m}")
+    # empty calls are no-ops
+    g.pdf_xfxq2_xgrid(spec.pids, x[:0].cuda(), q[:0].cuda(), 3)
+    g.pdf_xfxq2_xgrid(spec.pids, x.cuda(), q.cuda(), 0)
