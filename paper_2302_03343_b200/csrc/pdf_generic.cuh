@@ -243,6 +243,119 @@ k_xfxq2_xgrid(const __grid_constant__ GridDev G, const __grid_constant__ ColMap 
     if (errs) atomicAdd(G.err_count, errs);
 }
 
+// The same call with the stencil of a (member, cell) read ONCE for all points of the cell.  A CTA takes a
+// tile of kXcT consecutive points: their plans (2 x 4 node indices and weights, 96 B) go to shared memory and
+// consecutive interior points with the same 16 nodes form a run (any order of points is correct; sorted x at
+// one Q2, the paper's workload, gives runs of ~9-60 points).  Thread (g, j) serves member g of the CTA's
+// current group of kXcMem members and flavour pair j (6 pairs = one 96-byte row per 6 threads): it holds
+// V[16 nodes][2 flavours] of its member for the run in registers and walks the run's points with their
+// weights broadcast from shared memory, in stencil_col's summation order (bit-identical rows).  The six
+// threads of a member write one contiguous 88-byte row per point; consecutive points fill the sectors
+// while the lines are still in L2.
+constexpr int kXcT = 64, kXcThreads = 128, kXcMem = kXcThreads / 6;     // 21 members x 6 pairs = 126 threads
+struct XcPoint { double wx[4], wq[4]; int xi[4], qi[4]; };
+
+__global__ void __launch_bounds__(kXcThreads, 4)
+k_xfxq2_xgrid_cell(const __grid_constant__ GridDev G, long long npts, const double *__restrict__ x,
+                   const double *__restrict__ q2, int nrep, const int *__restrict__ members, double *__restrict__ out)
+{
+    __shared__ __align__(16) XcPoint sp[kXcT];
+    __shared__ int s_kind[kXcT];               // 0 invalid, 1 interior, 2 extrapolated
+    __shared__ int s_run[kXcT + 1];
+    __shared__ int s_nrun;
+    const long long p0 = (long long)blockIdx.x * kXcT;
+    const int np = (int)((npts - p0) < kXcT ? (npts - p0) : kXcT);
+    if ((int)threadIdx.x < np) {
+        const double xv = x[p0 + threadIdx.x], qv = q2[p0 + threadIdx.x];
+        int kind = 0;
+        if (classify(G, xv, qv) != kRegionInvalid) {
+            QueryPlan P;
+            make_plan(G, xv, qv, P);
+            kind = (!P.X.low && !P.lowq && !P.Q.high) ? 1 : 2;
+            XcPoint &d = sp[threadIdx.x];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { d.wx[k] = P.X.p0.w[k]; d.wq[k] = P.Q.p0.w[k]; d.xi[k] = P.X.p0.idx[k]; d.qi[k] = P.Q.p0.idx[k]; }
+        }
+        s_kind[threadIdx.x] = kind;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {                    // runs: maximal stretches of interior points on the same 16 nodes
+        int n = 0;
+        for (int p = 0; p < np; ++p) {
+            bool fresh = p == 0 || s_kind[p] != 1 || s_kind[p - 1] != 1;
+            if (!fresh)
+                for (int k = 0; k < 4; ++k) fresh |= sp[p].xi[k] != sp[p - 1].xi[k] || sp[p].qi[k] != sp[p - 1].qi[k];
+            if (fresh) s_run[n++] = p;
+        }
+        s_run[n] = np;
+        s_nrun = n;
+    }
+    __syncthreads();
+    const int nrun = s_nrun;
+    const int g = threadIdx.x / 6, j = threadIdx.x - 6 * g;
+    unsigned long long errs = 0;
+    if (g < kXcMem)
+    for (int r = blockIdx.y * kXcMem + g; r < nrep; r += gridDim.y * kXcMem) {
+        const int mem = members ? __ldg(members + r) : r;
+        const bool okm = mem >= 0 && mem < G.nmem;
+        const double *Vm = G.V + (size_t)(okm ? mem : 0) * G.memstride;
+        double *orow0 = out + ((long long)r * npts + p0) * 11;
+        for (int run = 0; run < nrun; ++run) {
+            const int a0 = s_run[run], a1 = s_run[run + 1];
+            const int kind = s_kind[a0];
+            if (kind == 1 && okm) {
+                double2 v[4][4];
+#pragma unroll
+                for (int b = 0; b < 4; ++b)
+#pragma unroll
+                    for (int a = 0; a < 4; ++a)
+                        v[b][a] = __ldg(reinterpret_cast<const double2 *>(Vm + ((size_t)sp[a0].qi[b] * G.nx + sp[a0].xi[a]) * 12) + j);
+                if (run + 1 < nrun && s_kind[s_run[run + 1]] == 1) {          // the next run's rows, under this run's arithmetic
+                    const XcPoint &nx = sp[s_run[run + 1]];
+#pragma unroll
+                    for (int b = 0; b < 4; ++b)
+#pragma unroll
+                        for (int a = 0; a < 4; ++a) {
+                            const double *row = Vm + ((size_t)nx.qi[b] * G.nx + nx.xi[a]) * 12 + 2 * j;
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(row));
+                        }
+                }
+                for (int p = a0; p < a1; ++p) {
+                    const double2 wx01 = *reinterpret_cast<const double2 *>(&sp[p].wx[0]), wx23 = *reinterpret_cast<const double2 *>(&sp[p].wx[2]);
+                    const double2 wq01 = *reinterpret_cast<const double2 *>(&sp[p].wq[0]), wq23 = *reinterpret_cast<const double2 *>(&sp[p].wq[2]);
+                    const double wx[4] = {wx01.x, wx01.y, wx23.x, wx23.y}, wq[4] = {wq01.x, wq01.y, wq23.x, wq23.y};
+                    double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        double rb0 = 0.0, rb1 = 0.0;
+#pragma unroll
+                        for (int a = 0; a < 4; ++a) { rb0 = fma(wx[a], v[b][a].x, rb0); rb1 = fma(wx[a], v[b][a].y, rb1); }
+                        acc0 = fma(wq[b], rb0, acc0); acc1 = fma(wq[b], rb1, acc1);
+                    }
+                    double *o = orow0 + (long long)p * 11 + 2 * j;
+                    o[0] = acc0;
+                    if (j < 5) o[1] = acc1;
+                }
+            } else if (kind == 1) {                                           // member id out of range: NaN rows
+                for (int p = a0; p < a1; ++p) {
+                    double *o = orow0 + (long long)p * 11 + 2 * j;
+                    o[0] = qnan();
+                    if (j < 5) o[1] = qnan();
+                    if (j == 0) ++errs;
+                }
+            } else if (j == 0) {                                              // a single invalid or extrapolated point
+                double *o = orow0 + (long long)a0 * 11;
+                if (kind == 2 && okm) xgrid_slow_row(G, Vm, x[p0 + a0], q2[p0 + a0], o);
+                else {
+                    for (int f = 0; f < 11; ++f) o[f] = qnan();
+                    ++errs;
+                }
+            }
+        }
+    }
+    if (errs) atomicAdd(G.err_count, errs);
+}
+
 // ---- a-6: alpha_s ----------------------------------------------------------------------------
 // Per cell the Hermite cubic of C-5 is kept in monomial form in t (built once by k_alphas_cells from
 // the same cell constants the PDF path uses):  with H00 = A_c, H01 = A_{c+1},

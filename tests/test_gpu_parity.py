@@ -355,18 +355,42 @@ def test_table33_workload_parity(B, oracle_mod, path):
     assert not np.allclose(out[: synth.TABLE33_NX], out[synth.TABLE33_NX: 2 * synth.TABLE33_NX], rtol=1e-6, atol=0)
 
 
-def test_xgrid_matches_member_major_calls(B, oracle_mod):
+def _xgrid_call(B, g, kernel, pids, x, q, members, reps):
+    """pdf_xfxq2_xgrid with the member list repeated `reps` times (large lists reach the cell-shared kernel under
+    PDF_PATH_AUTO); checks which kernel ran and that every repeat gives the same rows; returns the first copy."""
+    nrep = members.numel()
+    mm = members.repeat(reps)
+    B.pdf_profile_enable(True)
+    out = g.pdf_xfxq2_xgrid(pids, x.cuda(), q.cuda(), mm.numel(), members=mm.cuda())
+    torch.cuda.synchronize()
+    names = [n for n, _ in B.pdf_profile_read(64)]
+    B.pdf_profile_enable(False)
+    assert names == [kernel], names
+    out = out.cpu()
+    for k in range(1, reps):
+        assert torch.equal(out[k * nrep:(k + 1) * nrep].nan_to_num(nan=-1.0), out[:nrep].nan_to_num(nan=-1.0))
+    return out[:nrep]
+
+
+XGRID_KERNELS = [("direct", "k_xfxq2_xgrid", 1), ("auto", "k_xfxq2_xgrid", 1), ("auto", "k_xfxq2_xgrid_cell", 0)]
+
+
+@pytest.mark.parametrize("path,kernel,reps", XGRID_KERNELS)
+def test_xgrid_matches_member_major_calls(B, oracle_mod, path, kernel, reps):
     """pdf_xfxq2_xgrid (NEXT-3): every member on one shared point list == pdf_xfxq2_ex on the member-major
-    expansion, bit for bit against its direct path, and within tolerance of the oracle."""
+    expansion, bit for bit against its direct path, and within tolerance of the oracle; the per-point kernel
+    and the (member, cell)-shared kernel (PDF_PATH_AUTO, large member lists)."""
     nrep = 23
     spec = synth.grid_c1(nmem=nrep)
-    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, "direct")
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path)
     xg = synth.xgrid_table33()
     npts = xg.numel()
     q = torch.full((npts,), synth.TABLE33_Q2, dtype=torch.float64)
     x, qq, mem = synth.queries_table33(nrep)
+    g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_DIRECT)
     want = g.pdf_xfxq2(spec.pids, x.cuda(), qq.cuda(), member=mem.cuda()).cpu()
-    got = g.pdf_xfxq2_xgrid(spec.pids, xg.cuda(), q.cuda(), nrep).cpu()
+    g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_DIRECT if path == "direct" else B.PDF_PATH_AUTO)
+    got = _xgrid_call(B, g, kernel, spec.pids, xg, q, torch.arange(nrep, dtype=torch.int32), reps or 8)
     assert got.shape == (nrep, npts, 11)
     assert torch.equal(got.reshape(-1, 11), want)
     ref, S = og.xfxq2(spec.pids, x.numpy(), qq.numpy(), member=mem.numpy(), want_scale=True)
@@ -374,38 +398,53 @@ def test_xgrid_matches_member_major_calls(B, oracle_mod):
     assert g.pdf_error_count() == 0
 
 
-def test_xgrid_edge_cases(B, oracle_mod):
+@pytest.mark.parametrize("path,kernel,reps", XGRID_KERNELS)
+def test_xgrid_edge_cases(B, oracle_mod, path, kernel, reps):
     """ragged point count, extrapolated and invalid points, a member list with repeats and a bad id, a pid
     subset with an unknown pid, padded rows; error count = invalid (point, member) pairs"""
     spec = synth.grid_c1(nmem=7)
-    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, "direct")
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path)
     npts = 1000 + 13
-    x, q = synth.queries_c2(spec, npts, synth.BASE_SEED + 77)        # 5 % extrapolated, all classes
+    x, q = synth.queries_c2(spec, npts, synth.BASE_SEED + 77)        # 5 % extrapolated, all classes, unsorted
     x[5] = 2.0                                                        # x > x_max: invalid
     x[600] = float("nan")
     members = torch.tensor([3, 0, 6, 3, 7, 1], dtype=torch.int32)     # 7 is out of range
     nrep = members.numel()
+    reps = reps or 64
+
+    def check(got, pids_, xs, qs, what):
+        n_bad = 0
+        for r, m in enumerate(members.tolist()):
+            if m >= spec.nmem:
+                assert np.isnan(got[r]).all()
+                n_bad += xs.numel()
+                continue
+            ref, S = og.xfxq2(pids_, xs.numpy(), qs.numpy(), member=np.full(xs.numel(), m, dtype=np.int32), want_scale=True)
+            assert_values(got[r], ref, S, f"{what} member {m}")
+            n_bad += int(np.isnan(ref[:, 0]).sum())
+        return n_bad
+
+    # pid subset with an unknown pid, padded rows: always the per-point kernel
     pids = [21, 2, 99, -5]
     out = torch.full((nrep, npts, 6), -7.0, dtype=torch.float64, device="cuda")
     g.pdf_xfxq2_xgrid(pids, x.cuda(), q.cuda(), nrep, members=members.cuda(), out=out, ld_out=6)
     out = out.cpu().numpy()
     assert np.all(out[:, :, 4:] == -7.0)                              # padding untouched
-    n_bad = 0
-    for r, m in enumerate(members.tolist()):
-        if m >= spec.nmem:
-            assert np.isnan(out[r, :, :4]).all()
-            n_bad += npts
-            continue
-        ref, S = og.xfxq2(pids, x.numpy(), q.numpy(), member=np.full(npts, m, dtype=np.int32), want_scale=True)
-        assert_values(out[r, :, :4], ref, S, f"xgrid edge member {m}")
-        assert np.all(out[r, ~np.isnan(ref[:, 0]), 2] == 0.0)         # unknown pid -> 0.0
-        n_bad += int(np.isnan(ref[:, 0]).sum())
+    n_bad = check(out[:, :, :4], pids, x, q, "xgrid subset")
+    ok_rows = ~np.isnan(out[0, :, 0])
+    assert np.all(out[0, ok_rows, 2] == 0.0)                          # unknown pid -> 0.0
     assert g.pdf_error_count() == n_bad
-    # all 11 flavours, contiguous rows (the coalesced store path) on the same ragged, mixed point list
-    got = g.pdf_xfxq2_xgrid(spec.pids, x.cuda(), q.cuda(), 7).cpu().numpy()
-    for m in range(7):
-        ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), member=np.full(npts, m, dtype=np.int32), want_scale=True)
-        assert_values(got[m], ref, S, f"xgrid full member {m}")
+    # all 11 flavours, contiguous rows, on the same ragged, mixed, unsorted point list (runs of one point)
+    got = _xgrid_call(B, g, kernel, spec.pids, x, q, members, reps).numpy()
+    n_bad = check(got, spec.pids, x, q, "xgrid full")
+    assert g.pdf_error_count() == n_bad * reps
+    # sorted points at two Q2 values: runs of many points, run boundaries inside and across tiles
+    xs = torch.sort(x[torch.isfinite(x) & (x <= 1.0)])[0][:900]
+    qs = torch.where(torch.arange(xs.numel()) % 200 < 100, torch.tensor(50.0, dtype=torch.float64),
+                     torch.tensor(3.0e4, dtype=torch.float64))
+    got = _xgrid_call(B, g, kernel, spec.pids, xs, qs, members, reps + 8).numpy()
+    check(got, spec.pids, xs, qs, "xgrid sorted")
+    g.pdf_error_count()
     # empty calls are no-ops
     g.pdf_xfxq2_xgrid(spec.pids, x[:0].cuda(), q[:0].cuda(), 3)
     g.pdf_xfxq2_xgrid(spec.pids, x.cuda(), q.cuda(), 0)
