@@ -114,8 +114,8 @@ k_xfxq2_direct(GridDev G, ColMap cm, long long n, const double *__restrict__ x,
 // leave as 11 coalesced 256-byte stores (a lane writing its own row would touch 32 sectors per
 // instruction).  Extrapolated points and other layouts take plan_value column by column.
 // Measured (Table 3.3 shape, N_rep = 400): 0.092 ms against 0.169 ms for the direct kernel; what bounds it is
-// the L1 request path (96 LDG.128 per (point, member), 4-5 distinct rows per warp instruction): the next
-// step is one read of a (member, cell) stencil shared by the cell's points.
+// the L1 request path (96 LDG.128 per (point, member), 4-5 distinct rows per warp instruction): large member
+// lists go to k_xfxq2_xgrid_cell below, which reads a (member, cell) stencil once.
 constexpr int kXgridThreads = 128;
 
 // an extrapolated point of the 11-flavour layout: full plan, column by column (rare; kept out of line so
