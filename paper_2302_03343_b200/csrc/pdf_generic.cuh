@@ -279,16 +279,30 @@ k_xfxq2_xgrid_cell(const __grid_constant__ GridDev G, long long npts, const doub
         s_kind[threadIdx.x] = kind;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {                    // runs: maximal stretches of interior points on the same 16 nodes
-        int n = 0;
-        for (int p = 0; p < np; ++p) {
-            bool fresh = p == 0 || s_kind[p] != 1 || s_kind[p - 1] != 1;
+    // runs: maximal stretches of interior points on the same 16 nodes.  Thread p flags whether point p opens a
+    // run; the two warps that hold the tile's points ballot, and a flagged thread's rank among the flags is
+    // its run number.
+    {
+        __shared__ unsigned s_ballot[2];
+        bool fresh = false;
+        const int p = threadIdx.x;
+        if (p < np) {
+            fresh = p == 0 || s_kind[p] != 1 || s_kind[p - 1] != 1;
             if (!fresh)
+#pragma unroll
                 for (int k = 0; k < 4; ++k) fresh |= sp[p].xi[k] != sp[p - 1].xi[k] || sp[p].qi[k] != sp[p - 1].qi[k];
-            if (fresh) s_run[n++] = p;
         }
-        s_run[n] = np;
-        s_nrun = n;
+        if (p < kXcT) {
+            const unsigned bal = __ballot_sync(0xffffffffu, fresh);
+            if ((p & 31) == 0) s_ballot[p >> 5] = bal;
+        }
+        __syncthreads();
+        const unsigned b0 = s_ballot[0], b1 = s_ballot[1];
+        if (fresh) {
+            const int idx = p < 32 ? __popc(b0 & ((1u << p) - 1u)) : __popc(b0) + __popc(b1 & ((1u << (p - 32)) - 1u));
+            s_run[idx] = p;
+        }
+        if (p == 0) { const int n = __popc(b0) + __popc(b1); s_run[n] = np; s_nrun = n; }
     }
     __syncthreads();
     const int nrun = s_nrun;
@@ -332,6 +346,7 @@ k_xfxq2_xgrid_cell(const __grid_constant__ GridDev G, long long npts, const doub
                         for (int a = 0; a < 4; ++a) { rb0 = fma(wx[a], v[b][a].x, rb0); rb1 = fma(wx[a], v[b][a].y, rb1); }
                         acc0 = fma(wq[b], rb0, acc0); acc1 = fma(wq[b], rb1, acc1);
                     }
+                    // (16-byte stores with the pairs shifted on odd rows were measured: no gain, 0.074 ms either way)
                     double *o = orow0 + (long long)p * 11 + 2 * j;
                     o[0] = acc0;
                     if (j < 5) o[1] = acc1;

@@ -96,8 +96,11 @@ int pdf_xfxq2_xgrid(const pdf_grid *g, const int *pids, int npid, long long npts
     if (ident && g->path != PDF_PATH_DIRECT) {   // the (member, cell)-shared form (contiguous 11-flavour rows); PDF_PATH_DIRECT keeps the per-point kernel
         const long long tiles = (npts + kXcT - 1) / kXcT, groups = ((long long)nrep + kXcMem - 1) / kXcMem;
         // worth it once (tile, member group) pairs fill the machine; measured on the Table 3.3 shape:
-        // N_rep = 50: 0.037 against 0.026 ms per-point, 100: 0.040 / 0.038, 200: 0.049 / 0.054, 400: 0.074 / 0.091
+        // N_rep = 50: 0.037 against 0.026 ms per-point, 100: 0.040 / 0.038, 200: 0.041 / 0.054, 400: 0.066 / 0.091
         if (tiles <= 0x7fffffffLL && tiles * groups >= 2LL * sms) {
+            // one wave of co-resident CTAs (4 per SM); a CTA walks the member groups in strides of the grid's
+            // rows (one (tile, group) pair per CTA in several waves measured slower: 0.077 against 0.074 ms (then) at
+            // N_rep = 400, every wave pays the tile's plan phase again)
             long long gy = ((long long)sms * 4) / tiles;
             if (gy > groups) gy = groups;
             if (gy > 65535) gy = 65535;
