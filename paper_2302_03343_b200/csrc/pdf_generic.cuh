@@ -334,11 +334,13 @@ k_xfxq2_xgrid_cell(const __grid_constant__ GridDev G, long long npts, const doub
                             asm volatile("prefetch.global.L2 [%0];" ::"l"(row));
                         }
                 }
-                for (int p = a0; p < a1; ++p) {
+                // two points per step: their 2 x 10 dependent-FMA chains interleave (with one point per step the
+                // loop waited on its own chains: profile r1k, 27 % "wait" at 3 warps per scheduler)
+                auto point = [&](int p, double &acc0, double &acc1) {
                     const double2 wx01 = *reinterpret_cast<const double2 *>(&sp[p].wx[0]), wx23 = *reinterpret_cast<const double2 *>(&sp[p].wx[2]);
                     const double2 wq01 = *reinterpret_cast<const double2 *>(&sp[p].wq[0]), wq23 = *reinterpret_cast<const double2 *>(&sp[p].wq[2]);
                     const double wx[4] = {wx01.x, wx01.y, wx23.x, wx23.y}, wq[4] = {wq01.x, wq01.y, wq23.x, wq23.y};
-                    double acc0 = 0.0, acc1 = 0.0;
+                    acc0 = 0.0; acc1 = 0.0;
 #pragma unroll
                     for (int b = 0; b < 4; ++b) {
                         double rb0 = 0.0, rb1 = 0.0;
@@ -346,10 +348,22 @@ k_xfxq2_xgrid_cell(const __grid_constant__ GridDev G, long long npts, const doub
                         for (int a = 0; a < 4; ++a) { rb0 = fma(wx[a], v[b][a].x, rb0); rb1 = fma(wx[a], v[b][a].y, rb1); }
                         acc0 = fma(wq[b], rb0, acc0); acc1 = fma(wq[b], rb1, acc1);
                     }
-                    // (16-byte stores with the pairs shifted on odd rows were measured: no gain, 0.074 ms either way)
-                    double *o = orow0 + (long long)p * 11 + 2 * j;
-                    o[0] = acc0;
-                    if (j < 5) o[1] = acc1;
+                };
+                double *o = orow0 + (long long)a0 * 11 + 2 * j;
+                int p = a0;
+#pragma unroll 1
+                for (; p + 1 < a1; p += 2, o += 22) {
+                    double c0, c1, d0, d1;
+                    point(p, c0, c1);
+                    point(p + 1, d0, d1);
+                    o[0] = c0; o[11] = d0;
+                    if (j < 5) { o[1] = c1; o[12] = d1; }
+                }
+                if (p < a1) {
+                    double c0, c1;
+                    point(p, c0, c1);
+                    o[0] = c0;
+                    if (j < 5) o[1] = c1;
                 }
             } else if (kind == 1) {                                           // member id out of range: NaN rows
                 for (int p = a0; p < a1; ++p) {
