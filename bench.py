@@ -424,7 +424,7 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
         og.set_coupling(spec.coupling.numpy())
         lref, ls = og.lumi(*lumi_sample[:4], want_scale=True)
         lerr = np.abs(lumi_sample[4] - lref)
-        ltol = 1e-12 * np.abs(lref) + 1e-14 * ls
+        ltol = oracle.tolerance(lref, ls)
         lok = ~np.isnan(lref)
         line["lumi"]["parity_sample"] = {"n": int(lref.size), "worst_err_over_tol": float(np.max(lerr[lok] / np.maximum(ltol[lok], 1e-300))),
                                          "nan_match": bool(np.array_equal(np.isnan(lumi_sample[4]), ~lok))}
@@ -435,7 +435,7 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
                                     nmem=ms_.nmem)
             mref, mS = mog.xfxq2(ms_.pids, mx, mq, member=mm, want_scale=True)
             mok = ~np.isnan(mref)
-            mtol = 1e-12 * np.abs(mref) + 1e-14 * mS
+            mtol = oracle.tolerance(mref, mS)
             line["members"]["parity_sample"] = {"n": int(mx.size), "worst_err_over_tol": float(np.max(np.abs(mgot - mref)[mok] / np.maximum(mtol[mok], 1e-300))),
                                                 "nan_match": bool(np.array_equal(np.isnan(mgot), ~mok))}
         # and for the Table 3.3 workload (30 000 sampled rows of the N_rep = 400 call)
@@ -444,14 +444,14 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
             tog = oracle.OracleGrid(ts_.x_knots.numpy(), [q.numpy() for q in ts_.q2_subgrids], ts_.values.numpy(), ts_.pids,
                                     nmem=ts_.nmem)
             tref, tS = tog.xfxq2(ts_.pids, tx_, tq_, member=tm_, want_scale=True)
-            ttol = 1e-12 * np.abs(tref) + 1e-14 * tS
+            ttol = oracle.tolerance(tref, tS)
             line["table33"]["parity_sample"] = {"n": int(tx_.size), "worst_err_over_tol": float(np.max(np.abs(tgot - tref) / np.maximum(ttol, 1e-300))),
                                                 "nan_match": bool(not np.isnan(tgot).any() and not np.isnan(tref).any())}
         np_ = min(200_000, ns)
         got = out_sample.cpu().numpy()[:np_]
         _, S = og.xfxq2(spec.pids, cx[:np_], cq[:np_], want_scale=True)
         err = np.abs(got - ref[:np_])
-        tol = 1e-12 * np.abs(ref[:np_]) + 1e-14 * S
+        tol = oracle.tolerance(ref[:np_], S)
         okn = ~np.isnan(ref[:np_])
         line["parity_sample"] = {"n": np_, "worst_err_over_tol": float(np.max(err[okn] / np.maximum(tol[okn], 1e-300))),
                                  "nan_match": bool(np.array_equal(np.isnan(got), ~okn))}

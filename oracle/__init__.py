@@ -25,16 +25,35 @@ REGION_LOWX_LOWQ, REGION_LOWX_HIGHQ, REGION_INVALID = 4, 5, 6
 ALPHAS_FREEZE, ALPHAS_LOGGRAD = 0, 1
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (-O2, OpenMP, no FMA contraction)."""
-    stale = (not os.path.exists(_LIB)) or any(
-        os.path.getmtime(p) > os.path.getmtime(_LIB) for p in (_SRC, _HDR))
+# Parity metric C-12: |gpu - ref| <= REL |ref| + FLOOR_S S[...,0] + FLOOR_T S[...,1].
+# REL is north_star's 1e-12.  FLOOR_S multiplies sum |Wx Wq V| (rounding of the 16-term stencil sum: each
+# side loses up to 16 x 2^-53 of it in the worst case, ~4e-16 typically); FLOOR_T multiplies the
+# t-sensitivity (each side's t carries a few 2^-52 (1 + |ln v|/delta) of rounding).  The values are the
+# tightest that the measured errors allow with a margin (C-12 lists the measured worst ratios).
+REL = 1e-12
+FLOOR_S = 2e-15
+FLOOR_T = 4 * 2.0 ** -52
+
+
+def tolerance(ref, scale):
+    """element-wise parity tolerance from the oracle's value and its two condition numbers"""
+    ref, scale = np.asarray(ref), np.asarray(scale)
+    return REL * np.abs(ref) + FLOOR_S * scale[..., 0] + FLOOR_T * scale[..., 1]
+
+
+def build(force: bool = False, variant: str = "") -> str:
+    """Compile the oracle with gcc (-O2, OpenMP, no FMA contraction).  `variant` = a compile-time
+    switch of pdf_oracle.c (e.g. "ORACLE_S3_BILINEAR"), built beside the default library."""
+    out = _LIB if not variant else os.path.join(_HERE, f"libpdf_oracle_{variant.lower()}.so")
+    stale = (not os.path.exists(out)) or any(
+        os.path.getmtime(p) > os.path.getmtime(out) for p in (_SRC, _HDR))
     if force or stale:
         cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
-               "-ffp-contract=off", "-Wall", "-Wextra", "-o", _LIB + ".tmp", _SRC, "-lm"]
+               "-ffp-contract=off", "-Wall", "-Wextra", *( [f"-D{variant}"] if variant else []),
+               "-o", out + ".tmp", _SRC, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
-        os.replace(_LIB + ".tmp", _LIB)
-    return _LIB
+        os.replace(out + ".tmp", out)
+    return out
 
 
 _lib = None
@@ -151,7 +170,7 @@ class OracleGrid:
         pid, pp = _i(pids)
         n = x.size
         out = np.empty((n, len(pid)))
-        sc = np.empty((n, len(pid))) if want_scale else None
+        sc = np.empty((n, len(pid), 2)) if want_scale else None
         mp = None
         if member is not None:
             member, mp = _i(member)
@@ -176,7 +195,7 @@ class OracleGrid:
         q, qp = _d(q2)
         w, wp = _d(weights)
         out = np.empty(a.size)
-        sc = np.empty(a.size) if want_scale else None
+        sc = np.empty((a.size, 2)) if want_scale else None
         rc = lib().oracle_lumi(self._h, a.size, ap, bp, qp, wp,
                                out.ctypes.data_as(C.POINTER(C.c_double)),
                                sc.ctypes.data_as(C.POINTER(C.c_double)) if want_scale else None)

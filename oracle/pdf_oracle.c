@@ -189,6 +189,15 @@ static double hermite_cell(int m, const double *w, const double *v, long stride,
 {
     double delta = w[c + 1] - w[c];
     double t = (wpt - w[c]) / delta;
+#ifdef ORACLE_S3_BILINEAR
+    /* S-3 reading B, the literal one ("near grid edges ... automatically switches to
+     * bilinear interpolation, which requires 2 neighbor knots only"): plain linear in an end cell of
+     * the knot line.  Documentation switch only: the default build (reading A, S-3) keeps the
+     * cubic with a one-sided end slope; tests/test_oracle_pins.py builds this variant to show what
+     * distinguishes the two (C1 at the first interior knot). */
+    if (c == 0 || c + 1 == m - 1)
+        return v[(long)c * stride] + t * (v[(long)(c + 1) * stride] - v[(long)c * stride]);
+#endif
     /* the four Hermite basis cubics 2t^3-3t^2+1, t^3-2t^2+t, -2t^3+3t^2, t^3-t^2, written in
      * factored form so that each keeps its relative accuracy where it vanishes (t -> 0, 1) */
     double omt = 1.0 - t;
@@ -216,10 +225,13 @@ static double hermite_cell_dt(int m, const double *w, const double *v, long stri
          + d01 * v[(long)(c + 1) * stride] + d11 * (delta * mc1);
 }
 
-/* KT converts a first-order t-rounding term into units of the scale S:
- * tol = 1e-12 |ref| + 1e-14 * scale, and t = (ln v - ln knot)/delta carries a rounding error of
- * up to 2^-52 (2 + 2 |ln v|/delta); a factor 2 covers the two sides  ->  KT = 4 * 2^-52 / 1e-14 */
-#define KT 0.0888178419700125
+/* Condition numbers returned for the parity metric (C-12) come in two parts, kept apart so
+ * that each has its own, physically meaningful floor:
+ *   S[0] = sum |Wx_a Wq_b V_ab|: what the rounding of the 16-term sum acts on;
+ *   S[1] = |df/dt_x| (1 + |ln x|/du) + |df/dt_q| (1 + |ln Q2|/ds): t = (ln v - ln knot)/delta is only
+ *          known to a few 2^-52 (1 + |ln v|/delta) (one ulp each of ln v and ln knot, divided by delta),
+ *          which moves the value by |df/dt| times that.
+ * Both are propagated to first order (same coefficients) through the extrapolation formulas. */
 static double t_cond(const double *w, int c, double wpt)
 {
     return 1.0 + fabs(wpt) / (w[c + 1] - w[c]);
@@ -315,7 +327,7 @@ static const double *block_ptr(const oracle_grid *g, int mem, int k)
     return g->values + (size_t)mem * g->memstride + g->suboff[k];
 }
 
-/* value and condition scale S = sum |Wx_a Wq_b V_ab| at an in-range point */
+/* value and, if S != NULL, the two condition numbers S[0], S[1] (see t_cond) at an in-range point */
 static void interior_value(const oracle_grid *g, int mem, int fcol, double x,
                            double q2, double *val, double *S)
 {
@@ -353,24 +365,31 @@ static void interior_value(const oracle_grid *g, int mem, int fcol, double x,
             rd[b - jlo] = hermite_cell_dt(g->nx, g->u, B + (long)b * g->nflav + fcol, xstride, i, lx);
         double dfx = hermite_cell(jhi - jlo + 1, sk + jlo, rd, 1, j - jlo, lq);
         double dfq = hermite_cell_dt(jhi - jlo + 1, sk + jlo, r, 1, j - jlo, lq);
-        *S = acc + KT * (fabs(dfx) * t_cond(g->u, i, lx) + fabs(dfq) * t_cond(sk, j, lq));
+        S[0] = acc;
+        S[1] = fabs(dfx) * t_cond(g->u, i, lx) + fabs(dfq) * t_cond(sk, j, lq);
     }
 }
 
 /* C-7 / C-8 switch: continuation from two anchor values at abscissa theta
  * (theta = 0 at anchor 0, 1 at anchor 1).  Log form iff both > 1e-3 (L1722). */
-static void continue_two(double f0, double S0, double f1, double S1, double theta,
+static void continue_two(double f0, const double *S0, double f1, const double *S1, double theta,
                          double theta_cond, double *val, double *S)
 {
     if (f0 > 1e-3 && f1 > 1e-3) {
         double l0 = log(f0), l1 = log(f1);
         double v = exp(l0 + theta * (l1 - l0));
         *val = v;
-        if (S) *S = fabs(v) * (fabs(1.0 - theta) * S0 / f0 + fabs(theta) * S1 / f1
-                               + KT * theta_cond * fabs(l1 - l0));
+        if (S) {
+            for (int c = 0; c < 2; ++c)
+                S[c] = fabs(v) * (fabs(1.0 - theta) * S0[c] / f0 + fabs(theta) * S1[c] / f1);
+            S[1] += fabs(v) * theta_cond * fabs(l1 - l0);       /* rounding of theta itself */
+        }
     } else {
         *val = f0 + theta * (f1 - f0);
-        if (S) *S = fabs(1.0 - theta) * S0 + fabs(theta) * S1 + KT * theta_cond * fabs(f1 - f0);
+        if (S) {
+            for (int c = 0; c < 2; ++c) S[c] = fabs(1.0 - theta) * S0[c] + fabs(theta) * S1[c];
+            S[1] += theta_cond * fabs(f1 - f0);
+        }
     }
 }
 
@@ -379,9 +398,9 @@ static void value_inq(const oracle_grid *g, int mem, int fcol, double x, double 
                       double *val, double *S)
 {
     if (x >= g->x[0]) { interior_value(g, mem, fcol, x, q2, val, S); return; }
-    double f0, f1, S0, S1;
-    interior_value(g, mem, fcol, g->x[0], q2, &f0, &S0);
-    interior_value(g, mem, fcol, g->x[1], q2, &f1, &S1);
+    double f0, f1, S0[2], S1[2];
+    interior_value(g, mem, fcol, g->x[0], q2, &f0, S ? S0 : NULL);
+    interior_value(g, mem, fcol, g->x[1], q2, &f1, S ? S1 : NULL);
     double theta = (log(x) - g->u[0]) / (g->u[1] - g->u[0]);
     continue_two(f0, S0, f1, S1, theta, t_cond(g->u, 0, log(x)), val, S);
 }
@@ -392,9 +411,9 @@ static void value_geqmin(const oracle_grid *g, int mem, int fcol, double x, doub
 {
     int last = g->nqtot - 1;
     if (q2 <= g->q2[last]) { value_inq(g, mem, fcol, x, q2, val, S); return; }
-    double g0, g1, S0, S1;
-    value_inq(g, mem, fcol, x, g->q2[last - 1], &g0, &S0);
-    value_inq(g, mem, fcol, x, g->q2[last], &g1, &S1);
+    double g0, g1, S0[2], S1[2];
+    value_inq(g, mem, fcol, x, g->q2[last - 1], &g0, S ? S0 : NULL);
+    value_inq(g, mem, fcol, x, g->q2[last], &g1, S ? S1 : NULL);
     double theta = (log(q2) - g->s[last - 1]) / (g->s[last] - g->s[last - 1]);
     continue_two(g0, S0, g1, S1, theta, t_cond(g->s, last - 1, log(q2)), val, S);
 }
@@ -405,9 +424,9 @@ static void value_any(const oracle_grid *g, int mem, int fcol, double x, double 
 {
     double q2min = g->q2[0];
     if (q2 >= q2min) { value_geqmin(g, mem, fcol, x, q2, val, S); return; }
-    double fmin, fplus, Smin, Splus;
-    value_geqmin(g, mem, fcol, x, q2min, &fmin, &Smin);
-    value_geqmin(g, mem, fcol, x, 1.01 * q2min, &fplus, &Splus);
+    double fmin, fplus, Smin[2], Splus[2];
+    value_geqmin(g, mem, fcol, x, q2min, &fmin, S ? Smin : NULL);
+    value_geqmin(g, mem, fcol, x, 1.01 * q2min, &fplus, S ? Splus : NULL);
     double r = q2 / q2min;
     double gamma = 1.0;
     int free_gamma = 0;
@@ -418,10 +437,13 @@ static void value_any(const oracle_grid *g, int mem, int fcol, double x, double 
     double v = fmin * pow(r, (gamma - 1.0) * r + 1.0);
     *val = v;
     if (S) {
-        double sc = (fmin != 0.0) ? fabs(v / fmin) * Smin : pow(r, (gamma - 1.0) * r + 1.0) * Smin;
-        if (free_gamma)
-            sc += fabs(v * log(r) * r) * (Splus / (0.01 * fmin) + fabs(fplus) * Smin / (0.01 * fmin * fmin));
-        *S = sc;
+        /* d v = (v/fmin) d fmin + v ln(r) r d gamma,  d gamma = d fplus/(0.01 fmin) - fplus d fmin/(0.01 fmin^2) */
+        for (int c = 0; c < 2; ++c) {
+            double sc = (fmin != 0.0) ? fabs(v / fmin) * Smin[c] : pow(r, (gamma - 1.0) * r + 1.0) * Smin[c];
+            if (free_gamma)
+                sc += fabs(v * log(r) * r) * (Splus[c] / (0.01 * fmin) + fabs(fplus) * Smin[c] / (0.01 * fmin * fmin));
+            S[c] = sc;
+        }
     }
 }
 
@@ -446,12 +468,12 @@ int oracle_xfxq2(const oracle_grid *g, const int *pids, int npid, long long n,
         int r = classify(g, x[e], q2[e]);
         if (mem < 0 || mem >= g->nmem) { r = ORACLE_REGION_INVALID; bad_member = 1; }
         for (int p = 0; p < npid; ++p) {
-            double v, S = 0.0;
-            if (r == ORACLE_REGION_INVALID) { v = NAN; S = NAN; }       /* C-10 */
-            else if (col[p] < 0) { v = 0.0; S = 0.0; }                  /* C-11 */
-            else value_any(g, mem, col[p], x[e], q2[e], &v, scale ? &S : NULL);
+            double v, S[2] = {0.0, 0.0};
+            if (r == ORACLE_REGION_INVALID) { v = NAN; S[0] = S[1] = NAN; }   /* C-10 */
+            else if (col[p] < 0) { v = 0.0; }                                 /* C-11 */
+            else value_any(g, mem, col[p], x[e], q2[e], &v, scale ? S : NULL);
             out[e * npid + p] = v;
-            if (scale) scale[e * npid + p] = S;
+            if (scale) { scale[(e * npid + p) * 2] = S[0]; scale[(e * npid + p) * 2 + 1] = S[1]; }
         }
     }
     free(col);
@@ -499,26 +521,26 @@ int oracle_lumi(const oracle_grid *g, long long n, const double *x1,
     for (long long e = 0; e < n; ++e) {
         int r1 = classify(g, x1[e], q2[e]), r2 = classify(g, x2[e], q2[e]);
         if (r1 == ORACLE_REGION_INVALID || r2 == ORACLE_REGION_INVALID) {
-            out[e] = NAN; if (scale) scale[e] = NAN; continue;
+            out[e] = NAN; if (scale) scale[2 * e] = scale[2 * e + 1] = NAN; continue;
         }
-        double f1[64], f2[64], s1[64], s2[64];
+        double f1[64], f2[64], s1[64][2], s2[64][2];
         for (int f = 0; f < nf; ++f) {
-            double v, S = 0.0;
-            value_any(g, 0, f, x1[e], q2[e], &v, scale ? &S : NULL);
-            f1[f] = v / x1[e]; s1[f] = S / x1[e];
-            value_any(g, 0, f, x2[e], q2[e], &v, scale ? &S : NULL);
-            f2[f] = v / x2[e]; s2[f] = S / x2[e];
+            double v, S[2] = {0.0, 0.0};
+            value_any(g, 0, f, x1[e], q2[e], &v, scale ? S : NULL);
+            f1[f] = v / x1[e]; s1[f][0] = S[0] / x1[e]; s1[f][1] = S[1] / x1[e];
+            value_any(g, 0, f, x2[e], q2[e], &v, scale ? S : NULL);
+            f2[f] = v / x2[e]; s2[f][0] = S[0] / x2[e]; s2[f][1] = S[1] / x2[e];
         }
-        double acc = 0.0, sacc = 0.0;
+        double acc = 0.0, sacc[2] = {0.0, 0.0};
         for (int i = 0; i < nf; ++i)
             for (int j = 0; j < nf; ++j) {
                 acc += g->C[i * nf + j] * f1[i] * f2[j];
-                /* first-order propagation of the per-flavour tolerance 1e-12 |f| + 1e-14 S */
-                sacc += fabs(g->C[i * nf + j]) * (s1[i] * fabs(f2[j]) + fabs(f1[i]) * s2[j]
-                                                   + 200.0 * fabs(f1[i] * f2[j]));
+                /* first-order propagation of the per-flavour condition numbers through the product */
+                for (int c = 0; c < 2; ++c)
+                    sacc[c] += fabs(g->C[i * nf + j]) * (s1[i][c] * fabs(f2[j]) + fabs(f1[i]) * s2[j][c]);
             }
         out[e] = weights[e] * acc;
-        if (scale) scale[e] = fabs(weights[e]) * sacc;
+        if (scale) { scale[2 * e] = fabs(weights[e]) * sacc[0]; scale[2 * e + 1] = fabs(weights[e]) * sacc[1]; }
     }
     return 0;
 }

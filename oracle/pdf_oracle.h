@@ -67,11 +67,13 @@ int oracle_locate(const oracle_grid *g, long long n, const double *x,
                   const double *q2, int *ix, int *iq, int *isub, int *region);
 
 /* C-5 ... C-11.  out is [n][npid] row-major; member may be NULL (member 0);
- * scale, if not NULL, receives [n][npid] condition scales used by the parity
- * metric C-12, tol = 1e-12 |ref| + 1e-14 scale:  scale = sum |Wx_a Wq_b V_ab|
- * (rounding of the 16-term sum) + KT (|df/dt_x| (1+|ln x|/du) + |df/dt_q|
- * (1+|ln Q2|/ds)) (rounding of t = (ln v - ln knot)/delta, KT = 4*2^-52/1e-14),
- * propagated to first order through the extrapolation formulas. */
+ * scale, if not NULL, receives [n][npid][2] condition numbers for the parity
+ * metric C-12, tol = REL |ref| + FLOOR_S scale[0] + FLOOR_T scale[1]:
+ *   scale[0] = sum |Wx_a Wq_b V_ab|  (what the rounding of the 16-term sum acts on),
+ *   scale[1] = |df/dt_x| (1 + |ln x|/du) + |df/dt_q| (1 + |ln Q2|/ds)  (what the rounding of
+ *              t = (ln v - ln knot)/delta acts on, in units of the relative rounding of a logarithm),
+ * both propagated to first order through the extrapolation formulas.  Pinned by
+ * tests/test_oracle_pins.py::test_scale_* against an independent restatement. */
 int oracle_xfxq2(const oracle_grid *g, const int *pids, int npid, long long n,
                  const double *x, const double *q2, const int *member,
                  double *out, double *scale);
@@ -80,9 +82,9 @@ int oracle_xfxq2(const oracle_grid *g, const int *pids, int npid, long long n,
 int oracle_alphas_q2(const oracle_grid *g, long long n, const double *q2,
                      double *out);
 
-/* C-L.  scale, if not NULL, receives [n] = |w| sum_ij |C_ij| (S1_i |f2_j| + |f1_i| S2_j +
- * 200 |f1_i f2_j|): the per-flavour tolerance (1e-12 |f| + 1e-14 S) propagated to first order
- * through the product, in units of 1e-14. */
+/* C-L.  scale, if not NULL, receives [n][2]: for c = 0, 1
+ *   scale[c] = |w| sum_ij |C_ij| (S1_i[c] |f2_j| + |f1_i| S2_j[c]),   S1 = scale of xf(x1)/x1, S2 of xf(x2)/x2:
+ * the per-flavour condition numbers propagated to first order through the product. */
 int oracle_lumi(const oracle_grid *g, long long n, const double *x1,
                 const double *x2, const double *q2, const double *weights,
                 double *out, double *scale);

@@ -470,7 +470,7 @@ def test_p10_three_orders(oracle_mod):
         b = g.interior_order(1, f, x.numpy(), q.numpy())
         c = g.interior_order(2, f, x.numpy(), q.numpy())
         _, S = g.xfxq2([spec.pids[f]], x.numpy(), q.numpy(), want_scale=True)
-        S = S[:, 0] + 1e-300
+        S = S[:, 0, 0] + 1e-300
         assert np.max(np.abs(a - b) / S) < 1e-14 and np.max(np.abs(a - c) / S) < 1e-14
 
 
@@ -580,6 +580,7 @@ def test_p13_lumi(oracle_mod):
     f2 = g.xfxq2(spec.pids, x2, q2) / x2[:, None]
     Cm = spec.coupling.numpy()
     want = w * np.einsum("ei,ij,ej->e", f1, Cm, f2)
+    sc = sc[:, 0]
     assert np.max(np.abs(out - want) / sc) < 1e-13
     # C = e_i e_j^T isolates one product
     E = np.zeros((11, 11)); E[2, 7] = 1.0
@@ -589,6 +590,211 @@ def test_p13_lumi(oracle_mod):
     g.set_coupling(Cm.T.copy())
     swapped = g.lumi(x2, x1, q2, w)
     assert np.max(np.abs(swapped - out) / sc) < 1e-13
+
+
+# ---------------------------------------------------------------------------
+# The condition numbers of the parity metric (C-12).  Every GPU parity assertion divides by
+# them, so a mistake that inflates them would loosen all parity tests: pinned here against an independent
+# restatement (SURVEY C-5's closed 4-weight form in the monomial basis, numerical derivatives of the
+# literal interpolant above, and the first-order propagation formulas written out on pinned inputs).
+# ---------------------------------------------------------------------------
+def closed_weights(lk, c, t):
+    """SURVEY C-5 4-weight form, monomial Hermite basis; lk = ln-knots of one (sub-)line, vectorised over queries"""
+    m = len(lk)
+    h00, h10 = 2 * t**3 - 3 * t**2 + 1, t**3 - 2 * t**2 + t
+    h01, h11 = -2 * t**3 + 3 * t**2, t**3 - t**2
+    d = lk[c + 1] - lk[c]
+    left, right = c > 0, c + 2 < m
+    rm = np.where(left, d / (lk[c] - lk[np.maximum(c - 1, 0)] + (~left) * 1.0), 0.0)
+    rp = np.where(right, d / (lk[np.minimum(c + 2, m - 1)] - lk[c + 1] + (~right) * 1.0), 0.0)
+    w = np.empty((4,) + t.shape)
+    w[0] = np.where(left, -0.5 * rm * h10, 0.0)
+    w[1] = np.where(left, h00 + 0.5 * (rm - 1) * h10, h00 - h10) - np.where(right, 0.5 * h11, h11)
+    w[2] = h01 + np.where(left, 0.5 * h10, h10) + np.where(right, 0.5 * (1 - rp) * h11, h11)
+    w[3] = np.where(right, 0.5 * rp * h11, 0.0)
+    return w
+
+
+def closed_stencil(spec, x, q2):
+    """per query: sub-grid k, cells, the 4 x 4 node weights and node values [n][4][4][nflav] (absent nodes: weight 0)"""
+    xk = spec.x_knots.numpy()
+    n = len(x)
+    W = np.zeros((n, 4, 4))
+    V = np.zeros((n, 4, 4, spec.nflav))
+    T = np.zeros((n, 4))     # t_x, t_q, du, ds
+    starts = np.array([float(q[0]) for q in spec.q2_subgrids])
+    ksub = np.searchsorted(starts, q2, side="right") - 1
+    for k, qk_t in enumerate(spec.q2_subgrids):
+        sel = np.nonzero(ksub == k)[0]
+        if not sel.size:
+            continue
+        qk = qk_t.numpy()
+        i = np.clip(np.searchsorted(xk, x[sel], side="right") - 1, 0, len(xk) - 2)
+        j = np.clip(np.searchsorted(qk, q2[sel], side="right") - 1, 0, len(qk) - 2)
+        lx, lq = np.log(xk), np.log(qk)
+        tx = (np.log(x[sel]) - lx[i]) / (lx[i + 1] - lx[i])
+        tq = (np.log(q2[sel]) - lq[j]) / (lq[j + 1] - lq[j])
+        wx, wq = closed_weights(lx, i, tx), closed_weights(lq, j, tq)
+        blk = spec.block(0, k).numpy()
+        for a in range(4):
+            ia = np.clip(i - 1 + a, 0, len(xk) - 1)
+            for b in range(4):
+                jb = np.clip(j - 1 + b, 0, len(qk) - 1)
+                W[sel, a, b] = wx[a] * wq[b]
+                V[sel, a, b, :] = blk[ia, jb, :]
+        T[sel] = np.stack([tx, tq, lx[i + 1] - lx[i], lq[j + 1] - lq[j]], axis=1)
+    return W, V, T
+
+
+@pytest.mark.parametrize("which", ["c1", "tiny"])
+def test_scale_interior_sum_part(oracle_mod, which):
+    """scale[0] == sum |Wx_a Wq_b V_ab| (and the value == sum Wx_a Wq_b V_ab) on 1e5 random interior queries"""
+    if which == "c1":
+        spec, n = synth.grid_c1(), 100_000
+    else:
+        spec, n = synth.tiny_grid(321, 5, [4, 2, 5], nflav=3), 20_000
+    g = make_oracle_grid(oracle_mod, spec)
+    x, q = synth.queries_inside(spec, n, 1234)
+    x, q = x.numpy(), q.numpy()
+    ref, S = g.xfxq2(spec.pids, x, q, want_scale=True)
+    W, V, _ = closed_stencil(spec, x, q)
+    want_S0 = np.einsum("nab,nabf->nf", np.abs(W), np.abs(V))
+    want_v = np.einsum("nab,nabf->nf", W, V)
+    assert S.shape == (n, spec.nflav, 2)
+    assert np.max(np.abs(S[:, :, 0] - want_S0) / (want_S0 + 1e-300)) < 1e-11     # monomial vs factored basis: ~1e-13
+    assert np.max(np.abs(ref - want_v) / (want_S0 + 1e-3 * S[:, :, 1] + 1e-300)) < 1e-12   # the two t's differ by their rounding
+    assert np.all(S[:, :, 0] >= np.abs(ref) * (1 - 1e-12))                       # |f| <= S always
+    assert np.all(S[:, :, 1] >= 0)
+
+
+def test_scale_interior_t_part(oracle_mod):
+    """scale[1] == |df/dt_x| (1 + |ln x|/du) + |df/dt_q| (1 + |ln Q2|/ds), derivatives taken numerically from
+    the literal second implementation (brute_interior)"""
+    spec = synth.tiny_grid(322, 5, [4, 5], nflav=2)
+    g = make_oracle_grid(oracle_mod, spec)
+    x, q = synth.queries_inside(spec, 400, 99)
+    x, q = x.numpy(), q.numpy()
+    _, S = g.xfxq2(spec.pids, x, q, want_scale=True)
+    _, _, T = closed_stencil(spec, x, q)
+    checked = 0
+    for e in range(len(x)):
+        tx, tq, du, ds = T[e]
+        if not (0.1 < tx < 0.9 and 0.1 < tq < 0.9):
+            continue                                        # the central difference must stay inside the cell
+        h = 1e-5
+        for f in range(spec.nflav):
+            dfx = (brute_interior(spec, x[e] * math.exp(h * du), q[e], f) - brute_interior(spec, x[e] * math.exp(-h * du), q[e], f)) / (2 * h)
+            dfq = (brute_interior(spec, x[e], q[e] * math.exp(h * ds), f) - brute_interior(spec, x[e], q[e] * math.exp(-h * ds), f)) / (2 * h)
+            want = abs(dfx) * (1 + abs(math.log(x[e])) / du) + abs(dfq) * (1 + abs(math.log(q[e])) / ds)
+            assert abs(S[e, f, 1] - want) <= 1e-6 * (want + S[e, f, 0])
+            checked += 1
+    assert checked > 200
+
+
+def test_scale_extrapolation_propagation(oracle_mod):
+    """first-order propagation through C-7 / C-8 / C-9, written out on the (pinned) interior numbers"""
+    spec = synth.grid_c1()
+    g = make_oracle_grid(oracle_mod, spec)
+    xk = spec.x_knots.numpy()
+    qall = np.concatenate([t.numpy() for t in spec.q2_subgrids])
+    q2min, q2max, qprev = qall[0], qall[-1], qall[-2]
+    u0, u1 = math.log(xk[0]), math.log(xk[1])
+    rng = np.random.default_rng(8)
+    n = 300
+
+    def two(f0, S0, f1, S1, theta, cond):
+        v = np.where((f0 > 1e-3) & (f1 > 1e-3), np.exp(np.log(np.abs(f0) + 1e-300) + theta * (np.log(np.abs(f1) + 1e-300) - np.log(np.abs(f0) + 1e-300))),
+                     f0 + theta * (f1 - f0))
+        logf = (f0 > 1e-3) & (f1 > 1e-3)
+        out = np.empty(S0.shape)
+        for c in range(2):
+            lin = np.abs(1 - theta) * S0[..., c] + np.abs(theta) * S1[..., c] + (c == 1) * cond * np.abs(f1 - f0)
+            with np.errstate(divide="ignore", invalid="ignore"):
+                lg = np.abs(v) * (np.abs(1 - theta) * S0[..., c] / f0 + np.abs(theta) * S1[..., c] / f1
+                                  + (c == 1) * cond * np.abs(np.log(f1) - np.log(f0)))
+            out[..., c] = np.where(logf, lg, lin)
+        return v, out
+
+    # C-7 low-x, Q2 inside
+    x = np.exp(rng.uniform(math.log(1e-12), u0, n)); x = x[x < xk[0]]
+    q = np.exp(rng.uniform(math.log(q2min), math.log(q2max), len(x)))
+    ref, S = g.xfxq2(spec.pids, x, q, want_scale=True)
+    f0, S0 = g.xfxq2(spec.pids, np.full(len(x), xk[0]), q, want_scale=True)
+    f1, S1 = g.xfxq2(spec.pids, np.full(len(x), xk[1]), q, want_scale=True)
+    theta = ((np.log(x) - u0) / (u1 - u0))[:, None]
+    cond = (1 + np.abs(np.log(x)) / (u1 - u0))[:, None]
+    v, want = two(f0, S0, f1, S1, theta, cond)
+    assert np.max(np.abs(ref - v) / (np.abs(v) + 1e-300)) < 1e-12
+    assert np.max(np.abs(S - want) / (want + 1e-300)) < 1e-10
+    assert ((f0 > 1e-3) & (f1 > 1e-3)).any() and (~((f0 > 1e-3) & (f1 > 1e-3))).any()    # both forms are exercised
+    # C-8 high-Q, x inside
+    x = np.exp(rng.uniform(u0, 0.0, n)).clip(xk[0], xk[-1])
+    q = np.exp(rng.uniform(math.log(q2max), math.log(q2max) + 4, n)); q = np.maximum(q, np.nextafter(q2max, 1e300))
+    ref, S = g.xfxq2(spec.pids, x, q, want_scale=True)
+    f0, S0 = g.xfxq2(spec.pids, x, np.full(n, qprev), want_scale=True)
+    f1, S1 = g.xfxq2(spec.pids, x, np.full(n, q2max), want_scale=True)
+    ds = math.log(q2max) - math.log(qprev)
+    theta = ((np.log(q) - math.log(qprev)) / ds)[:, None]
+    cond = (1 + np.abs(np.log(q)) / ds)[:, None]
+    v, want = two(f0, S0, f1, S1, theta, cond)
+    assert np.max(np.abs(ref - v) / (np.abs(v) + 1e-300)) < 1e-12
+    assert np.max(np.abs(S - want) / (want + 1e-300)) < 1e-10
+    # C-9 low-Q, x inside
+    q = np.exp(rng.uniform(math.log(q2min) - 4, math.log(q2min), n)); q = np.minimum(q, np.nextafter(q2min, 0))
+    ref, S = g.xfxq2(spec.pids, x, q, want_scale=True)
+    fm, Sm = g.xfxq2(spec.pids, x, np.full(n, q2min), want_scale=True)
+    fp, Sp = g.xfxq2(spec.pids, x, np.full(n, 1.01 * q2min), want_scale=True)
+    r = (q / q2min)[:, None]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        gfd = (fp - fm) / (0.01 * fm)
+    free = (fm > 1e-5) & (gfd > -2.5)
+    gamma = np.where(fm > 1e-5, np.maximum(gfd, -2.5), 1.0)
+    v = fm * r ** ((gamma - 1) * r + 1)
+    assert np.max(np.abs(ref - v) / (np.abs(v) + 1e-300)) < 1e-12
+    for c in range(2):
+        with np.errstate(divide="ignore", invalid="ignore"):
+            base = np.where(fm != 0, np.abs(v / fm) * Sm[..., c], r ** ((gamma - 1) * r + 1) * Sm[..., c])
+            extra = np.abs(v * np.log(r) * r) * (Sp[..., c] / (0.01 * fm) + np.abs(fp) * Sm[..., c] / (0.01 * fm * fm))
+        want = base + np.where(free, extra, 0.0)
+        assert np.max(np.abs(S[..., c] - want) / (want + 1e-300)) < 1e-10
+    assert free.any() and (~free).any()
+
+
+def test_scale_lumi_formula(oracle_mod):
+    """oracle_lumi's scale == |w| sum_ij |C_ij| (S1_i |f2_j| + |f1_i| S2_j) per component (pdf_oracle.h)"""
+    spec = synth.grid_c1()
+    g = make_oracle_grid(oracle_mod, spec)
+    x1, x2, q2, w = [t.numpy() for t in synth.events_c4(2000, seed=5)]
+    _, sc = g.lumi(x1, x2, q2, w, want_scale=True)
+    v1, S1 = g.xfxq2(spec.pids, x1, q2, want_scale=True)
+    v2, S2 = g.xfxq2(spec.pids, x2, q2, want_scale=True)
+    f1, f2 = np.abs(v1 / x1[:, None]), np.abs(v2 / x2[:, None])
+    aC = np.abs(spec.coupling.numpy())
+    assert sc.shape == (2000, 2)
+    for c in range(2):
+        s1, s2 = S1[..., c] / x1[:, None], S2[..., c] / x2[:, None]
+        want = np.abs(w) * (np.einsum("ei,ij,ej->e", s1, aC, f2) + np.einsum("ei,ij,ej->e", f1, aC, s2))
+        assert np.max(np.abs(sc[:, c] - want) / want) < 1e-12
+
+
+def test_s3_reading_b_switch(oracle_mod):
+    """SURVEY S-3: the literal reading B (pure linear end cells) exists as a compile-time switch
+    of the oracle; what distinguishes it from the default reading A is C1 at the first interior knot."""
+    import ctypes as C
+    path = oracle_mod.build(variant="ORACLE_S3_BILINEAR")
+    L = C.CDLL(path)
+    dp = C.POINTER(C.c_double)
+    L.oracle_weights_1d.argtypes = [C.c_int, dp, C.c_double, C.c_int, dp]
+    lk = np.log(np.array([1.0, 2.0, 4.5, 9.0, 20.0]))
+    for lib_, end_is_linear in ((oracle_mod.lib(), False), (L, True)):
+        w = np.zeros(4)
+        lib_.oracle_weights_1d(5, lk.ctypes.data_as(dp), float(lk[0] + 0.3 * (lk[1] - lk[0])), 0, w.ctypes.data_as(dp))
+        assert abs(w.sum() - 1) < 1e-15
+        is_lin = abs(w[1] - 0.7) < 1e-15 and abs(w[2] - 0.3) < 1e-15 and w[3] == 0
+        assert is_lin == end_is_linear
+        w2 = np.zeros(4)                     # interior cells are the same cubic under both readings
+        lib_.oracle_weights_1d(5, lk.ctypes.data_as(dp), float(lk[1] + 0.3 * (lk[2] - lk[1])), 1, w2.ctypes.data_as(dp))
+        assert abs(w2[0]) > 1e-3 and abs(w2[3]) > 1e-3
 
 
 # ---------------------------------------------------------------------------
