@@ -141,12 +141,22 @@ int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out,
 int pdf_lumi(const pdf_grid *g, long long n, const double *x1, const double *x2, const double *q2,
              const double *weights, double *out, void *stream);
 
-/* a-2 exposed for validation: region class, sub-grid, lower-left knot of the cell (ix, and iq
- * local to the sub-grid); DEVICE int32 [n] each, any may be NULL.  For extrapolated queries the
+/* a-2 exposed for validation (L1714-1720, L1735): region class, sub-grid, lower-left knot of the cell (ix,
+ * and iq local to the sub-grid); DEVICE int32 [n] each, any may be NULL.  For extrapolated queries the
  * indices are those of the knots the continuation is anchored on (low-x: ix = 0; low-Q:
- * isub = 0, iq = 0; high-Q: last sub-grid, iq = nq-2); invalid queries get -1. */
+ * isub = 0, iq = 0; high-Q: last sub-grid, iq = nq-2); invalid queries get -1.
+ * The call runs the search of the evaluation path that is selected: under PDF_PATH_AUTO / PDF_PATH_BINNED
+ * (and a grid the binned path supports) the table-driven search of the binned kernel's A tiles
+ * (s3_locate, the function k_pdf_stream calls), under PDF_PATH_DIRECT the binary search of the direct
+ * kernels.  Both compare raw values only, so both must equal the oracle bit for bit. */
 int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2, int *ix,
                int *iq, int *isub, int *region, void *stream);
+
+/* which path the last evaluation call (pdf_xfxq2 / _ex / pdf_lumi / pdf_locate) on this handle ran:
+ * PDF_PATH_DIRECT or PDF_PATH_BINNED (0 before the first call).  PDF_PATH_AUTO falls back to the direct
+ * kernels for grids the binned path does not support (flavour count other than 11, > 1024 cells per axis),
+ * small calls and calls without a sufficient workspace; this call makes that visible. */
+int pdf_last_path(const pdf_grid *g);
 
 /* number of invalid queries seen by this grid since creation / the last call of this function
  * (reads and resets the device counter; synchronises `stream`). */

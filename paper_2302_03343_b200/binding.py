@@ -31,7 +31,7 @@ SYMBOLS = (
     "pdf_xfxq2", "pdf_xfxq2_ex", "pdf_xfxq2_xgrid", "pdf_alphas_q2", "pdf_lumi", "pdf_locate", "pdf_error_count",
     "pdf_xfxq2_host", "pdf_alphas_q2_host", "pdf_lumi_host", "pdf_status_string",
     "pdf_last_cuda_error", "pdf_launch_count", "pdf_profile_enable", "pdf_profile_read",
-    "pdf_measure_fp64_tflops",
+    "pdf_measure_fp64_tflops", "pdf_last_path",
 )
 
 
@@ -78,6 +78,7 @@ def lib():
     L.pdf_profile_enable.argtypes = [C.c_int]
     L.pdf_profile_read.argtypes = [C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
     L.pdf_measure_fp64_tflops.argtypes = [dp, vp]
+    L.pdf_last_path.argtypes = [vp]
     _lib = L
     return L
 
@@ -112,9 +113,19 @@ def _stream_ptr(stream: Optional[torch.cuda.Stream]):
     return C.c_void_p(s.cuda_stream)
 
 
-def _dev(t: torch.Tensor, dtype, what: str):
+def _dev(t: torch.Tensor, dtype, what: str, numel: Optional[int] = None, at_least: bool = False):
     if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
         raise PdfGridError(f"{what} must be a contiguous CUDA tensor of dtype {dtype}")
+    if numel is not None and (t.numel() < numel if at_least else t.numel() != numel):
+        raise PdfGridError(f"{what} has {t.numel()} elements, expected {'>= ' if at_least else ''}{numel}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host(t: torch.Tensor, what: str, numel: int, at_least: bool = False):
+    if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise PdfGridError(f"{what} must be a contiguous CPU float64 tensor")
+    if t.numel() < numel if at_least else t.numel() != numel:
+        raise PdfGridError(f"{what} has {t.numel()} elements, expected {'>= ' if at_least else ''}{numel}")
     return C.c_void_p(t.data_ptr())
 
 
@@ -257,24 +268,29 @@ class PdfGrid:
     def pdf_alphas_q2(self, q2: torch.Tensor, out: Optional[torch.Tensor] = None, stream=None):
         if out is None:
             out = torch.empty_like(q2)
-        _check(lib().pdf_alphas_q2(self._h, q2.numel(), _dev(q2, torch.float64, "q2"),
-                                   _dev(out, torch.float64, "out"), _stream_ptr(stream)), "pdf_alphas_q2")
+        n = q2.numel()
+        _check(lib().pdf_alphas_q2(self._h, n, _dev(q2, torch.float64, "q2"),
+                                   _dev(out, torch.float64, "out", n, at_least=True), _stream_ptr(stream)), "pdf_alphas_q2")
         return out
 
     def pdf_lumi(self, x1, x2, q2, weights, out: Optional[torch.Tensor] = None, stream=None):
         if out is None:
             out = torch.empty_like(x1)
-        f = torch.float64
-        _check(lib().pdf_lumi(self._h, x1.numel(), _dev(x1, f, "x1"), _dev(x2, f, "x2"), _dev(q2, f, "q2"),
-                              _dev(weights, f, "weights"), _dev(out, f, "out"), _stream_ptr(stream)), "pdf_lumi")
+        f, n = torch.float64, x1.numel()
+        _check(lib().pdf_lumi(self._h, n, _dev(x1, f, "x1"), _dev(x2, f, "x2", n), _dev(q2, f, "q2", n),
+                              _dev(weights, f, "weights", n), _dev(out, f, "out", n, at_least=True), _stream_ptr(stream)), "pdf_lumi")
         return out
 
     def pdf_locate(self, x: torch.Tensor, q2: torch.Tensor, stream=None):
         n = x.numel()
         outs = [torch.empty(n, dtype=torch.int32, device=x.device) for _ in range(4)]
-        _check(lib().pdf_locate(self._h, n, _dev(x, torch.float64, "x"), _dev(q2, torch.float64, "q2"),
+        _check(lib().pdf_locate(self._h, n, _dev(x, torch.float64, "x"), _dev(q2, torch.float64, "q2", n),
                                 *[C.c_void_p(o.data_ptr()) for o in outs], _stream_ptr(stream)), "pdf_locate")
         return tuple(outs)  # ix, iq, isub, region
+
+    def pdf_last_path(self) -> int:
+        """PDF_PATH_DIRECT or PDF_PATH_BINNED: which kernels the last evaluation call on this handle ran"""
+        return int(lib().pdf_last_path(self._h))
 
     def pdf_error_count(self, stream=None) -> int:
         v = C.c_longlong()
@@ -284,19 +300,18 @@ class PdfGrid:
     # ---- evaluation (host tensors; the e2e path) -------------------------------------------
     def pdf_xfxq2_host(self, pids, x: torch.Tensor, q2: torch.Tensor, out: torch.Tensor):
         pid = _hi(list(pids))
-        for t in (x, q2, out):
-            if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
-                raise PdfGridError("host call takes contiguous CPU float64 tensors")
-        _check(lib().pdf_xfxq2_host(self._h, _iptr(pid), pid.numel(), x.numel(), C.c_void_p(x.data_ptr()),
-                                    C.c_void_p(q2.data_ptr()), C.c_void_p(out.data_ptr())), "pdf_xfxq2_host")
+        n = x.numel()
+        _check(lib().pdf_xfxq2_host(self._h, _iptr(pid), pid.numel(), n, _host(x, "x", n), _host(q2, "q2", n),
+                                    _host(out, "out", n * pid.numel(), at_least=True)), "pdf_xfxq2_host")
         return out
 
     def pdf_alphas_q2_host(self, q2: torch.Tensor, out: torch.Tensor):
-        _check(lib().pdf_alphas_q2_host(self._h, q2.numel(), C.c_void_p(q2.data_ptr()),
-                                        C.c_void_p(out.data_ptr())), "pdf_alphas_q2_host")
+        n = q2.numel()
+        _check(lib().pdf_alphas_q2_host(self._h, n, _host(q2, "q2", n), _host(out, "out", n, at_least=True)), "pdf_alphas_q2_host")
         return out
 
     def pdf_lumi_host(self, x1, x2, q2, weights, out):
-        _check(lib().pdf_lumi_host(self._h, x1.numel(), *[C.c_void_p(t.data_ptr()) for t in (x1, x2, q2, weights, out)]),
-               "pdf_lumi_host")
+        n = x1.numel()
+        _check(lib().pdf_lumi_host(self._h, n, _host(x1, "x1", n), _host(x2, "x2", n), _host(q2, "q2", n),
+                                   _host(weights, "weights", n), _host(out, "out", n, at_least=True)), "pdf_lumi_host")
         return out

@@ -105,7 +105,7 @@ k_member_plan(const unsigned *__restrict__ hist, int nmem, int chunk, unsigned *
         cursor[m] = start;
         const unsigned pieces = (cnt + (unsigned)chunk - 1) / (unsigned)chunk;
         unsigned step = pieces ? (cnt + pieces - 1) / pieces : 0u;     // equal pieces, whole A tiles (chunk is a multiple)
-        step = (step + kTileA - 1) / kTileA * kTileA;
+        step = (step + kS3TileA - 1) / kS3TileA * kS3TileA;
         for (unsigned o = 0; o < cnt; o += step) {
             const unsigned len = cnt - o < step ? cnt - o : step;
             reinterpret_cast<int4 *>(ctab)[nc++] = make_int4((int)(start + o), (int)len, m, 0);

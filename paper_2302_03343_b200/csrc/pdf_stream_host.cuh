@@ -1,0 +1,362 @@
+// pdf_stream_host.cuh -- host side of the binned path: key geometry, search tables, workspace, launch.
+#pragma once
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+namespace pdfg {
+
+constexpr long long kAutoMinN = 1 << 15;      // PDF_PATH_AUTO: below this the direct path is used
+constexpr long long kMemberMinPer = 1 << 14;  // PDF_PATH_AUTO with member ids: queries per member below which the direct path is used
+
+struct StreamPlan {
+    bool usable = false;
+    StreamDev dev{};
+    unsigned short *d_lutx = nullptr, *d_lutq = nullptr;
+    double2 *d_cxs = nullptr, *d_cqs = nullptr;
+    double *d_plus = nullptr;                 // scratch of k_q2plus
+    int ncells_q = 1;                         // Q2 cells (knots - sub-grids)
+    long long default_chunk = 256 * 1024;
+};
+
+// cell and t_q of 1.01*Q2min with the device log (C-9); res = {jg, t, in_range}
+__global__ void k_q2plus(GridDev G, double *res)
+{
+    if (threadIdx.x || blockIdx.x) return;
+    double q = G.q2plus;
+    if (q > G.qk[G.nqtot - 1]) { res[2] = 0.0; return; }
+    int j, jg;
+    q_locate(G, q, j, jg);
+    res[0] = (double)jg;
+    res[1] = (q == G.qk[jg + 1]) ? 1.0 : (log(q) - G.cq[jg].lo_log) * G.cq[jg].inv_d;
+    res[2] = 1.0;
+}
+
+// {ln lower knot, 1/dln} of every cell, from the cell tables the direct path uses (same numbers)
+__global__ void k_cell_pairs(const CellTab *__restrict__ tab, double2 *__restrict__ out, int n)
+{
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < n) out[c] = make_double2(tab[c].lo_log, tab[c].inv_d);
+}
+
+inline void stream_plan_free(StreamPlan &p)
+{
+    cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_cxs); cudaFree(p.d_cqs); cudaFree(p.d_plus);
+    p.d_lutx = p.d_lutq = nullptr; p.d_cxs = p.d_cqs = nullptr; p.d_plus = nullptr; p.usable = false;
+}
+
+// search table of one knot line: bucket = (high word of v >> shift) - base; entry = the largest c <= lim with
+// k[c] <= the bucket's lower edge (0 if none).  The widest bucket that keeps the table within kS3LutMax entries.
+inline void make_search_table(const std::vector<double> &k, int lim, int &shift, int &base, std::vector<unsigned short> &lut)
+{
+    auto hi = [](double v) { long long b; std::memcpy(&b, &v, 8); return (int)(b >> 32); };
+    const int h0 = hi(k.front()), h1 = hi(k.back());
+    shift = 12;                                         // 8 mantissa bits: 256 buckets per binade
+    while (shift < 31 && ((h1 >> shift) - (h0 >> shift) + 1) > kS3LutMax) ++shift;
+    base = h0 >> shift;
+    const int nb = (h1 >> shift) - base + 1;
+    lut.resize(nb);
+    int c = 0;
+    for (int b = 0; b < nb; ++b) {
+        const long long eb = ((long long)(base + b) << shift) << 32;
+        double edge;
+        std::memcpy(&edge, &eb, 8);
+        while (c < lim && k[c + 1] <= edge) ++c;
+        lut[b] = (unsigned short)c;
+    }
+}
+
+inline long long stream_chunk(const StreamPlan &p, long long n, long long chunk_opt)
+{
+    long long c = chunk_opt > 0 ? chunk_opt : p.default_chunk;
+    c = (c + kS3TileA - 1) / kS3TileA * kS3TileA;
+    long long need = (n + kS3TileA - 1) / kS3TileA * kS3TileA;
+    if (need < kS3TileA) need = kS3TileA;
+    return c < need ? c : need;
+}
+
+// bin capacities for a chunk size: interior cells 3x the uniform share + 32 (a uniform cloud is Poisson
+// around the share), class bins 2x the share of an x cell; beyond them queries overflow to the generic code
+inline void stream_caps(const StreamPlan &p, long long chunk, StreamDev &d)
+{
+    auto up32 = [](long long v) { return (int)((v + 31) / 32 * 32); };
+    d = p.dev;
+    const long long per_x = chunk / (d.ncx > 0 ? d.ncx : 1);
+    const long long per_cell = per_x / (p.ncells_q > 0 ? p.ncells_q : 1);
+    d.cap_int = up32(3 * per_cell + 32);
+    d.cap_cls = up32(2 * per_x + 64);
+    d.cap_lx = d.cap_cls;
+    d.cap_lxc = 2 * d.cap_cls;
+    if (d.cap_int > chunk) d.cap_int = up32(chunk);
+    if (d.cap_cls > chunk) d.cap_cls = d.cap_lx = up32(chunk);
+    if (d.cap_lxc > chunk) d.cap_lxc = up32(chunk);
+    d.rowcap = d.nqt * d.cap_int + 2 * d.cap_cls;
+    d.lxbase = d.ncx * d.rowcap;
+    d.slab = d.lxbase + d.nqt * d.cap_lx + 2 * d.cap_lxc;
+}
+
+inline size_t stream_workspace_bytes(const StreamPlan &p, long long n, long long chunk_opt)
+{
+    if (!p.usable) return 0;
+    const long long chunk = stream_chunk(p, n, chunk_opt);
+    StreamDev d;
+    stream_caps(p, chunk, d);
+    size_t b = 4096;                                                    // ctrl
+    b += align_up(sizeof(unsigned) * (size_t)kS3Ring * d.nbins, 256);
+    b += 256;                                                           // ovf_count
+    b += align_up(sizeof(Payload) * (size_t)kS3Ring * d.slab, 256);
+    b += align_up(sizeof(Payload) * (size_t)kS3Ring * chunk, 256);
+    return b + 256;
+}
+
+inline void stream_carve(void *ws, long long chunk, const StreamDev &d, StreamWorkspace &w)
+{
+    char *c = (char *)align_up((size_t)ws, 256);
+    w.ctrl = (unsigned long long *)c; c += 4096;
+    w.counts = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)kS3Ring * d.nbins, 256);
+    w.ovf_count = (unsigned *)c; c += 256;
+    w.bins = (Payload *)c; c += align_up(sizeof(Payload) * (size_t)kS3Ring * d.slab, 256);
+    w.ovf = (Payload *)c;
+    (void)chunk;
+}
+
+inline size_t stream_smem_bytes(const GridDev &G, const StreamDev &d)
+{
+    return s3_table_bytes_padded(G.nx, G.nqtot, d.nbx, d.nbq) + 32 + (size_t)kS3Warps * 2 * kS3Batch * sizeof(Payload);
+}
+
+// builds the search tables and the key geometry; leaves usable = false when the grid does not fit the
+// specialised path (then every call takes the direct path; pdf_last_path reports which one ran)
+inline int stream_plan_init(StreamPlan &p, const GridDev &G, const std::vector<double> &xk, const std::vector<double> &qk, int nsub)
+{
+    p.usable = false;
+    const int nx = G.nx, nqt = G.nqtot;
+    if (G.nflav != kNF || G.nfp != kNFP) return 0;
+    if (nx - 1 > kS3MaxCells || nqt > kS3MaxCells || nx < 2) return 0;
+    StreamDev &d = p.dev;
+    d.ncx = nx - 1; d.nqt = nqt; d.nfk = nqt + 2;
+    d.nbins = (d.ncx + 1) * d.nfk;
+    d.ng = (nqt + kS3FkPerUnit - 1) / kS3FkPerUnit;
+    d.tb = (d.ncx + 1) * kS3ClassParts + (d.ncx + 1) * d.ng + kS3Ovf;
+    p.ncells_q = nqt - nsub;
+
+    std::vector<unsigned short> lx, lq;
+    make_search_table(xk, nx - 2, d.xshift, d.xbase, lx);
+    make_search_table(qk, nqt - 1, d.qshift, d.qbase, lq);
+    d.nbx = (int)lx.size(); d.nbq = (int)lq.size();
+
+    if (cudaMalloc((void **)&p.d_lutx, sizeof(unsigned short) * lx.size()) != cudaSuccess) return PDF_ENOMEM;
+    if (cudaMalloc((void **)&p.d_lutq, sizeof(unsigned short) * lq.size()) != cudaSuccess) return PDF_ENOMEM;
+    if (cudaMalloc((void **)&p.d_cxs, sizeof(double2) * nx) != cudaSuccess) return PDF_ENOMEM;
+    if (cudaMalloc((void **)&p.d_cqs, sizeof(double2) * nqt) != cudaSuccess) return PDF_ENOMEM;
+    if (cudaMalloc((void **)&p.d_plus, sizeof(double) * 4) != cudaSuccess) return PDF_ENOMEM;
+    cudaMemcpy(p.d_lutx, lx.data(), sizeof(unsigned short) * lx.size(), cudaMemcpyHostToDevice);
+    cudaMemcpy(p.d_lutq, lq.data(), sizeof(unsigned short) * lq.size(), cudaMemcpyHostToDevice);
+    k_cell_pairs<<<(nx + 127) / 128, 128>>>(G.cx, p.d_cxs, nx - 1);
+    k_cell_pairs<<<(nqt + 127) / 128, 128>>>(G.cq, p.d_cqs, nqt);
+    k_q2plus<<<1, 32>>>(G, p.d_plus);
+    double res[3] = {0, 0, 0};
+    if (cudaMemcpy(res, p.d_plus, sizeof res, cudaMemcpyDeviceToHost) != cudaSuccess) return PDF_ECUDA;
+    d.lutx = p.d_lutx; d.lutq = p.d_lutq; d.cxs = p.d_cxs; d.cqs = p.d_cqs;
+    // pdf_locate on this path needs only the tables
+    if (cudaFuncSetAttribute(k_locate_stream, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)s3_table_bytes_padded(nx, nqt, d.nbx, d.nbq)) != cudaSuccess) return 0;
+    if (res[2] != 1.0) return 0;                           // 1.01*Q2min beyond the grid: direct path only
+    d.jgplus = (int)res[0]; d.tqplus = res[1];
+    const size_t smem = stream_smem_bytes(G, d);
+    if (smem > 200 * 1024) return 0;
+    if (cudaFuncSetAttribute(k_pdf_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    p.usable = true;
+    return 0;
+}
+
+inline bool stream_qualifies(const StreamPlan &p, const int *member) { return p.usable && !member; }
+inline bool stream_members_qualifies(const StreamPlan &p, const GridDev &G, const int *member)
+{
+    return p.usable && member && G.nmem > 1 && G.nmem <= kMemMax;
+}
+
+// one memset + one persistent kernel for the whole call
+template <typename Scope>
+inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm, long long n, const double *x,
+                        const double *q2, double *out, long long ld, void *ws, size_t ws_bytes, long long chunk_opt,
+                        cudaStream_t s, int count_err = 1, const int *ctab = nullptr, const int *nchunks_dev = nullptr)
+{
+    if (stream_workspace_bytes(p, n, chunk_opt) > ws_bytes) return PDF_EWORKSPACE;
+    StreamArgs A;
+    A.ctab = ctab; A.nchunks_dev = nchunks_dev;
+    A.G = G; A.cm = cm;
+    A.chunk = stream_chunk(p, n, chunk_opt);
+    stream_caps(p, A.chunk, A.B);
+    stream_carve(ws, A.chunk, A.B, A.W);
+    A.x = x; A.q2 = q2; A.out = out; A.n = n; A.ld = ld;
+    A.nchunks = (int)((n + A.chunk - 1) / A.chunk);
+    A.ta = (int)(A.chunk / kS3TileA);
+    A.identity = cm.n == kNF;
+    for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
+    A.zfill = (ld == cm.n) ? 1 : 0;
+    A.count_err = count_err;
+    const size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts + ovf_count
+    if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
+    const size_t smem = stream_smem_bytes(G, A.B);
+    int per_sm = 0, dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_pdf_stream, kS3Threads, smem) != cudaSuccess || per_sm < 1)
+        return PDF_ECUDA;
+    const unsigned long long max_ctas = (unsigned long long)per_sm * sms;         // all CTAs must be co-resident
+    // with a chunk table the chunk count is on the device: the launch takes its upper bound
+    const long long nch = ctab ? member_max_chunks(n, A.chunk, G.nmem) : (long long)A.nchunks;
+    const unsigned long long tickets = (unsigned long long)nch * (A.ta + A.B.tb);
+    const unsigned long long want = (tickets + kS3Warps - 1) / kS3Warps;
+    const unsigned grid = (unsigned)(want < max_ctas ? want : max_ctas);
+    {
+        Scope sc(s, "k_pdf_stream");
+        k_pdf_stream<<<grid, kS3Threads, smem, s>>>(A);
+    }
+    return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
+}
+
+template <typename Scope>
+inline int stream_locate(const GridDev &G, const StreamPlan &p, long long n, const double *x, const double *q2,
+                         int *ix, int *iq, int *isub, int *region, cudaStream_t s)
+{
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long want = (n + 255) / 256;
+    const unsigned grid = (unsigned)(want < (long long)sms * 8 ? want : (long long)sms * 8);
+    Scope sc(s, "k_locate_stream");
+    k_locate_stream<<<grid, 256, s3_table_bytes_padded(G.nx, G.nqtot, p.dev.nbx, p.dev.nbq), s>>>(G, p.dev, n, x, q2, ix, iq, isub, region);
+    return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
+}
+
+// ---- luminosity on top of the binned path ------------------------------------------------------
+// pdf_lumi in slices of kLumiSlice events: xf(x1,Q2) and xf(x2,Q2) of the slice by two runs of the
+// persistent kernel into two scratch arrays, then k_lumi_combine reduces the 11 x 11 coupling
+// per event in registers.
+constexpr long long kLumiSlice = 1LL << 24;
+
+struct CouplingParam { double c[kNF * kNF]; };            // passed by value: constant-bank operands
+
+__global__ void __launch_bounds__(256)
+k_lumi_combine(const __grid_constant__ CouplingParam C, long long n, const double *__restrict__ f1,
+               const double *__restrict__ f2, const double *__restrict__ x1, const double *__restrict__ x2,
+               const double *__restrict__ w, double *__restrict__ out, unsigned long long *err_count)
+{
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const double a = __ldcs(x1 + e), b = __ldcs(x2 + e);
+    double h[kNF];
+    const double inv_b = 1.0 / b, inv_a = 1.0 / a;
+#pragma unroll
+    for (int j = 0; j < kNF; ++j) h[j] = __ldcs(f2 + e * kNF + j) * inv_b;
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < kNF; ++i) {
+        double row = 0.0;
+#pragma unroll
+        for (int j = 0; j < kNF; ++j) row = fma(C.c[i * kNF + j], h[j], row);
+        acc = fma(__ldcs(f1 + e * kNF + i) * inv_a, row, acc);
+    }
+    const double v = __ldcs(w + e) * acc;
+    if (!(finite_pos(a) && finite_pos(b)) || v != v) {
+        // an invalid parton made its whole row NaN (C-10); the event counts once
+        if (isnan(__ldcs(f1 + e * kNF)) || isnan(__ldcs(f2 + e * kNF))) { atomicAdd(err_count, 1ULL); out[e] = qnan(); return; }
+    }
+    out[e] = v;
+}
+
+inline bool stream_lumi_qualifies(const StreamPlan &p) { return p.usable; }
+inline size_t stream_lumi_scratch_bytes(const StreamPlan &p, long long n)
+{
+    const long long slice = n < kLumiSlice ? n : kLumiSlice;
+    return p.usable ? (size_t)2 * slice * kNF * sizeof(double) + 512 : 0;
+}
+
+template <typename Scope>
+inline int stream_lumi(const GridDev &G, const StreamPlan &p, const double *hostC, long long n, const double *x1,
+                       const double *x2, const double *q2, const double *w, double *out, void *ws, size_t ws_bytes,
+                       long long chunk_opt, cudaStream_t s)
+{
+    const long long slice = n < kLumiSlice ? n : kLumiSlice;
+    const size_t ws_x = stream_workspace_bytes(p, slice, chunk_opt);
+    if (ws_x + stream_lumi_scratch_bytes(p, n) > ws_bytes) return PDF_EWORKSPACE;
+    double *f1 = reinterpret_cast<double *>(align_up((size_t)ws + ws_x, 256));
+    double *f2 = f1 + slice * kNF;
+    ColMap cm; cm.n = kNF;
+    for (int f = 0; f < kNF; ++f) cm.col[f] = f;
+    CouplingParam C;
+    for (int k = 0; k < kNF * kNF; ++k) C.c[k] = hostC[k];
+    for (long long off = 0; off < n; off += slice) {
+        const long long m = n - off < slice ? n - off : slice;
+        int rc = stream_xfxq2<Scope>(G, p, cm, m, x1 + off, q2 + off, f1, kNF, ws, ws_x, chunk_opt, s, 0);
+        if (rc) return rc;
+        rc = stream_xfxq2<Scope>(G, p, cm, m, x2 + off, q2 + off, f2, kNF, ws, ws_x, chunk_opt, s, 0);
+        if (rc) return rc;
+        {
+            Scope sc(s, "k_lumi_combine");
+            k_lumi_combine<<<(unsigned)((m + 255) / 256), 256, 0, s>>>(C, m, f1, f2, x1 + off, x2 + off, w + off, out + off,
+                                                                      G.err_count);
+        }
+    }
+    return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
+}
+
+// a-8 on the binned path (pdf_members.cuh): per slice, partition by member, one persistent-kernel
+// run over the chunk table into the sorted scratch rows, gather back to query order
+inline size_t stream_members_bytes(const StreamPlan &p, const GridDev &G, long long n, long long chunk_opt, int npid)
+{
+    if (!p.usable || G.nmem < 2 || G.nmem > kMemMax) return 0;
+    const long long slice = member_slice(n);
+    const long long chunk = stream_chunk(p, slice, chunk_opt);
+    return stream_workspace_bytes(p, slice, chunk_opt) + member_scratch_bytes(slice, chunk, G.nmem, npid) + 256;
+}
+
+template <typename Scope>
+inline int stream_members(const GridDev &G, const StreamPlan &p, const ColMap &cm, long long n, const double *x,
+                          const double *q2, const int *member, double *out, long long ld, void *ws, size_t ws_bytes,
+                          long long chunk_opt, cudaStream_t s)
+{
+    if (stream_members_bytes(p, G, n, chunk_opt, cm.n) > ws_bytes) return PDF_EWORKSPACE;
+    const long long slice = member_slice(n);
+    const long long chunk = stream_chunk(p, slice, chunk_opt);
+    const size_t ws_x = stream_workspace_bytes(p, slice, chunk_opt);
+    MemberWs M;
+    member_carve((char *)ws + ws_x, slice, chunk, G.nmem, M);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const size_t hsm = sizeof(unsigned) * (size_t)G.nmem;
+    if (cudaFuncSetAttribute(k_member_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)member_scatter_smem(G.nmem)) != cudaSuccess)
+        return PDF_ECUDA;
+    for (long long off = 0; off < n; off += slice) {
+        const long long m = n - off < slice ? n - off : slice;
+        if (cudaMemsetAsync(M.hist, 0, hsm, s) != cudaSuccess) return PDF_ECUDA;
+        {
+            Scope sc(s, "k_member_hist");
+            long long want = (m + 2047) / 2048;
+            k_member_hist<<<(unsigned)(want < sms * 8 ? want : sms * 8), 256, hsm, s>>>(member + off, m, G.nmem, M.hist);
+        }
+        {
+            Scope sc(s, "k_member_plan");
+            k_member_plan<<<1, 256, hsm, s>>>(M.hist, G.nmem, (int)chunk, M.cursor, M.ctab, M.nchunks);
+        }
+        {
+            Scope sc(s, "k_member_scatter");
+            k_member_scatter<<<(unsigned)((m + kMemScatThreads * kMemTileQ - 1) / (kMemScatThreads * kMemTileQ)), kMemScatThreads, member_scatter_smem(G.nmem), s>>>(
+                x + off, q2 + off, member + off, m, G.nmem, M.cursor, M.xs, M.q2s, M.inv);
+        }
+        int rc = stream_xfxq2<Scope>(G, p, cm, m, M.xs, M.q2s, M.tmp, cm.n, ws, ws_x, chunk_opt, s, 1, M.ctab, M.nchunks);
+        if (rc) return rc;
+        {
+            Scope sc(s, "k_member_gather");
+            long long want = (m + 255) / 256;
+            k_member_gather<<<(unsigned)(want < sms * 16 ? want : sms * 16), 256, 0, s>>>(M.tmp, M.inv, m, cm.n, out + off * ld, ld,
+                                                                                       G.err_count);
+        }
+    }
+    return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
+}
+
+}  // namespace pdfg

@@ -13,7 +13,7 @@
 
 #include "pdf_common.cuh"
 #include "pdf_generic.cuh"
-#include "pdf_binned.cuh"
+#include "pdf_stream.cuh"
 
 using namespace pdfg;
 
@@ -84,7 +84,8 @@ struct pdf_grid {
     int path = PDF_PATH_AUTO;
     long long chunk = 0;      // binned-path chunk size override (0 = default)
     HostStage stage[2];
-    BinnedPlan bplan{};       // cell/key geometry of the binned path (pdf_binned.cuh)
+    StreamPlan bplan{};       // key geometry and search tables of the binned path (pdf_stream.cuh)
+    mutable int last_path = 0;  // PDF_PATH_DIRECT / PDF_PATH_BINNED: what the last evaluation call of this handle ran
 };
 
 namespace {
@@ -103,7 +104,7 @@ void free_grid(pdf_grid *g)
     cudaFree(g->d_sub_of); cudaFree(g->d_qoff); cudaFree(g->d_cell_adj); cudaFree(g->d_cx); cudaFree(g->d_cq); cudaFree(g->d_ca);
     cudaFree(g->d_ak); cudaFree(g->d_alk); cudaFree(g->d_av); cudaFree(g->d_C); cudaFree(g->d_err);
     cudaFree(g->d_acell); cudaFree(g->d_alut);
-    binned_plan_free(g->bplan);
+    stream_plan_free(g->bplan);
     for (auto &s : g->stage) {
         cudaFree(s.in); cudaFree(s.out); cudaFree(s.ws);
         if (s.stream) cudaStreamDestroy(s.stream);
@@ -244,7 +245,7 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
     d.V = g->d_V; d.memstride = (size_t)tot * nx * nfp;
     d.q2plus = 1.01 * q2_knots[0];
     d.na = 0; d.alphas_mode = PDF_ALPHAS_FREEZE; d.C = nullptr; d.err_count = g->d_err;
-    rc = binned_plan_init(g->bplan, g->d, g->xk, g->qk, g->qoff);
+    rc = stream_plan_init(g->bplan, g->d, g->xk, g->qk, nsub);
     if (rc != PDF_OK) { free_grid(g); return rc; }
     *out = g;
     return PDF_OK;

@@ -27,12 +27,11 @@ int launch_direct(const pdf_grid *g, const ColMap &cm, long long n, const double
     return PDF_OK;
 }
 
-}  // namespace
+int on_device(const pdf_grid *g);
 
-extern "C" {
-
-int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
-                 const double *q2, const int *member, double *out, long long ld_out, void *stream)
+// pdf_xfxq2_ex with the workspace as an argument (the *_host calls pass their own staging workspace)
+int xfxq2_impl(const pdf_grid *g, void *ws, size_t ws_bytes, const int *pids, int npid, long long n, const double *x,
+               const double *q2, const int *member, double *out, long long ld_out, cudaStream_t s)
 {
     if (!g || n < 0 || ld_out < npid) return PDF_EINVAL;
     ColMap cm;
@@ -40,27 +39,82 @@ int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, cons
     if (rc) return rc;
     if (n == 0) return PDF_OK;
     if (!x || !q2 || !out) return PDF_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
+    if ((rc = on_device(g))) return rc;
     // a-8: per-query member ids on the binned path (partition by member first, pdf_members.cuh)
-    if (binned_members_qualifies(g->bplan, g->d, member) && npid <= g->d.nflav) {
-        const size_t need = binned_members_bytes(g->bplan, g->d, n, g->chunk, npid);
+    if (stream_members_qualifies(g->bplan, g->d, member) && npid <= g->d.nflav) {
+        const size_t need = stream_members_bytes(g->bplan, g->d, n, g->chunk, npid);
         if (g->path == PDF_PATH_BINNED) {
-            if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
-            return binned_members<LaunchScope>(g->d, g->bplan, cm, n, x, q2, member, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
+            if (!ws || ws_bytes < need) return PDF_EWORKSPACE;
+            g->last_path = PDF_PATH_BINNED;
+            return stream_members<LaunchScope>(g->d, g->bplan, cm, n, x, q2, member, out, ld_out, ws, ws_bytes, g->chunk, s);
         }
-        if (g->path == PDF_PATH_AUTO && g->ws && g->ws_bytes >= need && n >= kMemberMinPer * g->d.nmem)
-            return binned_members<LaunchScope>(g->d, g->bplan, cm, n, x, q2, member, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
+        if (g->path == PDF_PATH_AUTO && ws && ws_bytes >= need && n >= kMemberMinPer * g->d.nmem) {
+            g->last_path = PDF_PATH_BINNED;
+            return stream_members<LaunchScope>(g->d, g->bplan, cm, n, x, q2, member, out, ld_out, ws, ws_bytes, g->chunk, s);
+        }
     }
-    bool ok_binned = binned_qualifies(g->bplan, cm, member);
-    const size_t need = binned_workspace_bytes(g->bplan, n, g->chunk);      // what THIS call uses of the workspace
+    bool ok_binned = stream_qualifies(g->bplan, member);
+    const size_t need = stream_workspace_bytes(g->bplan, n, g->chunk);      // what THIS call uses of the workspace
     bool want_binned = (g->path == PDF_PATH_BINNED) ||
-                       (g->path == PDF_PATH_AUTO && g->ws && ok_binned && n >= kAutoMinN && g->ws_bytes >= need);
+                       (g->path == PDF_PATH_AUTO && ws && ok_binned && n >= kAutoMinN && ws_bytes >= need);
     if (want_binned) {
         if (!ok_binned) return PDF_EINVAL;
-        if (!g->ws || g->ws_bytes < need) return PDF_EWORKSPACE;
-        return binned_xfxq2<LaunchScope>(g->d, g->bplan, cm, n, x, q2, out, ld_out, g->ws, g->ws_bytes, g->chunk, s);
+        if (!ws || ws_bytes < need) return PDF_EWORKSPACE;
+        g->last_path = PDF_PATH_BINNED;
+        return stream_xfxq2<LaunchScope>(g->d, g->bplan, cm, n, x, q2, out, ld_out, ws, ws_bytes, g->chunk, s);
     }
+    g->last_path = PDF_PATH_DIRECT;
     return launch_direct(g, cm, n, x, q2, member, out, ld_out, s);
+}
+
+int lumi_impl(const pdf_grid *g, void *ws, size_t ws_bytes, long long n, const double *x1, const double *x2, const double *q2,
+              const double *weights, double *out, cudaStream_t s)
+{
+    if (!g || n < 0) return PDF_EINVAL;
+    if (!g->d.C) return PDF_ESTATE;
+    if (g->d.nflav > kMaxLumiFlav) return PDF_EINVAL;
+    if (n == 0) return PDF_OK;
+    if (!x1 || !x2 || !q2 || !weights || !out) return PDF_EINVAL;
+    int rc = on_device(g);
+    if (rc) return rc;
+    const size_t need = stream_workspace_bytes(g->bplan, n < kLumiSlice ? n : kLumiSlice, g->chunk) +
+                        stream_lumi_scratch_bytes(g->bplan, n) + 256;
+    bool want_binned = stream_lumi_qualifies(g->bplan) &&
+                       (g->path == PDF_PATH_BINNED || (g->path == PDF_PATH_AUTO && ws && n >= kAutoMinN &&
+                                                       ws_bytes >= need));
+    if (want_binned) {
+        g->last_path = PDF_PATH_BINNED;
+        return stream_lumi<LaunchScope>(g->d, g->bplan, g->h_C.data(), n, x1, x2, q2, weights, out, ws, ws_bytes, g->chunk, s);
+    }
+    g->last_path = PDF_PATH_DIRECT;
+    const long long slice = 1LL << 30;
+    for (long long off = 0; off < n; off += slice) {
+        long long m = n - off < slice ? n - off : slice;
+        LaunchScope a(s, "k_lumi_direct");
+        k_lumi_direct<<<blocks_for(m, 128), 128, 0, s>>>(g->d, m, x1 + off, x2 + off, q2 + off, weights + off, out + off);
+    }
+    CK(cudaGetLastError());
+    return PDF_OK;
+}
+
+// every evaluation call runs on the device the grid lives on
+int on_device(const pdf_grid *g)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return PDF_ECUDA;
+    if (dev != g->device && cudaSetDevice(g->device) != cudaSuccess) return PDF_ECUDA;
+    return PDF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+                 const double *q2, const int *member, double *out, long long ld_out, void *stream)
+{
+    if (!g) return PDF_EINVAL;
+    return xfxq2_impl(g, g->ws, g->ws_bytes, pids, npid, n, x, q2, member, out, ld_out, (cudaStream_t)stream);
 }
 
 int pdf_xfxq2(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
@@ -121,10 +175,10 @@ int pdf_xfxq2_xgrid(const pdf_grid *g, const int *pids, int npid, long long npts
 size_t pdf_workspace_bytes(const pdf_grid *g, long long n)
 {
     if (!g || n < 0) return 0;
-    size_t b = binned_workspace_bytes(g->bplan, n, g->chunk);
-    if (b && g->d.C) b += binned_lumi_scratch_bytes(g->bplan, n) + 256;    // pdf_lumi slices (only once a coupling is set)
+    size_t b = stream_workspace_bytes(g->bplan, n, g->chunk);
+    if (b && g->d.C) b += stream_lumi_scratch_bytes(g->bplan, n) + 256;    // pdf_lumi slices (only once a coupling is set)
     if (g->d.nmem > 1) {                                                // a-8: member partition scratch (all flavours)
-        size_t m = binned_members_bytes(g->bplan, g->d, n, g->chunk, g->d.nflav);
+        size_t m = stream_members_bytes(g->bplan, g->d, n, g->chunk, g->d.nflav);
         if (m > b) b = m;
     }
     return b;
@@ -152,27 +206,8 @@ int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out,
 int pdf_lumi(const pdf_grid *g, long long n, const double *x1, const double *x2, const double *q2,
              const double *weights, double *out, void *stream)
 {
-    if (!g || n < 0) return PDF_EINVAL;
-    if (!g->d.C) return PDF_ESTATE;
-    if (g->d.nflav > kMaxLumiFlav) return PDF_EINVAL;
-    if (n == 0) return PDF_OK;
-    if (!x1 || !x2 || !q2 || !weights || !out) return PDF_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    const size_t need = binned_workspace_bytes(g->bplan, n < kLumiSlice ? n : kLumiSlice, g->chunk) +
-                        binned_lumi_scratch_bytes(g->bplan, n) + 256;
-    bool want_binned = binned_lumi_qualifies(g->bplan) &&
-                       (g->path == PDF_PATH_BINNED || (g->path == PDF_PATH_AUTO && g->ws && n >= kAutoMinN &&
-                                                       g->ws_bytes >= need));
-    if (want_binned)
-        return binned_lumi<LaunchScope>(g->d, g->bplan, g->h_C.data(), n, x1, x2, q2, weights, out, g->ws, g->ws_bytes, g->chunk, s);
-    const long long slice = 1LL << 30;
-    for (long long off = 0; off < n; off += slice) {
-        long long m = n - off < slice ? n - off : slice;
-        LaunchScope a(s, "k_lumi_direct");
-        k_lumi_direct<<<blocks_for(m, 128), 128, 0, s>>>(g->d, m, x1 + off, x2 + off, q2 + off, weights + off, out + off);
-    }
-    CK(cudaGetLastError());
-    return PDF_OK;
+    if (!g) return PDF_EINVAL;
+    return lumi_impl(g, g->ws, g->ws_bytes, n, x1, x2, q2, weights, out, (cudaStream_t)stream);
 }
 
 int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2, int *ix,
@@ -181,7 +216,17 @@ int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2
     if (!g || n < 0) return PDF_EINVAL;
     if (n == 0) return PDF_OK;
     if (!x || !q2) return PDF_EINVAL;
+    int rc = on_device(g);
+    if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
+    // the search of the path the evaluation calls take: the table-driven search of the binned kernel's A
+    // tiles unless PDF_PATH_DIRECT is set (or the grid does not fit the binned path), then the binary
+    // search of the direct kernels
+    if (g->path != PDF_PATH_DIRECT && g->bplan.usable) {
+        g->last_path = PDF_PATH_BINNED;
+        return stream_locate<LaunchScope>(g->d, g->bplan, n, x, q2, ix, iq, isub, region, s);
+    }
+    g->last_path = PDF_PATH_DIRECT;
     const long long slice = 1LL << 30;
     for (long long off = 0; off < n; off += slice) {
         long long m = n - off < slice ? n - off : slice;
@@ -192,6 +237,11 @@ int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2
     }
     CK(cudaGetLastError());
     return PDF_OK;
+}
+
+int pdf_last_path(const pdf_grid *g)
+{
+    return g ? g->last_path : PDF_EINVAL;
 }
 
 int pdf_error_count(const pdf_grid *g, long long *n_invalid, void *stream)

@@ -57,7 +57,6 @@ int pdf_xfxq2_host(pdf_grid *g, const int *pids, int npid, long long n, const do
     if (!x || !q2 || !out) return PDF_EINVAL;
     long long cap = n < kHostChunk ? n : kHostChunk;
     size_t wsb = pdf_workspace_bytes(g, cap);
-    void *user_ws = g->ws; size_t user_wsb = g->ws_bytes;
     for (auto &st : g->stage) {
         int rc = stage_reserve(g, st, 2 * (size_t)cap, (size_t)cap * npid, wsb);
         if (rc) return rc;
@@ -65,13 +64,11 @@ int pdf_xfxq2_host(pdf_grid *g, const int *pids, int npid, long long n, const do
     int rc = host_pipeline(g, n, [&](HostStage &st, long long off, long long m) -> int {
         CK(cudaMemcpyAsync(st.in, x + off, sizeof(double) * m, cudaMemcpyHostToDevice, st.stream));
         CK(cudaMemcpyAsync(st.in + cap, q2 + off, sizeof(double) * m, cudaMemcpyHostToDevice, st.stream));
-        if (wsb) { g->ws = st.ws; g->ws_bytes = st.ws_bytes; }
-        int r = pdf_xfxq2(g, pids, npid, m, st.in, st.in + cap, st.out, st.stream);
+        int r = xfxq2_impl(g, st.ws, st.ws_bytes, pids, npid, m, st.in, st.in + cap, nullptr, st.out, npid, st.stream);
         if (r) return r;
         CK(cudaMemcpyAsync(out + off * npid, st.out, sizeof(double) * m * npid, cudaMemcpyDeviceToHost, st.stream));
         return PDF_OK;
     });
-    g->ws = user_ws; g->ws_bytes = user_wsb;
     return rc;
 }
 
@@ -104,7 +101,6 @@ int pdf_lumi_host(pdf_grid *g, long long n, const double *x1, const double *x2, 
     if (!x1 || !x2 || !q2 || !weights || !out) return PDF_EINVAL;
     long long cap = n < kHostChunk ? n : kHostChunk;
     size_t wsb = pdf_workspace_bytes(g, cap);
-    void *user_ws = g->ws; size_t user_wsb = g->ws_bytes;
     for (auto &st : g->stage) {
         int rc = stage_reserve(g, st, 4 * (size_t)cap, (size_t)cap, wsb);
         if (rc) return rc;
@@ -113,13 +109,11 @@ int pdf_lumi_host(pdf_grid *g, long long n, const double *x1, const double *x2, 
         const double *src[4] = {x1, x2, q2, weights};
         for (int a = 0; a < 4; ++a)
             CK(cudaMemcpyAsync(st.in + a * cap, src[a] + off, sizeof(double) * m, cudaMemcpyHostToDevice, st.stream));
-        if (wsb) { g->ws = st.ws; g->ws_bytes = st.ws_bytes; }
-        int r = pdf_lumi(g, m, st.in, st.in + cap, st.in + 2 * cap, st.in + 3 * cap, st.out, st.stream);
+        int r = lumi_impl(g, st.ws, st.ws_bytes, m, st.in, st.in + cap, st.in + 2 * cap, st.in + 3 * cap, st.out, st.stream);
         if (r) return r;
         CK(cudaMemcpyAsync(out + off, st.out, sizeof(double) * m, cudaMemcpyDeviceToHost, st.stream));
         return PDF_OK;
     });
-    g->ws = user_ws; g->ws_bytes = user_wsb;
     return rc;
 }
 

@@ -4,7 +4,6 @@ must agree with the direct kernels."""
 import os
 import sys
 
-import numpy as np
 import torch
 
 sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
@@ -16,14 +15,16 @@ x, q = synth.queries_c2(spec, n, seed=synth.BASE_SEED + 31)
 g = B.PdfGrid.from_spec(spec, workspace_for=n)
 xd, qd = x.cuda(), q.cuda()
 g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_DIRECT)
-d = g.pdf_xfxq2(spec.pids, xd, qd).cpu().numpy()
+d = g.pdf_xfxq2(spec.pids, xd, qd)
 g.pdf_grid_set_option(B.PDF_OPT_PATH, B.PDF_PATH_BINNED)
 worst = 0
-for rep in range(3):
-    b = g.pdf_xfxq2(spec.pids, xd, qd).cpu().numpy()
-    assert np.array_equal(np.isnan(b), np.isnan(d))
-    err = np.abs(np.nan_to_num(b) - np.nan_to_num(d)) / (np.abs(np.nan_to_num(d)) + 1e-30)
-    bad = int((err.max(axis=1) > 1e-9).sum())
+for rep in range(3 if n <= 4_000_000 else 2):
+    b = g.pdf_xfxq2(spec.pids, xd, qd)
+    assert torch.equal(torch.isnan(b), torch.isnan(d))
+    # on the device: every row, relative difference of the two kernels' summation orders
+    err = (b.nan_to_num() - d.nan_to_num()).abs() / (d.nan_to_num().abs() + 1e-30)
+    bad = int((err.max(dim=1).values > 1e-9).sum())
     worst = max(worst, bad)
+    del b, err
 print("COLD_BAD_ROWS", worst)
 sys.exit(1 if worst else 0)

@@ -10,7 +10,7 @@ tests/test_oracle_pins.py::test_scale_*:
     factor (glibc's and CUDA's log may differ in the last bit); same for the extrapolation abscissa theta.
 Where the result cancels (|ref| << S: sign changes in Q2, x -> 1 where every flavour vanishes like 1 - t,
 flavours switched off below threshold) no evaluation can hold a strict relative bound.  The strict relative
-maximum over |ref| > STRICT_CUT * S[...,0] is reported and asserted by the C0/C1/C2 tests.
+maximum over the well-conditioned points is asserted <= 1e-12 by the C0/C1/C2 tests (see STRICT_COND below).
 NaN rows must match as NaN.
 """
 import numpy as np
@@ -18,7 +18,14 @@ import numpy as np
 import oracle
 
 REL = oracle.REL
-STRICT_CUT = 1e-3          # SURVEY C-12: "report also the strict maximum over points with |ref| > 1e-3 S"
+# SURVEY C-12: "report also the strict maximum over points with |ref| > 1e-3 S".  A strict relative bound can only
+# hold where the value is well conditioned in BOTH respects: at |ref| = 1e-3 S[0] the 16-term sum has lost 3 digits
+# (worst-case rounding 16 x 2^-53 S[0] = 1.8e-12 |ref| for any order of summation), and where the value vanishes
+# linearly in t (last x cell: every flavour is 0 at x = 1) the rounding of t alone gives 2^-52 / (1 - t) relative
+# (measured: 1.25e-12 on both GPU paths at the same C0 query).  So the strict 1e-12 bound is asserted over the points
+# with S[0] <= 100 |ref| and S[1] <= 100 |ref|, and the maximum at the survey's cut (|ref| > 1e-3 S[0]) is reported.
+STRICT_COND = 100.0
+STRICT_CUT_REPORT = 1e-3
 
 
 def value_errors(gpu, ref, S):
@@ -30,20 +37,24 @@ def value_errors(gpu, ref, S):
     tol = oracle.tolerance(ref[ok], S[ok])
     exact = err == 0
     ratio = np.where(exact, 0.0, err / np.where(tol > 0, tol, 1e-300))
-    strict_sel = np.abs(ref[ok]) > STRICT_CUT * S[ok][..., 0]
-    strict = float(np.max(err[strict_sel] / np.abs(ref[ok][strict_sel]))) if strict_sel.any() else 0.0
+    def strict_max(sel):
+        return float(np.max(err[sel] / np.abs(ref[ok][sel]))) if sel.any() else 0.0
+    aref = np.abs(ref[ok])
+    well = (S[ok][..., 0] <= STRICT_COND * aref) & (S[ok][..., 1] <= STRICT_COND * aref) & (aref > 0)
+    strict, strict_report = strict_max(well), strict_max(aref > STRICT_CUT_REPORT * S[ok][..., 0])
     # the same errors against tighter floors (what the floors could be lowered to): worst ratio per candidate
     probe = {}
     for fs in (1e-15, 5e-16):
         for ft in (2 * 2.0 ** -52, 2.0 ** -52):
             t2 = REL * np.abs(ref[ok]) + fs * S[ok][..., 0] + ft * S[ok][..., 1]
             probe[f"S{fs:g}_T{ft / 2.0 ** -52:g}ulp"] = float(np.max(np.where(exact, 0.0, err / np.where(t2 > 0, t2, 1e-300)))) if err.size else 0.0
-    return dict(worst=float(ratio.max()) if ratio.size else 0.0, strict_rel_max=strict,
+    return dict(worst=float(ratio.max()) if ratio.size else 0.0, strict_rel_max=strict, strict_rel_max_cut1e3=strict_report,
+                frac_well_conditioned=float(np.mean(well)) if well.size else 1.0,
                 frac_within_strict=float(np.mean(err <= REL * np.abs(ref[ok]))) if err.size else 1.0, probe=probe)
 
 
 def assert_values(gpu, ref, S, what="", strict=None):
-    """strict: if given, also assert the strict relative maximum (|ref| > STRICT_CUT S) <= strict"""
+    """strict: if given, also assert the strict relative maximum over the well-conditioned points <= strict"""
     st = value_errors(gpu, ref, S)
     assert st["worst"] <= 1.0, (what, st)
     if strict is not None:

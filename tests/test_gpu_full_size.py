@@ -1,19 +1,25 @@
-"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (PDF_PATH_AUTO
-with an attached workspace -> the binned persistent kernel): the CUDA path evaluates all n queries
-on seeded inputs generated on the device, the oracle evaluates a random sample of them one by one.
-Indices (region, sub-grid, cell) of the sample must be bit-exact, values obey tests/parity.py."""
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (PDF_PATH_AUTO with an
+attached workspace -> the binned persistent kernel): the CUDA path evaluates all n queries on seeded inputs
+generated on the device, and the oracle evaluates EVERY row of the same inputs in 1e7-row pieces (values by
+tests/parity.py; region, sub-grid and cell indices bit-exact).  PDF_FULL_PARITY_ROWS=<k> in the environment cuts
+the oracle's share to k evenly spread pieces of 1e6 rows (a fallback for slow hosts; default: all rows).
+The oracle's pass time is printed (SURVEY 8(d) "the oracle runs the full n in 1e7-query chunks")."""
+import os
+import time
+
 import numpy as np
 import pytest
 import torch
 
+import oracle as oracle_pkg
 from paper_2302_03343_b200 import synth
 from conftest import make_oracle_grid
-from parity import assert_values
+from parity import REL
 
 pytestmark = pytest.mark.gpu
 
 N_FULL = 100_000_000
-N_SAMPLE = 100_000
+PIECE = 10_000_000
 
 
 @pytest.fixture(scope="module")
@@ -24,17 +30,37 @@ def B():
     return binding
 
 
-def _sample(n, seed):
-    g = torch.Generator(device="cpu")
-    g.manual_seed(seed)
-    idx = torch.randint(0, n, (N_SAMPLE,), generator=g)
-    idx[:64] = torch.arange(64)                      # first tile
-    idx[64:128] = torch.arange(n - 64, n)            # ragged tail of the last chunk
-    return idx.cuda()
+def pieces(n):
+    k = int(os.environ.get("PDF_FULL_PARITY_ROWS", "0"))
+    if k <= 0:
+        return [(a, min(a + PIECE, n)) for a in range(0, n, PIECE)]
+    m = 1_000_000
+    starts = np.unique(np.concatenate([[0, n - m], np.linspace(0, n - m, k).astype(np.int64)]))
+    return [(int(a), int(a) + m) for a in starts]
 
 
-def test_c2_full_size_sampled(B, oracle_mod):
-    """configs[2]: 1e8 queries, 5 % extrapolated, 11 flavours, + alpha_s over the same Q2"""
+def check_piece(got, ref_fn, scale_fn, what, stats):
+    """got: GPU rows of the piece (numpy).  The oracle's values for every row; its condition numbers only for the
+    rows that are not already within the strict relative tolerance (they cost as much as the values)."""
+    ref = ref_fn()
+    nan_ref = np.isnan(ref)
+    assert np.array_equal(nan_ref, np.isnan(got)), f"{what}: NaN pattern differs"
+    err = np.abs(np.where(nan_ref, 0.0, got - ref))
+    loose = err > REL * np.abs(np.where(nan_ref, 0.0, ref))
+    rows = np.nonzero(loose.reshape(loose.shape[0], -1).any(axis=1))[0]
+    stats["rows"] += ref.shape[0]
+    stats["rows_needing_floor"] += int(rows.size)
+    if rows.size:
+        S = scale_fn(rows)
+        tol = oracle_pkg.tolerance(ref[rows], S)
+        ratio = err[rows] / np.maximum(tol, 1e-300)
+        worst = float(np.nanmax(ratio))
+        stats["worst"] = max(stats["worst"], worst)
+        assert worst <= 1.0, (what, worst, int(rows[np.nanargmax(ratio.reshape(rows.size, -1).max(axis=1))]))
+
+
+def test_c2_full_size_all_rows(B, oracle_mod):
+    """configs[2]: 1e8 queries, 5 % extrapolated, 11 flavours, + alpha_s over the same Q2; every row, every index"""
     spec = synth.grid_c1()
     n = N_FULL
     g = B.PdfGrid.from_spec(spec, workspace_for=n)
@@ -42,22 +68,29 @@ def test_c2_full_size_sampled(B, oracle_mod):
     x, q = synth.queries_c2(spec, n, device="cuda")
     out = g.pdf_xfxq2(spec.pids, x, q)
     assert g.pdf_error_count() == 0
-    idx = _sample(n, 5)
-    xs, qs = x[idx].cpu().numpy(), q[idx].cpu().numpy()
-    ref, S = og.xfxq2(spec.pids, xs, qs, want_scale=True)
-    assert_values(out[idx].cpu().numpy(), ref, S, "c2 full size")
-    ix, iq, isub, reg = og.locate(xs, qs)
-    gx, gq, gs, gr = [t.cpu().numpy() for t in g.pdf_locate(x[idx].contiguous(), q[idx].contiguous())]
-    assert np.array_equal(reg, gr) and np.array_equal(isub, gs) and np.array_equal(ix, gx) and np.array_equal(iq, gq)
-    assert len(np.unique(reg)) == 6                  # every class of Fig. 3.1(b) is in the sample
-    del out
     a = g.pdf_alphas_q2(q)
-    aref = og.alphas_q2(qs)
-    assert np.max(np.abs(a[idx].cpu().numpy() - aref) / np.abs(aref)) < 1e-12
+    gx, gq, gs, gr = g.pdf_locate(x, q)                      # the evaluation path's own search (PDF_PATH_AUTO)
+    stats = dict(rows=0, rows_needing_floor=0, worst=0.0)
+    regions = set()
+    t_oracle = 0.0
+    for a0, a1 in pieces(n):
+        xs, qs = x[a0:a1].cpu().numpy(), q[a0:a1].cpu().numpy()
+        t0 = time.perf_counter()
+        check_piece(out[a0:a1].cpu().numpy(), lambda: og.xfxq2(spec.pids, xs, qs),
+                    lambda rows: og.xfxq2(spec.pids, xs[rows], qs[rows], want_scale=True)[1], f"c2 rows {a0}..{a1}", stats)
+        t_oracle += time.perf_counter() - t0
+        ix, iq, isub, reg = og.locate(xs, qs)
+        assert np.array_equal(reg, gr[a0:a1].cpu().numpy()) and np.array_equal(isub, gs[a0:a1].cpu().numpy())
+        assert np.array_equal(ix, gx[a0:a1].cpu().numpy()) and np.array_equal(iq, gq[a0:a1].cpu().numpy())
+        regions |= set(np.unique(reg).tolist())
+        aref = og.alphas_q2(qs)
+        assert np.max(np.abs(a[a0:a1].cpu().numpy() - aref) / np.abs(aref)) < 1e-12
+    assert regions == {0, 1, 2, 3, 4, 5}                      # every class of Fig. 3.1(b)
+    print(f"\nc2 full size: {stats}, oracle pass {t_oracle:.1f} s on {oracle_mod.num_threads()} threads")
 
 
-def test_c3_full_size_sampled(B, oracle_mod):
-    """configs[3]: 1e8 queries over 100 member grids, one member id per query"""
+def test_c3_full_size_all_rows(B, oracle_mod):
+    """configs[3]: 1e8 queries over 100 member grids, one member id per query; every row"""
     spec = synth.grid_c1(nmem=100)
     n = N_FULL
     g = B.PdfGrid.from_spec(spec, workspace_for=n)
@@ -66,21 +99,58 @@ def test_c3_full_size_sampled(B, oracle_mod):
     mem = synth.members(spec, n, device="cuda")
     out = g.pdf_xfxq2(spec.pids, x, q, member=mem)
     assert g.pdf_error_count() == 0
-    idx = _sample(n, 6)
-    ref, S = og.xfxq2(spec.pids, x[idx].cpu().numpy(), q[idx].cpu().numpy(), member=mem[idx].cpu().numpy(), want_scale=True)
-    assert_values(out[idx].cpu().numpy(), ref, S, "c3 full size")
-    assert len(np.unique(mem[idx].cpu().numpy())) == 100
+    stats = dict(rows=0, rows_needing_floor=0, worst=0.0)
+    seen = set()
+    for a0, a1 in pieces(n):
+        xs, qs, ms = x[a0:a1].cpu().numpy(), q[a0:a1].cpu().numpy(), mem[a0:a1].cpu().numpy()
+        check_piece(out[a0:a1].cpu().numpy(), lambda: og.xfxq2(spec.pids, xs, qs, member=ms),
+                    lambda rows: og.xfxq2(spec.pids, xs[rows], qs[rows], member=ms[rows], want_scale=True)[1],
+                    f"c3 rows {a0}..{a1}", stats)
+        seen |= set(np.unique(ms).tolist())
+    assert len(seen) == 100
+    print(f"\nc3 full size: {stats}")
 
 
-def test_c4_full_size_sampled(B, oracle_mod):
-    """configs[4]: 1e8 events, x1, x2 log-uniform in [1e-6, 1], Q2 = x1 x2 s, weights, 11 x 11 coupling"""
+def test_c4_full_size_all_rows(B, oracle_mod):
+    """configs[4]: 1e8 events, x1, x2 log-uniform in [1e-6, 1], Q2 = x1 x2 s, weights, 11 x 11 coupling; every event"""
     spec = synth.grid_c1()
     n = N_FULL
     g = B.PdfGrid.from_spec(spec, workspace_for=n)
     og = make_oracle_grid(oracle_mod, spec)
     x1, x2, q2, w = synth.events_c4(n, device="cuda")
     out = g.pdf_lumi(x1, x2, q2, w)
-    idx = _sample(n, 7)
-    ref, S = og.lumi(*[t[idx].cpu().numpy() for t in (x1, x2, q2, w)], want_scale=True)
-    assert_values(out[idx].cpu().numpy(), ref, S, "c4 full size")
     assert g.pdf_error_count() == int(torch.isnan(out).sum())
+    stats = dict(rows=0, rows_needing_floor=0, worst=0.0)
+    for a0, a1 in pieces(n):
+        ev = [t[a0:a1].cpu().numpy() for t in (x1, x2, q2, w)]
+        check_piece(out[a0:a1].cpu().numpy(), lambda: og.lumi(*ev),
+                    lambda rows: og.lumi(*[t[rows] for t in ev], want_scale=True)[1], f"c4 events {a0}..{a1}", stats)
+    print(f"\nc4 full size: {stats}")
+
+
+def test_c1_at_its_stated_size(B, oracle_mod):
+    """configs[1]: 1e7 queries log-uniform over the closed range of the LHAPDF-shaped grid; every row, every index"""
+    spec = synth.grid_c1()
+    n = 10_000_000
+    g = B.PdfGrid.from_spec(spec, workspace_for=n)
+    og = make_oracle_grid(oracle_mod, spec)
+    x, q = synth.queries_inside(spec, n, synth.BASE_SEED + 11, device="cuda")
+    out = g.pdf_xfxq2(spec.pids, x, q).cpu().numpy()
+    xs, qs = x.cpu().numpy(), q.cpu().numpy()
+    stats = dict(rows=0, rows_needing_floor=0, worst=0.0)
+    check_piece(out, lambda: og.xfxq2(spec.pids, xs, qs),
+                lambda rows: og.xfxq2(spec.pids, xs[rows], qs[rows], want_scale=True)[1], "c1 1e7", stats)
+    ix, iq, isub, reg = og.locate(xs, qs)
+    gx, gq, gs, gr = [t.cpu().numpy() for t in g.pdf_locate(x, q)]
+    assert np.array_equal(reg, gr) and np.array_equal(isub, gs) and np.array_equal(ix, gx) and np.array_equal(iq, gq)
+    print(f"\nc1 1e7: {stats}")
+
+
+def test_binned_vs_direct_all_rows_fresh_process():
+    """all 1e8 rows of the binned kernel against the direct kernel, first calls of a fresh process (cold caches:
+    the waits of the persistent kernel's pipeline are really taken)"""
+    import subprocess
+    import sys
+    script = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cold_check.py")
+    r = subprocess.run([sys.executable, script, str(N_FULL)], capture_output=True, text=True, timeout=1200)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
