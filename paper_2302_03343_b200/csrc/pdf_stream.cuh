@@ -1,5 +1,5 @@
 // pdf_stream.cuh -- the binned, cell-coherent evaluation path (PDF_PATH_BINNED), version 3:
-// one persistent kernel of independent WARPS, bins per CELL, no CTA barrier on the path.
+// one persistent kernel of independent WARPS, one bin per CELL, no CTA barrier on the path.
 //
 // Why binning at all: a query needs a 4 x 4 stencil x 11 flavours = 1408 B of grid
 // data; gathered per lane that is >= 12 clk/query/SM of L1 / shared-memory bandwidth against a
@@ -9,93 +9,112 @@
 //
 // What changed against version 2 (one coarse bin per x cell, tile-local counting sorts in shared
 // memory in A, payload staging + counting sort by Q2 cell in B, 46 warp instructions per query, 16
-// warps/SM, profiles/r1i, r1j): the bin IS the cell.
+// warps/SM, profiles/r1i, r1j): the bin IS the cell, and every work item belongs to ONE warp.
 //   A tile (one warp, 256 queries): coalesced loads of x, Q2; validity / region class on the bit
 //     patterns; cell search from a table indexed by the exponent and top mantissa bits (integer
 //     compares on the raw knots: C-3 / C-4 bit-exact, FP64 pipe untouched); t_x, t_q (two logs);
 //     ONE global atomic per query reserves a slot in the cell's bin, the 32-byte payload
-//     {a, b, idx} is stored as one whole sector.  The tile's output rows are zero-filled with
+//     {a, b, idx, cell} is stored as one whole sector.  The tile's output rows are zero-filled with
 //     coalesced 32-byte stores first, so that the scattered 88-byte rows of B merge into valid
 //     L2-resident sectors (scattered partial-sector stores into untouched
 //     memory run at 0.9 TB/s).  No shared-memory sort, no barrier.
-//   B unit (one warp, 8 consecutive Q2 cells of one x cell): reads the 8 counts, then per cell the
-//     16 x 11 values as 8 fragment registers per lane (L1/L2), its payloads in batches of 32
-//     through a double-buffered cp.async stage, and runs DMMA m8n8k4 tiles of 8 queries x 8
-//     flavours; rows leave from the accumulator fragments.  No staging of grid columns, no
-//     counting sort, no batch descriptors.
-//   Extrapolation classes (a-5) are bins of their own ((x cell, low-Q), (x cell, high-Q), (low-x,
-//   Q2 cell), two corners) and run the same DMMA contraction with class-specific node sets and
-//   weights, followed by the per-flavour continuation formulas (C-7 ... C-9) on the fragments.
+//   B unit (one warp, 8 consecutive Q2 cells of one x cell): reads the 8 counts, then walks the
+//     cells' payload batches (<= 32 queries) through a double-buffered cp.async stage that also
+//     carries the cell's 16 node rows (the next batch and the next cell's values are in flight
+//     under the current batch's arithmetic), and runs DMMA m8n8k4 tiles of 8 queries x 8 flavours;
+//     rows leave from the accumulator fragments.  No counting sort, no batch descriptors.
+//   E unit (one warp): the extrapolation classes (a-5) are 5 % of configs[2] but cost ~40 x an
+//     interior query each (11 flavours x two logarithms and an exponential); as bins of the cell
+//     pipeline their units ran 250 us and stalled the ring (first build of this version, profile
+//     r2b).  They go to per-class lists of the chunk instead (one warp-aggregated atomic per warp
+//     and class), and E units claim batches of 32 entries from the lists dynamically: one query per
+//     lane, node rows gathered through L1 (8 rows per query; C-9's second anchor row, the values at
+//     1.01 Q2min, is tabulated once per grid), class-uniform branches.  Queries beyond a cell bin's
+//     capacity go to a sixth list that the same evaluator serves with the full 16-row stencil:
+//     correctness never depends on the distribution of the queries.
 // Work is handed out per warp by a global ticket counter in the order
-//      round r = [ A(r) tiles | B(r - kLag) units ],
-// B(c) waits until every A tile of chunk c has been released, A(c) until B(c - kRing) has drained
-// the ring slot; a ticket only ever waits on lower tickets and every CTA is resident, so the
-// scheme cannot deadlock.  Queries beyond a bin's capacity go to an overflow list evaluated by the
-// generic per-thread code: correctness never depends on the distribution of the queries.
+//      round r = [ A(r) tiles | E(r - kLag), B(r - kLag) units ],
+// B/E(c) wait until every A tile of chunk c has been released, A(c) until the units of chunk
+// c - kRing have drained the ring slot; a ticket only ever waits on lower tickets and every CTA is
+// resident, so the scheme cannot deadlock.
 #pragma once
+#include <climits>
 #include "pdf_common.cuh"
 #include "pdf_generic.cuh"
 
 namespace pdfg {
 
-#ifndef PDF_S3_THREADS
-#define PDF_S3_THREADS 256
+#ifndef PDF_S3_GRP
+#define PDF_S3_GRP 2
 #endif
-#ifndef PDF_S3_MINB
-#define PDF_S3_MINB 3
+#ifndef PDF_S3_EDIV
+#define PDF_S3_EDIV 1024                             // one E unit per this many queries of a chunk
 #endif
 #ifndef PDF_S3_LAG
-#define PDF_S3_LAG 1
+#define PDF_S3_LAG 2
 #endif
 #ifndef PDF_S3_RING
-#define PDF_S3_RING 3
+#define PDF_S3_RING 8
 #endif
-#ifndef PDF_S3_GRP
-#define PDF_S3_GRP 4
+#ifndef PDF_S3_MINB
+#define PDF_S3_MINB 2                                // 2 CTAs of 256 threads per SM: 128 registers, no spills (80 registers
+                                                     // and 3 CTAs spilled ~250 B per thread and ran 1.5x slower)
 #endif
-constexpr int kS3Threads = PDF_S3_THREADS;          // CTA size of the persistent kernel; every warp works alone
+constexpr int kS3Threads = 256;                      // CTA size of the persistent kernel; every warp works alone
 constexpr int kS3Warps = kS3Threads / 32;
-constexpr int kS3TileQ = 8;                          // queries per lane in an A tile
+#ifndef PDF_S3_TILEQ
+#define PDF_S3_TILEQ 8
+#endif
+constexpr int kS3TileQ = PDF_S3_TILEQ;               // queries per lane in an A tile
 constexpr int kS3TileA = 32 * kS3TileQ;              // 256 queries per A tile (one warp)
 constexpr int kS3Grp = PDF_S3_GRP;                   // queries of a lane that go through the A steps together
 static_assert(kS3TileQ % kS3Grp == 0, "kS3TileQ must be a multiple of kS3Grp");
 constexpr int kS3Batch = 32;                         // payloads per cp.async stage
-constexpr int kS3FkPerUnit = 8;                      // fine keys (Q2 cells) per B unit
-constexpr int kS3ClassParts = 2;                     // B units per x key that share its two extrapolation-class bins (low-Q, high-Q)
-constexpr int kS3Ovf = 8;                            // B units per chunk that drain the overflow list
+#ifndef PDF_S3_FKU
+#define PDF_S3_FKU 8
+#endif
+constexpr int kS3FkPerUnit = PDF_S3_FKU;             // Q2 cells per B unit
 constexpr int kS3Lag = PDF_S3_LAG;                   // B(c) tickets follow A(c) tickets by this many rounds
 constexpr int kS3Ring = PDF_S3_RING;                 // chunk slots in flight
 static_assert(kS3Ring >= kS3Lag + 2, "A(c) must find the slot of B(c - kRing) drained");
 constexpr int kS3LutMax = 2048;                      // search-table buckets per axis
 constexpr int kNF = 11, kNFP = 12;                   // the path is specialised for 11 flavours (rows padded to 12)
-constexpr int kS3MaxCells = 1024;                    // x cells / Q2 knots the path supports (u16 tables, 32-bit payload offsets)
+constexpr int kS3MaxCells = 1024;                    // x cells / Q2 knots the path supports (u16 tables)
+// lists of the E units: entries that are not evaluated from a cell bin (1..5 = the region codes)
+constexpr int kListOvf = 0, kListLowX = 1, kListLowQ = 2, kListHighQ = 3, kListLowXLowQ = 4, kListLowXHighQ = 5, kNumLists = 6;
+static_assert(kListLowX == kRegionLowX && kListLowQ == kRegionLowQ && kListHighQ == kRegionHighQ &&
+              kListLowXLowQ == kRegionLowXLowQ && kListLowXHighQ == kRegionLowXHighQ, "list numbers are the region codes");
+constexpr int kStageP = kS3Batch * 32;               // bytes of a payload stage (32 payloads)
+constexpr int kStageV = 16 * kNFP * 8;               // bytes of a value stage (a cell's 16 node rows)
+constexpr int kStageBytes = 2 * kStageP + 2 * kStageV; // per warp: two payload stages (by batch parity), two value stages (by cell parity)
 
 struct __align__(32) Payload {                       // one sector
     double a, b;                                     // class-dependent abscissae (t_x, t_q / theta / r)
-    unsigned idx, pad0;                              // query index inside its chunk
-    double pad1;
+    unsigned idx;                                    // query index inside its chunk
+    unsigned cell;                                   // lists: x cell (low-Q, high-Q), Q2 cell (low-x), i | jg << 16 (overflow)
+    double pad;
 };
 
 // geometry of the key space and the search tables; host copy in StreamPlan, passed by value
 struct StreamDev {
-    int ncx, nqt, nfk, nbins;                        // x cells, Q2 knots, fine keys per x key (nqt + 2), bins ((ncx + 1) * nfk)
+    int ncx, nqt, nbins;                             // x cells, Q2 knots, cell bins (ncx * nqt; a last knot of a sub-grid owns an unused bin)
     int jgplus;                                      // cell (global lower-knot index) of 1.01*Q2min
     double tqplus;                                   // and its t_q  (C-9)
-    int cap_int, cap_cls, cap_lx, cap_lxc;           // bin capacities: interior cell, (x cell, class), (low-x, Q2 cell), corner
-    int rowcap, lxbase, slab;                        // payloads per x key, offset of the low-x key, payloads per ring slot
-    int ng, tb;                                      // fine-key groups per x key, B units per chunk
+    int cap;                                         // payloads per cell bin
+    int ng, ne, tb;                                  // Q2-cell groups per x cell, E units per chunk, B + E units per chunk
     int xshift, xbase, nbx, qshift, qbase, nbq;      // bucket = (high word >> shift) - base
     const unsigned short *lutx, *lutq;               // [nbx], [nbq] cell at the lower edge of the bucket
-    const double2 *cxs, *cqs;                        // [ncx], [nqt] {ln lower knot, 1/dln} per cell
+    const double *rowplus;                           // [nmem][nx][12]: the grid's values at Q2 = 1.01 Q2min (C-9's second anchor), per x knot
 };
 
 struct StreamWorkspace {                             // carved out of the caller's workspace
     unsigned long long *ctrl;                        // [0] ticket; then per ring slot a_done, b_fin, b_done, each on a 128-byte line of its own
-    unsigned *counts;                                // [kS3Ring][nbins]
-    unsigned *ovf_count;                             // [kS3Ring]
-    Payload *bins;                                   // [kS3Ring][slab]
-    Payload *ovf;                                    // [kS3Ring][chunk]  (raw x, q2)
+    unsigned *counts;                                // [kS3Ring][nbins + 32]: cell bins, then list counts [kNumLists] and list cursors [kNumLists]
+    Payload *bins;                                   // [kS3Ring][nbins * cap]
+    Payload *lists;                                  // [kS3Ring][kNumLists][chunk]
 };
+constexpr int kCtrlWords = 1024;                     // 8 KB control block
+constexpr int kCtrlSlot0 = 32, kCtrlSlotStride = 48; // u64 words: 3 counters x 128 B per slot
 
 struct StreamArgs {
     GridDev G;
@@ -129,12 +148,12 @@ __device__ __forceinline__ double2 lds_v2f64(unsigned a)
 // loads of data written by other SMs during this launch (counters, payloads): through L2, never L1
 __device__ __forceinline__ unsigned ldcg_u32(const unsigned *p) { unsigned v; asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v; }
 // The counters of the pipeline are polled with RELAXED gpu-scope loads and bumped with RELEASE atomics: neither
-// invalidates L1 (an acquire load or __threadfence emits CCTL.IVALL, which with 24 independent warps per SM
-// signalling every few microseconds left no L1 at all for the grid values, and ~3000 warps spinning with
-// acquire loads on one line starved the ticket and release atomics behind them: profile r2b, 90 % of the
-// samples in the wait loops).  That is sound here because everything another SM wrote during this launch
-// (counters, payloads, overflow entries) is read through L2 (.cg / cp.async.cg), never through L1, and is
-// only read after the poll that observed the release has returned (the loop exit depends on its value).
+// invalidates L1 (an acquire load or __threadfence emits CCTL.IVALL; with independent warps signalling every few
+// microseconds that left no L1 for the grid values, and ~3000 warps spinning with acquire loads on one line
+// starved the ticket and release atomics behind them: profile r2b, 90 % of the samples in the wait loops).
+// That is sound here because everything another SM wrote during this launch (counters, payloads, list
+// entries) is read through L2 (.cg / cp.async.cg), never through L1, and is only read after the poll that
+// observed the release has returned (the loop exit depends on its value).
 __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p)
 {
     unsigned long long v;
@@ -144,14 +163,14 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
 // called by all 32 lanes of a converged warp: lane 0 polls (one request per iteration), the warp leaves together
 __device__ __forceinline__ void warp_wait(const unsigned long long *p, unsigned long long target)
 {
-    unsigned ns = 64;
+    unsigned ns = 256;
     for (;;) {
         unsigned long long v = 0;
         if ((threadIdx.x & 31) == 0) v = ld_relaxed_u64(p);
         v = __shfl_sync(0xffffffffu, v, 0);
         if (v >= target) break;
         __nanosleep(ns);
-        if (ns < 2048) ns <<= 1;
+        if (ns < 4096) ns <<= 1;
     }
 }
 // release by one warp: every lane's stores are ordered before lane 0's release by the warp barrier, and the
@@ -165,36 +184,26 @@ __device__ __forceinline__ unsigned long long warp_release_add(unsigned long lon
     return __shfl_sync(0xffffffffu, old, 0);
 }
 // one payload = one 32-byte sector, stored whole (STG.256): never a partial-sector write
-__device__ __forceinline__ void store_payload(Payload *dst, double a, double b, unsigned idx)
+__device__ __forceinline__ void store_payload(Payload *dst, double a, double b, unsigned idx, unsigned cell)
 {
-    const double w2 = __hiloint2double(0, (int)idx);
+    const double w2 = __hiloint2double((int)cell, (int)idx);       // low word idx, high word cell
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(dst), "d"(a), "d"(b), "d"(w2), "d"(0.0) : "memory");
 }
-__device__ __forceinline__ void cp_async16(unsigned saddr, const void *g)
+__device__ __forceinline__ void cp_async16_cg(unsigned saddr, const void *g)
 {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async16_ca(unsigned saddr, const void *g)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(g) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// ---- key space ---------------------------------------------------------------------------------
-// x key X in [0, ncx]: the x cell, or ncx for x < X_0.  Fine key fk: the Q2 cell (global lower-knot
-// index), nqt for Q2 < Q2min, nqt + 1 for Q2 > Q2max.  A (X, fk) pair is one cell or one
-// extrapolation class (a-5): every batch is class-uniform and every branch warp-uniform.
-__device__ __forceinline__ int bin_off(const StreamDev &B, int X, int fk)
-{
-    if (X < B.ncx) return X * B.rowcap + (fk < B.nqt ? fk * B.cap_int : B.nqt * B.cap_int + (fk - B.nqt) * B.cap_cls);
-    return B.lxbase + (fk < B.nqt ? fk * B.cap_lx : B.nqt * B.cap_lx + (fk - B.nqt) * B.cap_lxc);
-}
-__device__ __forceinline__ int bin_cap(const StreamDev &B, int X, int fk)
-{
-    if (X < B.ncx) return fk < B.nqt ? B.cap_int : B.cap_cls;
-    return fk < B.nqt ? B.cap_lx : B.cap_lxc;
-}
 
 // ---- a-2 on this path: region class and cell from the raw bit patterns ---------------------------
 struct StreamTab {        // shared-window addresses of the tables staged once per CTA
-    unsigned xk, qk, cxs, cqs, lutx, lutq;
+    unsigned xk, qk, cx, cq, lutx, lutq;       // knots, cell tables (CellTab, 48 B each), search tables
 };
 constexpr long long kInfBits = 0x7ff0000000000000LL;
 
@@ -237,10 +246,12 @@ __device__ __forceinline__ Located s3_locate(const GridDev &G, const StreamDev &
     return L;
 }
 
-// pdf_locate on this path: the search the evaluation kernel runs, exported (ix, iq local to the sub-grid)
-__global__ void __launch_bounds__(256)
-k_locate_stream(const __grid_constant__ GridDev G, const __grid_constant__ StreamDev B, long long n,
-                const double *__restrict__ x, const double *__restrict__ q2, int *ix, int *iq, int *isub, int *region);
+// Out-of-line copies of the transcendental pieces: inlined, the two logarithms of a query and the continuation
+// formulas made the kernel 22 700 instructions (364 KB) with a 25 KB A loop, and warps of three different work
+// kinds per SM evicted one another's code from the instruction caches (~20 clk per issued instruction).
+__device__ __noinline__ double s3_log(double v) { return log(v); }
+__device__ __noinline__ double s3_two(double f0, double f1, double theta) { return continue_two(f0, f1, theta); }
+__device__ __noinline__ double s3_lowq(double fmin, double fplus, double r, double lnr) { return lowq_continue_ln(fmin, fplus, r, lnr); }
 
 // ---- A tile: classify, locate, t_x / t_q, one slot per query in its cell's bin -----------------
 // zero-fill rows [r0, r1) of `out` (contiguous rows of ld doubles) with coalesced 32-byte stores of one warp
@@ -271,8 +282,10 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
     long long t1 = t0 + kS3TileA;
     if (t1 > chunk_end) t1 = chunk_end;
     if (t0 >= t1) return;
-    unsigned *counts = A.W.counts + (size_t)slot * B.nbins;
-    Payload *bins = A.W.bins + (size_t)slot * B.slab;
+    unsigned *counts = A.W.counts + (size_t)slot * (B.nbins + 32);
+    unsigned *lcount = counts + B.nbins;
+    Payload *bins = A.W.bins + (size_t)slot * B.nbins * B.cap;
+    Payload *lists = A.W.lists + (size_t)slot * kNumLists * A.chunk;
     if (A.zfill) zero_fill_warp(A.out, A.ld, t0, t1, lane);
     __syncwarp();                                      // the NaN rows below are written by other lanes than the zeros
     const int nx = G.nx, nqt = G.nqtot;
@@ -296,51 +309,70 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) L[q] = s3_locate(G, B, T, xv[q], qv[q], xminb, xmaxb, qminb, qmaxb);
         double pa[kS3Grp], pb[kS3Grp];
-        int bin[kS3Grp];
+        int key[kS3Grp];                               // >= 0: cell bin; -1 - k: list k; INT_MIN: invalid or no query
+        unsigned cell[kS3Grp];
+        bool any_list = false;
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
+            const long long e = t0 + (g0 + q) * 32 + lane;
             const int r = L[q].region;
             const bool lowx = r == kRegionLowX || r == kRegionLowXLowQ || r == kRegionLowXHighQ;
             const bool lowq = r == kRegionLowQ || r == kRegionLowXLowQ, highq = r == kRegionHighQ || r == kRegionLowXHighQ;
             const int i = L[q].i;
             const int jg = L[q].g < nqt - 1 ? L[q].g : nqt - 2;       // only Q2 == Q2max lands on the last knot: it belongs to the last cell
-            const double2 ci = lds_v2f64(T.cxs + 16u * i), cj = lds_v2f64(T.cqs + 16u * jg);
+            const double2 ci = lds_v2f64(T.cx + 48u * i), cj = lds_v2f64(T.cq + 48u * jg);   // {ln lower knot, 1/dln}
             double lx = 0.0, lq = 0.0;
-            if (r != kRegionInvalid) { lx = log(xv[q]); lq = log(qv[q]); }
+            if (r != kRegionInvalid) { lx = s3_log(xv[q]); lq = s3_log(qv[q]); }
             // t = 1 exactly on the last knot (the only knot that belongs to the cell on its left, C-4)
             pa[q] = lowx ? (lx - u0) * inv_du0                                    // theta_x (C-7)
                          : (__double_as_longlong(xv[q]) == xmaxb) ? 1.0 : (lx - ci.x) * ci.y;
             pb[q] = lowq ? qv[q] * inv_qmin                                       // r (C-9)
                   : highq ? (lq - sA) * inv_ds                                    // theta_q (C-8)
                           : (__double_as_longlong(qv[q]) == qmaxb) ? 1.0 : (lq - cj.x) * cj.y;
-            const int X = lowx ? B.ncx : i;
-            const int fk = lowq ? nqt : highq ? nqt + 1 : jg;
-            bin[q] = r == kRegionInvalid ? -1 : X * B.nfk + fk;
+            key[q] = r == kRegionInterior ? i * nqt + jg : -1 - r;               // region codes 1..5 are the list numbers
+            cell[q] = r == kRegionInterior ? ((unsigned)i | ((unsigned)jg << 16)) : lowx ? (unsigned)jg : (unsigned)i;
+            if (e >= t1 || r == kRegionInvalid) key[q] = INT_MIN;
+            any_list |= key[q] < 0 && key[q] != INT_MIN;
         }
         unsigned pos[kS3Grp];
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
-            const long long e = t0 + (g0 + q) * 32 + lane;
             pos[q] = 0u;
-            if (e < t1 && bin[q] >= 0) pos[q] = atomicAdd(counts + bin[q], 1u);
+            if (key[q] >= 0) pos[q] = atomicAdd(counts + key[q], 1u);
+        }
+#pragma unroll
+        for (int q = 0; q < kS3Grp; ++q)
+            if (key[q] >= 0 && pos[q] >= (unsigned)B.cap) { key[q] = -1 - kListOvf; any_list = true; }   // bin full: to the overflow list
+        // list entries (extrapolated queries, bin overflow; rare): one atomic per warp and list reserves the run of
+        // the list's lanes
+        if (__any_sync(0xffffffffu, any_list)) {
+#pragma unroll
+            for (int q = 0; q < kS3Grp; ++q) {
+                const bool mine = key[q] < 0 && key[q] != INT_MIN;
+                const unsigned act = __ballot_sync(0xffffffffu, mine);
+                if (act == 0u) continue;
+                if (mine) {
+                    const int k = -1 - key[q];
+                    const unsigned peers = __match_any_sync(act, k);
+                    const int leader = __ffs(peers) - 1;
+                    unsigned base = 0;
+                    if (lane == leader) base = atomicAdd(lcount + k, (unsigned)__popc(peers));
+                    base = __shfl_sync(peers, base, leader);
+                    pos[q] = base + (unsigned)__popc(peers & ((1u << lane) - 1u));
+                }
+            }
         }
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
             const long long e = t0 + (g0 + q) * 32 + lane;
             if (e >= t1) continue;
-            if (bin[q] < 0) {                                                     // C-10: NaN row, counted
+            const unsigned idx = (unsigned)(e - chunk_base);
+            if (key[q] == INT_MIN) {                                              // C-10: NaN row, counted
                 double *o = A.out + e * A.ld;
                 for (int p = 0; p < A.cm.n; ++p) o[p] = qnan();
                 if (A.count_err) ++err_local;
-                continue;
-            }
-            const int X = bin[q] / B.nfk, fk = bin[q] - X * B.nfk;
-            if (pos[q] < (unsigned)bin_cap(B, X, fk))
-                store_payload(bins + bin_off(B, X, fk) + pos[q], pa[q], pb[q], (unsigned)(e - chunk_base));
-            else {                                                                // bin full: raw query to the overflow list
-                const unsigned o = atomicAdd(A.W.ovf_count + slot, 1u);
-                store_payload(A.W.ovf + (size_t)slot * A.chunk + o, xv[q], qv[q], (unsigned)(e - chunk_base));
-            }
+            } else if (key[q] < 0) store_payload(lists + (size_t)(-1 - key[q]) * A.chunk + pos[q], pa[q], pb[q], idx, cell[q]);
+            else store_payload(bins + (size_t)key[q] * B.cap + pos[q], pa[q], pb[q], idx, cell[q]);
         }
     }
 }
@@ -359,23 +391,17 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
 }
 struct Acc { double d00, d01, d10, d11; };              // flavours 2t, 2t+1, 8+2t, 9+2t (the last two exist for t < 2, t == 0)
 __device__ __forceinline__ void kstep(Acc &d, double a, double2 f) { dmma884(d.d00, d.d01, a, f.x); dmma884(d.d10, d.d11, a, f.y); }
-// fragment of node (row, col): flavour g in .x, flavour 8 + g in .y (the 12th column of a row is a zero pad)
-__device__ __forceinline__ double2 fragld(const double *__restrict__ Vm, int nx, int row, int col, int g)
-{
-    const double *p = Vm + ((size_t)row * nx + col) * kNFP;
-    return make_double2(__ldg(p + g), g < 4 ? __ldg(p + 8 + g) : 0.0);
-}
 
 // node weight number t of the 1-D Hermite operator in the factored form
 //   w_t = (1-s)^2 (c0 + c1 s) + s^2 (c2 + c3 (1-s))        (same weights as hermite_weights)
 struct WCoef { double c0, c1, c2, c3; };
-__device__ __forceinline__ WCoef weight_coef(const CellTab &c, int t)
+__device__ __forceinline__ WCoef weight_coef(double aL, double bL, double aR, double bR, int t)
 {
     WCoef w;
     w.c0 = t == 1 ? 1.0 : 0.0;
-    w.c1 = t == 0 ? -c.bL : t == 1 ? 2.0 + c.bL - c.aL : t == 2 ? c.aL : 0.0;
+    w.c1 = t == 0 ? -bL : t == 1 ? 2.0 + bL - aL : t == 2 ? aL : 0.0;
     w.c2 = t == 2 ? 1.0 : 0.0;
-    w.c3 = t == 1 ? c.aR : t == 2 ? 2.0 - c.aR + c.bR : t == 3 ? -c.bR : 0.0;
+    w.c3 = t == 1 ? aR : t == 2 ? 2.0 - aR + bR : t == 3 ? -bR : 0.0;
     return w;
 }
 __device__ __forceinline__ double weight_eval(const WCoef &w, double s)
@@ -383,34 +409,11 @@ __device__ __forceinline__ double weight_eval(const WCoef &w, double s)
     double om = 1.0 - s, om2 = om * om, s2 = s * s;
     return fma(om2, fma(w.c1, s, w.c0), s2 * fma(w.c3, om, w.c2));
 }
-// Q2 row number tr (0..3) of cell jg: jg-1 .. jg+2, clamped at the ends of the sub-grid (q_point_cell)
-__device__ __forceinline__ int qrow(const CellTab &cq, int jg, int tr)
-{
-    return jg - 1 + tr + ((tr == 0 && cq.aL == 1.0) ? 1 : 0) - ((tr == 3 && cq.aR == 1.0) ? 1 : 0);
-}
 // x node number t (0..3) of cell i: i-1 .. i+2, clamped at the ends of the knot line (x_point_cell)
 __device__ __forceinline__ int xnode(int i, int t, int nx)
 {
     const int c = i - 1 + t;
     return c < 0 ? 0 : (c >= nx ? nx - 1 : c);
-}
-
-// the per-flavour continuation formulas on accumulator fragments (kept out of line: ~12 inlined
-// transcendental calls each)
-__device__ __noinline__ void acc_two(Acc &o, const Acc &a, const Acc &b, double theta, int t)
-{
-    o.d00 = continue_two(a.d00, b.d00, theta);
-    o.d01 = continue_two(a.d01, b.d01, theta);
-    o.d10 = t < 2 ? continue_two(a.d10, b.d10, theta) : 0.0;
-    o.d11 = t == 0 ? continue_two(a.d11, b.d11, theta) : 0.0;
-}
-__device__ __noinline__ void acc_lowq(Acc &o, const Acc &fmin, const Acc &fplus, double r, int t)
-{
-    const double lnr = log(r);
-    o.d00 = lowq_continue_ln(fmin.d00, fplus.d00, r, lnr);
-    o.d01 = lowq_continue_ln(fmin.d01, fplus.d01, r, lnr);
-    o.d10 = t < 2 ? lowq_continue_ln(fmin.d10, fplus.d10, r, lnr) : 0.0;
-    o.d11 = t == 0 ? lowq_continue_ln(fmin.d11, fplus.d11, r, lnr) : 0.0;
 }
 
 // one row from the accumulator fragments: 4 lanes write one row
@@ -429,56 +432,75 @@ __device__ __forceinline__ void store_row(const StreamArgs &A, double *rp, int t
     }
 }
 
-// payload batches of one bin through a double-buffered cp.async stage (one warp): the caller's
-// body(n, sbuf) sees n <= 32 payloads at shared-window address sbuf
-template <typename Body>
-__device__ __forceinline__ void for_batches(const Payload *bin, int first, int count, unsigned sbuf, int lane, Body body)
-{
-    if (count <= 0) return;
-    auto issue = [&](int o, unsigned dst) {
-        const int n = min(kS3Batch, count - o);
-        if (lane < n) {
-            const char *src = reinterpret_cast<const char *>(bin + first + o + lane);
-            cp_async16(dst + 32u * lane, src);
-            cp_async16(dst + 32u * lane + 16u, src + 16);
-        }
-        cp_async_commit();
-    };
-    issue(0, sbuf);
-    int p = 0;
-    for (int o = 0; o < count; o += kS3Batch) {
-        if (o + kS3Batch < count) { issue(o + kS3Batch, sbuf + (unsigned)((p ^ 1) * kS3Batch * 32)); cp_async_wait<1>(); }
-        else cp_async_wait<0>();
-        __syncwarp();
-        body(min(kS3Batch, count - o), sbuf + (unsigned)(p * kS3Batch * 32));
-        __syncwarp();
-        p ^= 1;
-    }
-}
-
-// interior cells (X = i < ncx, fine keys [fk0, fk1) are Q2 cells)
-__device__ __forceinline__ void b_unit_interior(const StreamArgs &A, const double *__restrict__ Vm, int slot, long long chunk_base,
-                                                int i, int fk0, int fk1, unsigned sbuf)
+// interior cells of x cell i, Q2 cells [fk0, fk1): the (cell, batch of <= 32 payloads) sequence of the unit runs
+// through the warp's stages: two payload stages (batch parity) and two value stages (cell parity; a cell's 16 node
+// rows, node n = 4 * (Q2 row) + (x node)).  The fragments are re-read from the value stage per 8-query tile (8
+// LDS.64): held in registers across the loop they spilled to local memory at 80 registers (profile r2f).
+__device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, const double *__restrict__ Vm, int slot,
+                                       long long chunk_base, int i, int fk0, int fk1, unsigned sbuf)
 {
     const GridDev &G = A.G;
     const StreamDev &B = A.B;
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-    const unsigned *counts = A.W.counts + (size_t)slot * B.nbins + (size_t)i * B.nfk;
-    const Payload *bins = A.W.bins + (size_t)slot * B.slab;
+    const unsigned *counts = A.W.counts + (size_t)slot * (B.nbins + 32) + (size_t)i * B.nqt;
+    const Payload *bins = A.W.bins + ((size_t)slot * B.nbins + (size_t)i * B.nqt) * B.cap;
     int mycnt = 0;
-    if (fk0 + lane < fk1) mycnt = min((int)ldcg_u32(counts + fk0 + lane), B.cap_int);
-    if (__ballot_sync(0xffffffffu, mycnt > 0) == 0u) return;
-    const WCoef kx = weight_coef(G.cx[i], t);          // x-axis weight of this lane's node, fixed for the unit
-    const int xc = xnode(i, t, G.nx);
-    for (int fk = fk0; fk < fk1; ++fk) {
-        const int cnt = __shfl_sync(0xffffffffu, mycnt, fk - fk0);
-        if (cnt == 0) continue;
-        const CellTab cq = G.cq[fk];
-        const WCoef kq = weight_coef(cq, t);
-        double2 f[4];
+    if (fk0 + lane < fk1) mycnt = min((int)ldcg_u32(counts + fk0 + lane), B.cap);
+    unsigned live = __ballot_sync(0xffffffffu, mycnt > 0);      // cells of the unit that hold queries
+    if (live == 0u) return;
+    const int nx = G.nx;
+    WCoef kx;
+    {
+        const double2 ab = lds_v2f64(T.cx + 48u * i + 16u), cd = lds_v2f64(T.cx + 48u * i + 32u);
+        kx = weight_coef(ab.x, ab.y, cd.x, cd.y, t);            // x-axis weight of this lane's node, fixed for the unit
+    }
+    // the 96 16-byte pieces of a cell's 16 node rows are copied by 32 lanes x 3: piece e = lane + 32 k,
+    // node = e / 6 = 4 b + a; x-node columns are fixed for the unit, Q2 rows follow the cell
+    const unsigned sP = sbuf, sV = sbuf + 2u * kStageP;
+    auto issue = [&](int j, int o, int pp, int vp, bool with_values) {
+        const int fk = fk0 + j;
+        const int n = min(kS3Batch, __shfl_sync(0xffffffffu, mycnt, j) - o);
+        if (lane < n) {
+            const char *src = reinterpret_cast<const char *>(bins + (size_t)fk * B.cap + o + lane);
+            const unsigned dst = sP + (unsigned)(pp * kStageP) + 32u * lane;
+            cp_async16_cg(dst, src);
+            cp_async16_cg(dst + 16u, src + 16);
+        }
+        if (with_values) {
+            const double aL = lds_f64(T.cq + 48u * fk + 16u), aR = lds_f64(T.cq + 48u * fk + 32u);
+            const int elo = aL == 1.0 ? 1 : 0, ehi = aR == 1.0 ? 1 : 0;       // one-sided ends of a sub-grid (q_point_cell)
 #pragma unroll
-        for (int r = 0; r < 4; ++r) f[r] = fragld(Vm, G.nx, qrow(cq, fk, t ^ r), xc, g);
-        for_batches(bins + bin_off(B, i, fk), 0, cnt, sbuf, lane, [&](int nact, unsigned sb) {
+            for (int k = 0; k < 3; ++k) {
+                const int e = lane + 32 * k, node = e / 6, piece = e - node * 6, b = node >> 2;
+                const int row = fk - 1 + b + (b == 0 ? elo : 0) - (b == 3 ? ehi : 0);
+                cp_async16_ca(sV + (unsigned)(vp * kStageV) + 16u * e,
+                              Vm + ((size_t)row * nx + xnode(i, node & 3, nx)) * kNFP + 2 * piece);
+            }
+        }
+        cp_async_commit();
+    };
+    int j = __ffs(live) - 1, o = 0, pp = 0, vp = 0;
+    issue(j, 0, 0, 0, true);
+    bool fresh = true;                                          // the current batch opens a cell
+    WCoef kq;
+    // this lane's fragment offsets inside a value stage: step r pairs Q2 row (t ^ r) with x node t
+    const unsigned fo = (unsigned)(t * kNFP * 8 + 8 * g);
+    for (;;) {
+        // successor of (j, o)
+        int jn = j, on = o + kS3Batch;
+        const int cntj = __shfl_sync(0xffffffffu, mycnt, j);
+        if (on >= cntj) { live &= live - 1; jn = live ? __ffs(live) - 1 : -1; on = 0; }
+        if (jn >= 0) { issue(jn, on, pp ^ 1, jn != j ? vp ^ 1 : vp, jn != j); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncwarp();
+        if (fresh) {
+            const int fk = fk0 + j;
+            const double2 ab = lds_v2f64(T.cq + 48u * fk + 16u), cd = lds_v2f64(T.cq + 48u * fk + 32u);
+            kq = weight_coef(ab.x, ab.y, cd.x, cd.y, t);
+        }
+        const unsigned sb = sP + (unsigned)(pp * kStageP), sv = sV + (unsigned)(vp * kStageV) + fo;
+        const int nact = min(kS3Batch, cntj - o);
+        {
             // the next tile's abscissae are fetched under this tile's arithmetic
             bool vn = g < nact;
             double2 abn = make_double2(0.0, 0.0);
@@ -497,167 +519,206 @@ __device__ __forceinline__ void b_unit_interior(const StreamArgs &A, const doubl
                 const double wq2 = __shfl_xor_sync(0xffffffffu, wq0, 2);
                 const double wq3 = __shfl_xor_sync(0xffffffffu, wq0, 3);
                 Acc d = {0.0, 0.0, 0.0, 0.0};
-                kstep(d, wq0 * wx, f[0]);
-                kstep(d, wq1 * wx, f[1]);
-                kstep(d, wq2 * wx, f[2]);
-                kstep(d, wq3 * wx, f[3]);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const unsigned pn = sv + (unsigned)(4 * (t ^ r) * kNFP * 8);
+                    double2 f;
+                    f.x = lds_f64(pn);
+                    f.y = g < 4 ? lds_f64(pn + 64u) : 0.0;
+                    kstep(d, (r == 0 ? wq0 : r == 1 ? wq1 : r == 2 ? wq2 : wq3) * wx, f);
+                }
                 if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, d);
             }
-        });
+        }
+        __syncwarp();                                           // the stages are free for the copies after next
+        if (jn < 0) break;
+        fresh = jn != j;
+        if (fresh) vp ^= 1;
+        j = jn; o = on; pp ^= 1;
     }
 }
 
-// extrapolation classes (a-5): bin (X, fk) with X == ncx (x < X_0) or fk >= nqt (Q2 outside); slots
-// [first, first + count) of the bin.  Same 4-lanes-per-query layout: the linear parts are k-steps on node
-// sets fixed by the class, the continuation formulas run on the fragments.
-//   X < ncx, fk == nqt   (low-Q, C-9):   a = t_x, b = r        e0 = row Q2min,       e1 = cell of 1.01 Q2min at tqplus
-//   X < ncx, fk == nqt+1 (high-Q, C-8):  a = t_x, b = theta_q  e0 = row last-1,      e1 = row last
-//   X == ncx, fk < nqt   (low-x, C-7):   a = theta_x, b = t_q  e0 = column X_0,      e1 = column X_1 (4 rows of cell fk)
-//   X == ncx, fk == nqt  (corner):       a = theta_x, b = r    x rule on (Q2min) and on (1.01 Q2min), then C-9  (L1744)
-//   X == ncx, fk == nqt+1 (corner):      a = theta_x, b = theta_q   x rule on rows last-1 and last, then C-8
-__device__ __noinline__ void b_unit_class(const StreamArgs &A, const double *__restrict__ Vm, long long chunk_base,
-                                          const Payload *bin, int first, int count, int X, int fk, unsigned sbuf)
+// ---- E units: the lists (extrapolation classes, bin overflow), one query per lane -----------------
+// flavour pair p (columns 2p, 2p+1) of a node row; rows are 96 B = 6 pairs, the 12th column is a zero pad
+__device__ __forceinline__ double2 ldpair(const double *__restrict__ row, int p) { return __ldg(reinterpret_cast<const double2 *>(row) + p); }
+
+// the row of one list entry into `v[12]`.  Warp-uniform `list`; lanes differ in their cells.
+//   kListLowQ  (C-9):  a = t_x, b = r;  anchors: row Q2min and the tabulated row at 1.01 Q2min, x cell `cell`
+//   kListHighQ (C-8):  a = t_x, b = theta_q;  anchors: rows last-1 and last, x cell `cell`
+//   kListLowX  (C-7):  a = theta_x, b = t_q;  anchors: columns X_0 and X_1 on the 4 rows of Q2 cell `cell`
+//   corners (L1744): the x rule on both Q2 anchors, then the Q2 rule
+//   kListOvf: a = t_x, b = t_q, cell = i | jg << 16: the full 16-node sum
+__device__ __noinline__ void list_row(const StreamArgs &A, const double *__restrict__ Vm, const double *__restrict__ RPm, int list,
+                                      double a, double b, unsigned cell, double v[kNFP])
 {
     const GridDev &G = A.G;
-    const StreamDev &B = A.B;
-    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int nx = G.nx, last = G.nqtot - 1;
-    const bool lowx = X == B.ncx;
-    const int i = lowx ? 0 : X;
-    const WCoef kx = weight_coef(G.cx[i], t);
-    const int xc = xnode(i, t, nx);
-    const CellTab cqp = G.cq[B.jgplus];
-    const double unit0 = t == 0 ? 1.0 : 0.0;           // k-step weight that picks node slot 0 alone
-    // weights of the cell of 1.01*Q2min at tqplus (C-9), by row
-    double wqp[4];
+    const size_t rs = (size_t)nx * kNFP;                       // doubles per Q2 row
+    if (list == kListLowQ || list == kListHighQ) {
+        const int i = (int)cell;
+        double wx[4];
+        hermite_weights(a, G.cx[i], wx);
+        const double *r0 = list == kListLowQ ? Vm : Vm + (size_t)(last - 1) * rs;
+        const double *r1 = list == kListLowQ ? RPm : Vm + (size_t)last * rs;
+        const double lnr = list == kListLowQ ? s3_log(b) : 0.0;
+        int xn[4];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) wqp[r] = weight_eval(weight_coef(cqp, r), B.tqplus);
-    const CellTab cqf = G.cq[fk < B.nqt ? fk : 0];
-    const WCoef kq = weight_coef(cqf, t);
-    for_batches(bin, first, count, sbuf, lane, [&](int nact, unsigned sb) {
-        for (int m0 = 0; m0 < nact; m0 += 8) {
-            const int q = m0 + g;
-            const bool valid = q < nact;
-            double pa = 0.0, pb = 1.0;
-            unsigned idx = 0;
-            if (valid) { const double2 ab = lds_v2f64(sb + 32u * q); pa = ab.x; pb = ab.y; idx = lds_u32(sb + 32u * q + 16u); }
-            Acc o;
-            if (!lowx) {
-                const double wx = weight_eval(kx, pa);
-                Acc e0 = {0.0, 0.0, 0.0, 0.0}, e1 = {0.0, 0.0, 0.0, 0.0};
-                if (fk == B.nqt) {
-                    kstep(e0, wx, fragld(Vm, nx, 0, xc, g));
+        for (int k = 0; k < 4; ++k) xn[k] = xnode(i, k, nx) * kNFP;
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        // step r pairs row (t ^ r) with x-node t: the row weight is a select among the 4 constants
-                        const int tr = t ^ r;
-                        const double w = tr == 0 ? wqp[0] : tr == 1 ? wqp[1] : tr == 2 ? wqp[2] : wqp[3];
-                        kstep(e1, w * wx, fragld(Vm, nx, qrow(cqp, B.jgplus, tr), xc, g));
-                    }
-                    acc_lowq(o, e0, e1, pb, t);
-                } else {
-                    kstep(e0, wx, fragld(Vm, nx, last - 1, xc, g));
-                    kstep(e1, wx, fragld(Vm, nx, last, xc, g));
-                    acc_two(o, e0, e1, pb, t);
-                }
-            } else if (fk < B.nqt) {
-                const double wq = weight_eval(kq, pb);
-                const int row = qrow(cqf, fk, t);
-                Acc e0 = {0.0, 0.0, 0.0, 0.0}, e1 = {0.0, 0.0, 0.0, 0.0};
-                kstep(e0, wq, fragld(Vm, nx, row, 0, g));
-                kstep(e1, wq, fragld(Vm, nx, row, 1, g));
-                acc_two(o, e0, e1, pa, t);
-            } else {
-                Acc e0 = {0.0, 0.0, 0.0, 0.0}, e1 = {0.0, 0.0, 0.0, 0.0}, e2 = {0.0, 0.0, 0.0, 0.0}, e3 = {0.0, 0.0, 0.0, 0.0};
-                if (fk == B.nqt) {
-                    const double w = t == 0 ? wqp[0] : t == 1 ? wqp[1] : t == 2 ? wqp[2] : wqp[3];
-                    const int row = qrow(cqp, B.jgplus, t);
-                    kstep(e0, unit0, fragld(Vm, nx, 0, 0, g));
-                    kstep(e1, unit0, fragld(Vm, nx, 0, 1, g));
-                    kstep(e2, w, fragld(Vm, nx, row, 0, g));
-                    kstep(e3, w, fragld(Vm, nx, row, 1, g));
-                } else {
-                    kstep(e0, unit0, fragld(Vm, nx, last - 1, 0, g));
-                    kstep(e1, unit0, fragld(Vm, nx, last - 1, 1, g));
-                    kstep(e2, unit0, fragld(Vm, nx, last, 0, g));
-                    kstep(e3, unit0, fragld(Vm, nx, last, 1, g));
-                }
-                Acc lo, hi;
-                acc_two(lo, e0, e1, pa, t);
-                acc_two(hi, e2, e3, pa, t);
-                if (fk == B.nqt) acc_lowq(o, lo, hi, pb, t); else acc_two(o, lo, hi, pb, t);
+        for (int p = 0; p < 6; ++p) {
+            double2 e0 = make_double2(0.0, 0.0), e1 = e0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double2 u0 = ldpair(r0 + xn[k], p), u1 = ldpair(r1 + xn[k], p);
+                e0.x = fma(wx[k], u0.x, e0.x); e0.y = fma(wx[k], u0.y, e0.y);
+                e1.x = fma(wx[k], u1.x, e1.x); e1.y = fma(wx[k], u1.y, e1.y);
             }
-            if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, o);
+            if (list == kListLowQ) { v[2 * p] = s3_lowq(e0.x, e1.x, b, lnr); v[2 * p + 1] = p < 5 ? s3_lowq(e0.y, e1.y, b, lnr) : 0.0; }
+            else { v[2 * p] = s3_two(e0.x, e1.x, b); v[2 * p + 1] = p < 5 ? s3_two(e0.y, e1.y, b) : 0.0; }
         }
-    });
+    } else if (list == kListLowX) {
+        const int jg = (int)cell;
+        const CellTab cq = G.cq[jg];
+        double wq[4];
+        hermite_weights(b, cq, wq);
+        size_t qn[4];
+        qn[0] = (size_t)((cq.aL == 1.0) ? jg : jg - 1) * rs; qn[1] = (size_t)jg * rs; qn[2] = (size_t)(jg + 1) * rs;
+        qn[3] = (size_t)((cq.aR == 1.0) ? jg + 1 : jg + 2) * rs;
+#pragma unroll
+        for (int p = 0; p < 6; ++p) {
+            double2 e0 = make_double2(0.0, 0.0), e1 = e0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double2 u0 = ldpair(Vm + qn[k], p), u1 = ldpair(Vm + qn[k] + kNFP, p);
+                e0.x = fma(wq[k], u0.x, e0.x); e0.y = fma(wq[k], u0.y, e0.y);
+                e1.x = fma(wq[k], u1.x, e1.x); e1.y = fma(wq[k], u1.y, e1.y);
+            }
+            v[2 * p] = s3_two(e0.x, e1.x, a); v[2 * p + 1] = p < 5 ? s3_two(e0.y, e1.y, a) : 0.0;
+        }
+    } else if (list == kListLowXLowQ || list == kListLowXHighQ) {
+        const bool lq = list == kListLowXLowQ;
+        const double *r0 = lq ? Vm : Vm + (size_t)(last - 1) * rs;
+        const double *r1 = lq ? RPm : Vm + (size_t)last * rs;
+        const double lnr = lq ? s3_log(b) : 0.0;
+#pragma unroll
+        for (int p = 0; p < 6; ++p) {
+            const double2 u00 = ldpair(r0, p), u01 = ldpair(r0 + kNFP, p), u10 = ldpair(r1, p), u11 = ldpair(r1 + kNFP, p);
+            const double lox = s3_two(u00.x, u01.x, a), hix = s3_two(u10.x, u11.x, a);
+            v[2 * p] = lq ? s3_lowq(lox, hix, b, lnr) : s3_two(lox, hix, b);
+            if (p < 5) {
+                const double loy = s3_two(u00.y, u01.y, a), hiy = s3_two(u10.y, u11.y, a);
+                v[2 * p + 1] = lq ? s3_lowq(loy, hiy, b, lnr) : s3_two(loy, hiy, b);
+            } else v[2 * p + 1] = 0.0;
+        }
+    } else {
+        const int i = (int)(cell & 0xffffu), jg = (int)(cell >> 16);
+        const CellTab cq = G.cq[jg];
+        double wx[4], wq[4];
+        hermite_weights(a, G.cx[i], wx);
+        hermite_weights(b, cq, wq);
+        size_t qn[4];
+        qn[0] = (size_t)((cq.aL == 1.0) ? jg : jg - 1) * rs; qn[1] = (size_t)jg * rs; qn[2] = (size_t)(jg + 1) * rs;
+        qn[3] = (size_t)((cq.aR == 1.0) ? jg + 1 : jg + 2) * rs;
+        int xn[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) xn[k] = xnode(i, k, nx) * kNFP;
+#pragma unroll
+        for (int p = 0; p < 6; ++p) {
+            double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int bq = 0; bq < 4; ++bq) {
+                double2 rb = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double2 u = ldpair(Vm + qn[bq] + xn[k], p);
+                    rb.x = fma(wx[k], u.x, rb.x); rb.y = fma(wx[k], u.y, rb.y);
+                }
+                acc.x = fma(wq[bq], rb.x, acc.x); acc.y = fma(wq[bq], rb.y, acc.y);
+            }
+            v[2 * p] = acc.x; v[2 * p + 1] = acc.y;
+        }
+    }
 }
 
-// low-x key, fine keys [fk0, fk1) are Q2 cells: one class bin per cell
-__device__ __forceinline__ void b_unit_lowx(const StreamArgs &A, const double *__restrict__ Vm, int slot, long long chunk_base,
-                                            int fk0, int fk1, unsigned sbuf)
+// claims batches of 32 entries from the chunk's lists until they are drained
+__device__ __forceinline__ void e_unit(const StreamArgs &A, const double *__restrict__ Vm, const double *__restrict__ RPm, int slot,
+                                       long long chunk_base)
 {
     const StreamDev &B = A.B;
     const int lane = threadIdx.x & 31;
-    const unsigned *counts = A.W.counts + (size_t)slot * B.nbins + (size_t)B.ncx * B.nfk;
-    const Payload *bins = A.W.bins + (size_t)slot * B.slab;
-    int mycnt = 0;
-    if (fk0 + lane < fk1) mycnt = min((int)ldcg_u32(counts + fk0 + lane), B.cap_lx);
-    for (int fk = fk0; fk < fk1; ++fk) {
-        const int cnt = __shfl_sync(0xffffffffu, mycnt, fk - fk0);
-        if (cnt) b_unit_class(A, Vm, chunk_base, bins + bin_off(B, B.ncx, fk), 0, cnt, B.ncx, fk, sbuf);
+    unsigned *lcount = A.W.counts + (size_t)slot * (B.nbins + 32) + B.nbins, *lcursor = lcount + kNumLists;
+    const Payload *lists = A.W.lists + (size_t)slot * kNumLists * A.chunk;
+    // lanes 0..5 hold the lists' lengths and claim for their list
+    unsigned len = 0, claim = 0;
+    if (lane < kNumLists) {
+        len = ldcg_u32(lcount + lane);
+        if (lane == kListOvf && len > (unsigned)A.chunk) len = (unsigned)A.chunk;
+        claim = len ? atomicAdd(lcursor + lane, (unsigned)kS3Batch) : 0u;
     }
-}
-
-// overflow list: raw queries evaluated by the generic per-thread code (rare)
-__device__ __noinline__ void ovf_unit(const StreamArgs &A, const double *V, int slot, long long chunk_base, int part)
-{
-    const unsigned cnt = ldcg_u32(A.W.ovf_count + slot);
-    const Payload *ovf = A.W.ovf + (size_t)slot * A.chunk;
-    for (unsigned e = part * 32 + (threadIdx.x & 31); e < cnt; e += kS3Ovf * 32) {
-        const double2 ab = __ldcg(reinterpret_cast<const double2 *>(ovf + e));
-        const unsigned idx = __ldcg(reinterpret_cast<const unsigned *>(ovf + e) + 4);
-        QueryPlan P;
-        make_plan(A.G, ab.x, ab.y, P);
-        double *o = A.out + (chunk_base + idx) * A.ld;
-        for (int p = 0; p < A.cm.n; ++p) {
-            const int c = A.cm.col[p];
-            o[p] = c < 0 ? 0.0 : plan_value(A.G, V, P, c);
+    for (;;) {
+        const unsigned open = __ballot_sync(0xffffffffu, lane < kNumLists && claim < len);
+        if (open == 0u) break;
+        const int list = __ffs(open) - 1;
+        const unsigned first = __shfl_sync(0xffffffffu, claim, list), n = __shfl_sync(0xffffffffu, len, list);
+        if (lane == list) claim = atomicAdd(lcursor + lane, (unsigned)kS3Batch);      // the next claim travels under this batch
+        const bool active = first + lane < n;
+        double a = 0.5, b = 0.5;
+        unsigned idx = 0, cell = 0;
+        if (active) {
+            const Payload *e = lists + (size_t)list * A.chunk + first + lane;
+            const double2 ab = __ldcg(reinterpret_cast<const double2 *>(e));
+            const uint2 ic = __ldcg(reinterpret_cast<const uint2 *>(e) + 2);
+            a = ab.x; b = ab.y; idx = ic.x; cell = ic.y;
+        }
+        double v[kNFP];
+        list_row(A, Vm, RPm, list, a, b, cell, v);
+        if (active) {
+            double *o = A.out + (chunk_base + idx) * A.ld;
+            if (A.identity) {
+#pragma unroll
+                for (int f = 0; f < kNF; ++f) o[f] = v[f];
+            } else {
+                for (int p = 0; p < A.cm.n; ++p) {
+                    const int c = A.cm.col[p];
+                    double w = 0.0;
+#pragma unroll
+                    for (int f = 0; f < kNF; ++f) w = c == f ? v[f] : w;
+                    o[p] = w;
+                }
+            }
         }
     }
 }
 
 // ---- the persistent kernel -----------------------------------------------------------------------
-// dynamic shared memory: [x knots | Q2 knots | x cell {ln lo, 1/d} | Q2 cell {ln lo, 1/d} | lutx | lutq | per-warp payload stage]
+// dynamic shared memory: [x knots | Q2 knots | x cell tables | Q2 cell tables | lutx | lutq | per-warp stages]
 __host__ __device__ inline size_t s3_table_bytes(int nx, int nqt, int nbx, int nbq)
 {
-    size_t b = sizeof(double) * (size_t)(nx + nqt) + 16u * (size_t)(nx + nqt) + 2u * (size_t)(nbx + nbq);
-    return (b + 31) / 32 * 32;
+    size_t b = sizeof(double) * (size_t)(nx + nqt) + sizeof(CellTab) * (size_t)(nx + nqt) + 2u * (size_t)(nbx + nbq);
+    return (b + 31) / 32 * 32 + 64;                      // + alignment slack of the 16-byte aligned cell tables
 }
 __device__ __forceinline__ StreamTab s3_stage_tables(const GridDev &G, const StreamDev &B, unsigned char *smem, int nthreads)
 {
     double *s_xk = reinterpret_cast<double *>(smem);
     double *s_qk = s_xk + G.nx;
-    double2 *s_cx = reinterpret_cast<double2 *>(s_qk + G.nqtot + ((G.nx + G.nqtot) & 1));
-    double2 *s_cq = s_cx + G.nx;
-    unsigned short *s_lx = reinterpret_cast<unsigned short *>(s_cq + G.nqtot);
+    double *s_cx = s_qk + G.nqtot + ((G.nx + G.nqtot) & 1);      // 16-byte aligned
+    double *s_cq = s_cx + 6 * G.nx;
+    unsigned short *s_lx = reinterpret_cast<unsigned short *>(s_cq + 6 * G.nqtot);
     unsigned short *s_lq = s_lx + B.nbx;
     for (int k = threadIdx.x; k < G.nx; k += nthreads) s_xk[k] = G.xk[k];
     for (int k = threadIdx.x; k < G.nqtot; k += nthreads) s_qk[k] = G.qk[k];
-    for (int k = threadIdx.x; k < B.ncx; k += nthreads) s_cx[k] = B.cxs[k];
-    for (int k = threadIdx.x; k < G.nqtot; k += nthreads) s_cq[k] = B.cqs[k];
+    for (int k = threadIdx.x; k < 6 * B.ncx; k += nthreads) s_cx[k] = reinterpret_cast<const double *>(G.cx)[k];
+    for (int k = threadIdx.x; k < 6 * G.nqtot; k += nthreads) s_cq[k] = reinterpret_cast<const double *>(G.cq)[k];
     for (int k = threadIdx.x; k < B.nbx; k += nthreads) s_lx[k] = B.lutx[k];
     for (int k = threadIdx.x; k < B.nbq; k += nthreads) s_lq[k] = B.lutq[k];
     StreamTab T;
     T.xk = (unsigned)__cvta_generic_to_shared(s_xk); T.qk = (unsigned)__cvta_generic_to_shared(s_qk);
-    T.cxs = (unsigned)__cvta_generic_to_shared(s_cx); T.cqs = (unsigned)__cvta_generic_to_shared(s_cq);
+    T.cx = (unsigned)__cvta_generic_to_shared(s_cx); T.cq = (unsigned)__cvta_generic_to_shared(s_cq);
     T.lutx = (unsigned)__cvta_generic_to_shared(s_lx); T.lutq = (unsigned)__cvta_generic_to_shared(s_lq);
     return T;
 }
-__host__ __device__ inline size_t s3_table_bytes_padded(int nx, int nqt, int nbx, int nbq)
-{
-    return s3_table_bytes(nx, nqt, nbx, nbq) + 64;       // alignment slack of the double2 tables
-}
 
+// pdf_locate on this path: the search the evaluation kernel runs, exported (ix, iq local to the sub-grid)
 __global__ void __launch_bounds__(256)
 k_locate_stream(const __grid_constant__ GridDev G, const __grid_constant__ StreamDev B, long long n,
                 const double *__restrict__ x, const double *__restrict__ q2, int *ix, int *iq, int *isub, int *region)
@@ -692,11 +753,10 @@ __global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __
 {
     extern __shared__ __align__(32) unsigned char smem_raw[];
     const StreamTab T = s3_stage_tables(A.G, A.B, smem_raw, kS3Threads);
-    const unsigned stage0 = (unsigned)__cvta_generic_to_shared(smem_raw) +
-                            (unsigned)s3_table_bytes_padded(A.G.nx, A.G.nqtot, A.B.nbx, A.B.nbq);
+    const unsigned stage0 = (unsigned)__cvta_generic_to_shared(smem_raw) + (unsigned)s3_table_bytes(A.G.nx, A.G.nqtot, A.B.nbx, A.B.nbq);
     __syncthreads();                                   // the only CTA barrier: every warp works alone from here on
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned sbuf = ((stage0 + 31u) & ~31u) + (unsigned)(warp * 2 * kS3Batch * 32);
+    const unsigned sbuf = ((stage0 + 31u) & ~31u) + (unsigned)(warp * kStageBytes);
 
     unsigned long long *ctrl = A.W.ctrl;
     const StreamDev &B = A.B;
@@ -713,14 +773,15 @@ __global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __
         seen_p = p; seen_v = target;
     };
 
-    // the next ticket is fetched while the current item runs (a global atomic is ~1 us)
-    unsigned long long next_t = 0;
-    if (lane == 0) next_t = atomicAdd(ctrl, 1ULL);
+    // A ticket is fetched when the warp is free to start it, not earlier: a prefetched ticket sits unstarted behind
+    // the holder's current item and its waits, which doubles the window of unfinished tickets that the lag and the
+    // ring have to cover (measured: with prefetch B units waited 29 us on average even at lag 3).
     for (;;) {
-        const unsigned long long t = __shfl_sync(0xffffffffu, next_t, 0);
+        unsigned long long t = 0;
+        if (lane == 0) t = atomicAdd(ctrl, 1ULL);
+        t = __shfl_sync(0xffffffffu, t, 0);
         if (t >= total) break;
-        if (lane == 0) next_t = atomicAdd(ctrl, 1ULL);
-        // ticket order, lag L = kS3Lag rounds:  round r = [A(r) tiles | B(r-L) units]
+        // ticket order, lag L = kS3Lag rounds:  round r = [A(r) tiles | E(r-L), B(r-L) units]
         bool isA; long long c; int sub;
         {
             const unsigned long long RA = (unsigned long long)(nchunks < kS3Lag ? nchunks : kS3Lag);   // A-only rounds
@@ -741,51 +802,33 @@ __global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __
         }
         const int slot = (int)(c % kS3Ring);
         const unsigned long long gen = (unsigned long long)(c / kS3Ring);
-        unsigned long long *a_done = ctrl + 32 + slot * 48, *b_fin = a_done + 16, *b_done = a_done + 32;
+        unsigned long long *a_done = ctrl + kCtrlSlot0 + slot * kCtrlSlotStride, *b_fin = a_done + 16, *b_done = a_done + 32;
         long long chunk_base = c * A.chunk, chunk_end = chunk_base + A.chunk;
         if (chunk_end > A.n) chunk_end = A.n;
-        const double *V = A.G.V;
+        const double *V = A.G.V, *RP = B.rowplus;
         if (A.ctab) {                                              // a-8: the chunk is a piece of one member's run
             const int4 ce = __ldg(reinterpret_cast<const int4 *>(A.ctab) + c);
             chunk_base = ce.x; chunk_end = (long long)ce.x + ce.y;
             V += (size_t)ce.z * A.G.memstride;
+            RP += (size_t)ce.z * A.G.nx * kNFP;
         }
         if (isA) {
-            // the ring slot must have been drained by B(c - kS3Ring) before this tile touches its bins
+            // the ring slot must have been drained by the units of chunk c - kS3Ring before this tile touches its bins
             if (gen) wait_for(b_done, gen * TB);
             a_tile(A, T, slot, chunk_base, chunk_end, sub, err_local);
             warp_release_add(a_done, 1ULL);
         } else {
             wait_for(a_done, (gen + 1) * TA);                      // every tile of A(c) has been released
-            const int ncls = (B.ncx + 1) * kS3ClassParts;
-            const int ncell = (B.ncx + 1) * B.ng;
-            if (sub < ncls) {                                      // class bins first: the long units must not end the round
-                const int X = B.ncx - sub / kS3ClassParts, part = sub % kS3ClassParts;
-                unsigned c2 = 0;
-                if (lane < 2) c2 = ldcg_u32(A.W.counts + (size_t)slot * B.nbins + (size_t)X * B.nfk + B.nqt + lane);
-                for (int cls = 0; cls < 2; ++cls) {                // low-Q, then high-Q
-                    const int fk = B.nqt + cls;
-                    const int cap = bin_cap(B, X, fk), seg = (cap + kS3ClassParts - 1) / kS3ClassParts;
-                    int cnt = (int)__shfl_sync(0xffffffffu, c2, cls);
-                    cnt = cnt < cap ? cnt : cap;
-                    const int first = part * seg, cntp = min(seg, cnt - first);
-                    if (cntp > 0)
-                        b_unit_class(A, V, chunk_base, A.W.bins + (size_t)slot * B.slab + bin_off(B, X, fk), first, cntp, X, fk, sbuf);
-                }
-            } else if (sub < ncls + ncell) {
-                const int v = sub - ncls;
-                const int X = B.ncx - v / B.ng, grp = v % B.ng;    // the low-x key first
-                const int fk0 = grp * kS3FkPerUnit, fk1 = min(B.nqt, fk0 + kS3FkPerUnit);
-                if (X == B.ncx) b_unit_lowx(A, V, slot, chunk_base, fk0, fk1, sbuf);
-                else b_unit_interior(A, V, slot, chunk_base, X, fk0, fk1, sbuf);
-            } else {
-                ovf_unit(A, V, slot, chunk_base, sub - ncls - ncell);
+            if (sub < B.ne) e_unit(A, V, RP, slot, chunk_base);    // list units first: their queries are the expensive ones
+            else {
+                const int v = sub - B.ne;
+                const int i = v / B.ng, grp = v - i * B.ng;
+                b_unit(A, T, V, slot, chunk_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf);
             }
             const unsigned long long old = warp_release_add(b_fin, 1ULL);
             if (old + 1 == (gen + 1) * TB) {                       // last unit of the chunk: the slot's counters are reset for the ring
-                unsigned *cz = A.W.counts + (size_t)slot * B.nbins;
-                for (int k = lane; k < B.nbins; k += 32) cz[k] = 0u;
-                if (lane == 0) A.W.ovf_count[slot] = 0u;
+                unsigned *cz = A.W.counts + (size_t)slot * (B.nbins + 32);
+                for (int k = lane; k < B.nbins + 32; k += 32) cz[k] = 0u;
                 warp_release_add(b_done, TB);
             }
         }

@@ -1,6 +1,7 @@
 // pdf_stream_host.cuh -- host side of the binned path: key geometry, search tables, workspace, launch.
 #pragma once
 #include <cmath>
+#include <cstdio>
 #include <cstring>
 #include <vector>
 
@@ -13,9 +14,11 @@ struct StreamPlan {
     bool usable = false;
     StreamDev dev{};
     unsigned short *d_lutx = nullptr, *d_lutq = nullptr;
-    double2 *d_cxs = nullptr, *d_cqs = nullptr;
+    double *d_rowplus = nullptr;              // [nmem][nx][12] values at 1.01*Q2min (C-9's second anchor row)
     double *d_plus = nullptr;                 // scratch of k_q2plus
     int ncells_q = 1;                         // Q2 cells (knots - sub-grids)
+    bool locate_ok = false;                   // the search tables exist (pdf_locate can run this path's search)
+
     long long default_chunk = 256 * 1024;
 };
 
@@ -32,17 +35,29 @@ __global__ void k_q2plus(GridDev G, double *res)
     res[2] = 1.0;
 }
 
-// {ln lower knot, 1/dln} of every cell, from the cell tables the direct path uses (same numbers)
-__global__ void k_cell_pairs(const CellTab *__restrict__ tab, double2 *__restrict__ out, int n)
+// a-1 for C-9: the grid's values at Q2 = 1.01 Q2min for every member and x knot, RP[m][ix][f] =
+// sum_b wq_b V[m][row_b][ix][f] with the 4 node weights of cell jgplus at tqplus (the Q2 direction of the
+// second anchor of eq. 3.4 does not depend on the query, so it is tabulated once per grid)
+__global__ void k_rowplus(GridDev G, int jgplus, double tqplus, double *__restrict__ rp)
 {
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c < n) out[c] = make_double2(tab[c].lo_log, tab[c].inv_d);
+    const size_t per = (size_t)G.nx * G.nfp;
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= per * G.nmem) return;
+    const int m = (int)(e / per);
+    const size_t r = e % per;
+    Point1D qp;
+    q_point_cell(G, jgplus, tqplus, qp);
+    const double *Vm = G.V + (size_t)m * G.memstride;
+    double acc = 0.0;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) acc = fma(qp.w[b], Vm[(size_t)qp.idx[b] * per + r], acc);
+    rp[e] = acc;
 }
 
 inline void stream_plan_free(StreamPlan &p)
 {
-    cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_cxs); cudaFree(p.d_cqs); cudaFree(p.d_plus);
-    p.d_lutx = p.d_lutq = nullptr; p.d_cxs = p.d_cqs = nullptr; p.d_plus = nullptr; p.usable = false;
+    cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_rowplus); cudaFree(p.d_plus);
+    p.d_lutx = p.d_lutq = nullptr; p.d_rowplus = nullptr; p.d_plus = nullptr; p.usable = false; p.locate_ok = false;
 }
 
 // search table of one knot line: bucket = (high word of v >> shift) - base; entry = the largest c <= lim with
@@ -75,24 +90,17 @@ inline long long stream_chunk(const StreamPlan &p, long long n, long long chunk_
     return c < need ? c : need;
 }
 
-// bin capacities for a chunk size: interior cells 3x the uniform share + 32 (a uniform cloud is Poisson
-// around the share), class bins 2x the share of an x cell; beyond them queries overflow to the generic code
+// per-chunk geometry: a cell bin holds 3x the uniform share + 32 (a uniform cloud is Poisson around the share;
+// beyond it queries overflow to a list), one E unit per 1024 queries of the chunk
 inline void stream_caps(const StreamPlan &p, long long chunk, StreamDev &d)
 {
-    auto up32 = [](long long v) { return (int)((v + 31) / 32 * 32); };
     d = p.dev;
-    const long long per_x = chunk / (d.ncx > 0 ? d.ncx : 1);
-    const long long per_cell = per_x / (p.ncells_q > 0 ? p.ncells_q : 1);
-    d.cap_int = up32(3 * per_cell + 32);
-    d.cap_cls = up32(2 * per_x + 64);
-    d.cap_lx = d.cap_cls;
-    d.cap_lxc = 2 * d.cap_cls;
-    if (d.cap_int > chunk) d.cap_int = up32(chunk);
-    if (d.cap_cls > chunk) d.cap_cls = d.cap_lx = up32(chunk);
-    if (d.cap_lxc > chunk) d.cap_lxc = up32(chunk);
-    d.rowcap = d.nqt * d.cap_int + 2 * d.cap_cls;
-    d.lxbase = d.ncx * d.rowcap;
-    d.slab = d.lxbase + d.nqt * d.cap_lx + 2 * d.cap_lxc;
+    const long long per_cell = chunk / ((long long)(d.ncx > 0 ? d.ncx : 1) * (p.ncells_q > 0 ? p.ncells_q : 1));
+    long long cap = (3 * per_cell + 32 + 31) / 32 * 32;
+    if (cap > chunk) cap = (chunk + 31) / 32 * 32;
+    d.cap = (int)cap;
+    d.ne = (int)((chunk + PDF_S3_EDIV - 1) / PDF_S3_EDIV);
+    d.tb = d.ne + d.ncx * d.ng;
 }
 
 inline size_t stream_workspace_bytes(const StreamPlan &p, long long n, long long chunk_opt)
@@ -101,28 +109,26 @@ inline size_t stream_workspace_bytes(const StreamPlan &p, long long n, long long
     const long long chunk = stream_chunk(p, n, chunk_opt);
     StreamDev d;
     stream_caps(p, chunk, d);
-    size_t b = 4096;                                                    // ctrl
-    b += align_up(sizeof(unsigned) * (size_t)kS3Ring * d.nbins, 256);
-    b += 256;                                                           // ovf_count
-    b += align_up(sizeof(Payload) * (size_t)kS3Ring * d.slab, 256);
-    b += align_up(sizeof(Payload) * (size_t)kS3Ring * chunk, 256);
+    size_t b = sizeof(unsigned long long) * kCtrlWords;
+    b += align_up(sizeof(unsigned) * (size_t)kS3Ring * (d.nbins + 32), 256);
+    b += align_up(sizeof(Payload) * (size_t)kS3Ring * d.nbins * d.cap, 256);
+    b += align_up(sizeof(Payload) * (size_t)kS3Ring * kNumLists * chunk, 256);
     return b + 256;
 }
 
 inline void stream_carve(void *ws, long long chunk, const StreamDev &d, StreamWorkspace &w)
 {
     char *c = (char *)align_up((size_t)ws, 256);
-    w.ctrl = (unsigned long long *)c; c += 4096;
-    w.counts = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)kS3Ring * d.nbins, 256);
-    w.ovf_count = (unsigned *)c; c += 256;
-    w.bins = (Payload *)c; c += align_up(sizeof(Payload) * (size_t)kS3Ring * d.slab, 256);
-    w.ovf = (Payload *)c;
+    w.ctrl = (unsigned long long *)c; c += sizeof(unsigned long long) * kCtrlWords;
+    w.counts = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)kS3Ring * (d.nbins + 32), 256);
+    w.bins = (Payload *)c; c += align_up(sizeof(Payload) * (size_t)kS3Ring * d.nbins * d.cap, 256);
+    w.lists = (Payload *)c;
     (void)chunk;
 }
 
 inline size_t stream_smem_bytes(const GridDev &G, const StreamDev &d)
 {
-    return s3_table_bytes_padded(G.nx, G.nqtot, d.nbx, d.nbq) + 32 + (size_t)kS3Warps * 2 * kS3Batch * sizeof(Payload);
+    return s3_table_bytes(G.nx, G.nqtot, d.nbx, d.nbq) + 32 + (size_t)kS3Warps * kStageBytes;
 }
 
 // builds the search tables and the key geometry; leaves usable = false when the grid does not fit the
@@ -134,10 +140,9 @@ inline int stream_plan_init(StreamPlan &p, const GridDev &G, const std::vector<d
     if (G.nflav != kNF || G.nfp != kNFP) return 0;
     if (nx - 1 > kS3MaxCells || nqt > kS3MaxCells || nx < 2) return 0;
     StreamDev &d = p.dev;
-    d.ncx = nx - 1; d.nqt = nqt; d.nfk = nqt + 2;
-    d.nbins = (d.ncx + 1) * d.nfk;
+    d.ncx = nx - 1; d.nqt = nqt;
+    d.nbins = d.ncx * nqt;
     d.ng = (nqt + kS3FkPerUnit - 1) / kS3FkPerUnit;
-    d.tb = (d.ncx + 1) * kS3ClassParts + (d.ncx + 1) * d.ng + kS3Ovf;
     p.ncells_q = nqt - nsub;
 
     std::vector<unsigned short> lx, lq;
@@ -147,22 +152,24 @@ inline int stream_plan_init(StreamPlan &p, const GridDev &G, const std::vector<d
 
     if (cudaMalloc((void **)&p.d_lutx, sizeof(unsigned short) * lx.size()) != cudaSuccess) return PDF_ENOMEM;
     if (cudaMalloc((void **)&p.d_lutq, sizeof(unsigned short) * lq.size()) != cudaSuccess) return PDF_ENOMEM;
-    if (cudaMalloc((void **)&p.d_cxs, sizeof(double2) * nx) != cudaSuccess) return PDF_ENOMEM;
-    if (cudaMalloc((void **)&p.d_cqs, sizeof(double2) * nqt) != cudaSuccess) return PDF_ENOMEM;
     if (cudaMalloc((void **)&p.d_plus, sizeof(double) * 4) != cudaSuccess) return PDF_ENOMEM;
     cudaMemcpy(p.d_lutx, lx.data(), sizeof(unsigned short) * lx.size(), cudaMemcpyHostToDevice);
     cudaMemcpy(p.d_lutq, lq.data(), sizeof(unsigned short) * lq.size(), cudaMemcpyHostToDevice);
-    k_cell_pairs<<<(nx + 127) / 128, 128>>>(G.cx, p.d_cxs, nx - 1);
-    k_cell_pairs<<<(nqt + 127) / 128, 128>>>(G.cq, p.d_cqs, nqt);
     k_q2plus<<<1, 32>>>(G, p.d_plus);
     double res[3] = {0, 0, 0};
     if (cudaMemcpy(res, p.d_plus, sizeof res, cudaMemcpyDeviceToHost) != cudaSuccess) return PDF_ECUDA;
-    d.lutx = p.d_lutx; d.lutq = p.d_lutq; d.cxs = p.d_cxs; d.cqs = p.d_cqs;
+    d.lutx = p.d_lutx; d.lutq = p.d_lutq;
     // pdf_locate on this path needs only the tables
     if (cudaFuncSetAttribute(k_locate_stream, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)s3_table_bytes_padded(nx, nqt, d.nbx, d.nbq)) != cudaSuccess) return 0;
+                             (int)s3_table_bytes(nx, nqt, d.nbx, d.nbq)) != cudaSuccess) return 0;
+    p.locate_ok = true;
     if (res[2] != 1.0) return 0;                           // 1.01*Q2min beyond the grid: direct path only
     d.jgplus = (int)res[0]; d.tqplus = res[1];
+    const size_t nrp = (size_t)G.nmem * nx * kNFP;
+    if (cudaMalloc((void **)&p.d_rowplus, sizeof(double) * nrp) != cudaSuccess) return PDF_ENOMEM;
+    k_rowplus<<<(unsigned)((nrp + 255) / 256), 256>>>(G, d.jgplus, d.tqplus, p.d_rowplus);
+    if (cudaDeviceSynchronize() != cudaSuccess) return PDF_ECUDA;
+    d.rowplus = p.d_rowplus;
     const size_t smem = stream_smem_bytes(G, d);
     if (smem > 200 * 1024) return 0;
     if (cudaFuncSetAttribute(k_pdf_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
@@ -196,7 +203,7 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
     A.zfill = (ld == cm.n) ? 1 : 0;
     A.count_err = count_err;
-    const size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts + ovf_count
+    const size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts
     if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
     const size_t smem = stream_smem_bytes(G, A.B);
     int per_sm = 0, dev = 0, sms = 0;
@@ -227,7 +234,7 @@ inline int stream_locate(const GridDev &G, const StreamPlan &p, long long n, con
     const long long want = (n + 255) / 256;
     const unsigned grid = (unsigned)(want < (long long)sms * 8 ? want : (long long)sms * 8);
     Scope sc(s, "k_locate_stream");
-    k_locate_stream<<<grid, 256, s3_table_bytes_padded(G.nx, G.nqtot, p.dev.nbx, p.dev.nbq), s>>>(G, p.dev, n, x, q2, ix, iq, isub, region);
+    k_locate_stream<<<grid, 256, s3_table_bytes(G.nx, G.nqtot, p.dev.nbx, p.dev.nbq), s>>>(G, p.dev, n, x, q2, ix, iq, isub, region);
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }
 

@@ -37,9 +37,9 @@ int cuda_fail(cudaError_t e, const char *what)
 // every kernel launch of the library goes through these two: count it, optionally time it
 struct LaunchScope {
     cudaStream_t s; const char *name; ProfEntry pe{}; bool on;
-    LaunchScope(cudaStream_t st, const char *nm) : s(st), name(nm)
+    LaunchScope(cudaStream_t st, const char *nm, int launches = 1) : s(st), name(nm)
     {
-        g_launches.fetch_add(1, std::memory_order_relaxed);
+        g_launches.fetch_add(launches, std::memory_order_relaxed);
         on = g_prof_on;
         if (on) { cudaEventCreate(&pe.a); cudaEventCreate(&pe.b); pe.name = nm; cudaEventRecord(pe.a, s); }
     }

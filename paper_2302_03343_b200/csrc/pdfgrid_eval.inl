@@ -222,7 +222,7 @@ int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2
     // the search of the path the evaluation calls take: the table-driven search of the binned kernel's A
     // tiles unless PDF_PATH_DIRECT is set (or the grid does not fit the binned path), then the binary
     // search of the direct kernels
-    if (g->path != PDF_PATH_DIRECT && g->bplan.usable) {
+    if (g->path != PDF_PATH_DIRECT && g->bplan.locate_ok) {
         g->last_path = PDF_PATH_BINNED;
         return stream_locate<LaunchScope>(g->d, g->bplan, n, x, q2, ix, iq, isub, region, s);
     }
