@@ -185,6 +185,10 @@ int pdf_profile_read(int max_entries, const char **names, float *ms);
  * the measured denominator of the "alu" roofline of pdf_lumi. */
 int pdf_measure_fp64_tflops(double *tflops, void *stream);
 
+/* diagnostic: out[i] = the logarithm the path computes its abscissae with (t = (ln v - ln knot)/delta, L1716), for
+ * finite x[i] > 0; DEVICE [n] each.  Tested against the host's log (<= 1 ulp). */
+int pdf_log_f64(long long n, const double *x, double *out, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -31,8 +31,8 @@ ALPHAS_FREEZE, ALPHAS_LOGGRAD = 0, 1
 # t-sensitivity (each side's t carries a few 2^-52 (1 + |ln v|/delta) of rounding).  The values are the
 # tightest that the measured errors allow with a margin (C-12 lists the measured worst ratios).
 REL = 1e-12
-FLOOR_S = 2e-15
-FLOOR_T = 4 * 2.0 ** -52
+FLOOR_S = 1e-15
+FLOOR_T = 2 * 2.0 ** -52
 
 
 def tolerance(ref, scale):

@@ -31,7 +31,7 @@ SYMBOLS = (
     "pdf_xfxq2", "pdf_xfxq2_ex", "pdf_xfxq2_xgrid", "pdf_alphas_q2", "pdf_lumi", "pdf_locate", "pdf_error_count",
     "pdf_xfxq2_host", "pdf_alphas_q2_host", "pdf_lumi_host", "pdf_status_string",
     "pdf_last_cuda_error", "pdf_launch_count", "pdf_profile_enable", "pdf_profile_read",
-    "pdf_measure_fp64_tflops", "pdf_last_path",
+    "pdf_measure_fp64_tflops", "pdf_last_path", "pdf_log_f64",
 )
 
 
@@ -79,6 +79,7 @@ def lib():
     L.pdf_profile_read.argtypes = [C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
     L.pdf_measure_fp64_tflops.argtypes = [dp, vp]
     L.pdf_last_path.argtypes = [vp]
+    L.pdf_log_f64.argtypes = [ll, vp, vp, vp]
     _lib = L
     return L
 
@@ -148,6 +149,12 @@ def pdf_measure_fp64_tflops(stream=None) -> float:
     v = C.c_double()
     _check(lib().pdf_measure_fp64_tflops(C.byref(v), _stream_ptr(stream)), "pdf_measure_fp64_tflops")
     return v.value
+
+
+def pdf_log_f64(x: torch.Tensor, stream=None) -> torch.Tensor:
+    out = torch.empty_like(x)
+    _check(lib().pdf_log_f64(x.numel(), _dev(x, torch.float64, "x"), _dev(out, torch.float64, "out"), _stream_ptr(stream)), "pdf_log_f64")
+    return out
 
 
 class PdfGrid:

@@ -8,7 +8,7 @@
 
 namespace pdfg {
 
-constexpr int kAlphaLut = 256;     // search-acceleration buckets of the alpha_s knot line
+constexpr int kAlphaLutMax = 2048;  // search-table buckets of the alpha_s knot line (indexed by exponent and top mantissa bits)
 constexpr int kMaxLumiFlav = 16;   // generic pdf_lumi keeps both flavour vectors in registers/local
 constexpr int kRegionInterior = 0, kRegionLowX = 1, kRegionLowQ = 2, kRegionHighQ = 3,
               kRegionLowXLowQ = 4, kRegionLowXHighQ = 5, kRegionInvalid = 6;
@@ -43,8 +43,8 @@ struct GridDev {
     const double *ak, *alk, *av;  // raw knots, ln knots, values
     const CellTab *ca;            // [na-1]
     const double *acell;          // [na-1][6] per-cell cubic: ln lower knot, 1/dln, c0..c3 (alpha_s = c0 + t(c1 + t(c2 + t c3)))
-    const short *alut;            // [kAlphaLut] start guesses of the alpha_s knot search
-    double alut_scale;            // buckets per unit of ln Q2
+    const unsigned short *alut;   // [nalut] cell at the lower edge of bucket (high word of Q2 >> ashift) - abase
+    int ashift, abase, nalut;
     // luminosity coupling [nflav][nflav]
     const double *C;
     unsigned long long *err_count;
@@ -54,6 +54,45 @@ struct Point1D {      // a cell, its 4 clamped node indices and node weights
     int idx[4];
     double w[4];
 };
+
+// ln v for finite v > 0: the logarithm behind every abscissa of the path (t_x, t_q, theta: C-1, C-5, C-7, C-8) and
+// behind the ln-knot tables, so that t == 0 exactly on a knot on every path.  The library routine is ~85
+// instructions per call with its special cases (5 of the 42 warp instructions per query of the binned kernel,
+// profile r2k); this one is 38 and inlines.  v = m 2^e, m in [sqrt(1/2), sqrt 2), f = m - 1 (exact),
+// s = f / (2 + f), z = s^2:
+//   ln m = 2 atanh(s) = f - f^2/2 + s (f^2/2 + R),   R = z (2/3 + z (2/5 + z (2/7 + ...))),   z <= 0.0295,
+// summed in the order that keeps the exact f for last, with ln 2 split so that e ln2_hi is exact.
+// Measured against glibc on the GPU box (tests/test_gpu_parity.py::test_path_logarithm): <= 1 ulp.
+__device__ __forceinline__ double pdf_log(double v)
+{
+    int hi = __double2hiint(v), lo = __double2loint(v);
+    int e = -1023;
+    if (hi < 0x00100000) {                               // subnormal: scale by 2^54
+        v *= 18014398509481984.0;
+        hi = __double2hiint(v); lo = __double2loint(v);
+        e -= 54;
+    }
+    e += hi >> 20;
+    hi = (hi & 0x000fffff) | 0x3ff00000;                 // m in [1, 2)
+    if (hi >= 0x3ff6a09f) { hi -= 0x00100000; ++e; }     // m in [sqrt(1/2), sqrt 2)
+    const double f = __hiloint2double(hi, lo) - 1.0;
+    const double d = 2.0 + f;
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    r = fma(fma(-d, r, 1.0), r, r);
+    r = fma(fma(-d, r, 1.0), r, r);
+    double s = f * r;
+    s = fma(fma(-d, s, f), r, s);                        // s = f / d to the last bit or two
+    const double z = s * s;
+    double R = 2.0 / 21.0;
+    R = fma(R, z, 2.0 / 19.0); R = fma(R, z, 2.0 / 17.0); R = fma(R, z, 2.0 / 15.0); R = fma(R, z, 2.0 / 13.0);
+    R = fma(R, z, 2.0 / 11.0); R = fma(R, z, 2.0 / 9.0);  R = fma(R, z, 2.0 / 7.0);  R = fma(R, z, 2.0 / 5.0);
+    R = fma(R, z, 2.0 / 3.0);
+    R *= z;
+    const double hfsq = 0.5 * f * f, de = (double)e;
+    // ln 2 = ln2_hi + ln2_lo, the low 21 bits of ln2_hi are zero: e ln2_hi is exact for |e| < 2^11
+    return fma(de, 0x1.62e42fee00000p-1, -((hfsq - fma(s, hfsq + R, de * 0x1.a39ef35793c76p-33)) - f));
+}
 
 __device__ __forceinline__ bool finite_pos(double v) { return v > 0.0 && v < __longlong_as_double(0x7ff0000000000000LL); }
 
@@ -117,7 +156,7 @@ __device__ __forceinline__ int x_point(const GridDev &G, double x, Point1D &p)
 {
     int i = find_cell(G.xk, G.nx, x);
     // t = 1 exactly on the last knot (the only knot that belongs to the cell on its left, C-4)
-    double t = (x == G.xk[i + 1]) ? 1.0 : (log(x) - G.cx[i].lo_log) * G.cx[i].inv_d;
+    double t = (x == G.xk[i + 1]) ? 1.0 : (pdf_log(x) - G.cx[i].lo_log) * G.cx[i].inv_d;
     x_point_cell(G, i, t, p);
     return i;
 }
@@ -149,7 +188,7 @@ __device__ __forceinline__ void q_point(const GridDev &G, double q2, Point1D &p)
 {
     int j, jg;
     q_locate(G, q2, j, jg);
-    double t = (q2 == G.qk[jg + 1]) ? 1.0 : (log(q2) - G.cq[jg].lo_log) * G.cq[jg].inv_d;
+    double t = (q2 == G.qk[jg + 1]) ? 1.0 : (pdf_log(q2) - G.cq[jg].lo_log) * G.cq[jg].inv_d;
     q_point_cell(G, jg, t, p);
 }
 
@@ -164,7 +203,7 @@ __device__ __forceinline__ void make_xdesc(const GridDev &G, double x, XDesc &d)
     if (!d.low) { x_point(G, x, d.p0); return; }
     x_point_cell(G, 0, 0.0, d.p0);
     if (G.nx >= 3) x_point_cell(G, 1, 0.0, d.p1); else x_point_cell(G, 0, 1.0, d.p1);
-    d.theta = (log(x) - G.uk[0]) / (G.uk[1] - G.uk[0]);
+    d.theta = (pdf_log(x) - G.uk[0]) / (G.uk[1] - G.uk[0]);
 }
 
 __device__ __forceinline__ void make_qdesc(const GridDev &G, double q2, QDesc &d)
@@ -174,7 +213,7 @@ __device__ __forceinline__ void make_qdesc(const GridDev &G, double q2, QDesc &d
     if (!d.high) { q_point(G, q2, d.p0); return; }
     q_point_cell(G, last - 1, 0.0, d.p0);
     q_point_cell(G, last - 1, 1.0, d.p1);
-    d.theta = (log(q2) - G.sk[last - 1]) / (G.sk[last] - G.sk[last - 1]);
+    d.theta = (pdf_log(q2) - G.sk[last - 1]) / (G.sk[last] - G.sk[last - 1]);
 }
 
 // C-7 / C-8 switch (L1722): log form iff both anchors exceed 1e-3, per flavour

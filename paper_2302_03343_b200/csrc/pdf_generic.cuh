@@ -7,11 +7,11 @@
 namespace pdfg {
 
 // ---- a-1: grid layout ------------------------------------------------------------------------
-// ln of the knots with the device log (so that t == 0 exactly on a knot), one thread per knot
+// ln of the knots with the path's own logarithm (so that t == 0 exactly on a knot), one thread per knot
 __global__ void k_log_knots(const double *__restrict__ k, double *__restrict__ lk, int n)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) lk[i] = log(k[i]);
+    if (i < n) lk[i] = pdf_log(k[i]);
 }
 
 // per-cell Hermite constants of one knot line [first, first+m) (a sub-grid, the x line, alpha_s)
@@ -409,6 +409,8 @@ __global__ void k_alphas_cells(const CellTab *__restrict__ ca, const double *__r
 
 constexpr int kAlphasIlp = 4;
 
+// The cell comes from a table on the bit pattern of Q2 (exponent and top mantissa bits) and a walk on the raw
+// knots (C-4, exact), so the search does not wait for the logarithm; ln Q2 is pdf_log (38 instructions).
 __global__ void __launch_bounds__(256)
 k_alphas(GridDev G, long long n, const double *__restrict__ q2, double *__restrict__ out)
 {
@@ -417,12 +419,13 @@ k_alphas(GridDev G, long long n, const double *__restrict__ q2, double *__restri
     double *ak = sm;                               // [na] raw knots
     double *av = sm + m;                           // [na] values
     double *cell = sm + 2 * m;                     // [na-1][6]
-    short *lut = reinterpret_cast<short *>(cell + 6 * (m - 1));
+    unsigned short *lut = reinterpret_cast<unsigned short *>(cell + 6 * (m - 1));
     for (int i = threadIdx.x; i < m; i += blockDim.x) { ak[i] = G.ak[i]; av[i] = G.av[i]; }
     for (int i = threadIdx.x; i < 6 * (m - 1); i += blockDim.x) cell[i] = G.acell[i];
-    for (int i = threadIdx.x; i < kAlphaLut; i += blockDim.x) lut[i] = G.alut[i];
+    for (int i = threadIdx.x; i < G.nalut; i += blockDim.x) lut[i] = G.alut[i];
     __syncthreads();
-    const double kmin = ak[0], kmax = ak[m - 1], l0 = cell[0], scale = G.alut_scale;
+    const double kmin = ak[0], kmax = ak[m - 1];
+    const int shift = G.ashift, base = G.abase, nb = G.nalut;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long e0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; e0 < n; e0 += stride * kAlphasIlp) {
         double q[kAlphasIlp], v[kAlphasIlp];
@@ -437,21 +440,26 @@ k_alphas(GridDev G, long long n, const double *__restrict__ q2, double *__restri
                 v[k] = G.alphas_mode ? av[0] * pow(qq / kmin, log(av[1] / av[0]) / log(ak[1] / kmin)) : av[0];
                 continue;
             }
-            const double lq = log(qq);
-            int b = (int)((lq - l0) * scale);
-            b = b < 0 ? 0 : (b >= kAlphaLut ? kAlphaLut - 1 : b);
-            int c = lut[b];                                                // start guess; the walk makes it exact (C-4)
-            while (c > 0 && ak[c] > qq) --c;
-            while (c < m - 2 && ak[c + 1] <= qq) ++c;
+            int b = (__double2hiint(qq) >> shift) - base;
+            b = b < 0 ? 0 : (b >= nb ? nb - 1 : b);
+            int c = lut[b];                                                // at the bucket's lower edge: never above the cell
+            while (c < m - 2 && ak[c + 1] <= qq) ++c;                      // C-4 on the raw knots
             const double2 *cc = reinterpret_cast<const double2 *>(cell + 6 * c);
             const double2 c01 = cc[0], c23 = cc[1], c45 = cc[2];
-            const double t = (lq - c01.x) * c01.y;
+            const double t = (pdf_log(qq) - c01.x) * c01.y;
             const double poly = fma(fma(fma(c45.y, t, c45.x), t, c23.y), t, c23.x);
             v[k] = (qq == ak[c + 1]) ? av[c + 1] : poly;                   // a knot returns its stored value
         }
 #pragma unroll
         for (int k = 0; k < kAlphasIlp; ++k) { long long e = e0 + k * stride; if (e < n) __stcs(out + e, v[k]); }
     }
+}
+
+// the path's logarithm on an array (diagnostic: pdf_log_f64 of the C ABI, tested against the host's)
+__global__ void k_log_f64(long long n, const double *__restrict__ x, double *__restrict__ out)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < n) out[e] = pdf_log(x[e]);
 }
 
 // ---- a-7: direct luminosity ------------------------------------------------------------------

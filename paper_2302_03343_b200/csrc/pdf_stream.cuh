@@ -246,9 +246,9 @@ __device__ __forceinline__ Located s3_locate(const GridDev &G, const StreamDev &
     return L;
 }
 
-// Out-of-line copies of the transcendental pieces: inlined, the two logarithms of a query and the continuation
-// formulas made the kernel 22 700 instructions (364 KB) with a 25 KB A loop, and warps of three different work
-// kinds per SM evicted one another's code from the instruction caches (~20 clk per issued instruction).
+// Out-of-line copies of the transcendental pieces of the E units: inlined, the library logarithms and the
+// continuation formulas made the kernel 22 700 instructions (364 KB), and warps of three different work kinds
+// per SM evicted one another's code from the instruction caches (~20 clk per issued instruction).
 __device__ __noinline__ double s3_log(double v) { return log(v); }
 __device__ __noinline__ double s3_two(double f0, double f1, double theta) { return continue_two(f0, f1, theta); }
 __device__ __noinline__ double s3_lowq(double fmin, double fplus, double r, double lnr) { return lowq_continue_ln(fmin, fplus, r, lnr); }
@@ -322,7 +322,7 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
             const int jg = L[q].g < nqt - 1 ? L[q].g : nqt - 2;       // only Q2 == Q2max lands on the last knot: it belongs to the last cell
             const double2 ci = lds_v2f64(T.cx + 48u * i), cj = lds_v2f64(T.cq + 48u * jg);   // {ln lower knot, 1/dln}
             double lx = 0.0, lq = 0.0;
-            if (r != kRegionInvalid) { lx = s3_log(xv[q]); lq = s3_log(qv[q]); }
+            if (r != kRegionInvalid) { lx = pdf_log(xv[q]); lq = pdf_log(qv[q]); }
             // t = 1 exactly on the last knot (the only knot that belongs to the cell on its left, C-4)
             pa[q] = lowx ? (lx - u0) * inv_du0                                    // theta_x (C-7)
                          : (__double_as_longlong(xv[q]) == xmaxb) ? 1.0 : (lx - ci.x) * ci.y;

@@ -31,7 +31,7 @@ __global__ void k_q2plus(GridDev G, double *res)
     int j, jg;
     q_locate(G, q, j, jg);
     res[0] = (double)jg;
-    res[1] = (q == G.qk[jg + 1]) ? 1.0 : (log(q) - G.cq[jg].lo_log) * G.cq[jg].inv_d;
+    res[1] = (q == G.qk[jg + 1]) ? 1.0 : (pdf_log(q) - G.cq[jg].lo_log) * G.cq[jg].inv_d;
     res[2] = 1.0;
 }
 

@@ -76,7 +76,7 @@ struct pdf_grid {
     int *d_sub_of = nullptr, *d_qoff = nullptr, *d_cell_adj = nullptr;
     CellTab *d_cx = nullptr, *d_cq = nullptr, *d_ca = nullptr;
     double *d_ak = nullptr, *d_alk = nullptr, *d_av = nullptr, *d_C = nullptr, *d_acell = nullptr;
-    short *d_alut = nullptr;
+    unsigned short *d_alut = nullptr;
     unsigned long long *d_err = nullptr;
     std::vector<double> h_av, h_ak, h_C;
     // caller-owned workspace of the binned path
@@ -268,23 +268,18 @@ int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double
     g->d_ak = g->d_alk = g->d_av = g->d_acell = nullptr; g->d_ca = nullptr; g->d_alut = nullptr; g->d.na = 0;
     int rc;
     if ((rc = dev_alloc(&g->d_ak, n)) || (rc = dev_alloc(&g->d_alk, n)) || (rc = dev_alloc(&g->d_av, n)) ||
-        (rc = dev_alloc(&g->d_ca, n)) || (rc = dev_alloc(&g->d_acell, 6 * (size_t)n)) || (rc = dev_alloc(&g->d_alut, kAlphaLut))) return rc;
+        (rc = dev_alloc(&g->d_ca, n)) || (rc = dev_alloc(&g->d_acell, 6 * (size_t)n)) || (rc = dev_alloc(&g->d_alut, kAlphaLutMax))) return rc;
     CK(cudaMemcpy(g->d_ak, q2_knots, sizeof(double) * n, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(g->d_av, values, sizeof(double) * n, cudaMemcpyHostToDevice));
     { LaunchScope a(0, "k_log_knots"); k_log_knots<<<(n + 127) / 128, 128>>>(g->d_ak, g->d_alk, n); }
     { LaunchScope a(0, "k_cell_tables"); k_cell_tables<<<(n + 127) / 128, 128>>>(g->d_alk, g->d_ca, 0, n); }
     { LaunchScope a(0, "k_alphas_cells"); k_alphas_cells<<<(n + 127) / 128, 128>>>(g->d_ca, g->d_av, g->d_acell, n); }
-    {   // search LUT over ln Q2 (a start guess only: host log here, exact walk on the device)
-        std::vector<short> lut(kAlphaLut);
-        double l0 = std::log(q2_knots[0]), l1 = std::log(q2_knots[n - 1]);
-        g->d.alut_scale = kAlphaLut / (l1 - l0) * (1.0 - 1e-12);
-        int c = 0;
-        for (int b = 0; b < kAlphaLut; ++b) {
-            double edge = std::exp(l0 + b / g->d.alut_scale);
-            while (c < n - 2 && q2_knots[c + 1] <= edge) ++c;
-            lut[b] = (short)c;
-        }
-        CK(cudaMemcpy(g->d_alut, lut.data(), sizeof(short) * kAlphaLut, cudaMemcpyHostToDevice));
+    {   // search table on the bit pattern of Q2: entry = the cell at the bucket's lower edge (the walk on the device makes it exact)
+        std::vector<double> k(q2_knots, q2_knots + n);
+        std::vector<unsigned short> lut;
+        make_search_table(k, n - 2, g->d.ashift, g->d.abase, lut);
+        g->d.nalut = (int)lut.size();
+        CK(cudaMemcpy(g->d_alut, lut.data(), sizeof(unsigned short) * lut.size(), cudaMemcpyHostToDevice));
     }
     CK(cudaDeviceSynchronize());
     g->d.na = n; g->d.ak = g->d_ak; g->d.alk = g->d_alk; g->d.av = g->d_av; g->d.ca = g->d_ca;

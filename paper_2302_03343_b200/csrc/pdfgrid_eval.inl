@@ -196,7 +196,7 @@ int pdf_alphas_q2(const pdf_grid *g, long long n, const double *q2, double *out,
     long long want = (n + 255) / 256;
     unsigned grid = (unsigned)(want < (long long)sms * 8 ? want : (long long)sms * 8);
     LaunchScope a(s, "k_alphas");
-    size_t smem = sizeof(double) * (2 * g->d.na + 6 * (g->d.na - 1)) + sizeof(short) * kAlphaLut + 16;
+    size_t smem = sizeof(double) * (2 * g->d.na + 6 * (g->d.na - 1)) + sizeof(short) * g->d.nalut + 16;
     if (smem > 48 * 1024) return PDF_EINVAL;
     k_alphas<<<grid, 256, smem, s>>>(g->d, n, q2, out);
     CK(cudaGetLastError());
@@ -253,6 +253,18 @@ int pdf_error_count(const pdf_grid *g, long long *n_invalid, void *stream)
     CK(cudaMemsetAsync(g->d_err, 0, sizeof v, s));
     CK(cudaStreamSynchronize(s));
     *n_invalid = (long long)v;
+    return PDF_OK;
+}
+
+int pdf_log_f64(long long n, const double *x, double *out, void *stream)
+{
+    if (n < 0) return PDF_EINVAL;
+    if (n == 0) return PDF_OK;
+    if (!x || !out) return PDF_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    LaunchScope a(s, "k_log_f64");
+    k_log_f64<<<blocks_for(n, 256), 256, 0, s>>>(n, x, out);
+    CK(cudaGetLastError());
     return PDF_OK;
 }
 

@@ -21,9 +21,13 @@ worst = 0
 for rep in range(3 if n <= 4_000_000 else 2):
     b = g.pdf_xfxq2(spec.pids, xd, qd)
     assert torch.equal(torch.isnan(b), torch.isnan(d))
-    # on the device: every row, relative difference of the two kernels' summation orders
-    err = (b.nan_to_num() - d.nan_to_num()).abs() / (d.nan_to_num().abs() + 1e-30)
-    bad = int((err.max(dim=1).values > 1e-9).sum())
+    # on the device: every row; the two kernels sum in different orders, so an element may differ by a few ulp of
+    # the stencil's scale (bounded below by the row's largest value) where it cancels, else by ~1e-15 relative
+    dz = d.nan_to_num()
+    err = (b.nan_to_num() - dz).abs()
+    tol = 1e-9 * dz.abs() + 1e-11 * dz.abs().max(dim=1, keepdim=True).values + 1e-300
+    bad = int(((err > tol).any(dim=1)).sum())
+    del dz, tol
     worst = max(worst, bad)
     del b, err
 print("COLD_BAD_ROWS", worst)

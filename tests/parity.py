@@ -44,8 +44,8 @@ def value_errors(gpu, ref, S):
     strict, strict_report = strict_max(well), strict_max(aref > STRICT_CUT_REPORT * S[ok][..., 0])
     # the same errors against tighter floors (what the floors could be lowered to): worst ratio per candidate
     probe = {}
-    for fs in (1e-15, 5e-16):
-        for ft in (2 * 2.0 ** -52, 2.0 ** -52):
+    for fs in (5e-16, 2.5e-16):
+        for ft in (2.0 ** -52, 0.5 * 2.0 ** -52):
             t2 = REL * np.abs(ref[ok]) + fs * S[ok][..., 0] + ft * S[ok][..., 1]
             probe[f"S{fs:g}_T{ft / 2.0 ** -52:g}ulp"] = float(np.max(np.where(exact, 0.0, err / np.where(t2 > 0, t2, 1e-300)))) if err.size else 0.0
     return dict(worst=float(ratio.max()) if ratio.size else 0.0, strict_rel_max=strict, strict_rel_max_cut1e3=strict_report,

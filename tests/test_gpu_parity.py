@@ -62,6 +62,27 @@ def test_locate_bitexact(B, oracle_mod, cfg):
     check_locate(B, og, g, bad_x, bad_q)
 
 
+def test_path_logarithm(B):
+    """pdf_log, the logarithm behind every abscissa of the path (C-1, C-5), against the host's log: <= 1 ulp apart
+    over the whole positive range, subnormals, the neighbourhood of 1 and exact powers of two"""
+    g = torch.Generator().manual_seed(12)
+    parts = [torch.exp(torch.empty(4_000_000, dtype=torch.float64).uniform_(-700.0, 700.0, generator=g)),
+             1.0 + torch.empty(1_000_000, dtype=torch.float64).uniform_(-0.3, 0.45, generator=g),
+             1.0 + 10.0 ** torch.empty(200_000, dtype=torch.float64).uniform_(-16.0, -1.0, generator=g),
+             1.0 - 10.0 ** torch.empty(200_000, dtype=torch.float64).uniform_(-16.0, -1.0, generator=g),
+             2.0 ** torch.arange(-1074, 1024, dtype=torch.float64),
+             torch.tensor([5e-324, 2.2250738585072014e-308, 2.225073858507201e-308, 1.0, 0.7071067811865476, 1.4142135623730951,
+                           1.7976931348623157e308], dtype=torch.float64)]
+    x = torch.cat(parts)
+    got = B.pdf_log_f64(x.cuda()).cpu().numpy()
+    ref = np.log(x.numpy())
+    ulp = np.spacing(np.abs(ref))
+    d = np.abs(got - ref) / np.where(ulp > 0, ulp, 5e-324)
+    assert got[x.numpy() == 1.0].tolist() == [0.0] * int((x == 1.0).sum())
+    print("\npdf_log: max |gpu - glibc| =", d.max(), "ulp; differing:", float(np.mean(d > 0)))
+    assert d.max() <= 1.0
+
+
 @pytest.mark.parametrize("path", PATHS)
 def test_c0_parity(B, oracle_mod, path):
     """configs[0]: 1e5 queries strictly inside the 50x30 single-sub-grid grid"""
