@@ -189,6 +189,40 @@ int pdf_measure_fp64_tflops(double *tflops, void *stream);
  * finite x[i] > 0; DEVICE [n] each.  Tested against the host's log (<= 1 ulp). */
 int pdf_log_f64(long long n, const double *x, double *out, void *stream);
 
+/* ---- Monte Carlo steps around the hot path -----------------------------
+ * All array arguments are DEVICE pointers unless marked HOST; calls enqueue on `stream`.  Random numbers are
+ * inputs (uniforms in [0, 1)): the library draws none. */
+
+/* RAMBO (section 1.3.5, eq. 1.103-1.104, 1.107-1.110, L1101-1180): npart (2..16) final-state momenta
+ * p[nev][npart][4] = (E, px, py, pz) in the frame P = (sqrt_s[e], 0, 0, 0) from the uniforms u[nev][npart][4], and the
+ * weight w[nev]: eq. 1.108 for massless particles (masses == NULL or all 0; HOST [npart]), w0 w_m of eq. 1.110 with
+ * the momenta of eq. 1.109 (xi by Newton's iteration on its energy constraint) otherwise.  ptmin > 0 sets w = 0
+ * for events with a final-state p_T below it (L2070); the momenta are written either way. */
+int pdf_rambo(long long nev, int npart, const double *sqrt_s, const double *masses, const double *u, double ptmin,
+              double *p, double *w, void *stream);
+
+/* VEGAS importance sampling (section 1.3.3): a separable density p(x) = prod_d p_d(x_d) (eq. 1.81), piecewise
+ * constant on nbins equally probable bins per dimension with edges[ndim][nbins + 1].
+ * pdf_vegas_map: u[n][ndim] -> x[n][ndim], jac[n] = 1/p(x) = prod_d nbins * width, bin[n][ndim] (may be NULL).
+ * pdf_vegas_accumulate: sums[0] = sum f jac, sums[1] = sum (f jac)^2 (eq. 1.74-1.75), hist[ndim][nbins] = per-bin sums
+ *   of |f jac| (L913; may be NULL); both are zeroed first.  Across GPUs these are the only numbers to all-reduce.
+ * pdf_vegas_estimate: res[0] = E_N (eq. 1.74), res[1] = variance of E_N (eq. 1.75 over N - 1).
+ * pdf_vegas_refine: new edges = nbins equal shares of the histogram, taken piecewise constant in the old bins and
+ *   damped by the exponent alpha (1 = none; not in the paper); scratch is DEVICE [ndim][2 nbins + 1] doubles.
+ * pdf_vegas_combine: res = {Ebar, S2bar, chi2/dof} of M iterations (eq. 1.82-1.83); E, S2 DEVICE [M]. */
+int pdf_vegas_map(int ndim, int nbins, const double *edges, long long n, const double *u, double *x, double *jac,
+                  int *bin, void *stream);
+int pdf_vegas_accumulate(int ndim, int nbins, long long n, const double *f, const double *jac, const int *bin,
+                         double *sums, double *hist, void *stream);
+int pdf_vegas_estimate(long long n, const double *sums, double *res, void *stream);
+int pdf_vegas_refine(int ndim, int nbins, const double *hist, double alpha, double *edges, double *scratch, void *stream);
+int pdf_vegas_combine(int M, const double *E, const double *S2, double *res, void *stream);
+
+/* unweighting (section 4.1.3): accept[e] = w[e] > u[e] * max_e w[e] (uint8).  scratch16 is 16 DEVICE
+ * bytes; wmax and n_accept (HOST, may be NULL) are read back after a stream synchronise when given. */
+int pdf_unweight(long long n, const double *w, const double *u, unsigned char *accept, void *scratch16,
+                 double *wmax, long long *n_accept, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -18,6 +18,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pdf_oracle.c")
 _HDR = os.path.join(_HERE, "pdf_oracle.h")
+_SRC_MC = os.path.join(_HERE, "mc_oracle.c")
+_HDR_MC = os.path.join(_HERE, "mc_oracle.h")
 _LIB = os.path.join(_HERE, "libpdf_oracle.so")
 
 REGION_INTERIOR, REGION_LOWX, REGION_LOWQ, REGION_HIGHQ = 0, 1, 2, 3
@@ -46,11 +48,11 @@ def build(force: bool = False, variant: str = "") -> str:
     switch of pdf_oracle.c (e.g. "ORACLE_S3_BILINEAR"), built beside the default library."""
     out = _LIB if not variant else os.path.join(_HERE, f"libpdf_oracle_{variant.lower()}.so")
     stale = (not os.path.exists(out)) or any(
-        os.path.getmtime(p) > os.path.getmtime(out) for p in (_SRC, _HDR))
+        os.path.getmtime(p) > os.path.getmtime(out) for p in (_SRC, _HDR, _SRC_MC, _HDR_MC))
     if force or stale:
         cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp",
                "-ffp-contract=off", "-Wall", "-Wextra", *( [f"-D{variant}"] if variant else []),
-               "-o", out + ".tmp", _SRC, "-lm"]
+               "-o", out + ".tmp", _SRC, _SRC_MC, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
         os.replace(out + ".tmp", out)
     return out
@@ -78,6 +80,15 @@ def lib():
         L.oracle_interior_order.argtypes = [vp, C.c_int, C.c_int, C.c_int, ll, dp, dp, dp]
         L.oracle_weights_1d.argtypes = [C.c_int, dp, C.c_double, C.c_int, dp]
         L.oracle_num_threads.restype = C.c_int
+        L.oracle_rambo_w0.argtypes = [C.c_int, C.c_double]
+        L.oracle_rambo_w0.restype = C.c_double
+        L.oracle_rambo.argtypes = [ll, C.c_int, dp, dp, dp, C.c_double, dp, dp]
+        L.oracle_vegas_map.argtypes = [C.c_int, C.c_int, dp, ll, dp, dp, dp, ip]
+        L.oracle_vegas_accumulate.argtypes = [C.c_int, C.c_int, ll, dp, dp, ip, dp, dp]
+        L.oracle_vegas_estimate.argtypes = [ll, dp, dp, dp]
+        L.oracle_vegas_refine.argtypes = [C.c_int, C.c_int, dp, C.c_double, dp]
+        L.oracle_vegas_combine.argtypes = [C.c_int, dp, dp, dp, dp, dp]
+        L.oracle_unweight.argtypes = [ll, dp, dp, dp, C.POINTER(C.c_ubyte), C.POINTER(ll)]
         _lib = L
     return _lib
 
@@ -212,3 +223,86 @@ class OracleGrid:
         if rc:
             raise ValueError(f"oracle_interior_order: {rc}")
         return out
+
+
+# ---- Monte Carlo steps around the hot path (mc_oracle.c) -------------
+def rambo_w0(n: int, s: float) -> float:
+    return float(lib().oracle_rambo_w0(int(n), float(s)))
+
+
+def rambo(sqrt_s, u, masses=None, ptmin: float = 0.0):
+    """u[nev][n][4] uniforms -> (p[nev][n][4] = (E, px, py, pz), w[nev])"""
+    u, up = _d(u)
+    nev, n = u.shape[0], u.shape[1]
+    rs, rp = _d(np.broadcast_to(np.asarray(sqrt_s, dtype=np.float64), (nev,)))
+    mp = None
+    if masses is not None:
+        masses, mp = _d(masses)
+    p, w = np.empty((nev, n, 4)), np.empty(nev)
+    rc = lib().oracle_rambo(nev, n, rp, mp, up, float(ptmin), p.ctypes.data_as(C.POINTER(C.c_double)),
+                            w.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc:
+        raise ValueError(f"oracle_rambo: {rc}")
+    return p, w
+
+
+def vegas_map(edges, u):
+    e, ep = _d(edges)
+    u, up = _d(u)
+    n, ndim = u.shape
+    nb = e.shape[1] - 1
+    x, jac, bins = np.empty((n, ndim)), np.empty(n), np.empty((n, ndim), dtype=np.int32)
+    rc = lib().oracle_vegas_map(ndim, nb, ep, n, up, x.ctypes.data_as(C.POINTER(C.c_double)),
+                                jac.ctypes.data_as(C.POINTER(C.c_double)), bins.ctypes.data_as(C.POINTER(C.c_int)))
+    if rc:
+        raise ValueError(f"oracle_vegas_map: {rc}")
+    return x, jac, bins
+
+
+def vegas_accumulate(nb: int, f, jac, bins):
+    f, fp = _d(f)
+    j, jp = _d(jac)
+    b, bp = _i(bins)
+    ndim = b.shape[1]
+    sums, hist = np.empty(2), np.empty((ndim, nb))
+    rc = lib().oracle_vegas_accumulate(ndim, nb, f.size, fp, jp, bp, sums.ctypes.data_as(C.POINTER(C.c_double)),
+                                       hist.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc:
+        raise ValueError(f"oracle_vegas_accumulate: {rc}")
+    return sums, hist
+
+
+def vegas_estimate(n: int, sums):
+    s, sp = _d(sums)
+    E, var = C.c_double(), C.c_double()
+    if lib().oracle_vegas_estimate(int(n), sp, C.byref(E), C.byref(var)):
+        raise ValueError("oracle_vegas_estimate")
+    return E.value, var.value
+
+
+def vegas_refine(hist, edges, alpha: float = 1.0):
+    h, hp = _d(hist)
+    e = np.array(edges, dtype=np.float64, order="C")
+    ndim, nb = h.shape
+    if lib().oracle_vegas_refine(ndim, nb, hp, float(alpha), e.ctypes.data_as(C.POINTER(C.c_double))):
+        raise ValueError("oracle_vegas_refine")
+    return e
+
+
+def vegas_combine(E, S2):
+    E, Ep = _d(E)
+    S, Sp = _d(S2)
+    a, b, c = C.c_double(), C.c_double(), C.c_double()
+    if lib().oracle_vegas_combine(E.size, Ep, Sp, C.byref(a), C.byref(b), C.byref(c)):
+        raise ValueError("oracle_vegas_combine")
+    return a.value, b.value, c.value
+
+
+def unweight(w, u):
+    w, wp = _d(w)
+    u, up = _d(u)
+    acc = np.empty(w.size, dtype=np.uint8)
+    wmax, cnt = C.c_double(), C.c_longlong()
+    if lib().oracle_unweight(w.size, wp, up, C.byref(wmax), acc.ctypes.data_as(C.POINTER(C.c_ubyte)), C.byref(cnt)):
+        raise ValueError("oracle_unweight")
+    return wmax.value, acc.astype(bool), int(cnt.value)

@@ -32,6 +32,8 @@ SYMBOLS = (
     "pdf_xfxq2_host", "pdf_alphas_q2_host", "pdf_lumi_host", "pdf_status_string",
     "pdf_last_cuda_error", "pdf_launch_count", "pdf_profile_enable", "pdf_profile_read",
     "pdf_measure_fp64_tflops", "pdf_last_path", "pdf_log_f64",
+    "pdf_rambo", "pdf_vegas_map", "pdf_vegas_accumulate", "pdf_vegas_estimate", "pdf_vegas_refine", "pdf_vegas_combine",
+    "pdf_unweight",
 )
 
 
@@ -80,6 +82,13 @@ def lib():
     L.pdf_measure_fp64_tflops.argtypes = [dp, vp]
     L.pdf_last_path.argtypes = [vp]
     L.pdf_log_f64.argtypes = [ll, vp, vp, vp]
+    L.pdf_rambo.argtypes = [ll, C.c_int, vp, dp, vp, C.c_double, vp, vp, vp]
+    L.pdf_vegas_map.argtypes = [C.c_int, C.c_int, vp, ll, vp, vp, vp, vp, vp]
+    L.pdf_vegas_accumulate.argtypes = [C.c_int, C.c_int, ll, vp, vp, vp, vp, vp, vp]
+    L.pdf_vegas_estimate.argtypes = [ll, vp, vp, vp]
+    L.pdf_vegas_refine.argtypes = [C.c_int, C.c_int, vp, C.c_double, vp, vp, vp]
+    L.pdf_vegas_combine.argtypes = [C.c_int, vp, vp, vp, vp]
+    L.pdf_unweight.argtypes = [ll, vp, vp, vp, vp, dp, C.POINTER(ll), vp]
     _lib = L
     return L
 
@@ -155,6 +164,77 @@ def pdf_log_f64(x: torch.Tensor, stream=None) -> torch.Tensor:
     out = torch.empty_like(x)
     _check(lib().pdf_log_f64(x.numel(), _dev(x, torch.float64, "x"), _dev(out, torch.float64, "out"), _stream_ptr(stream)), "pdf_log_f64")
     return out
+
+
+# ---- Monte Carlo steps around the hot path (argument marshalling only) -------------------------------------
+def pdf_rambo(sqrt_s: torch.Tensor, u: torch.Tensor, masses=None, ptmin: float = 0.0, stream=None):
+    """u [nev][npart][4] uniforms -> (p [nev][npart][4], w [nev])"""
+    nev, npart = u.shape[0], u.shape[1]
+    f = torch.float64
+    p = torch.empty((nev, npart, 4), dtype=f, device=u.device)
+    w = torch.empty(nev, dtype=f, device=u.device)
+    m = _hd(masses) if masses is not None else None
+    if m is not None and m.numel() != npart:
+        raise PdfGridError("masses must have npart entries")
+    _check(lib().pdf_rambo(nev, npart, _dev(sqrt_s, f, "sqrt_s", nev), _dptr(m) if m is not None else None,
+                           _dev(u, f, "u", nev * npart * 4), float(ptmin), _dev(p, f, "p"), _dev(w, f, "w"), _stream_ptr(stream)),
+           "pdf_rambo")
+    return p, w
+
+
+def pdf_vegas_map(edges: torch.Tensor, u: torch.Tensor, stream=None):
+    ndim, nb = edges.shape[0], edges.shape[1] - 1
+    n = u.shape[0]
+    f = torch.float64
+    x = torch.empty((n, ndim), dtype=f, device=u.device)
+    jac = torch.empty(n, dtype=f, device=u.device)
+    bins = torch.empty((n, ndim), dtype=torch.int32, device=u.device)
+    _check(lib().pdf_vegas_map(ndim, nb, _dev(edges, f, "edges"), n, _dev(u, f, "u", n * ndim), _dev(x, f, "x"), _dev(jac, f, "jac"),
+                               _dev(bins, torch.int32, "bin"), _stream_ptr(stream)), "pdf_vegas_map")
+    return x, jac, bins
+
+
+def pdf_vegas_accumulate(nb: int, fvals: torch.Tensor, jac: torch.Tensor, bins: torch.Tensor, stream=None):
+    n, ndim = bins.shape
+    f = torch.float64
+    sums = torch.empty(2, dtype=f, device=jac.device)
+    hist = torch.empty((ndim, nb), dtype=f, device=jac.device)
+    _check(lib().pdf_vegas_accumulate(ndim, nb, n, _dev(fvals, f, "f", n), _dev(jac, f, "jac", n), _dev(bins, torch.int32, "bin"),
+                                      _dev(sums, f, "sums"), _dev(hist, f, "hist"), _stream_ptr(stream)), "pdf_vegas_accumulate")
+    return sums, hist
+
+
+def pdf_vegas_estimate(n: int, sums: torch.Tensor, stream=None):
+    res = torch.empty(2, dtype=torch.float64, device=sums.device)
+    _check(lib().pdf_vegas_estimate(n, _dev(sums, torch.float64, "sums", 2), _dev(res, torch.float64, "res"), _stream_ptr(stream)),
+           "pdf_vegas_estimate")
+    return res
+
+
+def pdf_vegas_refine(hist: torch.Tensor, edges: torch.Tensor, alpha: float = 1.0, stream=None):
+    """refines `edges` in place"""
+    ndim, nb = hist.shape
+    scratch = torch.empty((ndim, 2 * nb + 1), dtype=torch.float64, device=hist.device)
+    _check(lib().pdf_vegas_refine(ndim, nb, _dev(hist, torch.float64, "hist"), float(alpha), _dev(edges, torch.float64, "edges", ndim * (nb + 1)),
+                                  _dev(scratch, torch.float64, "scratch"), _stream_ptr(stream)), "pdf_vegas_refine")
+    return edges
+
+
+def pdf_vegas_combine(E: torch.Tensor, S2: torch.Tensor, stream=None):
+    res = torch.empty(3, dtype=torch.float64, device=E.device)
+    _check(lib().pdf_vegas_combine(E.numel(), _dev(E, torch.float64, "E"), _dev(S2, torch.float64, "S2", E.numel()),
+                                   _dev(res, torch.float64, "res"), _stream_ptr(stream)), "pdf_vegas_combine")
+    return res
+
+
+def pdf_unweight(w: torch.Tensor, u: torch.Tensor, stream=None):
+    n = w.numel()
+    acc = torch.empty(n, dtype=torch.uint8, device=w.device)
+    scratch = torch.empty(16, dtype=torch.uint8, device=w.device)
+    wmax, cnt = C.c_double(), C.c_longlong()
+    _check(lib().pdf_unweight(n, _dev(w, torch.float64, "w"), _dev(u, torch.float64, "u", n), _dev(acc, torch.uint8, "accept"),
+                              _dev(scratch, torch.uint8, "scratch"), C.byref(wmax), C.byref(cnt), _stream_ptr(stream)), "pdf_unweight")
+    return wmax.value, acc.bool(), int(cnt.value)
 
 
 class PdfGrid:

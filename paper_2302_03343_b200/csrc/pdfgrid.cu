@@ -14,6 +14,7 @@
 #include "pdf_common.cuh"
 #include "pdf_generic.cuh"
 #include "pdf_stream.cuh"
+#include "mc_kernels.cuh"
 
 using namespace pdfg;
 
@@ -336,3 +337,4 @@ int pdf_grid_limits(const pdf_grid *g, double *xmin, double *xmax, double *q2min
 }  // extern "C"
 
 #include "pdfgrid_eval.inl"
+#include "mc_entry.inl"

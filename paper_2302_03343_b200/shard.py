@@ -19,3 +19,14 @@ def max_over_ranks(dist, seconds: float, device="cpu") -> float:
     t = torch.tensor([seconds], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def vegas_allreduce(dist, sums, hist=None):
+    """The one exchange step of the widened path: every rank samples its own share of an
+    iteration's points, so the sums of eq. 1.74-1.75 and the refinement histograms (L913) are
+    added over the ranks -- one all-reduce of 2 + ndim * nbins doubles per iteration (NCCL on GPUs, gloo in the CPU
+    tests); every rank then refines the same grid from the same histogram."""
+    dist.all_reduce(sums, op=dist.ReduceOp.SUM)
+    if hist is not None:
+        dist.all_reduce(hist, op=dist.ReduceOp.SUM)
+    return sums, hist

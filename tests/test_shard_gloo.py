@@ -75,3 +75,41 @@ def test_table33_generator_shape():
     assert torch.equal(x[:2415], xg) and torch.equal(x[2415:4830], xg)
     assert torch.equal(mem, torch.arange(3, dtype=torch.int32).repeat_interleave(2415))
     assert bool((q2 == synth.TABLE33_Q2).all())
+
+
+def _vegas_worker(rank, world, port, n, outdir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle
+    oracle.build()
+    nb = 16
+    edges = np.tile(np.linspace(0.0, 1.0, nb + 1), (2, 1))
+    u = np.random.default_rng(77).random((n, 2))
+    lo, hi = shard.shard_range(n, rank, world)
+    x, jac, bins = oracle.vegas_map(edges, u[lo:hi])
+    f = np.exp(-((x - 0.3) ** 2).sum(axis=1) / 0.02)
+    sums, hist = oracle.vegas_accumulate(nb, f, jac, bins)
+    ts, th = torch.tensor(sums), torch.tensor(hist)
+    shard.vegas_allreduce(dist, ts, th)
+    new = oracle.vegas_refine(th.numpy(), edges)
+    np.save(os.path.join(outdir, f"vegas{rank}.npy"), np.concatenate([ts.numpy(), th.numpy().ravel(), new.ravel()]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_vegas_sums_allreduce_two_ranks(tmp_path, oracle_mod):
+    """NEXT-1's only collective: two ranks sample halves of an iteration, all-reduce the sums and histograms, and both
+    end with the single-rank estimate and the single-rank refined grid"""
+    n, world, nb = 40_001, 2, 16
+    mp.spawn(_vegas_worker, args=(world, _free_port(), n, str(tmp_path)), nprocs=world, join=True)
+    a, b = np.load(tmp_path / "vegas0.npy"), np.load(tmp_path / "vegas1.npy")
+    assert np.array_equal(a, b)
+    edges = np.tile(np.linspace(0.0, 1.0, nb + 1), (2, 1))
+    u = np.random.default_rng(77).random((n, 2))
+    x, jac, bins = oracle_mod.vegas_map(edges, u)
+    f = np.exp(-((x - 0.3) ** 2).sum(axis=1) / 0.02)
+    sums, hist = oracle_mod.vegas_accumulate(nb, f, jac, bins)
+    new = oracle_mod.vegas_refine(hist, edges)
+    want = np.concatenate([sums, hist.ravel(), new.ravel()])
+    assert np.max(np.abs(a - want) / (np.abs(want) + 1e-300)) < 1e-12
