@@ -133,7 +133,14 @@ struct StreamArgs {
     // inside one member's run; ctab[c] = {first query, queries, member, 0}, *nchunks_dev chunks.
     const int *ctab;
     const int *nchunks_dev;
+    // fused luminosity (a-7): pass 1 (k_lumi_first) writes rows [xf_0..xf_10, w/(x1 x2)] of 12 doubles into `out` (the
+    // scratch), pass 2 (k_lumi_second) reads them back as `f1` and reduces the coupling against its own row on the fly
+    const double *x2, *w;      // pass 1: the other parton's x and the event weight (for the scale column)
+    const double *f1;          // pass 2: the rows of pass 1
+    const double *coup;        // pass 2: C[i][j] as [12][16] doubles, zero padded
 };
+constexpr int kModeRows = 0, kModeLumiFirst = 1, kModeLumiSecond = 2;
+constexpr int kCoupBytes = kNFP * 16 * 8;
 
 // ---- small device helpers ----------------------------------------------------------------------
 // explicit shared-window accessors (32-bit addresses)
@@ -184,10 +191,10 @@ __device__ __forceinline__ unsigned long long warp_release_add(unsigned long lon
     return __shfl_sync(0xffffffffu, old, 0);
 }
 // one payload = one 32-byte sector, stored whole (STG.256): never a partial-sector write
-__device__ __forceinline__ void store_payload(Payload *dst, double a, double b, unsigned idx, unsigned cell)
+__device__ __forceinline__ void store_payload(Payload *dst, double a, double b, unsigned idx, unsigned cell, double pad = 0.0)
 {
     const double w2 = __hiloint2double((int)cell, (int)idx);       // low word idx, high word cell
-    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(dst), "d"(a), "d"(b), "d"(w2), "d"(0.0) : "memory");
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(dst), "d"(a), "d"(b), "d"(w2), "d"(pad) : "memory");
 }
 __device__ __forceinline__ void cp_async16_cg(unsigned saddr, const void *g)
 {
@@ -272,6 +279,7 @@ __device__ __forceinline__ void zero_fill_warp(double *out, long long ld, long l
     if (lane < (int)(e - p)) p[lane] = 0.0;
 }
 
+template <int MODE>
 __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, int slot, long long chunk_base, long long chunk_end,
                                        int tile, unsigned long long &err_local)
 {
@@ -298,12 +306,15 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
     const double inv_qmin = 1.0 / __longlong_as_double(qminb);
 #pragma unroll 1
     for (int g0 = 0; g0 < kS3TileQ; g0 += kS3Grp) {
-        double xv[kS3Grp], qv[kS3Grp];
+        double xv[kS3Grp], qv[kS3Grp], sc[kS3Grp];
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
             const long long e = t0 + (g0 + q) * 32 + lane;
-            xv[q] = 1.0; qv[q] = 1.0;
-            if (e < t1) { xv[q] = __ldcs(A.x + e); qv[q] = __ldcs(A.q2 + e); }
+            xv[q] = 1.0; qv[q] = 1.0; sc[q] = 0.0;
+            if (e < t1) {
+                xv[q] = __ldcs(A.x + e); qv[q] = __ldcs(A.q2 + e);
+                if (MODE == kModeLumiFirst) sc[q] = __ldcs(A.w + e) / (xv[q] * __ldcs(A.x2 + e));   // f = xf / x on both sides (eq. 3.3)
+            }
         }
         Located L[kS3Grp];
 #pragma unroll
@@ -369,10 +380,11 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
             const unsigned idx = (unsigned)(e - chunk_base);
             if (key[q] == INT_MIN) {                                              // C-10: NaN row, counted
                 double *o = A.out + e * A.ld;
-                for (int p = 0; p < A.cm.n; ++p) o[p] = qnan();
+                const int ncol = MODE == kModeLumiFirst ? kNFP : A.cm.n;
+                for (int p = 0; p < ncol; ++p) o[p] = qnan();
                 if (A.count_err) ++err_local;
-            } else if (key[q] < 0) store_payload(lists + (size_t)(-1 - key[q]) * A.chunk + pos[q], pa[q], pb[q], idx, cell[q]);
-            else store_payload(bins + (size_t)key[q] * B.cap + pos[q], pa[q], pb[q], idx, cell[q]);
+            } else if (key[q] < 0) store_payload(lists + (size_t)(-1 - key[q]) * A.chunk + pos[q], pa[q], pb[q], idx, cell[q], sc[q]);
+            else store_payload(bins + (size_t)key[q] * B.cap + pos[q], pa[q], pb[q], idx, cell[q], sc[q]);
         }
     }
 }
@@ -436,8 +448,10 @@ __device__ __forceinline__ void store_row(const StreamArgs &A, double *rp, int t
 // through the warp's stages: two payload stages (batch parity) and two value stages (cell parity; a cell's 16 node
 // rows, node n = 4 * (Q2 row) + (x node)).  The fragments are re-read from the value stage per 8-query tile (8
 // LDS.64): held in registers across the loop they spilled to local memory at 80 registers (profile r2f).
+template <int MODE>
 __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, const double *__restrict__ Vm, int slot,
-                                       long long chunk_base, int i, int fk0, int fk1, unsigned sbuf)
+                                       long long chunk_base, int i, int fk0, int fk1, unsigned sbuf, unsigned sC,
+                                       unsigned long long &err_local)
 {
     const GridDev &G = A.G;
     const StreamDev &B = A.B;
@@ -513,6 +527,14 @@ __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, 
                 const int qn = m0 + 8 + g;
                 vn = qn < nact;
                 if (vn) { abn = lds_v2f64(sb + 32u * qn); idxn = lds_u32(sb + 32u * qn + 16u); }
+                // pass 2 of the luminosity: this query's row of pass 1 in the A-operand layout (flavour 4 s + t), fetched
+                // under the contraction; lane t = 3 of step 2 gets the scale column.  (Fetching it one tile ahead costs 6
+                // more registers, which spill: measured 12.25 against 11.80 ms per 1e8 events.)
+                double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+                if (MODE == kModeLumiSecond && valid) {
+                    const double *fr = A.f1 + (chunk_base + idx) * kNFP + t;
+                    a0 = __ldcs(fr); a1 = __ldcs(fr + 4); a2 = __ldcs(fr + 8);
+                }
                 const double wx = valid ? weight_eval(kx, tx) : 0.0;
                 const double wq0 = weight_eval(kq, tq);
                 const double wq1 = __shfl_xor_sync(0xffffffffu, wq0, 1);
@@ -527,7 +549,37 @@ __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, 
                     f.y = g < 4 ? lds_f64(pn + 64u) : 0.0;
                     kstep(d, (r == 0 ? wq0 : r == 1 ? wq1 : r == 2 ? wq2 : wq3) * wx, f);
                 }
-                if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, d);
+                if (MODE == kModeRows) {
+                    if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, d);
+                } else if (MODE == kModeLumiFirst) {
+                    // rows of 12 on 32-byte sectors: two stores write the three sectors whole (no zero fill needed)
+                    if (valid) {
+                        double *rp = A.out + (chunk_base + idx) * kNFP;
+                        *reinterpret_cast<double2 *>(rp + 2 * t) = make_double2(d.d00, d.d01);
+                        if (t == 0) *reinterpret_cast<double2 *>(rp + 8) = make_double2(d.d10, d.d11);
+                        if (t == 1) *reinterpret_cast<double2 *>(rp + 10) = make_double2(d.d10, lds_f64(sb + 32u * (m0 + g) + 24u));
+                    }
+                } else {
+                    // G[q][j] = sum_i f1[q][i] C[i][j] by 6 more DMMAs, then the dot with this row and the scale
+                    Acc gq = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                    for (int s = 0; s < 3; ++s) {
+                        const unsigned pc = sC + (unsigned)((4 * s + t) * 128 + 8 * g);
+                        double2 cf;
+                        cf.x = lds_f64(pc);
+                        cf.y = g < 4 ? lds_f64(pc + 64u) : 0.0;
+                        kstep(gq, s == 0 ? a0 : s == 1 ? a1 : (t == 3 ? 0.0 : a2), cf);
+                    }
+                    double dot = fma(d.d00, gq.d00, fma(d.d01, gq.d01, fma(d.d10, gq.d10, d.d11 * gq.d11)));
+                    dot += __shfl_xor_sync(0xffffffffu, dot, 1);
+                    dot += __shfl_xor_sync(0xffffffffu, dot, 2);
+                    const double scale = __shfl_sync(0xffffffffu, a2, lane | 3);
+                    if (valid && t == 0) {
+                        double v = scale * dot;
+                        if (v != v && a0 != a0) { v = qnan(); if (A.count_err) ++err_local; }   // the x1 parton was invalid (C-10): counted once
+                        A.out[chunk_base + idx] = v;
+                    }
+                }
             }
         }
         __syncwarp();                                           // the stages are free for the copies after next
@@ -641,8 +693,27 @@ __device__ __noinline__ void list_row(const StreamArgs &A, const double *__restr
 }
 
 // claims batches of 32 entries from the chunk's lists until they are drained
+// pass 2 of the luminosity for a list entry: w/(x1 x2) sum_ij f1_i C_ij f2_j with C broadcast from shared memory
+__device__ __noinline__ double list_lumi(const double *__restrict__ fr, unsigned sC, const double v[kNFP], bool &x1_invalid)
+{
+    double f1[kNFP];
+#pragma unroll
+    for (int p = 0; p < 6; ++p) { const double2 u = __ldcs(reinterpret_cast<const double2 *>(fr) + p); f1[2 * p] = u.x; f1[2 * p + 1] = u.y; }
+    double acc = 0.0;
+#pragma unroll
+    for (int i = 0; i < kNF; ++i) {
+        double row = 0.0;
+#pragma unroll
+        for (int j = 0; j < kNF; ++j) row = fma(lds_f64(sC + (unsigned)(i * 128 + 8 * j)), v[j], row);
+        acc = fma(f1[i], row, acc);
+    }
+    x1_invalid = f1[0] != f1[0];
+    return f1[11] * acc;
+}
+
+template <int MODE>
 __device__ __forceinline__ void e_unit(const StreamArgs &A, const double *__restrict__ Vm, const double *__restrict__ RPm, int slot,
-                                       long long chunk_base)
+                                       long long chunk_base, unsigned sC, unsigned long long &err_local)
 {
     const StreamDev &B = A.B;
     const int lane = threadIdx.x & 31;
@@ -664,15 +735,31 @@ __device__ __forceinline__ void e_unit(const StreamArgs &A, const double *__rest
         const bool active = first + lane < n;
         double a = 0.5, b = 0.5;
         unsigned idx = 0, cell = 0;
+        double pad = 0.0;
         if (active) {
             const Payload *e = lists + (size_t)list * A.chunk + first + lane;
             const double2 ab = __ldcg(reinterpret_cast<const double2 *>(e));
             const uint2 ic = __ldcg(reinterpret_cast<const uint2 *>(e) + 2);
             a = ab.x; b = ab.y; idx = ic.x; cell = ic.y;
+            if (MODE == kModeLumiFirst) pad = __ldcg(reinterpret_cast<const double *>(e) + 3);
         }
         double v[kNFP];
         list_row(A, Vm, RPm, list, a, b, cell, v);
-        if (active) {
+        if (MODE == kModeLumiFirst) {
+            if (active) {
+                double2 *o = reinterpret_cast<double2 *>(A.out + (chunk_base + idx) * kNFP);
+                v[11] = pad;
+#pragma unroll
+                for (int p = 0; p < 6; ++p) o[p] = make_double2(v[2 * p], v[2 * p + 1]);
+            }
+        } else if (MODE == kModeLumiSecond) {
+            if (active) {
+                bool bad;
+                double r = list_lumi(A.f1 + (chunk_base + idx) * kNFP, sC, v, bad);
+                if (bad) { r = qnan(); if (A.count_err) ++err_local; }                     // the x1 parton was invalid (C-10): counted once
+                A.out[chunk_base + idx] = r;
+            }
+        } else if (active) {
             double *o = A.out + (chunk_base + idx) * A.ld;
             if (A.identity) {
 #pragma unroll
@@ -749,7 +836,8 @@ k_locate_stream(const __grid_constant__ GridDev G, const __grid_constant__ Strea
     }
 }
 
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __grid_constant__ StreamArgs A)
+template <int MODE>
+__device__ __forceinline__ void stream_body(const StreamArgs &A)
 {
     extern __shared__ __align__(32) unsigned char smem_raw[];
     const StreamTab T = s3_stage_tables(A.G, A.B, smem_raw, kS3Threads);
@@ -757,6 +845,12 @@ __global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __
     __syncthreads();                                   // the only CTA barrier: every warp works alone from here on
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned sbuf = ((stage0 + 31u) & ~31u) + (unsigned)(warp * kStageBytes);
+    const unsigned sC = ((stage0 + 31u) & ~31u) + (unsigned)(kS3Warps * kStageBytes);       // the coupling table (pass 2)
+    if (MODE == kModeLumiSecond) {
+        for (int k = threadIdx.x; k < kCoupBytes / 8; k += kS3Threads)
+            asm volatile("st.shared.f64 [%0], %1;" ::"r"(sC + 8u * k), "d"(__ldg(A.coup + k)) : "memory");
+        __syncthreads();
+    }
 
     unsigned long long *ctrl = A.W.ctrl;
     const StreamDev &B = A.B;
@@ -815,15 +909,15 @@ __global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __
         if (isA) {
             // the ring slot must have been drained by the units of chunk c - kS3Ring before this tile touches its bins
             if (gen) wait_for(b_done, gen * TB);
-            a_tile(A, T, slot, chunk_base, chunk_end, sub, err_local);
+            a_tile<MODE>(A, T, slot, chunk_base, chunk_end, sub, err_local);
             warp_release_add(a_done, 1ULL);
         } else {
             wait_for(a_done, (gen + 1) * TA);                      // every tile of A(c) has been released
-            if (sub < B.ne) e_unit(A, V, RP, slot, chunk_base);    // list units first: their queries are the expensive ones
+            if (sub < B.ne) e_unit<MODE>(A, V, RP, slot, chunk_base, sC, err_local);   // list units first: their queries are the expensive ones
             else {
                 const int v = sub - B.ne;
                 const int i = v / B.ng, grp = v - i * B.ng;
-                b_unit(A, T, V, slot, chunk_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf);
+                b_unit<MODE>(A, T, V, slot, chunk_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf, sC, err_local);
             }
             const unsigned long long old = warp_release_add(b_fin, 1ULL);
             if (old + 1 == (gen + 1) * TB) {                       // last unit of the chunk: the slot's counters are reset for the ring
@@ -835,6 +929,10 @@ __global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __
     }
     if (err_local) atomicAdd(A.G.err_count, err_local);
 }
+
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __grid_constant__ StreamArgs A) { stream_body<kModeRows>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_first(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiFirst>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_second(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiSecond>(A); }
 
 __host__ __device__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 

@@ -15,6 +15,7 @@ struct StreamPlan {
     StreamDev dev{};
     unsigned short *d_lutx = nullptr, *d_lutq = nullptr;
     double *d_rowplus = nullptr;              // [nmem][nx][12] values at 1.01*Q2min (C-9's second anchor row)
+    double *d_coup = nullptr;                 // [12][16] zero-padded coupling of the call in flight (pass 2 of pdf_lumi)
     double *d_plus = nullptr;                 // scratch of k_q2plus
     int ncells_q = 1;                         // Q2 cells (knots - sub-grids)
     bool locate_ok = false;                   // the search tables exist (pdf_locate can run this path's search)
@@ -56,7 +57,7 @@ __global__ void k_rowplus(GridDev G, int jgplus, double tqplus, double *__restri
 
 inline void stream_plan_free(StreamPlan &p)
 {
-    cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_rowplus); cudaFree(p.d_plus);
+    cudaFree(p.d_lutx); cudaFree(p.d_lutq); cudaFree(p.d_rowplus); cudaFree(p.d_plus); cudaFree(p.d_coup); p.d_coup = nullptr;
     p.d_lutx = p.d_lutq = nullptr; p.d_rowplus = nullptr; p.d_plus = nullptr; p.usable = false; p.locate_ok = false;
 }
 
@@ -128,7 +129,7 @@ inline void stream_carve(void *ws, long long chunk, const StreamDev &d, StreamWo
 
 inline size_t stream_smem_bytes(const GridDev &G, const StreamDev &d)
 {
-    return s3_table_bytes(G.nx, G.nqtot, d.nbx, d.nbq) + 32 + (size_t)kS3Warps * kStageBytes;
+    return s3_table_bytes(G.nx, G.nqtot, d.nbx, d.nbq) + 32 + (size_t)kS3Warps * kStageBytes + kCoupBytes;
 }
 
 // builds the search tables and the key geometry; leaves usable = false when the grid does not fit the
@@ -173,6 +174,9 @@ inline int stream_plan_init(StreamPlan &p, const GridDev &G, const std::vector<d
     const size_t smem = stream_smem_bytes(G, d);
     if (smem > 200 * 1024) return 0;
     if (cudaFuncSetAttribute(k_pdf_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (cudaFuncSetAttribute(k_lumi_first, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (cudaFuncSetAttribute(k_lumi_second, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (cudaMalloc((void **)&p.d_coup, kCoupBytes) != cudaSuccess) return PDF_ENOMEM;
     p.usable = true;
     return 0;
 }
@@ -187,11 +191,13 @@ inline bool stream_members_qualifies(const StreamPlan &p, const GridDev &G, cons
 template <typename Scope>
 inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm, long long n, const double *x,
                         const double *q2, double *out, long long ld, void *ws, size_t ws_bytes, long long chunk_opt,
-                        cudaStream_t s, int count_err = 1, const int *ctab = nullptr, const int *nchunks_dev = nullptr)
+                        cudaStream_t s, int count_err = 1, const int *ctab = nullptr, const int *nchunks_dev = nullptr,
+                        int mode = kModeRows, const double *x2 = nullptr, const double *w = nullptr, const double *f1 = nullptr)
 {
     if (stream_workspace_bytes(p, n, chunk_opt) > ws_bytes) return PDF_EWORKSPACE;
     StreamArgs A;
     A.ctab = ctab; A.nchunks_dev = nchunks_dev;
+    A.x2 = x2; A.w = w; A.f1 = f1; A.coup = p.d_coup;
     A.G = G; A.cm = cm;
     A.chunk = stream_chunk(p, n, chunk_opt);
     stream_caps(p, A.chunk, A.B);
@@ -201,7 +207,7 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     A.ta = (int)(A.chunk / kS3TileA);
     A.identity = cm.n == kNF;
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
-    A.zfill = (ld == cm.n) ? 1 : 0;
+    A.zfill = (ld == cm.n && mode != kModeLumiFirst) ? 1 : 0;
     A.count_err = count_err;
     const size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts
     if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
@@ -209,7 +215,8 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     int per_sm = 0, dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_pdf_stream, kS3Threads, smem) != cudaSuccess || per_sm < 1)
+    const auto kern = mode == kModeLumiFirst ? k_lumi_first : mode == kModeLumiSecond ? k_lumi_second : k_pdf_stream;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kS3Threads, smem) != cudaSuccess || per_sm < 1)
         return PDF_ECUDA;
     const unsigned long long max_ctas = (unsigned long long)per_sm * sms;         // all CTAs must be co-resident
     // with a chunk table the chunk count is on the device: the launch takes its upper bound
@@ -218,8 +225,8 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     const unsigned long long want = (tickets + kS3Warps - 1) / kS3Warps;
     const unsigned grid = (unsigned)(want < max_ctas ? want : max_ctas);
     {
-        Scope sc(s, "k_pdf_stream");
-        k_pdf_stream<<<grid, kS3Threads, smem, s>>>(A);
+        Scope sc(s, mode == kModeLumiFirst ? "k_lumi_first" : mode == kModeLumiSecond ? "k_lumi_second" : "k_pdf_stream");
+        kern<<<grid, kS3Threads, smem, s>>>(A);
     }
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }
@@ -238,47 +245,21 @@ inline int stream_locate(const GridDev &G, const StreamPlan &p, long long n, con
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }
 
-// ---- luminosity on top of the binned path ------------------------------------------------------
-// pdf_lumi in slices of kLumiSlice events: xf(x1,Q2) and xf(x2,Q2) of the slice by two runs of the
-// persistent kernel into two scratch arrays, then k_lumi_combine reduces the 11 x 11 coupling
-// per event in registers.
+// ---- luminosity on top of the binned path (a-7) ------------------------------------------------
+// pdf_lumi in slices of kLumiSlice events, two runs of the persistent kernel per slice:
+//   k_lumi_first   bins the events by the cell of (x1, Q2) and writes rows [xf_0..xf_10(x1, Q2), w/(x1 x2)] of 12
+//                  doubles -- whole 32-byte sectors, so no zero fill -- into the slice's scratch;
+//   k_lumi_second  bins them by the cell of (x2, Q2); its epilogue reads the event's row of pass 1 straight into DMMA
+//                  A-operand fragments, forms G = f1 C by 6 more DMMAs, dots it with its own accumulator fragments and
+//                  writes the 8-byte result.  The 88 B / event of xf(x2) never leave the registers and there is no
+//                  separate reduction kernel.
 constexpr long long kLumiSlice = 1LL << 24;
-
-struct CouplingParam { double c[kNF * kNF]; };            // passed by value: constant-bank operands
-
-__global__ void __launch_bounds__(256)
-k_lumi_combine(const __grid_constant__ CouplingParam C, long long n, const double *__restrict__ f1,
-               const double *__restrict__ f2, const double *__restrict__ x1, const double *__restrict__ x2,
-               const double *__restrict__ w, double *__restrict__ out, unsigned long long *err_count)
-{
-    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n) return;
-    const double a = __ldcs(x1 + e), b = __ldcs(x2 + e);
-    double h[kNF];
-    const double inv_b = 1.0 / b, inv_a = 1.0 / a;
-#pragma unroll
-    for (int j = 0; j < kNF; ++j) h[j] = __ldcs(f2 + e * kNF + j) * inv_b;
-    double acc = 0.0;
-#pragma unroll
-    for (int i = 0; i < kNF; ++i) {
-        double row = 0.0;
-#pragma unroll
-        for (int j = 0; j < kNF; ++j) row = fma(C.c[i * kNF + j], h[j], row);
-        acc = fma(__ldcs(f1 + e * kNF + i) * inv_a, row, acc);
-    }
-    const double v = __ldcs(w + e) * acc;
-    if (!(finite_pos(a) && finite_pos(b)) || v != v) {
-        // an invalid parton made its whole row NaN (C-10); the event counts once
-        if (isnan(__ldcs(f1 + e * kNF)) || isnan(__ldcs(f2 + e * kNF))) { atomicAdd(err_count, 1ULL); out[e] = qnan(); return; }
-    }
-    out[e] = v;
-}
 
 inline bool stream_lumi_qualifies(const StreamPlan &p) { return p.usable; }
 inline size_t stream_lumi_scratch_bytes(const StreamPlan &p, long long n)
 {
     const long long slice = n < kLumiSlice ? n : kLumiSlice;
-    return p.usable ? (size_t)2 * slice * kNF * sizeof(double) + 512 : 0;
+    return p.usable ? (size_t)slice * kNFP * sizeof(double) + 512 : 0;
 }
 
 template <typename Scope>
@@ -290,22 +271,22 @@ inline int stream_lumi(const GridDev &G, const StreamPlan &p, const double *host
     const size_t ws_x = stream_workspace_bytes(p, slice, chunk_opt);
     if (ws_x + stream_lumi_scratch_bytes(p, n) > ws_bytes) return PDF_EWORKSPACE;
     double *f1 = reinterpret_cast<double *>(align_up((size_t)ws + ws_x, 256));
-    double *f2 = f1 + slice * kNF;
-    ColMap cm; cm.n = kNF;
-    for (int f = 0; f < kNF; ++f) cm.col[f] = f;
-    CouplingParam C;
-    for (int k = 0; k < kNF * kNF; ++k) C.c[k] = hostC[k];
+    ColMap cm12; cm12.n = kNF;
+    for (int f = 0; f < kNF; ++f) cm12.col[f] = f;
+    ColMap cm1; cm1.n = 1; cm1.col[0] = 0;
+    double Cp[kNFP * 16];
+    for (int k = 0; k < kNFP * 16; ++k) Cp[k] = 0.0;
+    for (int i = 0; i < kNF; ++i)
+        for (int j = 0; j < kNF; ++j) Cp[i * 16 + j] = hostC[i * kNF + j];
+    if (cudaMemcpyAsync(p.d_coup, Cp, sizeof Cp, cudaMemcpyHostToDevice, s) != cudaSuccess) return PDF_ECUDA;   // pageable source: staged before return
     for (long long off = 0; off < n; off += slice) {
         const long long m = n - off < slice ? n - off : slice;
-        int rc = stream_xfxq2<Scope>(G, p, cm, m, x1 + off, q2 + off, f1, kNF, ws, ws_x, chunk_opt, s, 0);
+        int rc = stream_xfxq2<Scope>(G, p, cm12, m, x1 + off, q2 + off, f1, kNFP, ws, ws_x, chunk_opt, s, 0, nullptr, nullptr,
+                                     kModeLumiFirst, x2 + off, w + off, nullptr);
         if (rc) return rc;
-        rc = stream_xfxq2<Scope>(G, p, cm, m, x2 + off, q2 + off, f2, kNF, ws, ws_x, chunk_opt, s, 0);
+        rc = stream_xfxq2<Scope>(G, p, cm1, m, x2 + off, q2 + off, out + off, 1, ws, ws_x, chunk_opt, s, 1, nullptr, nullptr,
+                                 kModeLumiSecond, nullptr, nullptr, f1);
         if (rc) return rc;
-        {
-            Scope sc(s, "k_lumi_combine");
-            k_lumi_combine<<<(unsigned)((m + 255) / 256), 256, 0, s>>>(C, m, f1, f2, x1 + off, x2 + off, w + off, out + off,
-                                                                      G.err_count);
-        }
     }
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }
