@@ -7,21 +7,22 @@
 //   k_member_hist     histogram of the member ids of the slice (shared-memory counters per CTA)
 //   k_member_plan     exclusive scan -> first slot of every member; chunk table: every member's run
 //                     is cut in equal pieces of <= chunk queries {first, count, member}
-//   k_member_scatter  x, q2 -> xs, q2s in member order; inv[i] = slot of query i.  A CTA ranks its
-//                     4096 queries per member in shared memory, reserves its runs with one global
-//                     atomic per (CTA, member), sorts the tile in shared memory and writes the runs out
-//                     in slot order (~40 consecutive slots per run at 100 members)
+//   k_member_scatter  x, q2 -> xs, q2s in member order; orig[slot] = the query the slot came from.  A
+//                     CTA ranks its 4096 queries per member in shared memory, reserves its runs with
+//                     one global atomic per (CTA, member), sorts the tile in shared memory and writes
+//                     the runs out in slot order (~40 consecutive slots per run at 100 members);
+//                     queries with a member id outside [0, nmem) get their NaN row here and count as
+//                     errors (C-10)
 //   k_pdf_stream      the persistent binned kernel over the chunk table: chunk c evaluates against
-//                     V + member(c) * memstride and writes rows in SORTED order to tmp
-//   k_member_gather   out[i][:] = tmp[inv[i]][:] (coalesced writes, row-granular reads); queries
-//                     with a member id outside [0, nmem) get a NaN row and count as errors (C-10)
+//                     V + member(c) * memstride; the payload carries orig[slot], so every row goes
+//                     straight to its query's place in `out` (no sorted copy, no gather pass)
 // The order of the queries inside a member's run is whatever the atomics gave: every row depends on
 // its own query only, so the result does not.
 #pragma once
 
 namespace pdfg {
 
-constexpr long long kMemSlice = 1 << 25;      // queries partitioned at a time (scratch: 108 B per query of a slice)
+constexpr long long kMemSlice = 1 << 25;      // queries partitioned at a time (scratch: 20 B per query of a slice)
 constexpr int kMemMax = 4096;                 // members the shared-memory histograms hold
 constexpr int kMemTileQ = 8;                  // queries per thread of k_member_scatter
 constexpr int kMemScatThreads = 512;          // its CTA: 4096 queries, sorted by member in shared memory before they leave
@@ -32,9 +33,8 @@ struct MemberWs {
     unsigned *cursor;     // [nmem] next free slot of every member's run
     int *nchunks;         // [1]
     int *ctab;            // [max_chunks][4]
-    unsigned *inv;        // [slice]
+    unsigned *orig;       // [slice] query (slice-local) of every slot
     double *xs, *q2s;     // [slice]
-    double *tmp;          // [slice][npid]
 };
 
 // slices of equal length for a call of n queries
@@ -54,7 +54,7 @@ inline size_t member_scratch_bytes(long long slice, long long chunk, int nmem, i
     b += align_up(sizeof(int) * 4 * (size_t)member_max_chunks(slice, chunk, nmem), 256);
     b += align_up(sizeof(unsigned) * (size_t)slice, 256);
     b += 2 * align_up(sizeof(double) * (size_t)slice, 256);
-    b += align_up(sizeof(double) * (size_t)slice * npid, 256);
+    (void)npid;
     return b + 256;
 }
 
@@ -66,10 +66,9 @@ inline void member_carve(void *p, long long slice, long long chunk, int nmem, Me
     w.cursor = (unsigned *)c; c += hb;
     w.nchunks = (int *)c; c += hb;
     w.ctab = (int *)c; c += align_up(sizeof(int) * 4 * (size_t)member_max_chunks(slice, chunk, nmem), 256);
-    w.inv = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)slice, 256);
+    w.orig = (unsigned *)c; c += align_up(sizeof(unsigned) * (size_t)slice, 256);
     w.xs = (double *)c; c += align_up(sizeof(double) * (size_t)slice, 256);
-    w.q2s = (double *)c; c += align_up(sizeof(double) * (size_t)slice, 256);
-    w.tmp = (double *)c;
+    w.q2s = (double *)c;
 }
 
 __global__ void __launch_bounds__(256)
@@ -118,13 +117,14 @@ k_member_plan(const unsigned *__restrict__ hist, int nmem, int chunk, unsigned *
 // shared memory of k_member_scatter: 3 counter arrays, warp totals, then the tile sorted by member
 inline size_t member_scatter_smem(int nmem)
 {
-    return align_up(sizeof(unsigned) * 3 * (size_t)nmem + 256, 16) + (size_t)kMemScatThreads * kMemTileQ * (8 + 8 + 2);
+    return align_up(sizeof(unsigned) * 3 * (size_t)nmem + 256, 16) + (size_t)kMemScatThreads * kMemTileQ * (8 + 8 + 2 + 2);
 }
 
 __global__ void __launch_bounds__(kMemScatThreads)
 k_member_scatter(const double *__restrict__ x, const double *__restrict__ q2, const int *__restrict__ member,
                  long long n, int nmem, unsigned *__restrict__ cursor, double *__restrict__ xs,
-                 double *__restrict__ q2s, unsigned *__restrict__ inv)
+                 double *__restrict__ q2s, unsigned *__restrict__ orig, double *__restrict__ out, long long ld, int npid,
+                 unsigned long long *err_count)
 {
     constexpr int T = kMemScatThreads, TILE = T * kMemTileQ;
     extern __shared__ __align__(16) unsigned char s_raw[];
@@ -135,6 +135,7 @@ k_member_scatter(const double *__restrict__ x, const double *__restrict__ q2, co
     double *sx = reinterpret_cast<double *>(s_raw + align_up(sizeof(unsigned) * 3 * (size_t)nmem + 256, 16));
     double *sq = sx + TILE;
     unsigned short *sm = reinterpret_cast<unsigned short *>(sq + TILE);
+    unsigned short *so = sm + TILE;                               // the query's place inside the tile
     for (int k = threadIdx.x; k < nmem; k += T) s_c[k] = 0u;
     __syncthreads();
     const long long t0 = (long long)blockIdx.x * TILE;
@@ -183,14 +184,15 @@ k_member_scatter(const double *__restrict__ x, const double *__restrict__ q2, co
     for (int q = 0; q < kMemTileQ; ++q) {
         const long long e = t0 + q * T + threadIdx.x;
         if (e >= n) continue;
-        unsigned pos = kNoSlot;
         if (tag[q] != kNoSlot) {
             const unsigned m = tag[q] >> 16, rank = tag[q] & 0xffffu;
             const unsigned l = s_l[m] + rank;
-            sx[l] = xv[q]; sq[l] = qv[q]; sm[l] = (unsigned short)m;
-            pos = s_b[m] + rank;
+            sx[l] = xv[q]; sq[l] = qv[q]; sm[l] = (unsigned short)m; so[l] = (unsigned short)(q * T + threadIdx.x);
+        } else {                                                  // no such member: NaN row, counted (C-10)
+            double *o = out + e * ld;
+            for (int p = 0; p < npid; ++p) o[p] = qnan();
+            atomicAdd(err_count, 1ULL);
         }
-        inv[e] = pos;
     }
     __syncthreads();
     // the sorted tile leaves in slot order: consecutive threads write consecutive slots of a run
@@ -199,42 +201,8 @@ k_member_scatter(const double *__restrict__ x, const double *__restrict__ q2, co
         const unsigned m = sm[j], g = s_b[m] + (j - s_l[m]);
         xs[g] = sx[j];
         q2s[g] = sq[j];
+        orig[g] = (unsigned)t0 + so[j];
     }
-}
-
-// out[i][p] = tmp[inv[i]][p]; a thread per output element, so that writes are coalesced and the
-// npid doubles of a row are read by adjacent lanes
-__global__ void __launch_bounds__(256)
-k_member_gather(const double *__restrict__ tmp, const unsigned *__restrict__ inv, long long n, int npid,
-                double *__restrict__ out, long long ld, unsigned long long *err_count)
-{
-    constexpr int U = 4;                                              // row reads in flight per thread (latency-bound gather)
-    unsigned long long bad = 0;
-    const unsigned per = 256u * (unsigned)npid;                       // elements of 256 rows
-    for (long long r0 = (long long)blockIdx.x * 256; r0 < n; r0 += (long long)gridDim.x * 256) {
-        const unsigned rows = n - r0 < 256 ? (unsigned)(n - r0) : 256u;
-        const unsigned lim = rows * (unsigned)npid;
-        for (unsigned k0 = threadIdx.x; k0 < per; k0 += 256u * U) {
-            unsigned il[U], p[U], pos[U];
-            double v[U];
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const unsigned kk = k0 + 256u * u;
-                il[u] = kk / (unsigned)npid; p[u] = kk - il[u] * (unsigned)npid;
-                pos[u] = kk < lim ? __ldg(inv + r0 + il[u]) : kNoSlot;
-            }
-#pragma unroll
-            for (int u = 0; u < U; ++u) v[u] = pos[u] != kNoSlot ? __ldcs(tmp + (size_t)pos[u] * npid + p[u]) : qnan();
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const unsigned kk = k0 + 256u * u;
-                if (kk >= lim) continue;
-                bad += (pos[u] == kNoSlot && p[u] == 0u) ? 1u : 0u;
-                __stcs(out + (r0 + il[u]) * ld + p[u], v[u]);
-            }
-        }
-    }
-    if (bad) atomicAdd(err_count, bad);
 }
 
 }  // namespace pdfg

@@ -127,12 +127,12 @@ struct StreamArgs {
     long long chunk;           // queries per chunk (multiple of kS3TileA)
     int nchunks, ta;           // chunks, A tiles per chunk
     int identity;              // 1: requested columns == the grid's 11 columns in order
-    int zfill;                 // 1: rows are contiguous (ld == npid): A tiles zero-fill their rows of `out`
     int count_err;             // 1: invalid queries bump the grid's error counter
     // member axis (a-8, pdf_members.cuh): the queries arrive sorted by member and every chunk lies
     // inside one member's run; ctab[c] = {first query, queries, member, 0}, *nchunks_dev chunks.
     const int *ctab;
     const int *nchunks_dev;
+    const unsigned *orig;      // with ctab: the query (row of `out`) of every sorted slot; the payload carries it
     // fused luminosity (a-7): pass 1 (k_lumi_first) writes rows [xf_0..xf_10, w/(x1 x2)] of 12 doubles into `out` (the
     // scratch), pass 2 (k_lumi_second) reads them back as `f1` and reduces the coupling against its own row on the fly
     const double *x2, *w;      // pass 1: the other parton's x and the event weight (for the scale column)
@@ -261,24 +261,6 @@ __device__ __noinline__ double s3_two(double f0, double f1, double theta) { retu
 __device__ __noinline__ double s3_lowq(double fmin, double fplus, double r, double lnr) { return lowq_continue_ln(fmin, fplus, r, lnr); }
 
 // ---- A tile: classify, locate, t_x / t_q, one slot per query in its cell's bin -----------------
-// zero-fill rows [r0, r1) of `out` (contiguous rows of ld doubles) with coalesced 32-byte stores of one warp
-__device__ __forceinline__ void zero_fill_warp(double *out, long long ld, long long r0, long long r1, int lane)
-{
-    double *p = out + r0 * ld, *e = out + r1 * ld;
-    if (p >= e) return;
-    // head: up to 3 doubles to the next 32-byte boundary
-    const int head = (int)(((32u - (unsigned)(reinterpret_cast<size_t>(p) & 31u)) & 31u) >> 3);
-    const long long tot = e - p;
-    const int h = (long long)head < tot ? head : (int)tot;
-    if (lane < h) p[lane] = 0.0;
-    p += h;
-    const long long n4 = (e - p) >> 2;
-    for (long long k = lane; k < n4; k += 32)
-        asm volatile("st.global.v4.f64 [%0], {%1,%1,%1,%1};" ::"l"(p + 4 * k), "d"(0.0) : "memory");
-    p += 4 * n4;
-    if (lane < (int)(e - p)) p[lane] = 0.0;
-}
-
 template <int MODE>
 __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, int slot, long long chunk_base, long long chunk_end,
                                        int tile, unsigned long long &err_local)
@@ -294,8 +276,6 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
     unsigned *lcount = counts + B.nbins;
     Payload *bins = A.W.bins + (size_t)slot * B.nbins * B.cap;
     Payload *lists = A.W.lists + (size_t)slot * kNumLists * A.chunk;
-    if (A.zfill) zero_fill_warp(A.out, A.ld, t0, t1, lane);
-    __syncwarp();                                      // the NaN rows below are written by other lanes than the zeros
     const int nx = G.nx, nqt = G.nqtot;
     const long long xminb = lds_s64(T.xk), xmaxb = lds_s64(T.xk + 8u * (nx - 1));
     const long long qminb = lds_s64(T.qk), qmaxb = lds_s64(T.qk + 8u * (nqt - 1));
@@ -377,9 +357,9 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
         for (int q = 0; q < kS3Grp; ++q) {
             const long long e = t0 + (g0 + q) * 32 + lane;
             if (e >= t1) continue;
-            const unsigned idx = (unsigned)(e - chunk_base);
+            const unsigned idx = A.orig ? __ldcs(A.orig + e) : (unsigned)(e - chunk_base);
             if (key[q] == INT_MIN) {                                              // C-10: NaN row, counted
-                double *o = A.out + e * A.ld;
+                double *o = A.out + (A.orig ? (long long)idx : e) * A.ld;
                 const int ncol = MODE == kModeLumiFirst ? kNFP : A.cm.n;
                 for (int p = 0; p < ncol; ++p) o[p] = qnan();
                 if (A.count_err) ++err_local;
@@ -913,11 +893,12 @@ __device__ __forceinline__ void stream_body(const StreamArgs &A)
             warp_release_add(a_done, 1ULL);
         } else {
             wait_for(a_done, (gen + 1) * TA);                      // every tile of A(c) has been released
-            if (sub < B.ne) e_unit<MODE>(A, V, RP, slot, chunk_base, sC, err_local);   // list units first: their queries are the expensive ones
+            const long long row_base = A.orig ? 0 : chunk_base;    // member axis: the payload's index is the row itself
+            if (sub < B.ne) e_unit<MODE>(A, V, RP, slot, row_base, sC, err_local);   // list units first: their queries are the expensive ones
             else {
                 const int v = sub - B.ne;
                 const int i = v / B.ng, grp = v - i * B.ng;
-                b_unit<MODE>(A, T, V, slot, chunk_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf, sC, err_local);
+                b_unit<MODE>(A, T, V, slot, row_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf, sC, err_local);
             }
             const unsigned long long old = warp_release_add(b_fin, 1ULL);
             if (old + 1 == (gen + 1) * TB) {                       // last unit of the chunk: the slot's counters are reset for the ring

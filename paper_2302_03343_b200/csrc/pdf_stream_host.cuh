@@ -192,12 +192,13 @@ template <typename Scope>
 inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm, long long n, const double *x,
                         const double *q2, double *out, long long ld, void *ws, size_t ws_bytes, long long chunk_opt,
                         cudaStream_t s, int count_err = 1, const int *ctab = nullptr, const int *nchunks_dev = nullptr,
-                        int mode = kModeRows, const double *x2 = nullptr, const double *w = nullptr, const double *f1 = nullptr)
+                        int mode = kModeRows, const double *x2 = nullptr, const double *w = nullptr, const double *f1 = nullptr,
+                        const unsigned *orig = nullptr)
 {
     if (stream_workspace_bytes(p, n, chunk_opt) > ws_bytes) return PDF_EWORKSPACE;
     StreamArgs A;
     A.ctab = ctab; A.nchunks_dev = nchunks_dev;
-    A.x2 = x2; A.w = w; A.f1 = f1; A.coup = p.d_coup;
+    A.x2 = x2; A.w = w; A.f1 = f1; A.coup = p.d_coup; A.orig = orig;
     A.G = G; A.cm = cm;
     A.chunk = stream_chunk(p, n, chunk_opt);
     stream_caps(p, A.chunk, A.B);
@@ -207,7 +208,6 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     A.ta = (int)(A.chunk / kS3TileA);
     A.identity = cm.n == kNF;
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
-    A.zfill = (ld == cm.n && mode != kModeLumiFirst) ? 1 : 0;
     A.count_err = count_err;
     const size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts
     if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
@@ -291,8 +291,8 @@ inline int stream_lumi(const GridDev &G, const StreamPlan &p, const double *host
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }
 
-// a-8 on the binned path (pdf_members.cuh): per slice, partition by member, one persistent-kernel
-// run over the chunk table into the sorted scratch rows, gather back to query order
+// a-8 on the binned path (pdf_members.cuh): per slice, partition by member, then one persistent-kernel
+// run over the chunk table whose rows go straight to their queries' places
 inline size_t stream_members_bytes(const StreamPlan &p, const GridDev &G, long long n, long long chunk_opt, int npid)
 {
     if (!p.usable || G.nmem < 2 || G.nmem > kMemMax) return 0;
@@ -333,16 +333,11 @@ inline int stream_members(const GridDev &G, const StreamPlan &p, const ColMap &c
         {
             Scope sc(s, "k_member_scatter");
             k_member_scatter<<<(unsigned)((m + kMemScatThreads * kMemTileQ - 1) / (kMemScatThreads * kMemTileQ)), kMemScatThreads, member_scatter_smem(G.nmem), s>>>(
-                x + off, q2 + off, member + off, m, G.nmem, M.cursor, M.xs, M.q2s, M.inv);
+                x + off, q2 + off, member + off, m, G.nmem, M.cursor, M.xs, M.q2s, M.orig, out + off * ld, ld, cm.n, G.err_count);
         }
-        int rc = stream_xfxq2<Scope>(G, p, cm, m, M.xs, M.q2s, M.tmp, cm.n, ws, ws_x, chunk_opt, s, 1, M.ctab, M.nchunks);
+        int rc = stream_xfxq2<Scope>(G, p, cm, m, M.xs, M.q2s, out + off * ld, ld, ws, ws_x, chunk_opt, s, 1, M.ctab, M.nchunks,
+                                     kModeRows, nullptr, nullptr, nullptr, M.orig);
         if (rc) return rc;
-        {
-            Scope sc(s, "k_member_gather");
-            long long want = (m + 255) / 256;
-            k_member_gather<<<(unsigned)(want < sms * 16 ? want : sms * 16), 256, 0, s>>>(M.tmp, M.inv, m, cm.n, out + off * ld, ld,
-                                                                                       G.err_count);
-        }
     }
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
 }
