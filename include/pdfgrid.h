@@ -47,7 +47,8 @@ enum {
     PDF_ENOMEM = -2,     /* host or device allocation failed                                     */
     PDF_ECUDA = -3,      /* a CUDA runtime call failed (see pdf_last_cuda_error)                 */
     PDF_EWORKSPACE = -4, /* the binned path needs a workspace and none / too small was supplied  */
-    PDF_ESTATE = -5      /* call needs data that was not set (alpha_s knots, coupling matrix)    */
+    PDF_ESTATE = -5,     /* call needs data that was not set (alpha_s knots, coupling matrix)    */
+    PDF_ELIMIT = -6      /* pdf_xfxq2_noalloc: n (or the grid) beyond what its static scratch holds */
 };
 
 /* region codes written by pdf_locate (Fig. 3.1(b)) */
@@ -157,6 +158,26 @@ int pdf_locate(const pdf_grid *g, long long n, const double *x, const double *q2
  * kernels for grids the binned path does not support (flavour count other than 11, > 1024 cells per axis),
  * small calls and calls without a sufficient workspace; this call makes that visible. */
 int pdf_last_path(const pdf_grid *g);
+
+/* ---- the no-allocation entry point ------------------------------------------------------------
+ * pdf_xfxq2 (same operation, same results: PAPER.md L1712-1746) for callers that may not
+ * allocate device memory -- code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+ * It runs the binned path's kernel with its scratch in a static device array of PDF_NOALLOC_SCRATCH_BYTES that every
+ * GPU which loads the library holds until the process exits; no workspace is attached or used, and the call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine (one memset and one launch on `stream`).
+ *   pids HOST [npid]; x, q2 DEVICE [n]; out DEVICE [n][npid] row-major (ld = npid).
+ *   max_n: HOST, optional; receives the largest n this grid's geometry allows (also when the call is rejected):
+ *          the whole call is one chunk in one ring slot, ~290 B of scratch per query plus 32 B x 32 per grid cell
+ *          (about 1.8e5 queries for a 196 x 54-knot grid).
+ * Errors: PDF_ELIMIT when n > *max_n, or when the grid does not fit the binned path (flavour count other than 11,
+ * > 1024 cells per axis) or the array at all; PDF_EINVAL on bad arguments; PDF_ECUDA if the array's address could
+ * not be resolved when the grid was created.  Invalid queries give NaN rows and count in pdf_error_count as usual.
+ * The array is shared by every call on a device and keeps the last call's contents (the call clears the counters it
+ * needs at zero, on `stream`): calls that overlap on the GPU -- different streams, or two grids on one device --
+ * race on it, so order them on one stream or with events. */
+#define PDF_NOALLOC_SCRATCH_BYTES (64u * 1024u * 1024u)
+int pdf_xfxq2_noalloc(const pdf_grid *g, const int *pids, int npid, long long n, const double *x, const double *q2,
+                      double *out, long long *max_n, void *stream);
 
 /* number of invalid queries seen by this grid since creation / the last call of this function
  * (reads and resets the device counter; synchronises `stream`). */

@@ -19,7 +19,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpdfgrid.so")
 
-PDF_OK, PDF_EINVAL, PDF_ENOMEM, PDF_ECUDA, PDF_EWORKSPACE, PDF_ESTATE = 0, -1, -2, -3, -4, -5
+PDF_OK, PDF_EINVAL, PDF_ENOMEM, PDF_ECUDA, PDF_EWORKSPACE, PDF_ESTATE, PDF_ELIMIT = 0, -1, -2, -3, -4, -5, -6
 PDF_PATH_AUTO, PDF_PATH_DIRECT, PDF_PATH_BINNED = 0, 1, 2
 PDF_OPT_PATH, PDF_OPT_ALPHAS_MODE, PDF_OPT_CHUNK = 1, 2, 3
 PDF_ALPHAS_FREEZE, PDF_ALPHAS_LOGGRAD = 0, 1
@@ -33,7 +33,7 @@ SYMBOLS = (
     "pdf_last_cuda_error", "pdf_launch_count", "pdf_profile_enable", "pdf_profile_read",
     "pdf_measure_fp64_tflops", "pdf_last_path", "pdf_log_f64",
     "pdf_rambo", "pdf_vegas_map", "pdf_vegas_accumulate", "pdf_vegas_estimate", "pdf_vegas_refine", "pdf_vegas_combine",
-    "pdf_unweight",
+    "pdf_unweight", "pdf_xfxq2_noalloc",
 )
 
 
@@ -64,6 +64,7 @@ def lib():
     L.pdf_grid_set_option.argtypes = [vp, C.c_int, ll]
     L.pdf_grid_limits.argtypes = [vp, dp, dp, dp, dp]
     L.pdf_xfxq2.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp]
+    L.pdf_xfxq2_noalloc.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, C.POINTER(ll), vp]
     L.pdf_xfxq2_ex.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp, ll, vp]
     L.pdf_xfxq2_xgrid.argtypes = [vp, ip, C.c_int, ll, vp, vp, C.c_int, vp, vp, ll, vp]
     L.pdf_alphas_q2.argtypes = [vp, ll, vp, vp, vp]
@@ -334,6 +335,21 @@ class PdfGrid:
             rc = lib().pdf_xfxq2_ex(self._h, _iptr(pid), pid.numel(), n, xp, qp, mp, op, ld, _stream_ptr(stream))
         _check(rc, "pdf_xfxq2")
         return out
+
+    def pdf_xfxq2_noalloc(self, pids, x: torch.Tensor, q2: torch.Tensor, out: torch.Tensor, stream=None) -> int:
+        """pdf_xfxq2 through the library's static scratch array: no workspace, no allocation in the call (the caller
+        passes `out`).  Returns the largest n the grid allows; raises PdfGridError (PDF_ELIMIT) beyond it."""
+        pid = _hi(list(pids))
+        n = x.numel()
+        xp, qp = _dev(x, torch.float64, "x", n), _dev(q2, torch.float64, "q2", n)
+        op = _dev(out, torch.float64, "out", n * pid.numel(), at_least=True)
+        max_n = C.c_longlong(0)
+        rc = lib().pdf_xfxq2_noalloc(self._h, _iptr(pid), pid.numel(), n, xp, qp, op, C.byref(max_n), _stream_ptr(stream))
+        if rc == PDF_ELIMIT:
+            raise PdfGridError(f"pdf_xfxq2_noalloc: n = {n} is beyond the {max_n.value} queries that the static scratch "
+                               f"array holds for this grid ({lib().pdf_status_string(rc).decode()}) ({rc})")
+        _check(rc, "pdf_xfxq2_noalloc")
+        return int(max_n.value)
 
     def pdf_xfxq2_xgrid(self, pids, x: torch.Tensor, q2: torch.Tensor, nrep: int,
                         members: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,

@@ -87,9 +87,12 @@ struct pdf_grid {
     HostStage stage[2];
     StreamPlan bplan{};       // key geometry and search tables of the binned path (pdf_stream.cuh)
     mutable int last_path = 0;  // PDF_PATH_DIRECT / PDF_PATH_BINNED: what the last evaluation call of this handle ran
+    void *noalloc_ws = nullptr; // device address of the static scratch array on this grid's device (pdf_noalloc.inl)
 };
 
 namespace {
+
+int noalloc_setup(int device, void **ptr);   // pdf_noalloc.inl
 
 int col_of_pid(const pdf_grid *g, int pid)
 {
@@ -126,6 +129,7 @@ const char *pdf_status_string(int status)
     case PDF_ECUDA: return "CUDA runtime error";
     case PDF_EWORKSPACE: return "workspace missing or too small";
     case PDF_ESTATE: return "required grid data not set";
+    case PDF_ELIMIT: return "size beyond what the static scratch of the no-allocation entry point holds (see its max_n)";
     default: return "unknown status";
     }
 }
@@ -248,6 +252,9 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
     d.na = 0; d.alphas_mode = PDF_ALPHAS_FREEZE; d.C = nullptr; d.err_count = g->d_err;
     rc = stream_plan_init(g->bplan, g->d, g->xk, g->qk, nsub);
     if (rc != PDF_OK) { free_grid(g); return rc; }
+    // pdf_xfxq2_noalloc: the static scratch array's address on this device (resolved once per device; no allocation).
+    // A failure leaves the pointer null and only that entry point unusable.
+    noalloc_setup(g->device, &g->noalloc_ws);
     *out = g;
     return PDF_OK;
 }
@@ -338,3 +345,4 @@ int pdf_grid_limits(const pdf_grid *g, double *xmin, double *xmax, double *q2min
 
 #include "pdfgrid_eval.inl"
 #include "mc_entry.inl"
+#include "pdf_noalloc.inl"
