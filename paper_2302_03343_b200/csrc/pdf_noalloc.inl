@@ -110,13 +110,14 @@ int pdf_xfxq2_noalloc(const pdf_grid *g, const int *pids, int npid, long long n,
     const size_t smem = stream_smem_bytes(g->d, A.B);
     int per_sm = 0, sms = 0;
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_pdf_stream, kS3Threads, smem));
+    const auto kern = A.identity ? k_pdf_stream : k_pdf_stream_cols;     // rows of npid doubles: the stride fits 32 bits
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kS3Threads, smem));
     if (per_sm < 1) return PDF_ECUDA;
     const unsigned long long max_ctas = (unsigned long long)per_sm * sms;         // all CTAs must be co-resident
     const unsigned long long tickets = (unsigned long long)(A.ta + A.B.tb);
     const unsigned long long want = (tickets + kS3Warps - 1) / kS3Warps;
     g_launches.fetch_add(1, std::memory_order_relaxed);
-    k_pdf_stream<<<(unsigned)(want < max_ctas ? want : max_ctas), kS3Threads, smem, s>>>(A);
+    kern<<<(unsigned)(want < max_ctas ? want : max_ctas), kS3Threads, smem, s>>>(A);
     CK(cudaGetLastError());
     g->last_path = PDF_PATH_BINNED;
     return PDF_OK;

@@ -408,27 +408,25 @@ __device__ __forceinline__ int xnode(int i, int t, int nx)
     return c < 0 ? 0 : (c >= nx ? nx - 1 : c);
 }
 
-// one row from the accumulator fragments: 4 lanes write one row
+// one row from the accumulator fragments through a column map: 4 lanes write one row (the general form; calls with the
+// grid's own 11 columns in order take the four fixed stores in b_unit)
 __device__ __forceinline__ void store_row(const StreamArgs &A, double *rp, int t, const Acc &d)
 {
-    if (A.identity) {
-        rp[2 * t] = d.d00; rp[2 * t + 1] = d.d01;
-        if (t < 2) rp[8 + 2 * t] = d.d10;
-        if (t == 0) rp[9] = d.d11;
-    } else {
-        for (int p = 0; p < A.cm.n; ++p) {
-            const int c = A.cm.col[p];
-            if (c < 0) { if (t == 0) rp[p] = 0.0; continue; }
-            if (((c & 7) >> 1) == t) rp[p] = (c & 8) ? ((c & 1) ? d.d11 : d.d10) : ((c & 1) ? d.d01 : d.d00);
-        }
+    for (int p = 0; p < A.cm.n; ++p) {
+        const int c = A.cm.col[p];
+        if (c < 0) { if (t == 0) rp[p] = 0.0; continue; }
+        if (((c & 7) >> 1) == t) rp[p] = (c & 8) ? ((c & 1) ? d.d11 : d.d10) : ((c & 1) ? d.d01 : d.d00);
     }
 }
 
 // interior cells of x cell i, Q2 cells [fk0, fk1): the (cell, batch of <= 32 payloads) sequence of the unit runs
 // through the warp's stages: two payload stages (batch parity) and two value stages (cell parity; a cell's 16 node
-// rows, node n = 4 * (Q2 row) + (x node)).  The fragments are re-read from the value stage per 8-query tile (8
-// LDS.64): held in registers across the loop they spilled to local memory at 80 registers (profile r2f).
-template <int MODE>
+// rows, node n = 4 * (Q2 row) + (x node)).  Version 4 of the loop (profile r2a: version 3 spent 108 warp instructions
+// per 8-query tile, 8 of them DMMAs): the cell's operand fragments and the coefficients of both node weights are read
+// once per cell and stay in registers, rows with the grid's own 11 columns (FAST) leave by four fixed stores from one
+// 64-bit multiply-add, lanes beyond the batch run on whatever the stage holds (a row of A only ever meets its own
+// row of D) and only their stores are predicated.
+template <int MODE, bool FAST>
 __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, const double *__restrict__ Vm, int slot,
                                        long long chunk_base, int i, int fk0, int fk1, unsigned sbuf, unsigned sC,
                                        unsigned long long &err_local)
@@ -437,25 +435,36 @@ __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, 
     const StreamDev &B = A.B;
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const unsigned *counts = A.W.counts + (size_t)slot * (B.nbins + 32) + (size_t)i * B.nqt;
-    const Payload *bins = A.W.bins + ((size_t)slot * B.nbins + (size_t)i * B.nqt) * B.cap;
     int mycnt = 0;
     if (fk0 + lane < fk1) mycnt = min((int)ldcg_u32(counts + fk0 + lane), B.cap);
     unsigned live = __ballot_sync(0xffffffffu, mycnt > 0);      // cells of the unit that hold queries
     if (live == 0u) return;
     const int nx = G.nx;
+    // this lane's payload of a batch: bins of x cell i, entry `lane`
+    const char *binl = reinterpret_cast<const char *>(A.W.bins + ((size_t)slot * B.nbins + (size_t)i * B.nqt) * B.cap) + 32u * lane;
+    const unsigned capb = 32u * (unsigned)B.cap;
     WCoef kx;
     {
         const double2 ab = lds_v2f64(T.cx + 48u * i + 16u), cd = lds_v2f64(T.cx + 48u * i + 32u);
         kx = weight_coef(ab.x, ab.y, cd.x, cd.y, t);            // x-axis weight of this lane's node, fixed for the unit
     }
     // the 96 16-byte pieces of a cell's 16 node rows are copied by 32 lanes x 3: piece e = lane + 32 k,
-    // node = e / 6 = 4 b + a; x-node columns are fixed for the unit, Q2 rows follow the cell
+    // node = e / 6 = 4 b + a; the x-node columns (byte offsets vo) are fixed for the unit, the Q2 rows follow the cell
     const unsigned sP = sbuf, sV = sbuf + 2u * kStageP;
-    auto issue = [&](int j, int o, int pp, int vp, bool with_values) {
+    unsigned vo[3];
+    int vb[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int e = lane + 32 * k, node = e / 6, piece = e - node * 6;
+        vb[k] = node >> 2;
+        vo[k] = (unsigned)((xnode(i, node & 3, nx) * kNFP + 2 * piece) * 8);
+    }
+    const char *Vb = reinterpret_cast<const char *>(Vm);
+    const unsigned rowb = (unsigned)(nx * kNFP * 8);
+    auto issue = [&](int j, int o, int cntj, int pp, int vp, bool with_values) {
         const int fk = fk0 + j;
-        const int n = min(kS3Batch, __shfl_sync(0xffffffffu, mycnt, j) - o);
-        if (lane < n) {
-            const char *src = reinterpret_cast<const char *>(bins + (size_t)fk * B.cap + o + lane);
+        if (lane < cntj - o) {                                   // at most 32 lanes
+            const char *src = binl + ((size_t)(unsigned)fk * capb + 32u * (unsigned)o);
             const unsigned dst = sP + (unsigned)(pp * kStageP) + 32u * lane;
             cp_async16_cg(dst, src);
             cp_async16_cg(dst + 16u, src + 16);
@@ -463,93 +472,113 @@ __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, 
         if (with_values) {
             const double aL = lds_f64(T.cq + 48u * fk + 16u), aR = lds_f64(T.cq + 48u * fk + 32u);
             const int elo = aL == 1.0 ? 1 : 0, ehi = aR == 1.0 ? 1 : 0;       // one-sided ends of a sub-grid (q_point_cell)
+            const unsigned dv = sV + (unsigned)(vp * kStageV) + 16u * lane;
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
-                const int e = lane + 32 * k, node = e / 6, piece = e - node * 6, b = node >> 2;
-                const int row = fk - 1 + b + (b == 0 ? elo : 0) - (b == 3 ? ehi : 0);
-                cp_async16_ca(sV + (unsigned)(vp * kStageV) + 16u * e,
-                              Vm + ((size_t)row * nx + xnode(i, node & 3, nx)) * kNFP + 2 * piece);
+                const int row = fk - 1 + vb[k] + (vb[k] == 0 ? elo : 0) - (vb[k] == 3 ? ehi : 0);
+                cp_async16_ca(dv + 512u * k, Vb + ((size_t)((unsigned)row * rowb) + vo[k]));
             }
         }
         cp_async_commit();
     };
     int j = __ffs(live) - 1, o = 0, pp = 0, vp = 0;
-    issue(j, 0, 0, 0, true);
+    int cntj = __shfl_sync(0xffffffffu, mycnt, j);
+    issue(j, 0, cntj, 0, 0, true);
     bool fresh = true;                                          // the current batch opens a cell
     WCoef kq;
-    // this lane's fragment offsets inside a value stage: step r pairs Q2 row (t ^ r) with x node t
+    double fb0, fb1, fb2, fb3, fc0, fc1, fc2, fc3;              // the cell's operand fragments: step r pairs Q2 row (t ^ r) with x node t
+    fb0 = fb1 = fb2 = fb3 = fc0 = fc1 = fc2 = fc3 = 0.0;
+    kq.c0 = kq.c1 = kq.c2 = kq.c3 = 0.0;
     const unsigned fo = (unsigned)(t * kNFP * 8 + 8 * g);
+    // pass 2 of the luminosity: the coupling's fragments (flavour 4 s + t of parton 1 against flavours g, 8 + g of parton 2)
+    double cf0x = 0.0, cf0y = 0.0, cf1x = 0.0, cf1y = 0.0, cf2x = 0.0, cf2y = 0.0;
+    if (MODE == kModeLumiSecond) {
+        cf0x = lds_f64(sC + (unsigned)((0 + t) * 128 + 8 * g)); cf1x = lds_f64(sC + (unsigned)((4 + t) * 128 + 8 * g));
+        cf2x = lds_f64(sC + (unsigned)((8 + t) * 128 + 8 * g));
+        if (g < 4) {
+            cf0y = lds_f64(sC + (unsigned)((0 + t) * 128 + 8 * g) + 64u); cf1y = lds_f64(sC + (unsigned)((4 + t) * 128 + 8 * g) + 64u);
+            cf2y = lds_f64(sC + (unsigned)((8 + t) * 128 + 8 * g) + 64u);
+        }
+    }
+    // FAST: rows of A.ld doubles, this lane's columns 2t, 2t+1 (all t), 8 + 2t (t < 2), 9 (t == 0)
+    const unsigned ldb = (unsigned)(A.ld * 8);
+    char *outl = reinterpret_cast<char *>(A.out + chunk_base * (MODE == kModeLumiFirst ? (long long)kNFP : A.ld)) + 16 * t;
     for (;;) {
         // successor of (j, o)
-        int jn = j, on = o + kS3Batch;
-        const int cntj = __shfl_sync(0xffffffffu, mycnt, j);
-        if (on >= cntj) { live &= live - 1; jn = live ? __ffs(live) - 1 : -1; on = 0; }
-        if (jn >= 0) { issue(jn, on, pp ^ 1, jn != j ? vp ^ 1 : vp, jn != j); cp_async_wait<1>(); }
+        int jn = j, on = o + kS3Batch, cntn = cntj;
+        if (on >= cntj) {
+            live &= live - 1; on = 0; jn = -1;
+            if (live) { jn = __ffs(live) - 1; cntn = __shfl_sync(0xffffffffu, mycnt, jn); }
+        }
+        if (jn >= 0) { issue(jn, on, cntn, pp ^ 1, jn != j ? vp ^ 1 : vp, jn != j); cp_async_wait<1>(); }
         else cp_async_wait<0>();
         __syncwarp();
         if (fresh) {
             const int fk = fk0 + j;
             const double2 ab = lds_v2f64(T.cq + 48u * fk + 16u), cd = lds_v2f64(T.cq + 48u * fk + 32u);
             kq = weight_coef(ab.x, ab.y, cd.x, cd.y, t);
+            const unsigned sv = sV + (unsigned)(vp * kStageV) + fo;
+            fb0 = lds_f64(sv + (unsigned)(4 * (t ^ 0) * kNFP * 8)); fb1 = lds_f64(sv + (unsigned)(4 * (t ^ 1) * kNFP * 8));
+            fb2 = lds_f64(sv + (unsigned)(4 * (t ^ 2) * kNFP * 8)); fb3 = lds_f64(sv + (unsigned)(4 * (t ^ 3) * kNFP * 8));
+            if (g < 4) {
+                fc0 = lds_f64(sv + (unsigned)(4 * (t ^ 0) * kNFP * 8) + 64u); fc1 = lds_f64(sv + (unsigned)(4 * (t ^ 1) * kNFP * 8) + 64u);
+                fc2 = lds_f64(sv + (unsigned)(4 * (t ^ 2) * kNFP * 8) + 64u); fc3 = lds_f64(sv + (unsigned)(4 * (t ^ 3) * kNFP * 8) + 64u);
+            }
         }
-        const unsigned sb = sP + (unsigned)(pp * kStageP), sv = sV + (unsigned)(vp * kStageV) + fo;
+        const unsigned sb = sP + (unsigned)(pp * kStageP) + 32u * g;
         const int nact = min(kS3Batch, cntj - o);
         {
             // the next tile's abscissae are fetched under this tile's arithmetic
-            bool vn = g < nact;
-            double2 abn = make_double2(0.0, 0.0);
-            unsigned idxn = 0;
-            if (vn) { abn = lds_v2f64(sb + 32u * g); idxn = lds_u32(sb + 32u * g + 16u); }
+            double2 abn = lds_v2f64(sb);
+            unsigned idxn = lds_u32(sb + 16u);
+#pragma unroll 1
             for (int m0 = 0; m0 < nact; m0 += 8) {
-                const bool valid = vn;
+                const bool valid = m0 + g < nact;
                 const double tx = abn.x, tq = abn.y;
                 const unsigned idx = idxn;
-                const int qn = m0 + 8 + g;
-                vn = qn < nact;
-                if (vn) { abn = lds_v2f64(sb + 32u * qn); idxn = lds_u32(sb + 32u * qn + 16u); }
+                const unsigned sn = sb + 32u * (unsigned)((m0 + 8) & (kS3Batch - 1));      // wraps to tile 0 after the last tile (unused)
+                abn = lds_v2f64(sn); idxn = lds_u32(sn + 16u);
                 // pass 2 of the luminosity: this query's row of pass 1 in the A-operand layout (flavour 4 s + t), fetched
-                // under the contraction; lane t = 3 of step 2 gets the scale column.  (Fetching it one tile ahead costs 6
-                // more registers, which spill: measured 12.25 against 11.80 ms per 1e8 events.)
+                // under the contraction; lane t = 3 of step 2 gets the scale column
                 double a0 = 0.0, a1 = 0.0, a2 = 0.0;
                 if (MODE == kModeLumiSecond && valid) {
                     const double *fr = A.f1 + (chunk_base + idx) * kNFP + t;
                     a0 = __ldcs(fr); a1 = __ldcs(fr + 4); a2 = __ldcs(fr + 8);
                 }
-                const double wx = valid ? weight_eval(kx, tx) : 0.0;
+                const double wx = weight_eval(kx, tx);
                 const double wq0 = weight_eval(kq, tq);
                 const double wq1 = __shfl_xor_sync(0xffffffffu, wq0, 1);
                 const double wq2 = __shfl_xor_sync(0xffffffffu, wq0, 2);
                 const double wq3 = __shfl_xor_sync(0xffffffffu, wq0, 3);
                 Acc d = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const unsigned pn = sv + (unsigned)(4 * (t ^ r) * kNFP * 8);
-                    double2 f;
-                    f.x = lds_f64(pn);
-                    f.y = g < 4 ? lds_f64(pn + 64u) : 0.0;
-                    kstep(d, (r == 0 ? wq0 : r == 1 ? wq1 : r == 2 ? wq2 : wq3) * wx, f);
-                }
+                kstep(d, wq0 * wx, make_double2(fb0, fc0));
+                kstep(d, wq1 * wx, make_double2(fb1, fc1));
+                kstep(d, wq2 * wx, make_double2(fb2, fc2));
+                kstep(d, wq3 * wx, make_double2(fb3, fc3));
                 if (MODE == kModeRows) {
-                    if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, d);
+                    if (FAST) {
+                        if (valid) {
+                            char *rp = outl + (size_t)idx * ldb;
+                            asm volatile("st.global.f64 [%0], %1;" ::"l"(rp), "d"(d.d00) : "memory");
+                            asm volatile("st.global.f64 [%0+8], %1;" ::"l"(rp), "d"(d.d01) : "memory");
+                            if (t < 2) asm volatile("st.global.f64 [%0+64], %1;" ::"l"(rp), "d"(d.d10) : "memory");
+                            if (t == 0) asm volatile("st.global.f64 [%0+72], %1;" ::"l"(rp), "d"(d.d11) : "memory");
+                        }
+                    } else if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, d);
                 } else if (MODE == kModeLumiFirst) {
                     // rows of 12 on 32-byte sectors: two stores write the three sectors whole (no zero fill needed)
                     if (valid) {
-                        double *rp = A.out + (chunk_base + idx) * kNFP;
-                        *reinterpret_cast<double2 *>(rp + 2 * t) = make_double2(d.d00, d.d01);
+                        double *rp = reinterpret_cast<double *>(outl + (size_t)idx * (unsigned)(kNFP * 8));
+                        *reinterpret_cast<double2 *>(rp) = make_double2(d.d00, d.d01);
                         if (t == 0) *reinterpret_cast<double2 *>(rp + 8) = make_double2(d.d10, d.d11);
-                        if (t == 1) *reinterpret_cast<double2 *>(rp + 10) = make_double2(d.d10, lds_f64(sb + 32u * (m0 + g) + 24u));
+                        if (t == 1) *reinterpret_cast<double2 *>(rp + 8) = make_double2(d.d10, lds_f64(sb + 32u * (unsigned)m0 + 24u));
                     }
                 } else {
                     // G[q][j] = sum_i f1[q][i] C[i][j] by 6 more DMMAs, then the dot with this row and the scale
                     Acc gq = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-                    for (int s = 0; s < 3; ++s) {
-                        const unsigned pc = sC + (unsigned)((4 * s + t) * 128 + 8 * g);
-                        double2 cf;
-                        cf.x = lds_f64(pc);
-                        cf.y = g < 4 ? lds_f64(pc + 64u) : 0.0;
-                        kstep(gq, s == 0 ? a0 : s == 1 ? a1 : (t == 3 ? 0.0 : a2), cf);
-                    }
+                    kstep(gq, a0, make_double2(cf0x, cf0y));
+                    kstep(gq, a1, make_double2(cf1x, cf1y));
+                    kstep(gq, t == 3 ? 0.0 : a2, make_double2(cf2x, cf2y));
                     double dot = fma(d.d00, gq.d00, fma(d.d01, gq.d01, fma(d.d10, gq.d10, d.d11 * gq.d11)));
                     dot += __shfl_xor_sync(0xffffffffu, dot, 1);
                     dot += __shfl_xor_sync(0xffffffffu, dot, 2);
@@ -566,7 +595,7 @@ __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, 
         if (jn < 0) break;
         fresh = jn != j;
         if (fresh) vp ^= 1;
-        j = jn; o = on; pp ^= 1;
+        j = jn; o = on; cntj = cntn; pp ^= 1;
     }
 }
 
@@ -816,7 +845,7 @@ k_locate_stream(const __grid_constant__ GridDev G, const __grid_constant__ Strea
     }
 }
 
-template <int MODE>
+template <int MODE, bool FAST>
 __device__ __forceinline__ void stream_body(const StreamArgs &A)
 {
     extern __shared__ __align__(32) unsigned char smem_raw[];
@@ -898,7 +927,7 @@ __device__ __forceinline__ void stream_body(const StreamArgs &A)
             else {
                 const int v = sub - B.ne;
                 const int i = v / B.ng, grp = v - i * B.ng;
-                b_unit<MODE>(A, T, V, slot, row_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf, sC, err_local);
+                b_unit<MODE, FAST>(A, T, V, slot, row_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf, sC, err_local);
             }
             const unsigned long long old = warp_release_add(b_fin, 1ULL);
             if (old + 1 == (gen + 1) * TB) {                       // last unit of the chunk: the slot's counters are reset for the ring
@@ -911,9 +940,12 @@ __device__ __forceinline__ void stream_body(const StreamArgs &A)
     if (err_local) atomicAdd(A.G.err_count, err_local);
 }
 
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __grid_constant__ StreamArgs A) { stream_body<kModeRows>(A); }
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_first(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiFirst>(A); }
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_second(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiSecond>(A); }
+// k_pdf_stream: rows of the grid's own 11 columns in order (any leading dimension below 2^29 doubles); k_pdf_stream_cols:
+// any column list (pid subsets, repeated or unknown pids)
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __grid_constant__ StreamArgs A) { stream_body<kModeRows, true>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream_cols(const __grid_constant__ StreamArgs A) { stream_body<kModeRows, false>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_first(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiFirst, false>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_second(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiSecond, false>(A); }
 
 __host__ __device__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
