@@ -220,7 +220,7 @@ __device__ __forceinline__ void make_qdesc(const GridDev &G, double q2, QDesc &d
 __device__ __forceinline__ double continue_two(double f0, double f1, double theta)
 {
     if (f0 > 1e-3 && f1 > 1e-3) {
-        double l0 = log(f0), l1 = log(f1);
+        double l0 = pdf_log(f0), l1 = pdf_log(f1);       // the path's own logarithm (<= 1 ulp, 38 instructions against ~85)
         return exp(l0 + theta * (l1 - l0));
     }
     return f0 + theta * (f1 - f0);

@@ -60,7 +60,10 @@ namespace pdfg {
 #define PDF_S3_MINB 2                                // 2 CTAs of 256 threads per SM: 128 registers, no spills (80 registers
                                                      // and 3 CTAs spilled ~250 B per thread and ran 1.5x slower)
 #endif
-constexpr int kS3Threads = 256;                      // CTA size of the persistent kernel; every warp works alone
+#ifndef PDF_S3_THREADS
+#define PDF_S3_THREADS 256
+#endif
+constexpr int kS3Threads = PDF_S3_THREADS;                      // CTA size of the persistent kernel; every warp works alone
 constexpr int kS3Warps = kS3Threads / 32;
 #ifndef PDF_S3_TILEQ
 #define PDF_S3_TILEQ 8
@@ -69,9 +72,9 @@ constexpr int kS3TileQ = PDF_S3_TILEQ;               // queries per lane in an A
 constexpr int kS3TileA = 32 * kS3TileQ;              // 256 queries per A tile (one warp)
 constexpr int kS3Grp = PDF_S3_GRP;                   // queries of a lane that go through the A steps together
 static_assert(kS3TileQ % kS3Grp == 0, "kS3TileQ must be a multiple of kS3Grp");
-constexpr int kS3Batch = 32;                         // payloads per cp.async stage
+constexpr int kS3Batch = 32;                         // list entries per E batch
 #ifndef PDF_S3_FKU
-#define PDF_S3_FKU 8
+#define PDF_S3_FKU 16
 #endif
 constexpr int kS3FkPerUnit = PDF_S3_FKU;             // Q2 cells per B unit
 constexpr int kS3Lag = PDF_S3_LAG;                   // B(c) tickets follow A(c) tickets by this many rounds
@@ -84,9 +87,19 @@ constexpr int kS3MaxCells = 1024;                    // x cells / Q2 knots the p
 constexpr int kListOvf = 0, kListLowX = 1, kListLowQ = 2, kListHighQ = 3, kListLowXLowQ = 4, kListLowXHighQ = 5, kNumLists = 6;
 static_assert(kListLowX == kRegionLowX && kListLowQ == kRegionLowQ && kListHighQ == kRegionHighQ &&
               kListLowXLowQ == kRegionLowXLowQ && kListLowXHighQ == kRegionLowXHighQ, "list numbers are the region codes");
-constexpr int kStageP = kS3Batch * 32;               // bytes of a payload stage (32 payloads)
-constexpr int kStageV = 16 * kNFP * 8;               // bytes of a value stage (a cell's 16 node rows)
-constexpr int kStageBytes = 2 * kStageP + 2 * kStageV; // per warp: two payload stages (by batch parity), two value stages (by cell parity)
+#ifndef PDF_EV_BATCH
+#define PDF_EV_BATCH 48
+#endif
+#ifndef PDF_EV_DEPTH
+#define PDF_EV_DEPTH 2
+#endif
+constexpr int kEvBatch = PDF_EV_BATCH;               // payloads per stage of a B unit (whole 8-query tiles)
+constexpr int kEvDepth = PDF_EV_DEPTH;               // stages per warp: kEvDepth - 1 batches are in flight under the arithmetic
+constexpr int kEvHdr = 32;                           // stage header {payloads, Q2 cell}
+constexpr int kStageV = 16 * kNFP * 8;               // bytes of a cell's 16 node rows
+constexpr int kEvStage = kEvHdr + kEvBatch * 32 + kStageV;   // a self-contained stage: header | payloads | node rows
+constexpr int kStageBytes = kEvDepth * kEvStage;     // per warp
+static_assert(kEvBatch % 8 == 0 && kEvBatch <= 64, "a stage holds whole 8-query tiles; its payload pieces are copied by 32 lanes x 4");
 
 struct __align__(32) Payload {                       // one sector
     double a, b;                                     // class-dependent abscissae (t_x, t_q / theta / r)
@@ -190,6 +203,17 @@ __device__ __forceinline__ unsigned long long warp_release_add(unsigned long lon
         asm volatile("atom.add.release.gpu.global.u64 %0, [%1], %2;" : "=l"(old) : "l"(p), "l"(v) : "memory");
     return __shfl_sync(0xffffffffu, old, 0);
 }
+// the count of a chunk's finished units needs no fence: a unit only READ the slot (its counts have been consumed, its
+// copies waited for) and wrote rows of `out` that nothing in this launch reads.  The unit that sees the full count
+// zeroes the slot's counters and publishes that with a release (b_done).
+__device__ __forceinline__ unsigned long long warp_count_add(unsigned long long *p, unsigned long long v)
+{
+    unsigned long long old = 0;
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0)
+        asm volatile("atom.add.relaxed.gpu.global.u64 %0, [%1], %2;" : "=l"(old) : "l"(p), "l"(v) : "memory");
+    return __shfl_sync(0xffffffffu, old, 0);
+}
 // one payload = one 32-byte sector, stored whole (STG.256): never a partial-sector write
 __device__ __forceinline__ void store_payload(Payload *dst, double a, double b, unsigned idx, unsigned cell, double pad = 0.0)
 {
@@ -256,7 +280,7 @@ __device__ __forceinline__ Located s3_locate(const GridDev &G, const StreamDev &
 // Out-of-line copies of the transcendental pieces of the E units: inlined, the library logarithms and the
 // continuation formulas made the kernel 22 700 instructions (364 KB), and warps of three different work kinds
 // per SM evicted one another's code from the instruction caches (~20 clk per issued instruction).
-__device__ __noinline__ double s3_log(double v) { return log(v); }
+__device__ __noinline__ double s3_log(double v) { return pdf_log(v); }
 __device__ __noinline__ double s3_two(double f0, double f1, double theta) { return continue_two(f0, f1, theta); }
 __device__ __noinline__ double s3_lowq(double fmin, double fplus, double r, double lnr) { return lowq_continue_ln(fmin, fplus, r, lnr); }
 
@@ -284,25 +308,33 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
     const double inv_du0 = 1.0 / (__ldg(G.uk + 1) - u0);
     const double sA = __ldg(G.sk + nqt - 2), inv_ds = 1.0 / (__ldg(G.sk + nqt - 1) - sA);
     const double inv_qmin = 1.0 / __longlong_as_double(qminb);
-#pragma unroll 1
-    for (int g0 = 0; g0 < kS3TileQ; g0 += kS3Grp) {
-        double xv[kS3Grp], qv[kS3Grp], sc[kS3Grp];
+    // The groups of kS3Grp queries per lane go through a software pipeline: the loads of group g + 1 are issued before
+    // group g is located and its logarithms taken, and the payloads of group g are stored after group g + 1 has been
+    // computed, so that the ~1 us of the input loads and the ~1-2 us of the slot atomics travel under arithmetic
+    // instead of adding up per group (phase clocks of profile note r2c: 19.9 us per 256-query tile, 40 % of every
+    // warp's time, with the four groups strictly one after the other).
+    struct Grp { double xv[kS3Grp], qv[kS3Grp], sc[kS3Grp]; };
+    struct Out { double pa[kS3Grp], pb[kS3Grp], sc[kS3Grp]; int key[kS3Grp]; unsigned cell[kS3Grp], pos[kS3Grp]; bool any_list; };
+    auto load = [&](int g0) {
+        Grp r;
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
             const long long e = t0 + (g0 + q) * 32 + lane;
-            xv[q] = 1.0; qv[q] = 1.0; sc[q] = 0.0;
+            r.xv[q] = 1.0; r.qv[q] = 1.0; r.sc[q] = 0.0;
             if (e < t1) {
-                xv[q] = __ldcs(A.x + e); qv[q] = __ldcs(A.q2 + e);
-                if (MODE == kModeLumiFirst) sc[q] = __ldcs(A.w + e) / (xv[q] * __ldcs(A.x2 + e));   // f = xf / x on both sides (eq. 3.3)
+                r.xv[q] = __ldcs(A.x + e); r.qv[q] = __ldcs(A.q2 + e);
+                if (MODE == kModeLumiFirst) r.sc[q] = __ldcs(A.w + e) / (r.xv[q] * __ldcs(A.x2 + e));   // f = xf / x on both sides (eq. 3.3)
             }
         }
+        return r;
+    };
+    // classify, locate, abscissae, and the slot atomics of the cell bins (in flight when this returns)
+    auto compute = [&](const Grp &in, int g0) {
+        Out o;
         Located L[kS3Grp];
 #pragma unroll
-        for (int q = 0; q < kS3Grp; ++q) L[q] = s3_locate(G, B, T, xv[q], qv[q], xminb, xmaxb, qminb, qmaxb);
-        double pa[kS3Grp], pb[kS3Grp];
-        int key[kS3Grp];                               // >= 0: cell bin; -1 - k: list k; INT_MIN: invalid or no query
-        unsigned cell[kS3Grp];
-        bool any_list = false;
+        for (int q = 0; q < kS3Grp; ++q) L[q] = s3_locate(G, B, T, in.xv[q], in.qv[q], xminb, xmaxb, qminb, qmaxb);
+        o.any_list = false;
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
             const long long e = t0 + (g0 + q) * 32 + lane;
@@ -313,43 +345,47 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
             const int jg = L[q].g < nqt - 1 ? L[q].g : nqt - 2;       // only Q2 == Q2max lands on the last knot: it belongs to the last cell
             const double2 ci = lds_v2f64(T.cx + 48u * i), cj = lds_v2f64(T.cq + 48u * jg);   // {ln lower knot, 1/dln}
             double lx = 0.0, lq = 0.0;
-            if (r != kRegionInvalid) { lx = pdf_log(xv[q]); lq = pdf_log(qv[q]); }
+            if (r != kRegionInvalid) { lx = pdf_log(in.xv[q]); lq = pdf_log(in.qv[q]); }
             // t = 1 exactly on the last knot (the only knot that belongs to the cell on its left, C-4)
-            pa[q] = lowx ? (lx - u0) * inv_du0                                    // theta_x (C-7)
-                         : (__double_as_longlong(xv[q]) == xmaxb) ? 1.0 : (lx - ci.x) * ci.y;
-            pb[q] = lowq ? qv[q] * inv_qmin                                       // r (C-9)
-                  : highq ? (lq - sA) * inv_ds                                    // theta_q (C-8)
-                          : (__double_as_longlong(qv[q]) == qmaxb) ? 1.0 : (lq - cj.x) * cj.y;
-            key[q] = r == kRegionInterior ? i * nqt + jg : -1 - r;               // region codes 1..5 are the list numbers
-            cell[q] = r == kRegionInterior ? ((unsigned)i | ((unsigned)jg << 16)) : lowx ? (unsigned)jg : (unsigned)i;
-            if (e >= t1 || r == kRegionInvalid) key[q] = INT_MIN;
-            any_list |= key[q] < 0 && key[q] != INT_MIN;
+            o.pa[q] = lowx ? (lx - u0) * inv_du0                                    // theta_x (C-7)
+                           : (__double_as_longlong(in.xv[q]) == xmaxb) ? 1.0 : (lx - ci.x) * ci.y;
+            o.pb[q] = lowq ? in.qv[q] * inv_qmin                                    // r (C-9)
+                    : highq ? (lq - sA) * inv_ds                                    // theta_q (C-8)
+                            : (__double_as_longlong(in.qv[q]) == qmaxb) ? 1.0 : (lq - cj.x) * cj.y;
+            o.sc[q] = in.sc[q];
+            o.key[q] = r == kRegionInterior ? i * nqt + jg : -1 - r;               // region codes 1..5 are the list numbers
+            o.cell[q] = r == kRegionInterior ? ((unsigned)i | ((unsigned)jg << 16)) : lowx ? (unsigned)jg : (unsigned)i;
+            if (e >= t1 || r == kRegionInvalid) o.key[q] = INT_MIN;
+            o.any_list |= o.key[q] < 0 && o.key[q] != INT_MIN;
         }
-        unsigned pos[kS3Grp];
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
-            pos[q] = 0u;
-            if (key[q] >= 0) pos[q] = atomicAdd(counts + key[q], 1u);
+            o.pos[q] = 0u;
+            if (o.key[q] >= 0) o.pos[q] = atomicAdd(counts + o.key[q], 1u);
         }
+        return o;
+    };
+    // bin overflow, list slots, payload stores (reads the atomics' results)
+    auto finish = [&](Out &o, int g0) {
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q)
-            if (key[q] >= 0 && pos[q] >= (unsigned)B.cap) { key[q] = -1 - kListOvf; any_list = true; }   // bin full: to the overflow list
+            if (o.key[q] >= 0 && o.pos[q] >= (unsigned)B.cap) { o.key[q] = -1 - kListOvf; o.any_list = true; }   // bin full: to the overflow list
         // list entries (extrapolated queries, bin overflow; rare): one atomic per warp and list reserves the run of
         // the list's lanes
-        if (__any_sync(0xffffffffu, any_list)) {
+        if (__any_sync(0xffffffffu, o.any_list)) {
 #pragma unroll
             for (int q = 0; q < kS3Grp; ++q) {
-                const bool mine = key[q] < 0 && key[q] != INT_MIN;
+                const bool mine = o.key[q] < 0 && o.key[q] != INT_MIN;
                 const unsigned act = __ballot_sync(0xffffffffu, mine);
                 if (act == 0u) continue;
                 if (mine) {
-                    const int k = -1 - key[q];
+                    const int k = -1 - o.key[q];
                     const unsigned peers = __match_any_sync(act, k);
                     const int leader = __ffs(peers) - 1;
                     unsigned base = 0;
                     if (lane == leader) base = atomicAdd(lcount + k, (unsigned)__popc(peers));
                     base = __shfl_sync(peers, base, leader);
-                    pos[q] = base + (unsigned)__popc(peers & ((1u << lane) - 1u));
+                    o.pos[q] = base + (unsigned)__popc(peers & ((1u << lane) - 1u));
                 }
             }
         }
@@ -358,15 +394,29 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
             const long long e = t0 + (g0 + q) * 32 + lane;
             if (e >= t1) continue;
             const unsigned idx = A.orig ? __ldcs(A.orig + e) : (unsigned)(e - chunk_base);
-            if (key[q] == INT_MIN) {                                              // C-10: NaN row, counted
-                double *o = A.out + (A.orig ? (long long)idx : e) * A.ld;
+            if (o.key[q] == INT_MIN) {                                              // C-10: NaN row, counted
+                double *op = A.out + (A.orig ? (long long)idx : e) * A.ld;
                 const int ncol = MODE == kModeLumiFirst ? kNFP : A.cm.n;
-                for (int p = 0; p < ncol; ++p) o[p] = qnan();
+                for (int p = 0; p < ncol; ++p) op[p] = qnan();
                 if (A.count_err) ++err_local;
-            } else if (key[q] < 0) store_payload(lists + (size_t)(-1 - key[q]) * A.chunk + pos[q], pa[q], pb[q], idx, cell[q], sc[q]);
-            else store_payload(bins + (size_t)key[q] * B.cap + pos[q], pa[q], pb[q], idx, cell[q], sc[q]);
+            } else if (o.key[q] < 0) store_payload(lists + (size_t)(-1 - o.key[q]) * A.chunk + o.pos[q], o.pa[q], o.pb[q], idx, o.cell[q], o.sc[q]);
+            else store_payload(bins + (size_t)o.key[q] * B.cap + o.pos[q], o.pa[q], o.pb[q], idx, o.cell[q], o.sc[q]);
         }
+    };
+    Grp next = load(0);
+    Out prev;
+    prev.any_list = false;
+#pragma unroll
+    for (int q = 0; q < kS3Grp; ++q) { prev.key[q] = INT_MIN; prev.pos[q] = 0u; prev.cell[q] = 0u; prev.pa[q] = prev.pb[q] = prev.sc[q] = 0.0; }
+#pragma unroll 1
+    for (int g0 = 0; g0 < kS3TileQ; g0 += kS3Grp) {
+        const Grp cur = next;
+        if (g0 + kS3Grp < kS3TileQ) next = load(g0 + kS3Grp);
+        Out o = compute(cur, g0);
+        if (g0 > 0) finish(prev, g0 - kS3Grp);
+        prev = o;
     }
+    finish(prev, kS3TileQ - kS3Grp);
 }
 
 // ---- B units: DMMA contractions on the cell's values ---------------------------------------------
@@ -419,13 +469,17 @@ __device__ __forceinline__ void store_row(const StreamArgs &A, double *rp, int t
     }
 }
 
-// interior cells of x cell i, Q2 cells [fk0, fk1): the (cell, batch of <= 32 payloads) sequence of the unit runs
-// through the warp's stages: two payload stages (batch parity) and two value stages (cell parity; a cell's 16 node
-// rows, node n = 4 * (Q2 row) + (x node)).  Version 4 of the loop (profile r2a: version 3 spent 108 warp instructions
-// per 8-query tile, 8 of them DMMAs): the cell's operand fragments and the coefficients of both node weights are read
-// once per cell and stay in registers, rows with the grid's own 11 columns (FAST) leave by four fixed stores from one
-// 64-bit multiply-add, lanes beyond the batch run on whatever the stage holds (a row of A only ever meets its own
-// row of D) and only their stores are predicated.
+// interior cells of x cell i, Q2 cells [fk0, fk1).  The unit is a stream of batches: <= kEvBatch payloads of ONE cell
+// together with that cell's 16 node rows (node n = 4 * (Q2 row) + (x node)), copied by cp.async into one of the warp's
+// kEvDepth self-contained stages [header | payloads | node rows].  The issuing side of the loop runs kEvDepth - 1
+// batches ahead of the arithmetic (one commit group per loop turn, empty ones once the unit's cells are exhausted), so
+// the ~1.5 us L2 latency of a batch is paid once per unit, not once per batch: with one batch in flight (versions 3
+// and 4) a warp computed ~0.4 us per batch and waited ~1 us for the next (profile note r2c).
+// The arithmetic of a tile (version 4, profile r2a: version 3 spent 108 warp instructions per 8-query tile, 8 of them
+// DMMAs): the cell's operand fragments and the coefficients of both node weights are read once per batch and stay in
+// registers, rows with the grid's own 11 columns (FAST) leave by four fixed stores from one 64-bit multiply-add, lanes
+// beyond the batch run on whatever the stage holds (a row of A only ever meets its own row of D) and only their
+// stores are predicated.
 template <int MODE, bool FAST>
 __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, const double *__restrict__ Vm, int slot,
                                        long long chunk_base, int i, int fk0, int fk1, unsigned sbuf, unsigned sC,
@@ -440,163 +494,153 @@ __device__ __forceinline__ void b_unit(const StreamArgs &A, const StreamTab &T, 
     unsigned live = __ballot_sync(0xffffffffu, mycnt > 0);      // cells of the unit that hold queries
     if (live == 0u) return;
     const int nx = G.nx;
-    // this lane's payload of a batch: bins of x cell i, entry `lane`
-    const char *binl = reinterpret_cast<const char *>(A.W.bins + ((size_t)slot * B.nbins + (size_t)i * B.nqt) * B.cap) + 32u * lane;
+    const char *bin0 = reinterpret_cast<const char *>(A.W.bins + ((size_t)slot * B.nbins + (size_t)i * B.nqt) * B.cap);
     const unsigned capb = 32u * (unsigned)B.cap;
+    const char *Vb = reinterpret_cast<const char *>(Vm);
+    const unsigned rowb = (unsigned)(nx * kNFP * 8);
+    int o = 0;                                                  // payloads of the current cell already issued
+    // the next batch into stage `st`; an empty commit group behind a zero header once the cells are exhausted
+    auto produce = [&](unsigned st) {
+        if (live == 0u) {
+            if (lane == 0) asm volatile("st.shared.v2.u32 [%0], {%1,%1};" ::"r"(st), "r"(0) : "memory");
+            cp_async_commit();
+            return;
+        }
+        const int j = __ffs(live) - 1, fk = fk0 + j;
+        const int cntj = __shfl_sync(0xffffffffu, mycnt, j);
+        const int n = min(kEvBatch, cntj - o);
+        {
+            // payloads: 2 n pieces of 16 bytes, contiguous in the bin
+            const char *src = bin0 + ((size_t)(unsigned)fk * capb + 32u * (unsigned)o);
+#pragma unroll
+            for (int k = 0; k < (2 * kEvBatch + 31) / 32; ++k) {
+                const int e = lane + 32 * k;
+                if (e < 2 * n) cp_async16_cg(st + kEvHdr + 16u * e, src + 16 * e);
+            }
+        }
+        {
+            // the cell's 16 node rows: 96 pieces, piece e = lane + 32 k, node = e / 6 = 4 b + a (Q2 row b, x node a)
+            const double aL = lds_f64(T.cq + 48u * fk + 16u), aR = lds_f64(T.cq + 48u * fk + 32u);
+            const int elo = aL == 1.0 ? 1 : 0, ehi = aR == 1.0 ? 1 : 0;       // one-sided ends of a sub-grid (q_point_cell)
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const int e = lane + 32 * k, node = e / 6, piece = e - node * 6, b = node >> 2;
+                const int row = fk - 1 + b + (b == 0 ? elo : 0) - (b == 3 ? ehi : 0);
+                cp_async16_ca(st + kEvHdr + kEvBatch * 32 + 16u * e,
+                              Vb + ((size_t)((unsigned)row * rowb) + (unsigned)((xnode(i, node & 3, nx) * kNFP + 2 * piece) * 8)));
+            }
+        }
+        if (lane == 0) asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(st), "r"(n), "r"(fk) : "memory");
+        cp_async_commit();
+        o += n;
+        if (o >= cntj) { live &= live - 1; o = 0; }
+    };
     WCoef kx;
     {
         const double2 ab = lds_v2f64(T.cx + 48u * i + 16u), cd = lds_v2f64(T.cx + 48u * i + 32u);
         kx = weight_coef(ab.x, ab.y, cd.x, cd.y, t);            // x-axis weight of this lane's node, fixed for the unit
     }
-    // the 96 16-byte pieces of a cell's 16 node rows are copied by 32 lanes x 3: piece e = lane + 32 k,
-    // node = e / 6 = 4 b + a; the x-node columns (byte offsets vo) are fixed for the unit, the Q2 rows follow the cell
-    const unsigned sP = sbuf, sV = sbuf + 2u * kStageP;
-    unsigned vo[3];
-    int vb[3];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        const int e = lane + 32 * k, node = e / 6, piece = e - node * 6;
-        vb[k] = node >> 2;
-        vo[k] = (unsigned)((xnode(i, node & 3, nx) * kNFP + 2 * piece) * 8);
-    }
-    const char *Vb = reinterpret_cast<const char *>(Vm);
-    const unsigned rowb = (unsigned)(nx * kNFP * 8);
-    auto issue = [&](int j, int o, int cntj, int pp, int vp, bool with_values) {
-        const int fk = fk0 + j;
-        if (lane < cntj - o) {                                   // at most 32 lanes
-            const char *src = binl + ((size_t)(unsigned)fk * capb + 32u * (unsigned)o);
-            const unsigned dst = sP + (unsigned)(pp * kStageP) + 32u * lane;
-            cp_async16_cg(dst, src);
-            cp_async16_cg(dst + 16u, src + 16);
-        }
-        if (with_values) {
-            const double aL = lds_f64(T.cq + 48u * fk + 16u), aR = lds_f64(T.cq + 48u * fk + 32u);
-            const int elo = aL == 1.0 ? 1 : 0, ehi = aR == 1.0 ? 1 : 0;       // one-sided ends of a sub-grid (q_point_cell)
-            const unsigned dv = sV + (unsigned)(vp * kStageV) + 16u * lane;
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const int row = fk - 1 + vb[k] + (vb[k] == 0 ? elo : 0) - (vb[k] == 3 ? ehi : 0);
-                cp_async16_ca(dv + 512u * k, Vb + ((size_t)((unsigned)row * rowb) + vo[k]));
-            }
-        }
-        cp_async_commit();
-    };
-    int j = __ffs(live) - 1, o = 0, pp = 0, vp = 0;
-    int cntj = __shfl_sync(0xffffffffu, mycnt, j);
-    issue(j, 0, cntj, 0, 0, true);
-    bool fresh = true;                                          // the current batch opens a cell
-    WCoef kq;
-    double fb0, fb1, fb2, fb3, fc0, fc1, fc2, fc3;              // the cell's operand fragments: step r pairs Q2 row (t ^ r) with x node t
-    fb0 = fb1 = fb2 = fb3 = fc0 = fc1 = fc2 = fc3 = 0.0;
-    kq.c0 = kq.c1 = kq.c2 = kq.c3 = 0.0;
-    const unsigned fo = (unsigned)(t * kNFP * 8 + 8 * g);
     // pass 2 of the luminosity: the coupling's fragments (flavour 4 s + t of parton 1 against flavours g, 8 + g of parton 2)
     double cf0x = 0.0, cf0y = 0.0, cf1x = 0.0, cf1y = 0.0, cf2x = 0.0, cf2y = 0.0;
     if (MODE == kModeLumiSecond) {
-        cf0x = lds_f64(sC + (unsigned)((0 + t) * 128 + 8 * g)); cf1x = lds_f64(sC + (unsigned)((4 + t) * 128 + 8 * g));
-        cf2x = lds_f64(sC + (unsigned)((8 + t) * 128 + 8 * g));
-        if (g < 4) {
-            cf0y = lds_f64(sC + (unsigned)((0 + t) * 128 + 8 * g) + 64u); cf1y = lds_f64(sC + (unsigned)((4 + t) * 128 + 8 * g) + 64u);
-            cf2y = lds_f64(sC + (unsigned)((8 + t) * 128 + 8 * g) + 64u);
-        }
+        const unsigned pc = sC + (unsigned)(t * 128 + 8 * g);
+        cf0x = lds_f64(pc); cf1x = lds_f64(pc + 512u); cf2x = lds_f64(pc + 1024u);
+        if (g < 4) { cf0y = lds_f64(pc + 64u); cf1y = lds_f64(pc + 512u + 64u); cf2y = lds_f64(pc + 1024u + 64u); }
     }
-    // FAST: rows of A.ld doubles, this lane's columns 2t, 2t+1 (all t), 8 + 2t (t < 2), 9 (t == 0)
+    // rows of A.ld doubles, this lane's columns 2t, 2t+1 (all t), 8 + 2t (t < 2), 9 (t == 0)
     const unsigned ldb = (unsigned)(A.ld * 8);
     char *outl = reinterpret_cast<char *>(A.out + chunk_base * (MODE == kModeLumiFirst ? (long long)kNFP : A.ld)) + 16 * t;
-    for (;;) {
-        // successor of (j, o)
-        int jn = j, on = o + kS3Batch, cntn = cntj;
-        if (on >= cntj) {
-            live &= live - 1; on = 0; jn = -1;
-            if (live) { jn = __ffs(live) - 1; cntn = __shfl_sync(0xffffffffu, mycnt, jn); }
-        }
-        if (jn >= 0) { issue(jn, on, cntn, pp ^ 1, jn != j ? vp ^ 1 : vp, jn != j); cp_async_wait<1>(); }
-        else cp_async_wait<0>();
+#pragma unroll 1
+    for (int k = 0; k < kEvDepth - 1; ++k) produce(sbuf + (unsigned)(k * kEvStage));
+#pragma unroll 1
+    for (unsigned seq = 0;; ++seq) {
+        produce(sbuf + (unsigned)(((seq + kEvDepth - 1) % kEvDepth) * kEvStage));
+        cp_async_wait<kEvDepth - 1>();
         __syncwarp();
-        if (fresh) {
-            const int fk = fk0 + j;
+        const unsigned st = sbuf + (unsigned)((seq % kEvDepth) * kEvStage);
+        int n, fk;
+        asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(n), "=r"(fk) : "r"(st));
+        if (n == 0) break;
+        WCoef kq;
+        {
             const double2 ab = lds_v2f64(T.cq + 48u * fk + 16u), cd = lds_v2f64(T.cq + 48u * fk + 32u);
             kq = weight_coef(ab.x, ab.y, cd.x, cd.y, t);
-            const unsigned sv = sV + (unsigned)(vp * kStageV) + fo;
-            fb0 = lds_f64(sv + (unsigned)(4 * (t ^ 0) * kNFP * 8)); fb1 = lds_f64(sv + (unsigned)(4 * (t ^ 1) * kNFP * 8));
-            fb2 = lds_f64(sv + (unsigned)(4 * (t ^ 2) * kNFP * 8)); fb3 = lds_f64(sv + (unsigned)(4 * (t ^ 3) * kNFP * 8));
-            if (g < 4) {
-                fc0 = lds_f64(sv + (unsigned)(4 * (t ^ 0) * kNFP * 8) + 64u); fc1 = lds_f64(sv + (unsigned)(4 * (t ^ 1) * kNFP * 8) + 64u);
-                fc2 = lds_f64(sv + (unsigned)(4 * (t ^ 2) * kNFP * 8) + 64u); fc3 = lds_f64(sv + (unsigned)(4 * (t ^ 3) * kNFP * 8) + 64u);
-            }
         }
-        const unsigned sb = sP + (unsigned)(pp * kStageP) + 32u * g;
-        const int nact = min(kS3Batch, cntj - o);
-        {
-            // the next tile's abscissae are fetched under this tile's arithmetic
-            double2 abn = lds_v2f64(sb);
-            unsigned idxn = lds_u32(sb + 16u);
+        // the cell's operand fragments: step r pairs Q2 row (t ^ r) with x node t; flavours g and 8 + g
+        const unsigned sv = st + kEvHdr + kEvBatch * 32 + (unsigned)(t * kNFP * 8 + 8 * g);
+        const double fb0 = lds_f64(sv + (unsigned)(4 * (t ^ 0) * kNFP * 8)), fb1 = lds_f64(sv + (unsigned)(4 * (t ^ 1) * kNFP * 8));
+        const double fb2 = lds_f64(sv + (unsigned)(4 * (t ^ 2) * kNFP * 8)), fb3 = lds_f64(sv + (unsigned)(4 * (t ^ 3) * kNFP * 8));
+        double fc0 = 0.0, fc1 = 0.0, fc2 = 0.0, fc3 = 0.0;
+        if (g < 4) {
+            fc0 = lds_f64(sv + (unsigned)(4 * (t ^ 0) * kNFP * 8) + 64u); fc1 = lds_f64(sv + (unsigned)(4 * (t ^ 1) * kNFP * 8) + 64u);
+            fc2 = lds_f64(sv + (unsigned)(4 * (t ^ 2) * kNFP * 8) + 64u); fc3 = lds_f64(sv + (unsigned)(4 * (t ^ 3) * kNFP * 8) + 64u);
+        }
+        const unsigned sb = st + kEvHdr + 32u * g;
+        // the next tile's abscissae are fetched under this tile's arithmetic
+        double2 abn = lds_v2f64(sb);
+        unsigned idxn = lds_u32(sb + 16u);
 #pragma unroll 1
-            for (int m0 = 0; m0 < nact; m0 += 8) {
-                const bool valid = m0 + g < nact;
-                const double tx = abn.x, tq = abn.y;
-                const unsigned idx = idxn;
-                const unsigned sn = sb + 32u * (unsigned)((m0 + 8) & (kS3Batch - 1));      // wraps to tile 0 after the last tile (unused)
-                abn = lds_v2f64(sn); idxn = lds_u32(sn + 16u);
-                // pass 2 of the luminosity: this query's row of pass 1 in the A-operand layout (flavour 4 s + t), fetched
-                // under the contraction; lane t = 3 of step 2 gets the scale column
-                double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-                if (MODE == kModeLumiSecond && valid) {
-                    const double *fr = A.f1 + (chunk_base + idx) * kNFP + t;
-                    a0 = __ldcs(fr); a1 = __ldcs(fr + 4); a2 = __ldcs(fr + 8);
-                }
-                const double wx = weight_eval(kx, tx);
-                const double wq0 = weight_eval(kq, tq);
-                const double wq1 = __shfl_xor_sync(0xffffffffu, wq0, 1);
-                const double wq2 = __shfl_xor_sync(0xffffffffu, wq0, 2);
-                const double wq3 = __shfl_xor_sync(0xffffffffu, wq0, 3);
-                Acc d = {0.0, 0.0, 0.0, 0.0};
-                kstep(d, wq0 * wx, make_double2(fb0, fc0));
-                kstep(d, wq1 * wx, make_double2(fb1, fc1));
-                kstep(d, wq2 * wx, make_double2(fb2, fc2));
-                kstep(d, wq3 * wx, make_double2(fb3, fc3));
-                if (MODE == kModeRows) {
-                    if (FAST) {
-                        if (valid) {
-                            char *rp = outl + (size_t)idx * ldb;
-                            asm volatile("st.global.f64 [%0], %1;" ::"l"(rp), "d"(d.d00) : "memory");
-                            asm volatile("st.global.f64 [%0+8], %1;" ::"l"(rp), "d"(d.d01) : "memory");
-                            if (t < 2) asm volatile("st.global.f64 [%0+64], %1;" ::"l"(rp), "d"(d.d10) : "memory");
-                            if (t == 0) asm volatile("st.global.f64 [%0+72], %1;" ::"l"(rp), "d"(d.d11) : "memory");
-                        }
-                    } else if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, d);
-                } else if (MODE == kModeLumiFirst) {
-                    // rows of 12 on 32-byte sectors: two stores write the three sectors whole (no zero fill needed)
+        for (int m0 = 0; m0 < n; m0 += 8) {
+            const bool valid = m0 + g < n;
+            const double tx = abn.x, tq = abn.y;
+            const unsigned idx = idxn;
+            const unsigned sn = sb + 32u * (unsigned)(m0 + 8 < kEvBatch ? m0 + 8 : 0);     // (the tile after the last is never used)
+            abn = lds_v2f64(sn); idxn = lds_u32(sn + 16u);
+            // pass 2 of the luminosity: this query's row of pass 1 in the A-operand layout (flavour 4 s + t), fetched
+            // under the contraction; lane t = 3 of step 2 gets the scale column
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+            if (MODE == kModeLumiSecond && valid) {
+                const double *fr = A.f1 + (chunk_base + idx) * kNFP + t;
+                a0 = __ldcs(fr); a1 = __ldcs(fr + 4); a2 = __ldcs(fr + 8);
+            }
+            const double wx = weight_eval(kx, tx);
+            const double wq0 = weight_eval(kq, tq);
+            const double wq1 = __shfl_xor_sync(0xffffffffu, wq0, 1);
+            const double wq2 = __shfl_xor_sync(0xffffffffu, wq0, 2);
+            const double wq3 = __shfl_xor_sync(0xffffffffu, wq0, 3);
+            Acc d = {0.0, 0.0, 0.0, 0.0};
+            kstep(d, wq0 * wx, make_double2(fb0, fc0));
+            kstep(d, wq1 * wx, make_double2(fb1, fc1));
+            kstep(d, wq2 * wx, make_double2(fb2, fc2));
+            kstep(d, wq3 * wx, make_double2(fb3, fc3));
+            if (MODE == kModeRows) {
+                if (FAST) {
                     if (valid) {
-                        double *rp = reinterpret_cast<double *>(outl + (size_t)idx * (unsigned)(kNFP * 8));
-                        *reinterpret_cast<double2 *>(rp) = make_double2(d.d00, d.d01);
-                        if (t == 0) *reinterpret_cast<double2 *>(rp + 8) = make_double2(d.d10, d.d11);
-                        if (t == 1) *reinterpret_cast<double2 *>(rp + 8) = make_double2(d.d10, lds_f64(sb + 32u * (unsigned)m0 + 24u));
+                        char *rp = outl + (size_t)idx * ldb;
+                        asm volatile("st.global.f64 [%0], %1;" ::"l"(rp), "d"(d.d00) : "memory");
+                        asm volatile("st.global.f64 [%0+8], %1;" ::"l"(rp), "d"(d.d01) : "memory");
+                        if (t < 2) asm volatile("st.global.f64 [%0+64], %1;" ::"l"(rp), "d"(d.d10) : "memory");
+                        if (t == 0) asm volatile("st.global.f64 [%0+72], %1;" ::"l"(rp), "d"(d.d11) : "memory");
                     }
-                } else {
-                    // G[q][j] = sum_i f1[q][i] C[i][j] by 6 more DMMAs, then the dot with this row and the scale
-                    Acc gq = {0.0, 0.0, 0.0, 0.0};
-                    kstep(gq, a0, make_double2(cf0x, cf0y));
-                    kstep(gq, a1, make_double2(cf1x, cf1y));
-                    kstep(gq, t == 3 ? 0.0 : a2, make_double2(cf2x, cf2y));
-                    double dot = fma(d.d00, gq.d00, fma(d.d01, gq.d01, fma(d.d10, gq.d10, d.d11 * gq.d11)));
-                    dot += __shfl_xor_sync(0xffffffffu, dot, 1);
-                    dot += __shfl_xor_sync(0xffffffffu, dot, 2);
-                    const double scale = __shfl_sync(0xffffffffu, a2, lane | 3);
-                    if (valid && t == 0) {
-                        double v = scale * dot;
-                        if (v != v && a0 != a0) { v = qnan(); if (A.count_err) ++err_local; }   // the x1 parton was invalid (C-10): counted once
-                        A.out[chunk_base + idx] = v;
-                    }
+                } else if (valid) store_row(A, A.out + (chunk_base + idx) * A.ld, t, d);
+            } else if (MODE == kModeLumiFirst) {
+                // rows of 12 on 32-byte sectors: two stores write the three sectors whole (no zero fill needed)
+                if (valid) {
+                    double *rp = reinterpret_cast<double *>(outl + (size_t)idx * (unsigned)(kNFP * 8));
+                    *reinterpret_cast<double2 *>(rp) = make_double2(d.d00, d.d01);
+                    if (t == 0) *reinterpret_cast<double2 *>(rp + 8) = make_double2(d.d10, d.d11);
+                    if (t == 1) *reinterpret_cast<double2 *>(rp + 8) = make_double2(d.d10, lds_f64(sb + 32u * (unsigned)m0 + 24u));
+                }
+            } else {
+                // G[q][j] = sum_i f1[q][i] C[i][j] by 6 more DMMAs, then the dot with this row and the scale
+                Acc gq = {0.0, 0.0, 0.0, 0.0};
+                kstep(gq, a0, make_double2(cf0x, cf0y));
+                kstep(gq, a1, make_double2(cf1x, cf1y));
+                kstep(gq, t == 3 ? 0.0 : a2, make_double2(cf2x, cf2y));
+                double dot = fma(d.d00, gq.d00, fma(d.d01, gq.d01, fma(d.d10, gq.d10, d.d11 * gq.d11)));
+                dot += __shfl_xor_sync(0xffffffffu, dot, 1);
+                dot += __shfl_xor_sync(0xffffffffu, dot, 2);
+                const double scale = __shfl_sync(0xffffffffu, a2, lane | 3);
+                if (valid && t == 0) {
+                    double v = scale * dot;
+                    if (v != v && a0 != a0) { v = qnan(); if (A.count_err) ++err_local; }   // the x1 parton was invalid (C-10): counted once
+                    A.out[chunk_base + idx] = v;
                 }
             }
         }
-        __syncwarp();                                           // the stages are free for the copies after next
-        if (jn < 0) break;
-        fresh = jn != j;
-        if (fresh) vp ^= 1;
-        j = jn; o = on; cntj = cntn; pp ^= 1;
+        __syncwarp();                                           // the stage is free for the copies after next
     }
+    cp_async_wait<0>();                                         // the empty groups behind the last batch
 }
 
 // ---- E units: the lists (extrapolation classes, bin overflow), one query per lane -----------------
@@ -929,7 +973,7 @@ __device__ __forceinline__ void stream_body(const StreamArgs &A)
                 const int i = v / B.ng, grp = v - i * B.ng;
                 b_unit<MODE, FAST>(A, T, V, slot, row_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf, sC, err_local);
             }
-            const unsigned long long old = warp_release_add(b_fin, 1ULL);
+            const unsigned long long old = warp_count_add(b_fin, 1ULL);
             if (old + 1 == (gen + 1) * TB) {                       // last unit of the chunk: the slot's counters are reset for the ring
                 unsigned *cz = A.W.counts + (size_t)slot * (B.nbins + 32);
                 for (int k = lane; k < B.nbins + 32; k += 32) cz[k] = 0u;
