@@ -30,9 +30,10 @@ METRIC = "PDF evaluations (points x flavours)/s"
 UNIT = "points*flavours/s"
 WORKLOAD = ("configs[2] (C2): 196x(6+8+40) LHAPDF-shaped grid, 11 flavours, "
             "5% of queries extrapolated, + alpha_s over the same Q2 (60 knots)")
-# dram__bytes_read.sum + dram__bytes_write.sum of k_pdf_stream at n = 1e8 (C2), one ncu capture of this
-# command line: profiles/r1i_traffic_pdf_stream_1e8.csv; null for any other n
-NCU_TRAFFIC_BYTES_1E8 = 5887876352 + 22069447424
+# roofline.traffic is a MEASUREMENT, not a constant of this file: dram__bytes_read.sum + dram__bytes_write.sum of
+# k_pdf_stream at n = 1e8 (C2) come from the newest ncu capture profiles/*_traffic_pdf_stream_1e8.csv, whose note
+# (same name, .md) records the sha256 of the csrc/ tree it was taken on; a capture of another source tree is stale
+# and the line carries null (there is no .git on the GPU box, so the tree is identified by content).
 # PAPER.md Table 3.3 (L1896-1905), seconds: N_rep -> (LHAPDF CPU, PDFFlow GPU, PDFFlow CPU) on the thesis's system P1
 PAPER_TABLE33 = {10: (0.08, 0.07, 0.05), 50: (0.41, 0.35, 0.28), 100: (0.83, 0.69, 0.56),
                  200: (1.87, 1.46, 1.12), 300: (2.85, 1.29, 1.79), 400: (3.63, 1.69, 2.12)}
@@ -57,6 +58,51 @@ def parse_args():
     ap.add_argument("--table33-reps", type=int, default=10, help="timed calls per N_rep of the Table 3.3 leg (0 = skip)")
     ap.add_argument("--skip-extras", action="store_true", help="only the headline step (no lumi/members/e2e/cpu)")
     return ap.parse_args()
+
+
+def csrc_sha256():
+    """sha256 over the names and contents of the CUDA sources (what a traffic capture is valid for)"""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2302_03343_b200", "csrc", "*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()
+
+
+def load_traffic(n):
+    """(bytes or None, source dict): the newest profiles/*_traffic_pdf_stream_1e8.csv if it matches this source tree"""
+    import csv
+    import glob
+    import re
+    if n != 100_000_000:
+        return None, {"traffic_source": None, "traffic_note": "captures exist for n = 1e8 only"}
+    caps = sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic_pdf_stream_1e8.csv")))
+    if not caps:
+        return None, {"traffic_source": None, "traffic_note": "no capture under profiles/"}
+    cap = caps[-1]
+    note = cap[:-4] + ".md"
+    want = None
+    if os.path.exists(note):
+        m = re.search(r"csrc_sha256:\s*([0-9a-f]{64})", open(note).read())
+        want = m.group(1) if m else None
+    src = {"traffic_source": os.path.relpath(cap, ROOT), "traffic_csrc_sha256": want}
+    if want != csrc_sha256():
+        src["traffic_note"] = "stale: the capture was taken on another csrc/ tree"
+        return None, src
+    rd = wr = None
+    for row in csv.reader(open(cap)):
+        if len(row) > 14 and "k_pdf_stream" in row[4]:
+            if row[12] == "dram__bytes_read.sum":
+                rd = float(row[14].replace(",", ""))
+            if row[12] == "dram__bytes_write.sum":
+                wr = float(row[14].replace(",", ""))
+    if rd is None or wr is None:
+        src["traffic_note"] = "capture unreadable"
+        return None, src
+    src["traffic_read_bytes"], src["traffic_write_bytes"] = rd, wr
+    return rd + wr, src
 
 
 def load_peaks():
@@ -239,8 +285,9 @@ def run_ours(args):
     table = kernel_table(prof, args.steps)
     value = world * n * 11 * args.steps / secs
     xf_kernels = [k for k in table if k != "k_alphas"]
-    roof = roofline_hbm(table, xf_kernels, BYTES_PER_QUERY * n, peak_gbs, peak_src,
-                        traffic=NCU_TRAFFIC_BYTES_1E8 if (n == 100_000_000 and args.path != "direct") else None)
+    traffic, traffic_src = load_traffic(n) if args.path != "direct" else (None, {"traffic_source": None})
+    roof = roofline_hbm(table, xf_kernels, BYTES_PER_QUERY * n, peak_gbs, peak_src, traffic=traffic)
+    roof.update(traffic_src)
     roof["algorithmic_bytes"] = BYTES_PER_QUERY * n
     roof["alphas"] = roofline_hbm(table, ["k_alphas"], BYTES_PER_ALPHAS * n, peak_gbs, peak_src)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

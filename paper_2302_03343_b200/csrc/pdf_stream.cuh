@@ -76,7 +76,13 @@ constexpr int kS3Batch = 32;                         // list entries per E batch
 #ifndef PDF_S3_FKU
 #define PDF_S3_FKU 16
 #endif
-constexpr int kS3FkPerUnit = PDF_S3_FKU;             // Q2 cells per B unit
+#ifndef PDF_S3_FKU_LUMI2
+#define PDF_S3_FKU_LUMI2 8
+#endif
+// Q2 cells per B unit (at most 32: a lane per cell): 16 for rows (7.71 -> 7.55 ms per 1e8 C2 queries against 8); pass 2 of
+// the luminosity, whose units also fetch the rows of pass 1, runs best with 8 (11.6 against 13.9 ms per 1e8 C4 events)
+constexpr int kS3FkPerUnit = PDF_S3_FKU, kS3FkPerUnitLumi2 = PDF_S3_FKU_LUMI2;
+static_assert(kS3FkPerUnit <= 32 && kS3FkPerUnitLumi2 <= 32, "a B unit keeps one cell count per lane");
 constexpr int kS3Lag = PDF_S3_LAG;                   // B(c) tickets follow A(c) tickets by this many rounds
 constexpr int kS3Ring = PDF_S3_RING;                 // chunk slots in flight
 static_assert(kS3Ring >= kS3Lag + 2, "A(c) must find the slot of B(c - kRing) drained");
@@ -114,7 +120,7 @@ struct StreamDev {
     int jgplus;                                      // cell (global lower-knot index) of 1.01*Q2min
     double tqplus;                                   // and its t_q  (C-9)
     int cap;                                         // payloads per cell bin
-    int ng, ne, tb;                                  // Q2-cell groups per x cell, E units per chunk, B + E units per chunk
+    int fku, ng, ne, tb;                             // Q2 cells per B unit, Q2-cell groups per x cell, E units per chunk, B + E units per chunk
     int xshift, xbase, nbx, qshift, qbase, nbq;      // bucket = (high word >> shift) - base
     const unsigned short *lutx, *lutq;               // [nbx], [nbq] cell at the lower edge of the bucket
     const double *rowplus;                           // [nmem][nx][12]: the grid's values at Q2 = 1.01 Q2min (C-9's second anchor), per x knot
@@ -971,7 +977,7 @@ __device__ __forceinline__ void stream_body(const StreamArgs &A)
             else {
                 const int v = sub - B.ne;
                 const int i = v / B.ng, grp = v - i * B.ng;
-                b_unit<MODE, FAST>(A, T, V, slot, row_base, i, grp * kS3FkPerUnit, min(B.nqt, (grp + 1) * kS3FkPerUnit), sbuf, sC, err_local);
+                b_unit<MODE, FAST>(A, T, V, slot, row_base, i, grp * B.fku, min(B.nqt, (grp + 1) * B.fku), sbuf, sC, err_local);
             }
             const unsigned long long old = warp_count_add(b_fin, 1ULL);
             if (old + 1 == (gen + 1) * TB) {                       // last unit of the chunk: the slot's counters are reset for the ring

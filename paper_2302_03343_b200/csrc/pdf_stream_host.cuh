@@ -93,9 +93,11 @@ inline long long stream_chunk(const StreamPlan &p, long long n, long long chunk_
 
 // per-chunk geometry: a cell bin holds 3x the uniform share + 32 (a uniform cloud is Poisson around the share;
 // beyond it queries overflow to a list), one E unit per 1024 queries of the chunk
-inline void stream_caps(const StreamPlan &p, long long chunk, StreamDev &d)
+inline void stream_caps(const StreamPlan &p, long long chunk, StreamDev &d, int mode = kModeRows)
 {
     d = p.dev;
+    d.fku = mode == kModeLumiSecond ? kS3FkPerUnitLumi2 : kS3FkPerUnit;
+    d.ng = (d.nqt + d.fku - 1) / d.fku;
     const long long per_cell = chunk / ((long long)(d.ncx > 0 ? d.ncx : 1) * (p.ncells_q > 0 ? p.ncells_q : 1));
     long long cap = (3 * per_cell + 32 + 31) / 32 * 32;
     if (cap > chunk) cap = (chunk + 31) / 32 * 32;
@@ -143,7 +145,7 @@ inline int stream_plan_init(StreamPlan &p, const GridDev &G, const std::vector<d
     StreamDev &d = p.dev;
     d.ncx = nx - 1; d.nqt = nqt;
     d.nbins = d.ncx * nqt;
-    d.ng = (nqt + kS3FkPerUnit - 1) / kS3FkPerUnit;
+    d.fku = kS3FkPerUnit; d.ng = (nqt + d.fku - 1) / d.fku;
     p.ncells_q = nqt - nsub;
 
     std::vector<unsigned short> lx, lq;
@@ -202,7 +204,7 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     A.x2 = x2; A.w = w; A.f1 = f1; A.coup = p.d_coup; A.orig = orig;
     A.G = G; A.cm = cm;
     A.chunk = stream_chunk(p, n, chunk_opt);
-    stream_caps(p, A.chunk, A.B);
+    stream_caps(p, A.chunk, A.B, mode);
     stream_carve(ws, A.chunk, A.B, A.W);
     A.x = x; A.q2 = q2; A.out = out; A.n = n; A.ld = ld;
     A.nchunks = (int)((n + A.chunk - 1) / A.chunk);
