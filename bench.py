@@ -465,6 +465,31 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
         dt = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": ns * 11 / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                                 "sample": f"first {ns} queries of this run's C2 batch, xfxq2 (11 flavours) + alphas, {dt:.1f} s"}
+        # SURVEY 8(d) "Oracle timing": the whole batch in slices of the sample size (the rows are discarded), and one
+        # thread on 1e6 queries (a child process: the OpenMP thread count is fixed when the library loads)
+        if n > ns and n <= 200_000_000:
+            t0 = time.perf_counter()
+            for a0 in range(ns, n, ns):
+                sx, sq = x[a0:a0 + ns].cpu().numpy(), q2[a0:a0 + ns].cpu().numpy()
+                og.xfxq2(spec.pids, sx, sq)
+                og.alphas_q2(sq)
+            line["cpu_baseline"]["full_n_seconds"] = dt + time.perf_counter() - t0
+            line["cpu_baseline"]["full_n"] = n
+        try:
+            n1 = min(1_000_000, ns)
+            code = ("import sys, time, json; sys.path.insert(0, %r); import oracle\n"
+                    "from paper_2302_03343_b200 import synth\n"
+                    "spec = synth.grid_c1(); x, q = synth.queries_c2(spec, %d); x, q = x.numpy(), q.numpy()\n"
+                    "og = oracle.OracleGrid(spec.x_knots.numpy(), [k.numpy() for k in spec.q2_subgrids], spec.values.numpy(), spec.pids)\n"
+                    "og.xfxq2(spec.pids, x[:10000], q[:10000]); t0 = time.perf_counter(); og.xfxq2(spec.pids, x, q); dt = time.perf_counter() - t0\n"
+                    "print(json.dumps({'threads': oracle.num_threads(), 'seconds': dt}))") % (ROOT, n1)
+            r = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, OMP_NUM_THREADS="1"), capture_output=True,
+                               text=True, timeout=300)
+            one = json.loads(r.stdout.strip().splitlines()[-1])
+            line["cpu_baseline"]["single_thread"] = {"value": n1 * 11 / one["seconds"], "unit": UNIT, "cores": one["threads"],
+                                                     "sample": f"{n1} queries of the C2 recipe, xfxq2 (11 flavours), {one['seconds']:.1f} s"}
+        except Exception as e:
+            line["cpu_baseline"]["single_thread"] = {"value": None, "error": repr(e)}
         # sampled parity at full size, in the timed launch configuration (oracle one by one on the sample)
         import numpy as np
         # the same for the luminosity call (50 000 sampled events of the 1e8 launch)
@@ -500,7 +525,11 @@ def extras(args, torch, dist, world, rank, local, binding, synth, spec, g, x, q2
         err = np.abs(got - ref[:np_])
         tol = oracle.tolerance(ref[:np_], S)
         okn = ~np.isnan(ref[:np_])
+        aref = np.abs(ref[:np_])
+        well = okn & (S[..., 0] <= 100.0 * aref) & (S[..., 1] <= 100.0 * aref) & (aref > 0)       # tests/parity.py STRICT_COND
         line["parity_sample"] = {"n": np_, "worst_err_over_tol": float(np.max(err[okn] / np.maximum(tol[okn], 1e-300))),
+                                 "strict_rel_max": float(np.max(err[well] / aref[well])) if well.any() else 0.0,
+                                 "strict_rel_max_over": "points with S0, S1 <= 100 |ref| (DESIGN.md C-12)",
                                  "nan_match": bool(np.array_equal(np.isnan(got), ~okn))}
 
 
