@@ -25,6 +25,7 @@ _LIB = os.path.join(_HERE, "libpdf_oracle.so")
 REGION_INTERIOR, REGION_LOWX, REGION_LOWQ, REGION_HIGHQ = 0, 1, 2, 3
 REGION_LOWX_LOWQ, REGION_LOWX_HIGHQ, REGION_INVALID = 4, 5, 6
 ALPHAS_FREEZE, ALPHAS_LOGGRAD = 0, 1
+EXTRAP_CONTINUATION, EXTRAP_FREEZE, EXTRAP_ERROR = 0, 1, 2
 
 
 # Parity metric C-12: |gpu - ref| <= REL |ref| + FLOOR_S S[...,0] + FLOOR_T S[...,1].
@@ -70,6 +71,7 @@ def lib():
         L.oracle_grid_create.argtypes = [C.POINTER(vp), C.c_int, dp, C.c_int, ip, dp, dp, C.c_int, ip, C.c_int]
         L.oracle_grid_set_alphas.argtypes = [vp, C.c_int, dp, dp]
         L.oracle_grid_set_alphas_mode.argtypes = [vp, C.c_int]
+        L.oracle_grid_set_extrapolation.argtypes = [vp, C.c_int]
         L.oracle_grid_set_coupling.argtypes = [vp, dp]
         L.oracle_grid_limits.argtypes = [vp, dp, dp, dp, dp]
         L.oracle_grid_destroy.argtypes = [vp]
@@ -164,6 +166,18 @@ class OracleGrid:
         a = [C.c_double() for _ in range(4)]
         lib().oracle_grid_limits(self._h, *[C.byref(t) for t in a])
         return tuple(t.value for t in a)
+
+    def set_extrapolation(self, mode: int):
+        """EXTRAP_CONTINUATION (default), EXTRAP_FREEZE, EXTRAP_ERROR"""
+        if lib().oracle_grid_set_extrapolation(self._h, mode):
+            raise ValueError("oracle_grid_set_extrapolation failed")
+
+    def xfxq(self, pids, x, q, member=None, want_scale: bool = False):
+        """xfxQ (the interface takes Q or Q2): by definition xfxQ2 at Q2 = Q * Q; Q <= 0 is invalid"""
+        q = np.asarray(q, dtype=np.float64)
+        with np.errstate(over="ignore", invalid="ignore"):
+            q2 = np.where(q > 0, q * q, np.nan)
+        return self.xfxq2(pids, x, q2, member=member, want_scale=want_scale)
 
     def locate(self, x, q2):
         x, xp = _d(x)

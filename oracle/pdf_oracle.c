@@ -37,6 +37,7 @@ struct oracle_grid {
     int na;         /* alpha_s knots                               */
     double *aq2, *as, *aval;
     int alphas_mode;
+    int extrap;                 /* ORACLE_EXTRAP_* (L1720) */
     double *C;      /* [nflav][nflav] or NULL                      */
 };
 
@@ -134,6 +135,13 @@ int oracle_grid_set_alphas(oracle_grid *g, int n, const double *q2_knots,
     for (int j = 0; j < n; ++j) {
         g->aq2[j] = q2_knots[j]; g->as[j] = log(q2_knots[j]); g->aval[j] = values[j];
     }
+    return 0;
+}
+
+int oracle_grid_set_extrapolation(oracle_grid *g, int mode)
+{
+    if (!g || mode < ORACLE_EXTRAP_CONTINUATION || mode > ORACLE_EXTRAP_ERROR) return -1;
+    g->extrap = mode;
     return 0;
 }
 
@@ -290,25 +298,40 @@ static int classify(const oracle_grid *g, double x, double q2)
     return lowq ? ORACLE_REGION_LOWQ : highq ? ORACLE_REGION_HIGHQ : ORACLE_REGION_INTERIOR;
 }
 
+/* L1720 (reading R-7): the point a valid query is evaluated at under the grid's extrapolation option */
+static void apply_extrapolation(const oracle_grid *g, double *x, double *q2)
+{
+    if (g->extrap == ORACLE_EXTRAP_CONTINUATION) return;
+    int r = classify(g, *x, *q2);
+    if (r == ORACLE_REGION_INVALID || r == ORACLE_REGION_INTERIOR) return;
+    if (g->extrap == ORACLE_EXTRAP_ERROR) { *x = NAN; return; }           /* an error: the query is invalid */
+    double q2min = g->q2[0], q2max = g->q2[g->nqtot - 1];                 /* freeze */
+    if (*x < g->x[0]) *x = g->x[0];
+    if (*q2 < q2min) *q2 = q2min;
+    if (*q2 > q2max) *q2 = q2max;
+}
+
 int oracle_locate(const oracle_grid *g, long long n, const double *x,
                   const double *q2, int *ix, int *iq, int *isub, int *region)
 {
     if (!g || n < 0 || !x || !q2) return -1;
 #pragma omp parallel for schedule(static)
     for (long long e = 0; e < n; ++e) {
-        int r = classify(g, x[e], q2[e]);
+        double xe = x[e], qe = q2[e];
+        apply_extrapolation(g, &xe, &qe);
+        int r = classify(g, xe, qe);
         int i = -1, j = -1, k = -1;
         if (r != ORACLE_REGION_INVALID) {
             /* low-x is anchored on knots X_0, X_1 */
             i = (r == ORACLE_REGION_LOWX || r == ORACLE_REGION_LOWX_LOWQ ||
-                 r == ORACLE_REGION_LOWX_HIGHQ) ? 0 : find_cell(g->nx, g->x, x[e]);
+                 r == ORACLE_REGION_LOWX_HIGHQ) ? 0 : find_cell(g->nx, g->x, xe);
             if (r == ORACLE_REGION_LOWQ || r == ORACLE_REGION_LOWX_LOWQ) {
                 k = 0; j = 0;                       /* anchored on Q2_min */
             } else if (r == ORACLE_REGION_HIGHQ || r == ORACLE_REGION_LOWX_HIGHQ) {
                 k = g->nsub - 1; j = g->nq[k] - 2; /* two highest knots  */
             } else {
-                k = find_subgrid(g, q2[e]);
-                j = find_cell(g->nq[k], g->q2 + g->qoff[k], q2[e]);
+                k = find_subgrid(g, qe);
+                j = find_cell(g->nq[k], g->q2 + g->qoff[k], qe);
             }
         }
         if (ix) ix[e] = i;
@@ -465,13 +488,15 @@ int oracle_xfxq2(const oracle_grid *g, const int *pids, int npid, long long n,
 #pragma omp parallel for schedule(static)
     for (long long e = 0; e < n; ++e) {
         int mem = member ? member[e] : 0;
-        int r = classify(g, x[e], q2[e]);
+        double xe = x[e], qe = q2[e];
+        apply_extrapolation(g, &xe, &qe);
+        int r = classify(g, xe, qe);
         if (mem < 0 || mem >= g->nmem) { r = ORACLE_REGION_INVALID; bad_member = 1; }
         for (int p = 0; p < npid; ++p) {
             double v, S[2] = {0.0, 0.0};
             if (r == ORACLE_REGION_INVALID) { v = NAN; S[0] = S[1] = NAN; }   /* C-10 */
             else if (col[p] < 0) { v = 0.0; }                                 /* C-11 */
-            else value_any(g, mem, col[p], x[e], q2[e], &v, scale ? S : NULL);
+            else value_any(g, mem, col[p], xe, qe, &v, scale ? S : NULL);
             out[e * npid + p] = v;
             if (scale) { scale[(e * npid + p) * 2] = S[0]; scale[(e * npid + p) * 2 + 1] = S[1]; }
         }
@@ -519,16 +544,19 @@ int oracle_lumi(const oracle_grid *g, long long n, const double *x1,
     int nf = g->nflav;
 #pragma omp parallel for schedule(static)
     for (long long e = 0; e < n; ++e) {
-        int r1 = classify(g, x1[e], q2[e]), r2 = classify(g, x2[e], q2[e]);
+        double xa = x1[e], qa = q2[e], xb = x2[e], qb = q2[e];       /* the points the two partons are evaluated at (L1720) */
+        apply_extrapolation(g, &xa, &qa);
+        apply_extrapolation(g, &xb, &qb);
+        int r1 = classify(g, xa, qa), r2 = classify(g, xb, qb);
         if (r1 == ORACLE_REGION_INVALID || r2 == ORACLE_REGION_INVALID) {
             out[e] = NAN; if (scale) scale[2 * e] = scale[2 * e + 1] = NAN; continue;
         }
         double f1[64], f2[64], s1[64][2], s2[64][2];
         for (int f = 0; f < nf; ++f) {
             double v, S[2] = {0.0, 0.0};
-            value_any(g, 0, f, x1[e], q2[e], &v, scale ? S : NULL);
+            value_any(g, 0, f, xa, qa, &v, scale ? S : NULL);
             f1[f] = v / x1[e]; s1[f][0] = S[0] / x1[e]; s1[f][1] = S[1] / x1[e];
-            value_any(g, 0, f, x2[e], q2[e], &v, scale ? S : NULL);
+            value_any(g, 0, f, xb, qb, &v, scale ? S : NULL);
             f2[f] = v / x2[e]; s2[f][0] = S[0] / x2[e]; s2[f][1] = S[1] / x2[e];
         }
         double acc = 0.0, sacc[2] = {0.0, 0.0};

@@ -43,6 +43,11 @@ enum {
 
 /* alpha_s behaviour below the first knot (PAPER.md L1746 vs L1835, S-16) */
 enum { ORACLE_ALPHAS_FREEZE = 0, ORACLE_ALPHAS_LOGGRAD = 1 };
+/* the extrapolation choices of LHAPDF 6.  CONTINUATION is the default (C-7 ... C-9); FREEZE returns
+ * "the PDF value at the closest grid knot", read (R-7) as the interpolant at the coordinates moved to the closest
+ * point of the grid's range (a coordinate inside its range is not touched); ERROR "raises an error if a point outside
+ * the grid range is queried": such a query is an invalid query (C-10: NaN, counted by the CUDA path). */
+enum { ORACLE_EXTRAP_CONTINUATION = 0, ORACLE_EXTRAP_FREEZE = 1, ORACLE_EXTRAP_ERROR = 2 };
 
 /* Grid format of PAPER.md L1714: knots in (x,Q2), Q2 split in sub-grids whose
  * last knot equals the first knot of the next one.  values is
@@ -59,6 +64,8 @@ int oracle_grid_set_coupling(oracle_grid *g, const double *C /*[nflav][nflav]*/)
 int oracle_grid_limits(const oracle_grid *g, double *xmin, double *xmax,
                        double *q2min, double *q2max);
 int oracle_grid_destroy(oracle_grid *g);
+/* L1720; applies to oracle_locate, oracle_xfxq2 and oracle_lumi (whose 1/x1, 1/x2 keep the query's own x) */
+int oracle_grid_set_extrapolation(oracle_grid *g, int mode);
 
 /* C-2, C-3, C-4: region class, sub-grid, lower-left knot (ix, iq local to the
  * sub-grid).  For out-of-range queries the indices are those of the cell the

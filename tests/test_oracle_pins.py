@@ -817,3 +817,91 @@ def test_workload_shapes(oracle_mod):
     assert np.all(reg == 0)
     s = np.bincount(isub, minlength=3) / len(isub)
     assert abs(s[0] - 0.036) < 3e-3 and abs(s[1] - 0.103) < 3e-3
+
+
+# ---------------------------------------------------------------------------
+# NEXT-4: the other extrapolation options of LHAPDF 6 and xfxQ (L1712)
+# ---------------------------------------------------------------------------
+def _outside_queries(spec, n=4000, seed=5):
+    """valid queries of every region class of Fig. 3.1(b), and some inside"""
+    rng = np.random.default_rng(seed)
+    xk = spec.x_knots.numpy()
+    qk = np.concatenate([q.numpy() for q in spec.q2_subgrids])
+    x = np.exp(rng.uniform(np.log(xk[0]) - 6.0, np.log(xk[-1]), n))
+    q = np.exp(rng.uniform(np.log(qk[0]) - 4.0, np.log(qk[-1]) + 4.0, n))
+    x[::7] = xk[0]; q[::11] = qk[0]; q[5::11] = qk[-1]            # on the range's edges
+    return x, q, xk, qk
+
+
+def test_freeze_returns_the_value_at_the_closest_point_of_the_range(oracle_mod):
+    """L1720 "freeze the grid edges": outside the range the value does not depend on how far outside the query
+    is; on a knot line of the boundary it is the STORED node value (P-1 through the option); inside nothing changes."""
+    spec = synth.grid_c1()
+    og = make_oracle_grid(oracle_mod, spec)
+    x, q, xk, qk = _outside_queries(spec)
+    base = og.xfxq2(spec.pids, x, q)
+    og.set_extrapolation(oracle_mod.EXTRAP_FREEZE)
+    fr = og.xfxq2(spec.pids, x, q)
+    inside = (x >= xk[0]) & (q >= qk[0]) & (q <= qk[-1])
+    assert inside.any() and (~inside).any()
+    assert np.array_equal(fr[inside], base[inside])
+    # twice as far out: the same numbers, bit for bit
+    x2 = np.where(x < xk[0], x * 1e-3, x)
+    q2 = np.where(q < qk[0], q * 1e-2, np.where(q > qk[-1], q * 1e2, q))
+    assert np.array_equal(og.xfxq2(spec.pids, x2, q2), fr)
+    # below the first x knot AND on a Q2 knot: the node value V[0][jq] itself
+    nx = len(xk)
+    nq0 = spec.q2_subgrids[0].numel()
+    V0 = spec.values.numpy()[: nx * nq0 * 11].reshape(nx, nq0, 11)
+    for jq in (1, 3):
+        got = og.xfxq2(spec.pids, np.array([xk[0] * 1e-4]), np.array([spec.q2_subgrids[0].numpy()[jq]]))[0]
+        assert np.array_equal(got, V0[0, jq])
+    # below Q2min AND on an x knot: V[ix][0]; above Q2max: the last node row
+    got = og.xfxq2(spec.pids, np.array([xk[17]]), np.array([qk[0] * 1e-3]))[0]
+    assert np.array_equal(got, V0[17, 0])
+    nql = spec.q2_subgrids[-1].numel()
+    Vl = spec.values.numpy()[-nx * nql * 11:].reshape(nx, nql, 11)
+    got = og.xfxq2(spec.pids, np.array([xk[40]]), np.array([qk[-1] * 50.0]))[0]
+    assert np.array_equal(got, Vl[40, nql - 1])
+    # the cell reported is the boundary cell, the region interior
+    ix, iq, isub, reg = og.locate(x, q)
+    assert set(np.unique(reg).tolist()) == {0}
+    assert (ix[x < xk[0]] == 0).all() and (isub[q < qk[0]] == 0).all() and (iq[q < qk[0]] == 0).all()
+    assert (isub[q > qk[-1]] == len(spec.q2_subgrids) - 1).all() and (iq[q > qk[-1]] == nql - 2).all()
+
+
+def test_error_option_rejects_every_query_outside_the_range(oracle_mod):
+    """L1720 "raise an error if a point outside the grid range is queried": NaN rows outside, nothing changes inside"""
+    spec = synth.grid_c1()
+    og = make_oracle_grid(oracle_mod, spec)
+    x, q, xk, qk = _outside_queries(spec)
+    base = og.xfxq2(spec.pids, x, q)
+    og.set_extrapolation(oracle_mod.EXTRAP_ERROR)
+    er = og.xfxq2(spec.pids, x, q)
+    inside = (x >= xk[0]) & (q >= qk[0]) & (q <= qk[-1])
+    assert np.array_equal(er[inside], base[inside])
+    assert np.isnan(er[~inside]).all() and not np.isnan(base[~inside]).any()
+    reg = og.locate(x, q)[3]
+    assert (reg[~inside] == 6).all() and (reg[inside] == 0).all()
+    og.set_extrapolation(oracle_mod.EXTRAP_CONTINUATION)
+    assert np.array_equal(og.xfxq2(spec.pids, x, q), base)
+
+
+def test_xfxq_is_xfxq2_at_q_squared(oracle_mod):
+    """L1712: PDF::xfxQ and PDF::xfxQ2 are the same function of Q and Q2.  On a grid whose Q2 knots are exact squares
+    the Q knots reproduce the node values (P-1); Q <= 0 is invalid although its square is not."""
+    xk = uniform_log_knots(1e-4, 1.0, 9)
+    qroot = np.array([2.0, 4.0, 8.0, 16.0, 32.0])
+    spec = spec_from_function(xk, [qroot * qroot], lambda U, S, f, k: np.sin(U) + 0.1 * S * S + f, nflav=2)
+    og = make_oracle_grid(oracle_mod, spec)
+    V = spec.values.numpy().reshape(9, 5, 2)
+    for ix in (0, 3, 8):
+        for jq in (0, 2, 4):
+            got = og.xfxq(spec.pids, np.array([xk[ix]]), np.array([qroot[jq]]))[0]
+            assert np.array_equal(got, V[ix, jq])
+    rng = np.random.default_rng(2)
+    x = np.exp(rng.uniform(np.log(1e-5), 0.0, 500))
+    Q = np.exp(rng.uniform(np.log(1.0), np.log(64.0), 500))
+    assert np.array_equal(og.xfxq(spec.pids, x, Q), og.xfxq2(spec.pids, x, Q * Q))
+    bad = og.xfxq(spec.pids, np.array([0.1, 0.1, 0.1]), np.array([-4.0, 0.0, np.inf]))
+    assert np.isnan(bad).all()
