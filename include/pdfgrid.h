@@ -76,7 +76,16 @@ enum {
                              by member (<= 4096 members, npid <= nflav); pdf_lumi: sliced binned
                              evaluation of both partons into workspace scratch + a combine kernel     */
 };
-enum { PDF_OPT_PATH = 1, PDF_OPT_ALPHAS_MODE = 2, PDF_OPT_CHUNK = 3 };
+enum { PDF_OPT_PATH = 1, PDF_OPT_ALPHAS_MODE = 2, PDF_OPT_CHUNK = 3, PDF_OPT_EXTRAPOLATION = 4 };
+
+/* extrapolation outside the grid's range (pdf_grid_set_option(PDF_OPT_EXTRAPOLATION, ...)):
+ * CONTINUATION is LHAPDF's default (low-x / high-Q continuation L1722, low-Q rule eq. 3.4-3.5); FREEZE "freezes the
+ * grid edges, returning the PDF value at the closest grid knot": the interpolant at the query moved to the closest
+ * point of the range (a coordinate inside its range is not touched); ERROR "raises an error if a point outside the
+ * grid range is queried": such a query gives a NaN row and counts in pdf_error_count, like any invalid query.
+ * The option acts on pdf_xfxq2 / _ex / _xgrid / _noalloc, pdf_xfxq, pdf_lumi (whose factors 1/x1, 1/x2 keep the
+ * query's own x) and pdf_locate (which reports the cell of the point that is evaluated). */
+enum { PDF_EXTRAP_CONTINUATION = 0, PDF_EXTRAP_FREEZE = 1, PDF_EXTRAP_ERROR = 2 };
 
 typedef struct pdf_grid pdf_grid; /* opaque; owns its device tables */
 
@@ -130,6 +139,11 @@ int pdf_xfxq2_ex(const pdf_grid *g, const int *pids, int npid, long long n, cons
  * and node weights are computed once per point.  A point outside the domain, or a member id outside
  * [0, nmem), gives a quiet-NaN row and one error count per (point, member).  npts == 0 or nrep == 0 is a
  * no-op.  Enqueues one kernel on `stream`; PDF_EINVAL on bad arguments. */
+/* xfxQ ("PDF::xfxQ(...) and PDF::xfxQ2(...)"): pdf_xfxq2 at Q2 = Q * Q; q DEVICE [n] holds Q in GeV.
+ * Q <= 0 or non-finite is an invalid query (NaN row, counted) although its square is not. */
+int pdf_xfxq(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+             const double *q, double *out, void *stream);
+
 int pdf_xfxq2_xgrid(const pdf_grid *g, const int *pids, int npid, long long npts, const double *x,
                     const double *q2, int nrep, const int *members, double *out, long long ld_out,
                     void *stream);

@@ -21,7 +21,8 @@ LIB_PATH = os.path.join(_HERE, "libpdfgrid.so")
 
 PDF_OK, PDF_EINVAL, PDF_ENOMEM, PDF_ECUDA, PDF_EWORKSPACE, PDF_ESTATE, PDF_ELIMIT = 0, -1, -2, -3, -4, -5, -6
 PDF_PATH_AUTO, PDF_PATH_DIRECT, PDF_PATH_BINNED = 0, 1, 2
-PDF_OPT_PATH, PDF_OPT_ALPHAS_MODE, PDF_OPT_CHUNK = 1, 2, 3
+PDF_OPT_PATH, PDF_OPT_ALPHAS_MODE, PDF_OPT_CHUNK, PDF_OPT_EXTRAPOLATION = 1, 2, 3, 4
+PDF_EXTRAP_CONTINUATION, PDF_EXTRAP_FREEZE, PDF_EXTRAP_ERROR = 0, 1, 2
 PDF_ALPHAS_FREEZE, PDF_ALPHAS_LOGGRAD = 0, 1
 
 # every symbol include/pdfgrid.h declares (tests check the library exports all of them)
@@ -33,7 +34,7 @@ SYMBOLS = (
     "pdf_last_cuda_error", "pdf_launch_count", "pdf_profile_enable", "pdf_profile_read",
     "pdf_measure_fp64_tflops", "pdf_last_path", "pdf_log_f64",
     "pdf_rambo", "pdf_vegas_map", "pdf_vegas_accumulate", "pdf_vegas_estimate", "pdf_vegas_refine", "pdf_vegas_combine",
-    "pdf_unweight", "pdf_xfxq2_noalloc",
+    "pdf_unweight", "pdf_xfxq2_noalloc", "pdf_xfxq",
 )
 
 
@@ -64,6 +65,7 @@ def lib():
     L.pdf_grid_set_option.argtypes = [vp, C.c_int, ll]
     L.pdf_grid_limits.argtypes = [vp, dp, dp, dp, dp]
     L.pdf_xfxq2.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp]
+    L.pdf_xfxq.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp]
     L.pdf_xfxq2_noalloc.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, C.POINTER(ll), vp]
     L.pdf_xfxq2_ex.argtypes = [vp, ip, C.c_int, ll, vp, vp, vp, vp, ll, vp]
     L.pdf_xfxq2_xgrid.argtypes = [vp, ip, C.c_int, ll, vp, vp, C.c_int, vp, vp, ll, vp]
@@ -334,6 +336,17 @@ class PdfGrid:
             mp = _dev(member, torch.int32, "member") if member is not None else None
             rc = lib().pdf_xfxq2_ex(self._h, _iptr(pid), pid.numel(), n, xp, qp, mp, op, ld, _stream_ptr(stream))
         _check(rc, "pdf_xfxq2")
+        return out
+
+    def pdf_xfxq(self, pids, x: torch.Tensor, q: torch.Tensor, out: Optional[torch.Tensor] = None, stream=None):
+        """xfxQ: `q` holds Q (GeV), not Q2"""
+        pid = _hi(list(pids))
+        n = x.numel()
+        if out is None:
+            out = torch.empty((n, pid.numel()), dtype=torch.float64, device=x.device)
+        xp, qp = _dev(x, torch.float64, "x", n), _dev(q, torch.float64, "q", n)
+        op = _dev(out, torch.float64, "out", n * pid.numel(), at_least=True)
+        _check(lib().pdf_xfxq(self._h, _iptr(pid), pid.numel(), n, xp, qp, op, _stream_ptr(stream)), "pdf_xfxq")
         return out
 
     def pdf_xfxq2_noalloc(self, pids, x: torch.Tensor, q2: torch.Tensor, out: torch.Tensor, stream=None) -> int:

@@ -10,6 +10,7 @@ namespace pdfg {
 
 constexpr int kAlphaLutMax = 2048;  // search-table buckets of the alpha_s knot line (indexed by exponent and top mantissa bits)
 constexpr int kMaxLumiFlav = 16;   // generic pdf_lumi keeps both flavour vectors in registers/local
+constexpr int kExtrapContinuation = 0, kExtrapFreeze = 1, kExtrapError = 2;
 constexpr int kRegionInterior = 0, kRegionLowX = 1, kRegionLowQ = 2, kRegionHighQ = 3,
               kRegionLowXLowQ = 4, kRegionLowXHighQ = 5, kRegionInvalid = 6;
 
@@ -39,6 +40,7 @@ struct GridDev {
     size_t memstride;             // nqtot*nx*nfp
     double q2plus;                // 1.01 * Q2min (C-9)
     // alpha_s (a-6)
+    int extrap;                   // kExtrap*
     int na, alphas_mode;
     const double *ak, *alk, *av;  // raw knots, ln knots, values
     const CellTab *ca;            // [na-1]
@@ -140,6 +142,20 @@ __device__ __forceinline__ int classify(const GridDev &G, double x, double q2)
     if (lowx) return lowq ? kRegionLowXLowQ : highq ? kRegionLowXHighQ : kRegionLowX;
     return lowq ? kRegionLowQ : highq ? kRegionHighQ : kRegionInterior;
 }
+
+// PAPER.md L1720, the other extrapolation options of LHAPDF 6, applied to a query before anything else looks at it:
+// freeze = the point moved to the closest point of the grid's range (a coordinate inside its range is not touched),
+// error = a valid query outside the range becomes an invalid one (C-10).  Warp-uniform branch on the option.
+__device__ __forceinline__ void apply_extrapolation(const GridDev &G, double &x, double &q2)
+{
+    if (G.extrap == kExtrapContinuation) return;
+    const double x0 = G.xk[0], q0 = G.qk[0], q1 = G.qk[G.nqtot - 1];
+    if (!(finite_pos(x) && finite_pos(q2)) || x > G.xk[G.nx - 1]) return;          // invalid stays invalid
+    if (G.extrap == kExtrapFreeze) { x = x < x0 ? x0 : x; q2 = q2 < q0 ? q0 : (q2 > q1 ? q1 : q2); }
+    else if (x < x0 || q2 < q0 || q2 > q1) x = __longlong_as_double(0x7ff8000000000000LL);
+}
+// xfxQ: Q -> Q2; Q <= 0 is invalid although its square is not
+__device__ __forceinline__ double q_to_q2(double q) { return q > 0.0 ? q * q : __longlong_as_double(0x7ff8000000000000LL); }
 
 // x-axis point inside the knot range: cell i, t = (ln x - u_i)/(u_{i+1}-u_i)
 __device__ __forceinline__ void x_point_cell(const GridDev &G, int i, double t, Point1D &p)

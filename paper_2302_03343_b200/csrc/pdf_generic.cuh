@@ -58,6 +58,7 @@ __global__ void k_locate(GridDev G, long long n, const double *__restrict__ x, c
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n) return;
     double xv = x[e], qv = q2[e];
+    apply_extrapolation(G, xv, qv);
     int r = classify(G, xv, qv);
     int i = -1, j = -1, k = -1;
     if (r != kRegionInvalid) {
@@ -80,11 +81,13 @@ struct ColMap { int n; int col[64]; };
 __global__ void __launch_bounds__(128)
 k_xfxq2_direct(GridDev G, ColMap cm, long long n, const double *__restrict__ x,
                const double *__restrict__ q2, const int *__restrict__ member,
-               double *__restrict__ out, long long ld)
+               double *__restrict__ out, long long ld, int q_is_q)
 {
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n) return;
     double xv = x[e], qv = q2[e];
+    if (q_is_q) qv = q_to_q2(qv);
+    apply_extrapolation(G, xv, qv);
     int mem = member ? member[e] : 0;
     int r = classify(G, xv, qv);
     double *o = out + e * ld;
@@ -137,7 +140,7 @@ k_xfxq2_xgrid(const __grid_constant__ GridDev G, const __grid_constant__ ColMap 
     const long long p0 = p - lane;                             // first point of the warp
     const bool live = p < npts;
     double xv = 1.0, qv = 1.0;
-    if (live) { xv = x[p]; qv = q2[p]; }
+    if (live) { xv = x[p]; qv = q2[p]; apply_extrapolation(G, xv, qv); }
     const bool valid = live && classify(G, xv, qv) != kRegionInvalid;
     // only the interior plan (2 x 4 node indices and weights) stays in registers across the member loop;
     // the rare extrapolated point rebuilds its full plan per member
@@ -266,7 +269,8 @@ k_xfxq2_xgrid_cell(const __grid_constant__ GridDev G, long long npts, const doub
     const long long p0 = (long long)blockIdx.x * kXcT;
     const int np = (int)((npts - p0) < kXcT ? (npts - p0) : kXcT);
     if ((int)threadIdx.x < np) {
-        const double xv = x[p0 + threadIdx.x], qv = q2[p0 + threadIdx.x];
+        double xv = x[p0 + threadIdx.x], qv = q2[p0 + threadIdx.x];
+        apply_extrapolation(G, xv, qv);
         int kind = 0;
         if (classify(G, xv, qv) != kRegionInvalid) {
             QueryPlan P;
@@ -469,19 +473,22 @@ k_lumi_direct(GridDev G, long long n, const double *__restrict__ x1, const doubl
 {
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= n) return;
-    double a = x1[e], b = x2[e], qv = q2[e];
-    if (classify(G, a, qv) == kRegionInvalid || classify(G, b, qv) == kRegionInvalid) {
+    const double a0 = x1[e], b0 = x2[e];
+    double a = a0, b = b0, qa = q2[e], qb = qa;            // the points the partons are evaluated at (L1720); 1/x keeps the query's x
+    apply_extrapolation(G, a, qa);
+    apply_extrapolation(G, b, qb);
+    if (classify(G, a, qa) == kRegionInvalid || classify(G, b, qb) == kRegionInvalid) {
         out[e] = qnan();
         atomicAdd(G.err_count, 1ULL);
         return;
     }
     double f2[kMaxLumiFlav];
     QueryPlan P;
-    make_plan(G, b, qv, P);
-    double inv_b = 1.0 / b;
+    make_plan(G, b, qb, P);
+    double inv_b = 1.0 / b0;
     for (int j = 0; j < G.nflav; ++j) f2[j] = plan_value(G, G.V, P, j) * inv_b;
-    make_plan(G, a, qv, P);
-    double inv_a = 1.0 / a;
+    make_plan(G, a, qa, P);
+    double inv_a = 1.0 / a0;
     double acc = 0.0;
     for (int i = 0; i < G.nflav; ++i) {
         double f1 = plan_value(G, G.V, P, i) * inv_a;

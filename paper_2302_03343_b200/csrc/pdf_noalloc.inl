@@ -104,6 +104,7 @@ int pdf_xfxq2_noalloc(const pdf_grid *g, const int *pids, int npid, long long n,
     A.identity = cm.n == kNF;
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
     A.count_err = 1;
+    A.q_is_q = 0;
     // the array keeps the last call's contents: the ticket, the slot's counters and the bin / list counts start at zero
     const size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);
     CK(cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s));

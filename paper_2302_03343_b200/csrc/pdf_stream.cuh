@@ -147,6 +147,7 @@ struct StreamArgs {
     int nchunks, ta;           // chunks, A tiles per chunk
     int identity;              // 1: requested columns == the grid's 11 columns in order
     int count_err;             // 1: invalid queries bump the grid's error counter
+    int q_is_q;                // 1: the q2 array holds Q (pdf_xfxq): squared on load
     // member axis (a-8, pdf_members.cuh): the queries arrive sorted by member and every chunk lies
     // inside one member's run; ctab[c] = {first query, queries, member, 0}, *nchunks_dev chunks.
     const int *ctab;
@@ -335,7 +336,9 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
             r.xv[q] = 1.0; r.qv[q] = 1.0; r.sc[q] = 0.0;
             if (e < t1) {
                 r.xv[q] = __ldcs(A.x + e); r.qv[q] = __ldcs(A.q2 + e);
-                if (MODE == kModeLumiFirst) r.sc[q] = __ldcs(A.w + e) / (r.xv[q] * __ldcs(A.x2 + e));   // f = xf / x on both sides (eq. 3.3)
+                if (MODE == kModeLumiFirst) r.sc[q] = __ldcs(A.w + e) / (r.xv[q] * __ldcs(A.x2 + e));   // f = xf / x on both sides (eq. 3.3): the query's own x
+                if (A.q_is_q) r.qv[q] = q_to_q2(r.qv[q]);
+                apply_extrapolation(G, r.xv[q], r.qv[q]);                                              // L1720 (no-op for the default option)
             }
         }
         return r;
@@ -870,7 +873,9 @@ k_locate_stream(const __grid_constant__ GridDev G, const __grid_constant__ Strea
     const long long xminb = lds_s64(T.xk), xmaxb = lds_s64(T.xk + 8u * (G.nx - 1));
     const long long qminb = lds_s64(T.qk), qmaxb = lds_s64(T.qk + 8u * (G.nqtot - 1));
     for (long long e = (long long)blockIdx.x * 256 + threadIdx.x; e < n; e += (long long)gridDim.x * 256) {
-        const Located L = s3_locate(G, B, T, x[e], q2[e], xminb, xmaxb, qminb, qmaxb);
+        double xe = x[e], qe = q2[e];
+        apply_extrapolation(G, xe, qe);
+        const Located L = s3_locate(G, B, T, xe, qe, xminb, xmaxb, qminb, qmaxb);
         const int r = L.region;
         int i = -1, j = -1, k = -1;
         if (r != kRegionInvalid) {

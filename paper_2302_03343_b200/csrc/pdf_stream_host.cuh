@@ -196,7 +196,7 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
                         const double *q2, double *out, long long ld, void *ws, size_t ws_bytes, long long chunk_opt,
                         cudaStream_t s, int count_err = 1, const int *ctab = nullptr, const int *nchunks_dev = nullptr,
                         int mode = kModeRows, const double *x2 = nullptr, const double *w = nullptr, const double *f1 = nullptr,
-                        const unsigned *orig = nullptr)
+                        const unsigned *orig = nullptr, int q_is_q = 0)
 {
     if (stream_workspace_bytes(p, n, chunk_opt) > ws_bytes) return PDF_EWORKSPACE;
     StreamArgs A;
@@ -212,6 +212,7 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     A.identity = cm.n == kNF;
     for (int f = 0; f < kNF && A.identity; ++f) A.identity = cm.col[f] == f;
     A.count_err = count_err;
+    A.q_is_q = q_is_q;
     const size_t zero_bytes = (size_t)((char *)A.W.bins - (char *)A.W.ctrl);      // ctrl + counts
     if (cudaMemsetAsync(A.W.ctrl, 0, zero_bytes, s) != cudaSuccess) return PDF_ECUDA;
     const size_t smem = stream_smem_bytes(G, A.B);

@@ -249,7 +249,7 @@ int pdf_grid_create(pdf_grid **out, int nx, const double *x_knots, int nsub, con
     d.sub_of = g->d_sub_of; d.qoff = g->d_qoff; d.cell_adj = g->d_cell_adj; d.cx = g->d_cx; d.cq = g->d_cq;
     d.V = g->d_V; d.memstride = (size_t)tot * nx * nfp;
     d.q2plus = 1.01 * q2_knots[0];
-    d.na = 0; d.alphas_mode = PDF_ALPHAS_FREEZE; d.C = nullptr; d.err_count = g->d_err;
+    d.na = 0; d.alphas_mode = PDF_ALPHAS_FREEZE; d.extrap = PDF_EXTRAP_CONTINUATION; d.C = nullptr; d.err_count = g->d_err;
     rc = stream_plan_init(g->bplan, g->d, g->xk, g->qk, nsub);
     if (rc != PDF_OK) { free_grid(g); return rc; }
     // pdf_xfxq2_noalloc: the static scratch array's address on this device (resolved once per device; no allocation).
@@ -324,6 +324,9 @@ int pdf_grid_set_option(pdf_grid *g, int option, long long value)
     case PDF_OPT_ALPHAS_MODE:
         if (value != PDF_ALPHAS_FREEZE && value != PDF_ALPHAS_LOGGRAD) return PDF_EINVAL;
         g->d.alphas_mode = (int)value; return PDF_OK;
+    case PDF_OPT_EXTRAPOLATION:
+        if (value < PDF_EXTRAP_CONTINUATION || value > PDF_EXTRAP_ERROR) return PDF_EINVAL;
+        g->d.extrap = (int)value; return PDF_OK;
     case PDF_OPT_CHUNK:
         if (value < 0) return PDF_EINVAL;
         g->chunk = value; return PDF_OK;

@@ -14,14 +14,14 @@ inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + th
 
 // direct path in slices of < 2^31 blocks (n is long long)
 int launch_direct(const pdf_grid *g, const ColMap &cm, long long n, const double *x, const double *q2,
-                  const int *member, double *out, long long ld, cudaStream_t s)
+                  const int *member, double *out, long long ld, cudaStream_t s, int q_is_q = 0)
 {
     const long long slice = 1LL << 30;
     for (long long off = 0; off < n; off += slice) {
         long long m = n - off < slice ? n - off : slice;
         LaunchScope a(s, "k_xfxq2_direct");
         k_xfxq2_direct<<<blocks_for(m, 128), 128, 0, s>>>(g->d, cm, m, x + off, q2 + off,
-                                                         member ? member + off : nullptr, out + off * ld, ld);
+                                                         member ? member + off : nullptr, out + off * ld, ld, q_is_q);
     }
     CK(cudaGetLastError());
     return PDF_OK;
@@ -31,9 +31,10 @@ int on_device(const pdf_grid *g);
 
 // pdf_xfxq2_ex with the workspace as an argument (the *_host calls pass their own staging workspace)
 int xfxq2_impl(const pdf_grid *g, void *ws, size_t ws_bytes, const int *pids, int npid, long long n, const double *x,
-               const double *q2, const int *member, double *out, long long ld_out, cudaStream_t s)
+               const double *q2, const int *member, double *out, long long ld_out, cudaStream_t s, int q_is_q = 0)
 {
     if (!g || n < 0 || ld_out < npid) return PDF_EINVAL;
+    if (q_is_q && member) return PDF_EINVAL;
     ColMap cm;
     int rc = build_colmap(g, pids, npid, cm);
     if (rc) return rc;
@@ -61,10 +62,11 @@ int xfxq2_impl(const pdf_grid *g, void *ws, size_t ws_bytes, const int *pids, in
         if (!ok_binned) return PDF_EINVAL;
         if (!ws || ws_bytes < need) return PDF_EWORKSPACE;
         g->last_path = PDF_PATH_BINNED;
-        return stream_xfxq2<LaunchScope>(g->d, g->bplan, cm, n, x, q2, out, ld_out, ws, ws_bytes, g->chunk, s);
+        return stream_xfxq2<LaunchScope>(g->d, g->bplan, cm, n, x, q2, out, ld_out, ws, ws_bytes, g->chunk, s, 1, nullptr, nullptr,
+                                         kModeRows, nullptr, nullptr, nullptr, nullptr, q_is_q);
     }
     g->last_path = PDF_PATH_DIRECT;
-    return launch_direct(g, cm, n, x, q2, member, out, ld_out, s);
+    return launch_direct(g, cm, n, x, q2, member, out, ld_out, s, q_is_q);
 }
 
 int lumi_impl(const pdf_grid *g, void *ws, size_t ws_bytes, long long n, const double *x1, const double *x2, const double *q2,
@@ -121,6 +123,13 @@ int pdf_xfxq2(const pdf_grid *g, const int *pids, int npid, long long n, const d
               const double *q2, double *out, void *stream)
 {
     return pdf_xfxq2_ex(g, pids, npid, n, x, q2, nullptr, out, npid, stream);
+}
+
+int pdf_xfxq(const pdf_grid *g, const int *pids, int npid, long long n, const double *x,
+             const double *q, double *out, void *stream)
+{
+    if (!g) return PDF_EINVAL;
+    return xfxq2_impl(g, g->ws, g->ws_bytes, pids, npid, n, x, q, nullptr, out, npid, (cudaStream_t)stream, 1);
 }
 
 int pdf_xfxq2_xgrid(const pdf_grid *g, const int *pids, int npid, long long npts, const double *x, const double *q2,

@@ -1,0 +1,75 @@
+"""NEXT-4 on the GPU: the extrapolation options of PAPER.md L1720 (freeze, error) and xfxQ (L1712), both evaluation
+paths, against the oracle under the same option; the luminosity and the multi-member call under 'freeze'."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2302_03343_b200 import synth
+from conftest import make_oracle_grid
+from parity import assert_values
+from test_gpu_parity import B, PATHS, check_locate, gpu_grid  # noqa: F401  (B is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("mode", ["freeze", "error"])
+def test_extrapolation_options_parity(B, oracle_mod, path, mode):
+    spec = synth.grid_c1()
+    n = 400_000
+    x, q = synth.queries_c2(spec, n, seed=77)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    og.set_extrapolation({"freeze": oracle_mod.EXTRAP_FREEZE, "error": oracle_mod.EXTRAP_ERROR}[mode])
+    g.pdf_grid_set_option(B.PDF_OPT_EXTRAPOLATION, {"freeze": B.PDF_EXTRAP_FREEZE, "error": B.PDF_EXTRAP_ERROR}[mode])
+    ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), want_scale=True)
+    out = g.pdf_xfxq2(spec.pids, x.cuda(), q.cuda()).cpu().numpy()
+    print("\n", mode, path, assert_values(out, ref, S, f"{mode} {path}", strict=1e-12))
+    n_nan = int(np.isnan(ref[:, 0]).sum())
+    assert g.pdf_error_count() == n_nan
+    assert (n_nan > 0.04 * n) if mode == "error" else (n_nan == 0)
+    check_locate(B, og, g, x.numpy(), q.numpy())
+    # back to the default option: the default numbers
+    og.set_extrapolation(oracle_mod.EXTRAP_CONTINUATION)
+    g.pdf_grid_set_option(B.PDF_OPT_EXTRAPOLATION, B.PDF_EXTRAP_CONTINUATION)
+    ref, S = og.xfxq2(spec.pids, x.numpy()[:50_000], q.numpy()[:50_000], want_scale=True)
+    assert_values(g.pdf_xfxq2(spec.pids, x[:50_000].cuda(), q[:50_000].cuda()).cpu().numpy(), ref, S, "default again")
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_freeze_lumi_and_members(B, oracle_mod, path):
+    spec = synth.grid_c1()
+    n = 200_000
+    x1, x2, qq, w = synth.events_c4(n, seed=31)
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    og.set_coupling(spec.coupling.numpy())
+    og.set_extrapolation(oracle_mod.EXTRAP_FREEZE)
+    g.pdf_grid_set_option(B.PDF_OPT_EXTRAPOLATION, B.PDF_EXTRAP_FREEZE)
+    ref, S = og.lumi(x1.numpy(), x2.numpy(), qq.numpy(), w.numpy(), want_scale=True)
+    out = g.pdf_lumi(x1.cuda(), x2.cuda(), qq.cuda(), w.cuda()).cpu().numpy()
+    print("\nlumi freeze", path, assert_values(out, ref, S, "lumi freeze"))
+    mspec = synth.grid_c1(nmem=5)
+    nm = 300_000
+    x, q = synth.queries_c2(mspec, nm, seed=78)
+    mem = synth.members(mspec, nm)
+    mog = oracle_mod.OracleGrid(mspec.x_knots.numpy(), [k.numpy() for k in mspec.q2_subgrids], mspec.values.numpy(), mspec.pids, nmem=5)
+    mog.set_extrapolation(oracle_mod.EXTRAP_FREEZE)
+    mg = gpu_grid(B, mspec, path, nm)
+    mg.pdf_grid_set_option(B.PDF_OPT_EXTRAPOLATION, B.PDF_EXTRAP_FREEZE)
+    ref, S = mog.xfxq2(mspec.pids, x.numpy(), q.numpy(), member=mem.numpy(), want_scale=True)
+    out = mg.pdf_xfxq2(mspec.pids, x.cuda(), q.cuda(), member=mem.cuda()).cpu().numpy()
+    print("\nmembers freeze", path, assert_values(out, ref, S, "members freeze"))
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_xfxq_parity(B, oracle_mod, path):
+    spec = synth.grid_c1()
+    n = 300_000
+    x, q2 = synth.queries_c2(spec, n, seed=79)
+    Q = torch.sqrt(q2)
+    Q[::1000] = -Q[::1000]                      # invalid although the square is not
+    Q[1::5000] = 0.0
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec, path, n)
+    ref, S = og.xfxq(spec.pids, x.numpy(), Q.numpy(), want_scale=True)
+    out = g.pdf_xfxq(spec.pids, x.cuda(), Q.cuda()).cpu().numpy()
+    print("\nxfxq", path, assert_values(out, ref, S, f"xfxq {path}", strict=1e-12))
+    assert g.pdf_error_count() == int(np.isnan(ref[:, 0]).sum()) > 0
