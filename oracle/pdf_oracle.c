@@ -123,9 +123,13 @@ int oracle_grid_set_alphas(oracle_grid *g, int n, const double *q2_knots,
                            const double *values)
 {
     if (!g || n < 2 || !q2_knots || !values) return -1;
+    /* knots increase; a knot may appear twice (a flavour threshold: the end of one sub-line and the start of the
+     * next, L1835 "the sub-grids mechanism ... flavor thresholds"), every sub-line has at least 2 knots */
     for (int j = 0; j < n; ++j) {
         if (!finite_pos(q2_knots[j]) || !isfinite(values[j])) return -1;
-        if (j && !(q2_knots[j] > q2_knots[j - 1])) return -1;
+        if (j && !(q2_knots[j] >= q2_knots[j - 1])) return -1;
+        if (j && q2_knots[j] == q2_knots[j - 1] && (j == 1 || j == n - 1 || q2_knots[j - 1] == q2_knots[j - 2] ||
+                                                      q2_knots[j + 1] == q2_knots[j])) return -1;
     }
     free(g->aq2); free(g->as); free(g->aval);
     g->na = n;
@@ -525,8 +529,13 @@ int oracle_alphas_q2(const oracle_grid *g, long long n, const double *q2, double
                                      log(g->aval[1] / g->aval[0]) / log(g->aq2[1] / g->aq2[0]));
             else v = g->aval[0];                                        /* L1835, PDFFlow  */
         } else {
-            int c = find_cell(m, g->aq2, q);
-            v = hermite_cell(m, g->as, g->aval, 1, c, log(q));
+            /* the sub-line of q: it starts at the last repeated knot <= q (a query on a threshold belongs to the
+             * upper sub-line, as C-3) and ends at the next repeated knot; C-5 inside it, one-sided slopes at its ends */
+            int lo = 0, hi = m - 1;
+            for (int j = 1; j < m; ++j)
+                if (g->aq2[j] == g->aq2[j - 1]) { if (g->aq2[j] <= q) lo = j; else { hi = j - 1; break; } }
+            int c = find_cell(hi - lo + 1, g->aq2 + lo, q);
+            v = hermite_cell(hi - lo + 1, g->as + lo, g->aval + lo, 1, c, log(q));
         }
         out[e] = v;
     }

@@ -905,3 +905,33 @@ def test_xfxq_is_xfxq2_at_q_squared(oracle_mod):
     assert np.array_equal(og.xfxq(spec.pids, x, Q), og.xfxq2(spec.pids, x, Q * Q))
     bad = og.xfxq(spec.pids, np.array([0.1, 0.1, 0.1]), np.array([-4.0, 0.0, np.inf]))
     assert np.isnan(bad).all()
+
+
+def test_alphas_subgrids_split_the_knot_line(oracle_mod):
+    """C-alpha / L1835 ("the sub-grids mechanism ... flavor thresholds"): a repeated knot splits the alpha_s line
+    exactly as C-3 splits the Q2 line.  Pins: each sub-line equals the SAME knots given as a line of their own
+    (nothing leaks across a threshold); the threshold belongs to the upper sub-line; the jump is reproduced."""
+    spec = synth.grid_c0()
+    og = make_oracle_grid(oracle_mod, spec)
+    a = np.array([1.0, 1.7, 2.28, 2.28, 5.0, 11.0, 24.2, 24.2, 90.0, 400.0, 1e4])
+    A = np.array([0.40, 0.37, 0.35, 0.352, 0.30, 0.26, 0.23, 0.2312, 0.19, 0.16, 0.12])
+    og.set_alphas(a, A)
+    rng = np.random.default_rng(3)
+    cuts = [(0, 3), (3, 7), (7, 11)]
+    for lo, hi in cuts:
+        q = np.exp(rng.uniform(np.log(a[lo]), np.log(a[hi - 1]), 400))
+        q = q[(q >= a[lo]) & (q < a[hi - 1])]
+        whole = og.alphas_q2(q)
+        og2 = make_oracle_grid(oracle_mod, spec)
+        og2.set_alphas(a[lo:hi], A[lo:hi])
+        assert np.array_equal(whole, og2.alphas_q2(q))
+    # nodes: every knot returns a stored value; on a threshold the upper one; just below it the lower sub-line's limit
+    got = og.alphas_q2(a)
+    exp = A.copy(); exp[2] = A[3]; exp[6] = A[7]
+    assert np.array_equal(got, exp)
+    below = og.alphas_q2(np.nextafter(a[[2, 6]], 0.0))
+    assert np.allclose(below, A[[2, 6]], rtol=0, atol=1e-12) and not np.array_equal(below, A[[3, 7]])
+    # malformed lines are refused: a triple knot (a one-knot sub-line), a repeated first or last knot
+    for bad in ([1.0, 2.0, 2.0, 2.0, 3.0], [1.0, 1.0, 2.0, 3.0], [1.0, 2.0, 3.0, 3.0]):
+        with pytest.raises(ValueError):
+            og.set_alphas(np.array(bad), np.linspace(0.3, 0.1, len(bad)))
