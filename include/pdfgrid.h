@@ -104,7 +104,10 @@ int pdf_grid_create(pdf_grid **g, int nx, const double *x_knots, int nsub, const
                     const int *flavour_pids, int nmem);
 int pdf_grid_destroy(pdf_grid *g);
 
-/* alpha_s knots (HOST [n], Q2 strictly increasing > 0, n >= 2) and values (HOST [n]); L1746 */
+/* alpha_s knots (HOST [n], Q2 > 0 increasing, n >= 2) and values (HOST [n]); L1746.  A knot may appear twice (not at
+ * the ends, not three times): a flavour threshold, the end of one sub-line and the start of the next with its own value
+ * on either side (L1835 "the sub-grids mechanism ... flavor thresholds"); the Hermite cubic then uses one-sided slopes
+ * at the ends of every sub-line and a query on a threshold belongs to the upper sub-line. */
 int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double *values);
 /* flavour-pair coupling C, HOST [nflav][nflav] row-major, in the grid's column order; eq. 4.1 */
 int pdf_grid_set_coupling(pdf_grid *g, const double *C);

@@ -268,9 +268,13 @@ int pdf_grid_destroy(pdf_grid *g)
 int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double *values)
 {
     if (!g || n < 2 || !q2_knots || !values) return PDF_EINVAL;
+    // knots increase; a knot may appear twice (a flavour threshold: the end of one sub-line and the start of the next,
+    // PAPER.md L1835), every sub-line has at least 2 knots
     for (int j = 0; j < n; ++j) {
         if (!finite_pos_h(q2_knots[j]) || !std::isfinite(values[j])) return PDF_EINVAL;
-        if (j && !(q2_knots[j] > q2_knots[j - 1])) return PDF_EINVAL;
+        if (j && !(q2_knots[j] >= q2_knots[j - 1])) return PDF_EINVAL;
+        if (j && q2_knots[j] == q2_knots[j - 1] && (j == 1 || j == n - 1 || q2_knots[j - 1] == q2_knots[j - 2] ||
+                                                      q2_knots[j + 1] == q2_knots[j])) return PDF_EINVAL;
     }
     cudaFree(g->d_ak); cudaFree(g->d_alk); cudaFree(g->d_av); cudaFree(g->d_ca); cudaFree(g->d_acell); cudaFree(g->d_alut);
     g->d_ak = g->d_alk = g->d_av = g->d_acell = nullptr; g->d_ca = nullptr; g->d_alut = nullptr; g->d.na = 0;
@@ -280,7 +284,17 @@ int pdf_grid_set_alphas(pdf_grid *g, int n, const double *q2_knots, const double
     CK(cudaMemcpy(g->d_ak, q2_knots, sizeof(double) * n, cudaMemcpyHostToDevice));
     CK(cudaMemcpy(g->d_av, values, sizeof(double) * n, cudaMemcpyHostToDevice));
     { LaunchScope a(0, "k_log_knots"); k_log_knots<<<(n + 127) / 128, 128>>>(g->d_ak, g->d_alk, n); }
-    { LaunchScope a(0, "k_cell_tables"); k_cell_tables<<<(n + 127) / 128, 128>>>(g->d_alk, g->d_ca, 0, n); }
+    // cell constants per sub-line (one-sided slopes at its ends, C-5); the zero-width cell between the two copies of a
+    // threshold is never selected: the search takes the LATER copy of a repeated knot (C-3)
+    CK(cudaMemset(g->d_ca, 0, sizeof(CellTab) * n));
+    for (int first = 0; first < n;) {
+        int last = first;
+        while (last + 1 < n && q2_knots[last + 1] != q2_knots[last]) ++last;
+        const int m = last - first + 1;
+        LaunchScope a(0, "k_cell_tables");
+        k_cell_tables<<<(m + 127) / 128, 128>>>(g->d_alk, g->d_ca, first, m);
+        first = last + 1;
+    }
     { LaunchScope a(0, "k_alphas_cells"); k_alphas_cells<<<(n + 127) / 128, 128>>>(g->d_ca, g->d_av, g->d_acell, n); }
     {   // search table on the bit pattern of Q2: entry = the cell at the bucket's lower edge (the walk on the device makes it exact)
         std::vector<double> k(q2_knots, q2_knots + n);

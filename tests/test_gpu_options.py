@@ -73,3 +73,30 @@ def test_xfxq_parity(B, oracle_mod, path):
     out = g.pdf_xfxq(spec.pids, x.cuda(), Q.cuda()).cpu().numpy()
     print("\nxfxq", path, assert_values(out, ref, S, f"xfxq {path}", strict=1e-12))
     assert g.pdf_error_count() == int(np.isnan(ref[:, 0]).sum()) > 0
+
+
+def test_alphas_subgrids_parity(B, oracle_mod):
+    """alpha_s knot line with two flavour thresholds (repeated knots, L1835): strict 1e-12 relative against the oracle,
+    stored values at every knot (the upper one on a threshold), both below-range modes"""
+    spec = synth.grid_c1()
+    a = np.exp(np.linspace(0.0, np.log(1e10), 58))
+    a = np.sort(np.concatenate([a, a[[9, 23]]]))                       # two repeated knots
+    A = 1.0 / (1.0 / 0.35 + (1.0 / 0.08 - 1.0 / 0.35) * (np.arange(60) / 59.0) ** 1.1)
+    dup = np.nonzero(a[1:] == a[:-1])[0] + 1
+    A[dup[0]:] *= 1.004; A[dup[1]:] *= 0.997                           # a jump at each threshold
+    og, g = make_oracle_grid(oracle_mod, spec), gpu_grid(B, spec)
+    rng = np.random.default_rng(8)
+    q = np.exp(rng.uniform(np.log(0.01), np.log(1e12), 500_000))
+    q[: len(a)] = a
+    q[len(a): len(a) + 2] = np.nextafter(a[dup], 0.0)
+    for mode_o, mode_g in ((oracle_mod.ALPHAS_FREEZE, B.PDF_ALPHAS_FREEZE), (oracle_mod.ALPHAS_LOGGRAD, B.PDF_ALPHAS_LOGGRAD)):
+        og.set_alphas(a, A, mode_o)
+        g.pdf_grid_set_alphas(torch.tensor(a), torch.tensor(A))
+        g.pdf_grid_set_option(B.PDF_OPT_ALPHAS_MODE, mode_g)
+        ref = og.alphas_q2(q)
+        got = g.pdf_alphas_q2(torch.tensor(q).cuda()).cpu().numpy()
+        assert np.max(np.abs(got - ref) / np.abs(ref)) < 1e-12
+        exp = A.copy(); exp[dup - 1] = A[dup]
+        assert np.array_equal(got[: len(a)], exp)
+    with pytest.raises(B.PdfGridError):
+        g.pdf_grid_set_alphas(torch.tensor([1.0, 2.0, 2.0, 2.0, 3.0]), torch.tensor([0.3, 0.25, 0.2, 0.15, 0.1]))
