@@ -111,7 +111,7 @@ int pdf_xfxq2_noalloc(const pdf_grid *g, const int *pids, int npid, long long n,
     const size_t smem = stream_smem_bytes(g->d, A.B);
     int per_sm = 0, sms = 0;
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device));
-    const auto kern = A.identity ? k_pdf_stream : k_pdf_stream_cols;     // rows of npid doubles: the stride fits 32 bits
+    const auto kern = g->d.extrap != kExtrapContinuation ? k_pdf_stream_opt : A.identity ? k_pdf_stream : k_pdf_stream_cols;   // rows of npid doubles: the stride fits 32 bits
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kS3Threads, smem));
     if (per_sm < 1) return PDF_ECUDA;
     const unsigned long long max_ctas = (unsigned long long)per_sm * sms;         // all CTAs must be co-resident

@@ -298,7 +298,7 @@ __device__ __noinline__ double s3_two(double f0, double f1, double theta) { retu
 __device__ __noinline__ double s3_lowq(double fmin, double fplus, double r, double lnr) { return lowq_continue_ln(fmin, fplus, r, lnr); }
 
 // ---- A tile: classify, locate, t_x / t_q, one slot per query in its cell's bin -----------------
-template <int MODE>
+template <int MODE, bool OPT>
 __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, int slot, long long chunk_base, long long chunk_end,
                                        int tile, unsigned long long &err_local)
 {
@@ -337,8 +337,9 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
             if (e < t1) {
                 r.xv[q] = __ldcs(A.x + e); r.qv[q] = __ldcs(A.q2 + e);
                 if (MODE == kModeLumiFirst) r.sc[q] = __ldcs(A.w + e) / (r.xv[q] * __ldcs(A.x2 + e));   // f = xf / x on both sides (eq. 3.3): the query's own x
-                if (A.q_is_q) r.qv[q] = q_to_q2(r.qv[q]);
-                apply_extrapolation(G, r.xv[q], r.qv[q]);                                              // L1720 (no-op for the default option)
+                // pdf_xfxq and the extrapolation options of L1720 (kernels of their own: even as two warp-uniform
+                // branches that are never taken they cost the default kernel 0.58 ms per 1e8 queries)
+                if (OPT) { if (A.q_is_q) r.qv[q] = q_to_q2(r.qv[q]); apply_extrapolation(G, r.xv[q], r.qv[q]); }
             }
         }
         return r;
@@ -385,13 +386,28 @@ __device__ __forceinline__ void a_tile(const StreamArgs &A, const StreamTab &T, 
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q)
             if (o.key[q] >= 0 && o.pos[q] >= (unsigned)B.cap) { o.key[q] = -1 - kListOvf; o.any_list = true; }   // bin full: to the overflow list
-        // list entries (extrapolated queries, bin overflow): one atomic per entry on the list's counter.  (Warp-
-        // aggregated reservations with match.any cost ~100 warp instructions per group, and at 5 % extrapolated
-        // queries nearly every group of 64 has an entry; the six counters see ~1 atomic per microsecond.)
+        // list entries (extrapolated queries, bin overflow).  With a few entries per warp (C2: 5 % of the queries) one
+        // atomic per entry is cheapest (the match.any reservation below costs ~50 warp instructions per query slot and
+        // nearly every group of 64 has an entry); with many (C4: 25 % of the events take the low-Q2 list) the entries of
+        // a warp reserve their run with ONE atomic per list, or the list's counter serialises them.
         if (__any_sync(0xffffffffu, o.any_list)) {
 #pragma unroll
-            for (int q = 0; q < kS3Grp; ++q)
-                if (o.key[q] < 0 && o.key[q] != INT_MIN) o.pos[q] = atomicAdd(lcount + (-1 - o.key[q]), 1u);
+            for (int q = 0; q < kS3Grp; ++q) {
+                const bool mine = o.key[q] < 0 && o.key[q] != INT_MIN;
+                const unsigned act = __ballot_sync(0xffffffffu, mine);
+                if (act == 0u) continue;
+                if (__popc(act) <= 3) {
+                    if (mine) o.pos[q] = atomicAdd(lcount + (-1 - o.key[q]), 1u);
+                } else if (mine) {
+                    const int k = -1 - o.key[q];
+                    const unsigned peers = __match_any_sync(act, k);
+                    const int leader = __ffs(peers) - 1;
+                    unsigned base = 0;
+                    if (lane == leader) base = atomicAdd(lcount + k, (unsigned)__popc(peers));
+                    base = __shfl_sync(peers, base, leader);
+                    o.pos[q] = base + (unsigned)__popc(peers & ((1u << lane) - 1u));
+                }
+            }
         }
 #pragma unroll
         for (int q = 0; q < kS3Grp; ++q) {
@@ -895,7 +911,7 @@ k_locate_stream(const __grid_constant__ GridDev G, const __grid_constant__ Strea
     }
 }
 
-template <int MODE, bool FAST>
+template <int MODE, bool FAST, bool OPT>
 __device__ __forceinline__ void stream_body(const StreamArgs &A)
 {
     extern __shared__ __align__(32) unsigned char smem_raw[];
@@ -968,7 +984,7 @@ __device__ __forceinline__ void stream_body(const StreamArgs &A)
         if (isA) {
             // the ring slot must have been drained by the units of chunk c - kS3Ring before this tile touches its bins
             if (gen) wait_for(b_done, gen * TB);
-            a_tile<MODE>(A, T, slot, chunk_base, chunk_end, sub, err_local);
+            a_tile<MODE, OPT>(A, T, slot, chunk_base, chunk_end, sub, err_local);
             warp_release_red(a_done, 1ULL);
         } else {
             wait_for(a_done, (gen + 1) * TA);                      // every tile of A(c) has been released
@@ -992,10 +1008,14 @@ __device__ __forceinline__ void stream_body(const StreamArgs &A)
 
 // k_pdf_stream: rows of the grid's own 11 columns in order (any leading dimension below 2^29 doubles); k_pdf_stream_cols:
 // any column list (pid subsets, repeated or unknown pids)
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __grid_constant__ StreamArgs A) { stream_body<kModeRows, true>(A); }
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream_cols(const __grid_constant__ StreamArgs A) { stream_body<kModeRows, false>(A); }
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_first(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiFirst, false>(A); }
-__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_second(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiSecond, false>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream(const __grid_constant__ StreamArgs A) { stream_body<kModeRows, true, false>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream_cols(const __grid_constant__ StreamArgs A) { stream_body<kModeRows, false, false>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_first(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiFirst, false, false>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_second(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiSecond, false, false>(A); }
+// the same with pdf_xfxq's Q -> Q2 and the extrapolation options of L1720 applied where an A tile loads its queries
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_pdf_stream_opt(const __grid_constant__ StreamArgs A) { stream_body<kModeRows, false, true>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_first_opt(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiFirst, false, true>(A); }
+__global__ void __launch_bounds__(kS3Threads, PDF_S3_MINB) k_lumi_second_opt(const __grid_constant__ StreamArgs A) { stream_body<kModeLumiSecond, false, true>(A); }
 
 __host__ __device__ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 

@@ -179,6 +179,9 @@ inline int stream_plan_init(StreamPlan &p, const GridDev &G, const std::vector<d
     if (cudaFuncSetAttribute(k_pdf_stream_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
     if (cudaFuncSetAttribute(k_lumi_first, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
     if (cudaFuncSetAttribute(k_lumi_second, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (cudaFuncSetAttribute(k_pdf_stream_opt, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (cudaFuncSetAttribute(k_lumi_first_opt, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (cudaFuncSetAttribute(k_lumi_second_opt, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
     if (cudaMalloc((void **)&p.d_coup, kCoupBytes) != cudaSuccess) return PDF_ENOMEM;
     p.usable = true;
     return 0;
@@ -220,7 +223,9 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const bool rows11 = A.identity && ld < (1LL << 29);              // the four fixed stores of b_unit (32-bit row stride in bytes)
-    const auto kern = mode == kModeLumiFirst ? k_lumi_first : mode == kModeLumiSecond ? k_lumi_second : rows11 ? k_pdf_stream : k_pdf_stream_cols;
+    const bool opt = q_is_q || G.extrap != kExtrapContinuation;      // pdf_xfxq / an extrapolation option of L1720: kernels of their own
+    const auto kern = opt ? (mode == kModeLumiFirst ? k_lumi_first_opt : mode == kModeLumiSecond ? k_lumi_second_opt : k_pdf_stream_opt)
+                          : (mode == kModeLumiFirst ? k_lumi_first : mode == kModeLumiSecond ? k_lumi_second : rows11 ? k_pdf_stream : k_pdf_stream_cols);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kS3Threads, smem) != cudaSuccess || per_sm < 1)
         return PDF_ECUDA;
     const unsigned long long max_ctas = (unsigned long long)per_sm * sms;         // all CTAs must be co-resident
@@ -230,7 +235,8 @@ inline int stream_xfxq2(const GridDev &G, const StreamPlan &p, const ColMap &cm,
     const unsigned long long want = (tickets + kS3Warps - 1) / kS3Warps;
     const unsigned grid = (unsigned)(want < max_ctas ? want : max_ctas);
     {
-        Scope sc(s, mode == kModeLumiFirst ? "k_lumi_first" : mode == kModeLumiSecond ? "k_lumi_second" : rows11 ? "k_pdf_stream" : "k_pdf_stream_cols");
+        Scope sc(s, opt ? (mode == kModeLumiFirst ? "k_lumi_first_opt" : mode == kModeLumiSecond ? "k_lumi_second_opt" : "k_pdf_stream_opt")
+                        : (mode == kModeLumiFirst ? "k_lumi_first" : mode == kModeLumiSecond ? "k_lumi_second" : rows11 ? "k_pdf_stream" : "k_pdf_stream_cols"));
         kern<<<grid, kS3Threads, smem, s>>>(A);
     }
     return cudaGetLastError() == cudaSuccess ? PDF_OK : PDF_ECUDA;
