@@ -280,6 +280,8 @@ def run_ours(args):
         g.pdf_alphas_q2(q2, out=aout)
 
     secs, clocks, prof, launches = timed_steps(torch, dist, world, step, args.steps, args.warmup, sampler_index=local)
+    # which kernels the timed pdf_xfxq2 calls took (pdf_alphas_q2 does not touch the record)
+    path_taken = {binding.PDF_PATH_DIRECT: "direct", binding.PDF_PATH_BINNED: "binned"}.get(g.pdf_last_path(), "?")
     n_invalid = g.pdf_error_count()
     out_sample = out[:200_000].clone()
     table = kernel_table(prof, args.steps)
@@ -294,7 +296,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD,
-                       "queries_per_gpu_per_step": n, "path": args.path, "n_invalid": n_invalid,
+                       "queries_per_gpu_per_step": n, "path": args.path, "path_taken": path_taken, "n_invalid": n_invalid,
                        "l2": "inputs (1.6 GB) and outputs (9.6 GB) per step exceed the 126 MB L2; no flush needed"},
             "clocks": clocks, "gpu_launches": launches, "kernels": table, "roofline": roof}
 
