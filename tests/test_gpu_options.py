@@ -100,3 +100,36 @@ def test_alphas_subgrids_parity(B, oracle_mod):
         assert np.array_equal(got[: len(a)], exp)
     with pytest.raises(B.PdfGridError):
         g.pdf_grid_set_alphas(torch.tensor([1.0, 2.0, 2.0, 2.0, 3.0]), torch.tensor([0.3, 0.25, 0.2, 0.15, 0.1]))
+
+
+@pytest.mark.parametrize("mode", ["freeze", "error"])
+def test_extrapolation_options_on_the_shared_point_list(B, oracle_mod, mode):
+    """pdf_xfxq2_xgrid (both of its kernels) and pdf_xfxq2_noalloc under the options of L1720"""
+    spec = synth.grid_c1(nmem=160)
+    og = make_oracle_grid(oracle_mod, spec)
+    og.set_extrapolation({"freeze": oracle_mod.EXTRAP_FREEZE, "error": oracle_mod.EXTRAP_ERROR}[mode])
+    opt = {"freeze": B.PDF_EXTRAP_FREEZE, "error": B.PDF_EXTRAP_ERROR}[mode]
+    npts = 2000
+    x, q = synth.queries_c2(spec, npts, seed=91)
+    for path, nrep in (("direct", 3), ("auto", 160)):                 # per-point kernel; (member, cell)-shared kernel
+        g = gpu_grid(B, spec, path)
+        g.pdf_grid_set_option(B.PDF_OPT_EXTRAPOLATION, opt)
+        got = g.pdf_xfxq2_xgrid(spec.pids, x.cuda(), q.cuda(), nrep).cpu().numpy()
+        n_bad = 0
+        for r in (0, nrep // 2, nrep - 1):
+            ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), member=np.full(npts, r, dtype=np.int32), want_scale=True)
+            assert_values(got[r], ref, S, f"xgrid {mode} {path} member {r}")
+            n_bad = int(np.isnan(ref[:, 0]).sum())
+        assert g.pdf_error_count() == n_bad * nrep
+        g.close()
+    spec1 = synth.grid_c1()
+    og1 = make_oracle_grid(oracle_mod, spec1)
+    og1.set_extrapolation({"freeze": oracle_mod.EXTRAP_FREEZE, "error": oracle_mod.EXTRAP_ERROR}[mode])
+    g = gpu_grid(B, spec1)
+    g.pdf_grid_set_option(B.PDF_OPT_EXTRAPOLATION, opt)
+    n = 60_000
+    x, q = synth.queries_c2(spec1, n, seed=92)
+    out = torch.empty((n, 11), dtype=torch.float64, device="cuda")
+    g.pdf_xfxq2_noalloc(spec1.pids, x.cuda(), q.cuda(), out)
+    ref, S = og1.xfxq2(spec1.pids, x.numpy(), q.numpy(), want_scale=True)
+    assert_values(out.cpu().numpy(), ref, S, f"noalloc {mode}")
