@@ -105,16 +105,20 @@ def test_alphas_subgrids_parity(B, oracle_mod):
 @pytest.mark.parametrize("mode", ["freeze", "error"])
 def test_extrapolation_options_on_the_shared_point_list(B, oracle_mod, mode):
     """pdf_xfxq2_xgrid (both of its kernels) and pdf_xfxq2_noalloc under the options of L1720"""
-    spec = synth.grid_c1(nmem=160)
+    spec = synth.grid_c1(nmem=210)
     og = make_oracle_grid(oracle_mod, spec)
     og.set_extrapolation({"freeze": oracle_mod.EXTRAP_FREEZE, "error": oracle_mod.EXTRAP_ERROR}[mode])
     opt = {"freeze": B.PDF_EXTRAP_FREEZE, "error": B.PDF_EXTRAP_ERROR}[mode]
     npts = 2000
     x, q = synth.queries_c2(spec, npts, seed=91)
-    for path, nrep in (("direct", 3), ("auto", 160)):                 # per-point kernel; (member, cell)-shared kernel
+    for path, nrep in (("direct", 3), ("auto", 210)):                 # per-point kernel; (member, cell)-shared kernel
         g = gpu_grid(B, spec, path)
         g.pdf_grid_set_option(B.PDF_OPT_EXTRAPOLATION, opt)
+        B.pdf_profile_enable(True)
         got = g.pdf_xfxq2_xgrid(spec.pids, x.cuda(), q.cuda(), nrep).cpu().numpy()
+        names = [k for k, _ in B.pdf_profile_read(64)]
+        B.pdf_profile_enable(False)
+        assert names == ["k_xfxq2_xgrid" if path == "direct" else "k_xfxq2_xgrid_cell"], names
         n_bad = 0
         for r in (0, nrep // 2, nrep - 1):
             ref, S = og.xfxq2(spec.pids, x.numpy(), q.numpy(), member=np.full(npts, r, dtype=np.int32), want_scale=True)
